@@ -1,0 +1,237 @@
+/*
+ * dovetail.h -- C ABI of libdovetail_draft.so
+ *
+ * The GPU-side draft step of Dovetail heterogeneous speculative decoding
+ * (arxiv 2412.18934), written from the paper for NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (paper citations are PAPER.md line numbers):
+ *   - Dynamic Gating Fusion of the target's hidden feature with the token
+ *     embedding: h1 = W1 f, h2 = W2 e, g = sigmoid(Wg [h1 || h2] + bg),
+ *     x = g * h1 + (1 - g) * h2                       (Fig. 5 :98)
+ *   - the deepened draft decoder stack, n_layers LLaMA blocks, run over the
+ *     rows of one level of a draft-token tree with tree attention against the
+ *     committed prefix KV cache and the row's tree ancestors
+ *
+ *   - LM head, per-node top-k expansion, cumulative-probability scoring,
+ *     frontier selection for the next round and the final rerank to the
+ *     top-gamma candidate set
+ *   - the KV bookkeeping after the target has verified the candidates
+ *                                                      (last sentence)
+ *
+ * Conventions
+ *   - All functions are extern "C", return 0 on success and a negative
+ *     dovetail_status_t on failure. Nothing throws, aborts or calls exit().
+ *   - "dev" pointers are CUDA device pointers on the current device of the
+ *     calling thread; "host" pointers are ordinary host memory. The library
+ *     never takes ownership of caller memory.
+ *   - Matrices are row-major [out, in] (y = W x), dtype = cfg.dtype.
+ *   - cuda_stream is a cudaStream_t passed as void* (NULL = default stream).
+ *   - There is no CPU fallback: every entry point fails with DOVETAIL_ECUDA
+ *     when no sm_100 device is usable.
+ */
+#ifndef DOVETAIL_H_
+#define DOVETAIL_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define DOVETAIL_MAX_DEPTH 16
+#define DOVETAIL_MAX_LAYERS 16
+
+typedef enum {
+  DOVETAIL_OK = 0,
+  DOVETAIL_EINVAL = -1,    /* null pointer, bad shape, bad tree spec, bad path */
+  DOVETAIL_ECAPACITY = -2, /* KV cache / tree pool too small for this call     */
+  DOVETAIL_ECUDA = -3,     /* CUDA error; text in dovetail_last_error()        */
+  DOVETAIL_ENOMEM = -4
+} dovetail_status_t;
+
+typedef enum { DOVETAIL_F32 = 0, DOVETAIL_BF16 = 1 } dovetail_dtype_t;
+
+/* Model shape. The block is the LLaMA-family decoder layer of the paper's
+ * target models: pre-RMSNorm, rotary embedding with half-split
+ * pairing (i, i + head_dim/2), grouped-query attention, SiLU-gated FFN, no
+ * linear biases. */
+typedef struct {
+  int32_t hidden;       /* d                                              */
+  int32_t n_q_heads;    /* Hq                                             */
+  int32_t n_kv_heads;   /* Hkv, divides Hq                                */
+  int32_t head_dim;     /* dh, 64 or 128                                  */
+  int32_t n_layers;     /* draft Transformer blocks (the paper's M), <= DOVETAIL_MAX_LAYERS */
+  int32_t ffn;          /* F                                              */
+  int32_t vocab;        /* V                                              */
+  float rope_theta;
+  float rms_eps;
+  int32_t dtype;        /* dovetail_dtype_t of weights, norm gains, bias and KV cache */
+  int32_t dgf_proj;     /* 1: W1, W2 present (paper). 0: W1 = W2 = identity          */
+  int32_t first_layer_input_norm; /* 1: layer 0 applies its input RMSNorm; 0: skips it */
+  int32_t final_norm;   /* 1: RMSNorm(g_final) before the LM head; 0: none           */
+  int32_t max_rows;     /* largest n_new and largest beam[] a step may use (<= 64)   */
+  int32_t max_tree_slots; /* largest sum over tree levels of forwarded rows (<= 128) */
+  int32_t max_branch;   /* largest branch[] a step may use (<= 32)                   */
+} dovetail_config_t;
+
+/* Device pointers to one decoder layer's weights. */
+typedef struct {
+  const void* g_attn; /* [d]        input RMSNorm gain          */
+  const void* wq;     /* [Hq*dh, d]                             */
+  const void* wk;     /* [Hkv*dh, d]                            */
+  const void* wv;     /* [Hkv*dh, d]                            */
+  const void* wo;     /* [d, Hq*dh]                             */
+  const void* g_ffn;  /* [d]        post-attention RMSNorm gain */
+  const void* wgate;  /* [F, d]                                 */
+  const void* wup;    /* [F, d]                                 */
+  const void* wdown;  /* [d, F]                                 */
+} dovetail_layer_weights_t;
+
+/* Device pointers to all weights. BORROWED: the caller keeps them alive and
+ * unchanged for the life of the handle. The struct itself (and layers[]) is
+ * host memory and is copied by dovetail_draft_init. */
+typedef struct {
+  const void* embed;   /* [V, d]  token embedding E                      */
+  const void* dgf_w1;  /* [d, d]  hidden-state branch; NULL iff dgf_proj == 0 */
+  const void* dgf_w2;  /* [d, d]  embedding branch;    NULL iff dgf_proj == 0 */
+  const void* dgf_wg;  /* [d, 2d] gate, input order [h1 || h2]           */
+  const void* dgf_bg;  /* [d]     gate bias                              */
+  const dovetail_layer_weights_t* layers; /* host array [n_layers]       */
+  const void* g_final; /* [d] or NULL (required iff final_norm)          */
+  const void* lm_head; /* [V, d]                                         */
+} dovetail_weights_t;
+
+/* Draft KV cache, caller-owned device memory.
+ *   k, v : [n_layers][n_kv_heads][capacity][head_dim], dtype = cfg.dtype,
+ *          K stored AFTER rotary embedding.
+ * Rows [0, committed_len) are the committed prefix; dovetail_draft_step writes
+ * rows >= committed_len and advances committed_len (see below). The struct
+ * lives in host memory. */
+typedef struct {
+  void* k;
+  void* v;
+  int32_t capacity;
+  int32_t committed_len;
+} dovetail_kv_cache_t;
+
+/* Draft tree shape (settings :184).
+ *   depth  D >= 1 : number of token levels below the root = number of draft
+ *                   forwards per step.
+ *   branch[l]     : children kept per expanded node of level l (l = 0 is the
+ *                   root, i.e. the last verified token). 1 <= branch <= max_branch.
+ *   beam[l], l>=1 : at most this many level-l nodes (best cumulative
+ *                   log-probability first) are forwarded and expanded;
+ *                   0 = all of them. beam[0] is ignored.
+ *   gamma         : number of candidates returned (root excluded).
+ * The paper's server preset is depth 7, branch = beam = 10, gamma = 16. */
+typedef struct {
+  int32_t depth;
+  int32_t branch[DOVETAIL_MAX_DEPTH];
+  int32_t beam[DOVETAIL_MAX_DEPTH];
+  int32_t gamma;
+} dovetail_tree_spec_t;
+
+/* Device output buffers of one step, each of capacity >= gamma.
+ * Candidates are emitted in pool (topological) order: parents[i] < i or -1
+ * (child of the root). scores[i] is the cumulative natural-log probability
+ * root -> node ("global acceptance probability"). */
+typedef struct {
+  int32_t* token_ids; /* dev [gamma]           */
+  float* scores;      /* dev [gamma]           */
+  int32_t* parents;   /* dev [gamma]           */
+  int32_t* depths;    /* dev [gamma] or NULL; level of the node, 1-based */
+  int32_t* n_out;     /* dev [1]; = min(gamma, pool size) */
+} dovetail_draft_out_t;
+
+typedef struct dovetail_draft dovetail_draft_t;
+
+/* Create a handle: validates cfg, records the borrowed weight pointers and
+ * allocates the scratch the step needs (activations in fp32, tree pool,
+ * per-CTA partials). Errors: EINVAL, ENOMEM, ECUDA. *out is NULL on failure. */
+int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cfg,
+                        dovetail_draft_t** out);
+
+/* One draft step: D forwards of the draft model and the
+ * final rerank, enqueued asynchronously on cuda_stream, no host
+ * synchronisation inside.
+ *   hidden_feats : dev fp32 [n_new, d]  target hidden states of the n_new
+ *                  newly verified tokens (the vector the target's LM head
+ *                  consumes), row i paired with tokens[i].
+ *   tokens       : dev int32 [n_new]
+ *   n_new        : 1 <= n_new <= cfg.max_rows
+ * Level 0 runs the n_new rows at positions committed_len + i with causal
+ * attention and appends their K/V at those cache rows; the last row's
+ * distribution seeds the tree. Tree level l >= 1 runs the selected frontier
+ * nodes at position committed_len + n_new + l - 1, each attending the prefix,
+ * its tree ancestors and itself; its input feature is the draft's own output
+ * hidden state of its parent row. Tree K/V go to cache rows after the prefix.
+ * On return (still asynchronous) kv->committed_len has been advanced by n_new.
+ * Needs committed_len + n_new + (tree rows) <= capacity, else ECAPACITY.
+ * Ties: top-k within a row by (logit desc, token id asc); frontier and final
+ * selection by (cumulative score desc, pool index asc).
+ * Errors: EINVAL (null pointers, n_new out of range, bad tree spec),
+ * ECAPACITY, ECUDA. On error nothing was enqueued and kv is untouched. */
+int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens,
+                        int32_t n_new, dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree,
+                        const dovetail_draft_out_t* out, void* cuda_stream);
+
+/* After verification: tell the draft which candidates the
+ * target accepted.
+ *   accepted_path : HOST int32 [n_acc], indices into the last step's output,
+ *                   root -> leaf (accepted_path[0] has parent -1, each next
+ *                   entry is a child of the previous one). n_acc may be 0.
+ *   mode 0 (the paper's flow): the tree K/V rows are discarded; committed_len
+ *          is unchanged; the caller feeds the accepted tokens with their true
+ *          target features to the next dovetail_draft_step.
+ *   mode 1 (extra): the K/V rows of the accepted nodes that were forwarded
+ *          during the step are moved to cache rows committed_len.. in path
+ *          order and committed_len advances by their count (the leading nodes
+ *          of the path; a leaf that was never forwarded has no K/V). The
+ *          count is returned in *n_committed (host, may be NULL). This mode
+ *          synchronises the stream once to read the device-side validation.
+ * Errors: EINVAL (bad path: cache untouched), ECUDA. */
+int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32_t* accepted_path,
+                       int32_t n_acc, int32_t mode, int32_t* n_committed, void* cuda_stream);
+
+/* Tree bookkeeping alone, for bit-exact checks of the
+ * integer path: replays expansion, scoring, frontier selection and the final
+ * rerank from caller-supplied per-row top-k lists instead of LM-head results.
+ *   cand_tokens, cand_logp : dev [n_rows, max_b] with max_b = max over levels
+ *        of branch[l]; row 0 is the root's list, then the forwarded rows of
+ *        level 1, level 2, ... in frontier order; entries sorted as the LM-head
+ *        stage would emit them (log-prob desc, token id asc).
+ * Writes out like dovetail_draft_step and, when non-NULL, the pool arrays
+ * (dev, capacity >= pool size): token, parent pool index, depth, cumulative
+ * score, and pool_size[1]. Asynchronous on cuda_stream. */
+int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree,
+                         const int32_t* cand_tokens, const float* cand_logp, int32_t n_rows,
+                         int32_t max_b, const dovetail_draft_out_t* out, int32_t* pool_token,
+                         int32_t* pool_parent, int32_t* pool_depth, float* pool_cum,
+                         int32_t* pool_size, void* cuda_stream);
+
+/* Optional taps for parity tests; pass NULL to disable (the default).
+ *   logits : dev fp32 [max rows of a step, V]; row r of the step (level-0 rows
+ *            first, then tree rows in cache-slot order) receives the LM-head
+ *            logits of that row (level 0: only the last row is computed).
+ *   hhat   : dev fp32 [max rows of a step, d]; the draft's output hidden state
+ *            of each row.
+ * Borrowed until replaced. */
+int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat);
+
+/* Number of kernel launches the last dovetail_draft_step enqueued. */
+int dovetail_last_launch_count(const dovetail_draft_t* h);
+
+/* Algorithmic HBM bytes of one forward over the given prefix length: all
+ * weight bytes + prefix K/V bytes. */
+int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len);
+
+void dovetail_draft_destroy(dovetail_draft_t* h);
+
+/* Text of the last error on this handle (or of the last failed init when
+ * h == NULL). Never NULL; valid until the next call on the same handle. */
+const char* dovetail_last_error(const dovetail_draft_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DOVETAIL_H_ */

@@ -1,0 +1,23 @@
+"""TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+The fp64 CPU oracle of the Dovetail draft step, written from the paper
+(arxiv 2412.18934). Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package. It imports
+nothing from the CUDA package.
+"""
+from .oracle import (  # noqa: F401
+    OracleConfig,
+    OracleWeights,
+    build,
+    dgf,
+    forward,
+    kv_commit,
+    lm_head,
+    log_softmax,
+    matvec,
+    rmsnorm,
+    rope,
+    step,
+    topk,
+    tree_replay,
+)
