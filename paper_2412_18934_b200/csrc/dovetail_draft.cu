@@ -1,0 +1,766 @@
+// dovetail_draft.cu -- host side of libdovetail_draft.so: the C ABI declared in
+// include/dovetail.h. It validates arguments, owns the scratch buffers and
+// enqueues the kernels of one draft step on the caller's
+// stream; every step of the method runs in the kernels of gemv.cuh,
+// attention.cuh and tree.cuh. There is no CPU fallback.
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/dovetail.h"
+#include "attention.cuh"
+#include "gemv.cuh"
+#include "state.cuh"
+#include "tree.cuh"
+
+using namespace dvt;
+
+namespace {
+
+constexpr int kSmemBudget = 200 * 1024;  // dynamic shared memory a GEMV CTA may use
+constexpr int kSmemMax = 227 * 1024;
+constexpr int kAttnStages = 4;
+
+char g_init_error[512] = "no error";
+
+struct LevelPlan {
+  int rows;        // rows forwarded at this level (level 0: n_new)
+  int rows_lm;     // rows whose LM-head lists are expanded (level 0: 1)
+  int row0;        // first step row
+  int t0;          // first tree-row index (levels >= 1)
+  int pool_begin;  // pool index of the level's first child
+};
+
+}  // namespace
+
+struct dovetail_draft {
+  dovetail_config_t cfg;
+  dovetail_weights_t w;
+  std::vector<dovetail_layer_weights_t> layers;
+  int num_sms = 0, es = 2;
+  int dq = 0, dkv = 0, ldq = 0;
+  int max_step_rows = 0, pool_cap = 0, attn_chunks_cap = 1, qv_cap = 1;
+  // device scratch (owned)
+  StepDyn* dyn = nullptr;
+  TreeState* ts = nullptr;
+  RowTables* rt = nullptr;  // [2]
+  float2* rope = nullptr;
+  double* inv_freq = nullptr;
+  float *hbuf = nullptr, *hhat = nullptr, *qkv = nullptr, *obuf = nullptr, *act = nullptr;
+  float* attn_ws = nullptr;
+  int32_t* attn_cnt = nullptr;
+  float* cand_val = nullptr;
+  int32_t* cand_id = nullptr;
+  float* stat = nullptr;
+  Pool pool{};
+  uint32_t* treemask = nullptr;
+  int32_t* out_pool_idx = nullptr;
+  TreeState* ts_host = nullptr;  // pinned
+  // taps (borrowed)
+  float* tap_logits = nullptr;
+  float* tap_hhat = nullptr;
+  // last step
+  bool have_step = false;
+  int last_n_new = 0, last_depth = 0, last_gamma = 0;
+  int last_launches = 0;
+  int launches = 0;
+  char err[512] = "no error";
+};
+
+namespace {
+
+int fail(dovetail_draft* h, int code, const char* fmt, ...) {
+  char* dst = h ? h->err : g_init_error;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return code;
+}
+
+// ---- launch helper: every kernel is launched with the programmatic-stream-
+// serialization attribute so that its prologue / weight prefetch overlaps the
+// tail of its predecessor; the kernels call griddepcontrol.wait themselves.
+template <typename... KArgs, typename... Args>
+cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                   cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  ++h->launches;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
+using GemvKernel = void (*)(const GemvParams);
+
+template <typename WT>
+GemvKernel pick_gemv(int MT, int NI) {
+  if (NI == 3) {
+    if (MT == 1) return k_gemv<WT, 1, 3>;
+    if (MT == 2) return k_gemv<WT, 2, 3>;
+    return k_gemv<WT, 4, 3>;
+  }
+  if (MT == 1) return k_gemv<WT, 1, 7>;
+  return k_gemv<WT, 2, 7>;
+}
+
+using AttnKernel = void (*)(const AttnParams);
+
+template <typename WT, int DH>
+AttnKernel pick_attn_qt(int QT) {
+  if (QT == 1) return k_tree_attention<WT, DH, 1>;
+  if (QT == 2) return k_tree_attention<WT, DH, 2>;
+  return k_tree_attention<WT, DH, 4>;
+}
+
+AttnKernel pick_attn(int dtype, int dh, int QT) {
+  if (dtype == DOVETAIL_BF16)
+    return dh == 128 ? pick_attn_qt<__nv_bfloat16, 128>(QT) : pick_attn_qt<__nv_bfloat16, 64>(QT);
+  return dh == 128 ? pick_attn_qt<float, 128>(QT) : pick_attn_qt<float, 64>(QT);
+}
+
+cudaError_t set_max_smem_all() {
+  cudaError_t e = cudaSuccess;
+  auto set = [&](const void* f) {
+    cudaError_t r = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+    if (r != cudaSuccess) e = r;
+  };
+  const int mts[3] = {1, 2, 4};
+  for (int mt : mts) {
+    set(reinterpret_cast<const void*>(pick_gemv<__nv_bfloat16>(mt, 3)));
+    set(reinterpret_cast<const void*>(pick_gemv<float>(mt, 3)));
+    if (mt <= 2) {
+      set(reinterpret_cast<const void*>(pick_gemv<__nv_bfloat16>(mt, 7)));
+      set(reinterpret_cast<const void*>(pick_gemv<float>(mt, 7)));
+    }
+    for (int dt = 0; dt < 2; ++dt)
+      for (int dh = 64; dh <= 128; dh += 64) set(reinterpret_cast<const void*>(pick_attn(dt, dh, mt)));
+  }
+  return e;
+}
+
+// How the GEMV of a [N, K] matrix is staged: rows per stage, ring depth, tile of draft rows.
+struct GemvShape {
+  int row_bytes, rows_per_stage, stage_bytes, n_stages, MT, NI, smem;
+  bool ok;
+};
+
+GemvShape gemv_shape(int K, int es, int M, int res_rows) {
+  GemvShape s{};
+  s.row_bytes = K * es;
+  const int units = s.row_bytes / 16;
+  const int ni = (units + kConsumerThreads - 1) / kConsumerThreads;
+  s.ok = (s.row_bytes % 16 == 0) && ni <= 7;
+  s.NI = ni <= 3 ? 3 : 7;
+  s.MT = M == 1 ? 1 : (M == 2 ? 2 : (s.NI == 7 ? 2 : 4));
+  s.rows_per_stage = 32768 / s.row_bytes;
+  if (s.rows_per_stage < 1) s.rows_per_stage = 1;
+  if (s.rows_per_stage > kRowsPerStageMax) s.rows_per_stage = kRowsPerStageMax;
+  s.stage_bytes = s.rows_per_stage * s.row_bytes;
+  const int fixed = 128 /*barriers*/ + 2 * kConsumerWarps * 16 * 4 /*part*/ + 16 + kConsumerWarps * 16 +
+                    res_rows * s.MT * 4 + 128;
+  s.n_stages = (kSmemBudget - fixed) / s.stage_bytes;
+  if (s.n_stages > 8) s.n_stages = 8;
+  if (s.n_stages < 2) s.ok = false;
+  s.smem = s.n_stages * s.stage_bytes + fixed;
+  return s;
+}
+
+int div_up(int a, int b) { return (a + b - 1) / b; }
+
+// Enqueue one GEMV: group list, K, M rows, epilogue.
+int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, int ctas_per_group) {
+  int res_rows = 0;
+  for (int g = 0; g < n_groups; ++g) {
+    const GemvGroup& G = p.g[g];
+    int r;
+    if (G.paired) r = G.n_mat * (div_up(G.rows[0], ctas_per_group) + 1);
+    else {
+      long tot = 0;
+      for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
+      r = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group) + 1;
+    }
+    if (r > res_rows) res_rows = r;
+  }
+  const GemvShape s = gemv_shape(p.K, h->es, p.M, res_rows);
+  if (!s.ok) return fail(h, DOVETAIL_EINVAL, "GEMV with K = %d is not supported (K * elem size must be a multiple of 16 and <= 28672 bytes)", p.K);
+  p.rows_per_stage = s.rows_per_stage;
+  p.n_stages = s.n_stages;
+  p.stage_bytes = s.stage_bytes;
+  p.row_bytes = s.row_bytes;
+  p.dyn = h->dyn;
+  GemvKernel k = h->es == 2 ? pick_gemv<__nv_bfloat16>(s.MT, s.NI) : pick_gemv<float>(s.MT, s.NI);
+  cudaError_t e = launch(h, k, dim3(ctas_per_group, n_groups), dim3(kThreads), s.smem, st, p);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV launch failed: %s", cudaGetErrorString(e));
+  return DOVETAIL_OK;
+}
+
+GemvGroup rows_group(const float* xsrc, int64_t xld, const int32_t* xidx, int from_dyn, const void* gain) {
+  GemvGroup g{};
+  g.xkind = X_ROWS;
+  g.xsrc = xsrc;
+  g.xld = xld;
+  g.xidx = xidx;
+  g.x_from_dyn = from_dyn;
+  g.gain = gain;
+  return g;
+}
+
+int validate_tree(dovetail_draft* h, const dovetail_tree_spec_t* t, int n_new, std::vector<LevelPlan>& plan,
+                  int& tree_rows, int& pool_total) {
+  const dovetail_config_t& c = h->cfg;
+  if (t->depth < 1 || t->depth > DOVETAIL_MAX_DEPTH) return fail(h, DOVETAIL_EINVAL, "tree depth %d out of range", t->depth);
+  if (t->gamma < 1) return fail(h, DOVETAIL_EINVAL, "gamma must be >= 1");
+  plan.resize(t->depth);
+  int m = 1, pool = 0;
+  tree_rows = 0;
+  for (int l = 0; l < t->depth; ++l) {
+    if (t->branch[l] < 1 || t->branch[l] > c.max_branch || t->branch[l] > c.vocab)
+      return fail(h, DOVETAIL_EINVAL, "branch[%d] = %d out of range [1, min(max_branch, vocab)]", l, t->branch[l]);
+    if (l >= 1) {
+      if (t->beam[l] < 0) return fail(h, DOVETAIL_EINVAL, "beam[%d] negative", l);
+      const long n = static_cast<long>(m) * t->branch[l - 1];
+      m = static_cast<int>((t->beam[l] > 0 && t->beam[l] < n) ? t->beam[l] : n);
+      if (m > c.max_rows) return fail(h, DOVETAIL_EINVAL, "level %d forwards %d rows > max_rows %d", l, m, c.max_rows);
+      plan[l].rows = m;
+      plan[l].rows_lm = m;
+      plan[l].t0 = tree_rows;
+      plan[l].row0 = n_new + tree_rows;
+      tree_rows += m;
+    } else {
+      plan[0].rows = n_new;
+      plan[0].rows_lm = 1;
+      plan[0].t0 = 0;
+      plan[0].row0 = 0;
+    }
+    plan[l].pool_begin = pool;
+    pool += plan[l].rows_lm * t->branch[l];
+  }
+  if (tree_rows > c.max_tree_slots) return fail(h, DOVETAIL_EINVAL, "tree forwards %d rows > max_tree_slots %d", tree_rows, c.max_tree_slots);
+  if (pool > h->pool_cap) return fail(h, DOVETAIL_EINVAL, "candidate pool %d exceeds capacity %d", pool, h->pool_cap);
+  pool_total = pool;
+  return DOVETAIL_OK;
+}
+
+template <typename T>
+cudaError_t dmalloc(T** p, size_t n) {
+  return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
+}
+
+void free_all(dovetail_draft* h) {
+  cudaFree(h->dyn); cudaFree(h->ts); cudaFree(h->rt); cudaFree(h->rope); cudaFree(h->inv_freq);
+  cudaFree(h->hbuf); cudaFree(h->hhat); cudaFree(h->qkv); cudaFree(h->obuf); cudaFree(h->act);
+  cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
+  cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
+  cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
+  if (h->ts_host) cudaFreeHost(h->ts_host);
+}
+
+}  // namespace
+
+extern "C" {
+
+int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cfg, dovetail_draft_t** out) {
+  if (out) *out = nullptr;
+  if (!w || !cfg || !out) return fail(nullptr, DOVETAIL_EINVAL, "null argument");
+  const dovetail_config_t& c = *cfg;
+  if (c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.n_q_heads % c.n_kv_heads != 0 ||
+      (c.head_dim != 64 && c.head_dim != 128) || c.n_layers < 1 || c.n_layers > DOVETAIL_MAX_LAYERS ||
+      c.ffn < 8 || c.vocab < 1 || !(c.rope_theta > 0.f) || !(c.rms_eps >= 0.f) ||
+      (c.dtype != DOVETAIL_F32 && c.dtype != DOVETAIL_BF16))
+    return fail(nullptr, DOVETAIL_EINVAL, "bad model shape");
+  if (c.max_rows < 1 || c.max_rows > kMaxRows || c.max_tree_slots < 0 || c.max_tree_slots > kMaxTreeSlots ||
+      c.max_branch < 1 || c.max_branch > kMaxBranch)
+    return fail(nullptr, DOVETAIL_EINVAL, "max_rows / max_tree_slots / max_branch out of range (<= 64 / 128 / 32)");
+  const int es = c.dtype == DOVETAIL_BF16 ? 2 : 4;
+  const int dq = c.n_q_heads * c.head_dim, dkv = c.n_kv_heads * c.head_dim;
+  const int Ks[4] = {c.hidden, 2 * c.hidden, dq, c.ffn};
+  for (int K : Ks)
+    if (!gemv_shape(K, es, 1, 1).ok)
+      return fail(nullptr, DOVETAIL_EINVAL, "dimension %d not supported: rows must be a multiple of 16 bytes and at most 28672 bytes", K);
+  if (!w->embed || !w->dgf_wg || !w->dgf_bg || !w->layers || !w->lm_head ||
+      (c.dgf_proj && (!w->dgf_w1 || !w->dgf_w2)) || (c.final_norm && !w->g_final))
+    return fail(nullptr, DOVETAIL_EINVAL, "missing weight pointer");
+  for (int l = 0; l < c.n_layers; ++l) {
+    const dovetail_layer_weights_t& L = w->layers[l];
+    if (!L.g_attn || !L.wq || !L.wk || !L.wv || !L.wo || !L.g_ffn || !L.wgate || !L.wup || !L.wdown)
+      return fail(nullptr, DOVETAIL_EINVAL, "missing weight pointer in layer %d", l);
+  }
+  int dev = 0;
+  cudaDeviceProp prop{};
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, dev);
+  if (e != cudaSuccess) return fail(nullptr, DOVETAIL_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+  if (prop.major != 10)
+    return fail(nullptr, DOVETAIL_ECUDA, "device %s is sm_%d%d; this library is built for sm_100a only", prop.name, prop.major, prop.minor);
+
+  dovetail_draft* h = new (std::nothrow) dovetail_draft();
+  if (!h) return fail(nullptr, DOVETAIL_ENOMEM, "out of host memory");
+  h->cfg = c;
+  h->w = *w;
+  h->layers.assign(w->layers, w->layers + c.n_layers);
+  h->w.layers = h->layers.data();
+  h->num_sms = prop.multiProcessorCount;
+  h->es = es;
+  h->dq = dq;
+  h->dkv = dkv;
+  h->ldq = dq + 2 * dkv;
+  h->max_step_rows = c.max_rows + c.max_tree_slots;
+  h->pool_cap = c.max_branch + c.max_tree_slots * c.max_branch;
+  const int grp = c.n_q_heads / c.n_kv_heads;
+  h->attn_chunks_cap = std::max(1, 2 * h->num_sms / c.n_kv_heads);
+  h->qv_cap = c.max_rows * grp;
+
+  e = set_max_smem_all();
+  const size_t R = c.max_rows, d = c.hidden;
+  auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+  A(dmalloc(&h->dyn, 1));
+  A(dmalloc(&h->ts, 1));
+  A(dmalloc(&h->rt, 2));
+  A(dmalloc(&h->rope, static_cast<size_t>(kMaxRows + kMaxDepth) * (c.head_dim / 2)));
+  A(dmalloc(&h->inv_freq, c.head_dim / 2));
+  A(dmalloc(&h->hbuf, R * 2 * d));
+  A(dmalloc(&h->hhat, static_cast<size_t>(h->max_step_rows) * d));
+  A(dmalloc(&h->qkv, R * h->ldq));
+  A(dmalloc(&h->obuf, R * dq));
+  A(dmalloc(&h->act, R * c.ffn));
+  A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
+  A(dmalloc(&h->attn_cnt, c.n_kv_heads));
+  A(dmalloc(&h->cand_val, R * h->num_sms * kMaxBranch));
+  A(dmalloc(&h->cand_id, R * h->num_sms * kMaxBranch));
+  A(dmalloc(&h->stat, R * h->num_sms * 2));
+  A(dmalloc(&h->pool.token, h->pool_cap));
+  A(dmalloc(&h->pool.parent, h->pool_cap));
+  A(dmalloc(&h->pool.depth, h->pool_cap));
+  A(dmalloc(&h->pool.cum, h->pool_cap));
+  A(dmalloc(&h->pool.row, h->pool_cap));
+  A(dmalloc(&h->treemask, static_cast<size_t>(kMaxTreeSlots) * kMaskWords));
+  A(dmalloc(&h->out_pool_idx, h->pool_cap));
+  A(cudaMallocHost(reinterpret_cast<void**>(&h->ts_host), sizeof(TreeState)));
+  if (e == cudaSuccess) e = cudaMemset(h->attn_cnt, 0, sizeof(int32_t) * c.n_kv_heads);
+  if (e == cudaSuccess) e = cudaMemset(h->ts, 0, sizeof(TreeState));
+  if (e == cudaSuccess) {
+    // theta^(-2i/dh) in fp64, the expression the rotary definition states (reading A3)
+    std::vector<double> inv(c.head_dim / 2);
+    for (int i = 0; i < c.head_dim / 2; ++i)
+      inv[i] = std::pow(static_cast<double>(c.rope_theta), -2.0 * i / c.head_dim);
+    e = cudaMemcpy(h->inv_freq, inv.data(), inv.size() * sizeof(double), cudaMemcpyHostToDevice);
+  }
+  if (e != cudaSuccess) {
+    const int code = e == cudaErrorMemoryAllocation ? DOVETAIL_ENOMEM : DOVETAIL_ECUDA;
+    fail(nullptr, code, "init failed: %s", cudaGetErrorString(e));
+    cudaGetLastError();
+    free_all(h);
+    delete h;
+    return code;
+  }
+  *out = h;
+  return DOVETAIL_OK;
+}
+
+int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens, int32_t n_new,
+                        dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree,
+                        const dovetail_draft_out_t* out, void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (!hidden_feats || !tokens || !kv || !tree || !out || !kv->k || !kv->v || !out->token_ids ||
+      !out->scores || !out->parents || !out->n_out)
+    return fail(h, DOVETAIL_EINVAL, "null argument");
+  const dovetail_config_t& c = h->cfg;
+  if (n_new < 1 || n_new > c.max_rows) return fail(h, DOVETAIL_EINVAL, "n_new = %d out of range [1, %d]", n_new, c.max_rows);
+  if (kv->committed_len < 0 || kv->capacity < 1) return fail(h, DOVETAIL_EINVAL, "bad KV cache state");
+  std::vector<LevelPlan> plan;
+  int tree_rows = 0, pool_total = 0;
+  int rc = validate_tree(h, tree, n_new, plan, tree_rows, pool_total);
+  if (rc != DOVETAIL_OK) return rc;
+  const int L = kv->committed_len, Lp = L + n_new;
+  if (static_cast<long>(Lp) + tree_rows > kv->capacity)
+    return fail(h, DOVETAIL_ECAPACITY, "KV cache too small: %d committed + %d new + %d tree rows > capacity %d", L, n_new, tree_rows, kv->capacity);
+
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  h->launches = 0;
+  const int d = c.hidden, F = c.ffn, V = c.vocab, dh = c.head_dim, half = dh / 2;
+  const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
+  const int grp = c.n_q_heads / c.n_kv_heads;
+  const bool bf16 = c.dtype == DOVETAIL_BF16;
+  cudaError_t e;
+
+  // S0: per-step state, level-0 row tables, rotary table
+  StepDyn dv{};
+  dv.feats = hidden_feats;
+  dv.tokens = tokens;
+  dv.kc = kv->k;
+  dv.vc = kv->v;
+  dv.capacity = kv->capacity;
+  dv.L = L;
+  dv.n_new = n_new;
+  dv.Lp = Lp;
+  dv.out_ids = out->token_ids;
+  dv.out_scores = out->scores;
+  dv.out_parents = out->parents;
+  dv.out_depths = out->depths;
+  dv.out_n = out->n_out;
+  e = launch(h, k_step_begin, dim3(n_new + tree->depth - 1), dim3(64), 0, st, dv, h->dyn, h->ts, h->rt, h->rope,
+             static_cast<const double*>(h->inv_freq), half, V);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+
+  for (int l = 0; l < tree->depth; ++l) {
+    const LevelPlan& lp = plan[l];
+    const int M = lp.rows;
+    RowTables* cur = h->rt + (l & 1);
+    RowTables* nxt = h->rt + ((l + 1) & 1);
+    float* x = h->hhat + static_cast<size_t>(lp.row0) * d;  // residual stream rows of this level
+
+    // S0 + S1: gather, DGF projections h1 = W1 f, h2 = W2 e
+    if (c.dgf_proj) {
+      GemvParams p{};
+      p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
+      p.g[0].w[0] = h->w.dgf_w1;
+      p.g[0].rows[0] = d;
+      p.g[0].n_mat = 1;
+      p.g[0].out_off = 0;
+      p.g[1] = GemvGroup{};
+      p.g[1].xkind = X_EMBED;
+      p.g[1].embed = h->w.embed;
+      p.g[1].tokens = cur->token;
+      p.g[1].w[0] = h->w.dgf_w2;
+      p.g[1].rows[0] = d;
+      p.g[1].n_mat = 1;
+      p.g[1].out_off = d;
+      p.K = d;
+      p.M = M;
+      p.epi = EPI_STORE;
+      p.out = h->hbuf;
+      p.out_ld = 2 * d;
+      rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)));
+      if (rc) return rc;
+    } else {
+      const int blocks = std::min(nsm, div_up(M * 2 * d, 256));
+      if (bf16)
+        e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
+                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
+                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d);
+      else
+        e = launch(h, k_fill_h<float>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
+                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
+                   static_cast<const float*>(h->w.embed), h->hbuf, M, d);
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+    }
+    {  // S1: gate, sigmoid, blend
+      GemvParams p{};
+      p.g[0] = rows_group(h->hbuf, 2 * d, nullptr, 0, nullptr);
+      p.g[0].w[0] = h->w.dgf_wg;
+      p.g[0].rows[0] = d;
+      p.g[0].n_mat = 1;
+      p.K = 2 * d;
+      p.M = M;
+      p.epi = EPI_DGF;
+      p.out = x;
+      p.out_ld = d;
+      p.hbuf = h->hbuf;
+      p.bias = h->w.dgf_bg;
+      p.d = d;
+      rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+      if (rc) return rc;
+    }
+
+    for (int ly = 0; ly < c.n_layers; ++ly) {
+      const dovetail_layer_weights_t& W = h->layers[ly];
+      {  // S2: RMSNorm + Q, K, V projections
+        GemvParams p{};
+        const void* gain = (ly == 0 && !c.first_layer_input_norm) ? nullptr : W.g_attn;
+        p.g[0] = rows_group(x, d, nullptr, 0, gain);
+        p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq;
+        p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv;
+        p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv;
+        p.g[0].n_mat = 3;
+        p.K = d;
+        p.M = M;
+        p.eps = c.rms_eps;
+        p.epi = EPI_STORE;
+        p.out = h->qkv;
+        p.out_ld = ldq;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq));
+        if (rc) return rc;
+      }
+      {  // S2 (RoPE, KV append) + S3 tree attention
+        AttnParams a{};
+        a.dyn = h->dyn;
+        a.qkv = h->qkv;
+        a.obuf = h->obuf;
+        a.rows = cur;
+        a.rope = h->rope;
+        a.rope_row0 = l == 0 ? 0 : n_new + l - 1;
+        a.rope_per_row = l == 0 ? 1 : 0;
+        a.M = M;
+        a.Hq = c.n_q_heads;
+        a.Hkv = c.n_kv_heads;
+        a.layer = ly;
+        a.level0 = l == 0 ? 1 : 0;
+        a.new_cnt = l == 0 ? n_new : lp.t0 + M;
+        a.n_stages = kAttnStages;
+        a.ws = h->attn_ws;
+        a.qv_cap = h->qv_cap;
+        a.counters = h->attn_cnt;
+        const int Lbase = l == 0 ? L : Lp;
+        int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
+        const int qv_tot = M * grp;
+        const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
+        const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
+        const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
+                            static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
+        e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
+        if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "attention launch failed: %s", cudaGetErrorString(e));
+      }
+      {  // S4: x += Wo o
+        GemvParams p{};
+        p.g[0] = rows_group(h->obuf, dq, nullptr, 0, nullptr);
+        p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        p.K = dq;
+        p.M = M;
+        p.epi = EPI_RESID;
+        p.out = x;
+        p.out_ld = d;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+        if (rc) return rc;
+      }
+      {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
+        GemvParams p{};
+        p.g[0] = rows_group(x, d, nullptr, 0, W.g_ffn);
+        p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F;
+        p.g[0].w[1] = W.wup; p.g[0].rows[1] = F;
+        p.g[0].n_mat = 2;
+        p.g[0].paired = 1;
+        p.K = d;
+        p.M = M;
+        p.eps = c.rms_eps;
+        p.epi = EPI_SWIGLU;
+        p.out = h->act;
+        p.out_ld = F;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, F));
+        if (rc) return rc;
+      }
+      {  // S5b: x += Wdown act
+        GemvParams p{};
+        p.g[0] = rows_group(h->act, F, nullptr, 0, nullptr);
+        p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        p.K = F;
+        p.M = M;
+        p.epi = EPI_RESID;
+        p.out = x;
+        p.out_ld = d;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+        if (rc) return rc;
+      }
+    }
+
+    const int lm_ctas = std::min(nsm, V);
+    {  // S6: LM head + per-CTA top-b + softmax statistics. Level 0: the last row seeds the tree.
+      GemvParams p{};
+      const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
+      p.g[0] = rows_group(xs, d, nullptr, 0, c.final_norm ? h->w.g_final : nullptr);
+      p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1;
+      p.K = d;
+      p.M = lp.rows_lm;
+      p.eps = c.rms_eps;
+      p.epi = EPI_LMHEAD;
+      p.b = tree->branch[l];
+      p.vocab = V;
+      p.cand_val = h->cand_val;
+      p.cand_id = h->cand_id;
+      p.stat = h->stat;
+      p.tap = h->tap_logits ? h->tap_logits + static_cast<size_t>(lp.row0 + (l == 0 ? n_new - 1 : 0)) * V : nullptr;
+      rc = run_gemv(h, st, p, 1, lm_ctas);
+      if (rc) return rc;
+    }
+    {  // S7 (+ S8 after the last level)
+      TreeLevelParams t{};
+      t.dyn = h->dyn;
+      t.ts = h->ts;
+      t.pool = h->pool;
+      t.treemask = h->treemask;
+      t.cand_val = h->cand_val;
+      t.cand_id = h->cand_id;
+      t.stat = h->stat;
+      t.nct = lm_ctas;
+      t.M = lp.rows_lm;
+      t.b = tree->branch[l];
+      t.level = l;
+      t.pool_begin = lp.pool_begin;
+      const bool last = l + 1 == tree->depth;
+      t.M_next = last ? 0 : plan[l + 1].rows;
+      t.next_row0 = last ? 0 : plan[l + 1].row0;
+      t.next_t0 = last ? 0 : plan[l + 1].t0;
+      t.n_new = n_new;
+      t.cur = cur;
+      t.next = nxt;
+      t.gamma = tree->gamma;
+      t.pool_total = pool_total;
+      t.out_pool_idx = h->out_pool_idx;
+      e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
+    }
+  }
+  if (h->tap_hhat) {
+    e = cudaMemcpyAsync(h->tap_hhat, h->hhat, static_cast<size_t>(n_new + tree_rows) * d * sizeof(float),
+                        cudaMemcpyDeviceToDevice, st);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap copy failed: %s", cudaGetErrorString(e));
+  }
+  e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
+  kv->committed_len = Lp;  // the level-0 rows are real, verified tokens
+  h->have_step = true;
+  h->last_n_new = n_new;
+  h->last_depth = tree->depth;
+  h->last_gamma = tree->gamma;
+  h->last_launches = h->launches;
+  return DOVETAIL_OK;
+}
+
+int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32_t* accepted_path, int32_t n_acc,
+                       int32_t mode, int32_t* n_committed, void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (n_committed) *n_committed = 0;
+  if (!kv || !kv->k || !kv->v || (n_acc > 0 && !accepted_path)) return fail(h, DOVETAIL_EINVAL, "null argument");
+  if (mode != 0 && mode != 1) return fail(h, DOVETAIL_EINVAL, "mode must be 0 or 1");
+  if (!h->have_step) return fail(h, DOVETAIL_EINVAL, "no draft step to commit");
+  if (n_acc < 0 || n_acc > h->last_depth) return fail(h, DOVETAIL_EINVAL, "n_acc = %d out of range [0, depth %d]", n_acc, h->last_depth);
+  for (int i = 0; i < n_acc; ++i)
+    if (accepted_path[i] < 0 || accepted_path[i] >= h->last_gamma)
+      return fail(h, DOVETAIL_EINVAL, "accepted_path[%d] = %d is not an output index", i, accepted_path[i]);
+  if (mode == 0) {  // the paper's flow: tree rows are simply dead
+    h->have_step = false;
+    return DOVETAIL_OK;
+  }
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const dovetail_config_t& c = h->cfg;
+  CommitPath path{};
+  path.n = n_acc;
+  for (int i = 0; i < n_acc; ++i) path.idx[i] = accepted_path[i];
+  const int row_bytes = c.head_dim * h->es;
+  k_commit_plan<<<1, 32, 0, st>>>(path, h->ts, h->pool, h->out_pool_idx, h->last_n_new);
+  k_commit_move<<<dim3(c.n_layers * c.n_kv_heads, 2), 128, static_cast<size_t>(kMaxDepth + 1) * row_bytes, st>>>(
+      h->ts, kv->k, kv->v, kv->capacity, kv->committed_len, row_bytes);
+  cudaError_t e = cudaMemcpyAsync(h->ts_host, h->ts, sizeof(TreeState), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "kv_commit failed: %s", cudaGetErrorString(e));
+  if (h->ts_host->commit_err) return fail(h, DOVETAIL_EINVAL, "accepted_path is not a root-to-node chain of the last step's output");
+  kv->committed_len += h->ts_host->commit_n;
+  if (n_committed) *n_committed = h->ts_host->commit_n;
+  h->have_step = false;
+  return DOVETAIL_OK;
+}
+
+int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, const int32_t* cand_tokens,
+                         const float* cand_logp, int32_t n_rows, int32_t max_b, const dovetail_draft_out_t* out,
+                         int32_t* pool_token, int32_t* pool_parent, int32_t* pool_depth, float* pool_cum,
+                         int32_t* pool_size, void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (!tree || !cand_tokens || !cand_logp || !out || !out->token_ids || !out->scores || !out->parents || !out->n_out)
+    return fail(h, DOVETAIL_EINVAL, "null argument");
+  std::vector<LevelPlan> plan;
+  int tree_rows = 0, pool_total = 0;
+  int rc = validate_tree(h, tree, 1, plan, tree_rows, pool_total);
+  if (rc != DOVETAIL_OK) return rc;
+  int need_rows = 1 + tree_rows - (tree->depth > 1 ? 0 : 0);
+  // rows consumed: the root and every forwarded row of levels 1 .. D-1
+  need_rows = 1;
+  for (int l = 1; l < tree->depth; ++l) need_rows += plan[l].rows;
+  int maxb = 0;
+  for (int l = 0; l < tree->depth; ++l) maxb = std::max(maxb, tree->branch[l]);
+  if (n_rows < need_rows || max_b < maxb) return fail(h, DOVETAIL_EINVAL, "replay needs %d rows of %d candidates", need_rows, maxb);
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  h->launches = 0;
+  cudaError_t e = cudaMemsetAsync(h->rt, 0xff, sizeof(RowTables), st);  // level-0 row: pool = -1
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "memset failed: %s", cudaGetErrorString(e));
+  int row = 0;
+  for (int l = 0; l < tree->depth; ++l) {
+    const LevelPlan& lp = plan[l];
+    TreeLevelParams t{};
+    t.dyn = h->dyn;
+    t.ts = h->ts;
+    t.pool = h->pool;
+    t.treemask = h->treemask;
+    t.rp_tokens = cand_tokens;
+    t.rp_logp = cand_logp;
+    t.rp_maxb = max_b;
+    t.rp_row0 = row;
+    t.M = lp.rows_lm;
+    t.b = tree->branch[l];
+    t.level = l;
+    t.pool_begin = lp.pool_begin;
+    const bool last = l + 1 == tree->depth;
+    t.M_next = last ? 0 : plan[l + 1].rows;
+    t.next_row0 = last ? 0 : plan[l + 1].row0;
+    t.next_t0 = last ? 0 : plan[l + 1].t0;
+    t.n_new = 1;
+    t.cur = h->rt + (l & 1);
+    t.next = h->rt + ((l + 1) & 1);
+    t.gamma = tree->gamma;
+    t.pool_total = pool_total;
+    t.out_pool_idx = h->out_pool_idx;
+    t.o_ids = out->token_ids;
+    t.o_scores = out->scores;
+    t.o_parents = out->parents;
+    t.o_depths = out->depths;
+    t.o_n = out->n_out;
+    e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
+    row += lp.rows_lm;
+  }
+  auto cp = [&](void* dst, const void* src, size_t n) {
+    if (dst && e == cudaSuccess) e = cudaMemcpyAsync(dst, src, n, cudaMemcpyDeviceToDevice, st);
+  };
+  cp(pool_token, h->pool.token, sizeof(int32_t) * pool_total);
+  cp(pool_parent, h->pool.parent, sizeof(int32_t) * pool_total);
+  cp(pool_depth, h->pool.depth, sizeof(int32_t) * pool_total);
+  cp(pool_cum, h->pool.cum, sizeof(float) * pool_total);
+  cp(pool_size, &h->ts->pool_size, sizeof(int32_t));
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "copy failed: %s", cudaGetErrorString(e));
+  h->have_step = false;
+  h->last_launches = h->launches;
+  return DOVETAIL_OK;
+}
+
+int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat) {
+  if (!h) return DOVETAIL_EINVAL;
+  h->tap_logits = logits;
+  h->tap_hhat = hhat;
+  return DOVETAIL_OK;
+}
+
+int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
+
+int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
+  if (!h) return 0;
+  const dovetail_config_t& c = h->cfg;
+  const int64_t d = c.hidden, F = c.ffn, dq = h->dq, dkv = h->dkv;
+  int64_t params = (c.dgf_proj ? 2 * d * d : 0) + 2 * d * d + d;
+  params += static_cast<int64_t>(c.n_layers) * (d * dq + 2 * d * dkv + dq * d + 3 * d * F + 2 * d);
+  params += static_cast<int64_t>(c.vocab) * d + (c.final_norm ? d : 0);
+  const int64_t kvb = static_cast<int64_t>(c.n_layers) * 2 * prefix_len * dkv;
+  return (params + kvb) * h->es;
+}
+
+void dovetail_draft_destroy(dovetail_draft_t* h) {
+  if (!h) return;
+  free_all(h);
+  delete h;
+}
+
+const char* dovetail_last_error(const dovetail_draft_t* h) { return h ? h->err : g_init_error; }
+
+}  // extern "C"

@@ -1,0 +1,411 @@
+// gemv.cuh -- the weight-streaming GEMV that carries > 95 % of the step's HBM
+// bytes (S1 DGF, S2 QKV, S4 O-proj, S5 FFN, S6 LM head).
+//
+//   Y[m, n] = sum_k X[m, k] * W[n, k]      m < M (draft rows, tiny), W row-major [N, K]
+//
+// Shape of the kernel (one CTA per SM, 8 consumer warps + 1 producer warp):
+//   * the matrix rows are dealt to the CTAs in contiguous ranges whose sizes
+//     differ by at most one row, so every SM streams the same number of bytes;
+//   * the producer warp copies whole rows (1-D bulk async copies, one per row)
+//     into a ring of shared-memory stages guarded by full/empty mbarriers; it
+//     starts before griddepcontrol.wait because weights never depend on the
+//     previous kernel (programmatic dependent launch hides ramp-up);
+//   * consumer thread t keeps the activations of the 16-byte units t, t+256, ...
+//     of K in registers (fp32) for MT rows and accumulates with packed fp32
+//     FMAs; a transposing shuffle reduction and a fixed-order cross-warp sum
+//     give one deterministic value per (row, m);
+//   * results of the CTA's rows are kept in shared memory and the fused
+//     epilogue (store / DGF gate+blend / residual add / SiLU*up / LM-head
+//     top-b + softmax statistics) runs over them once per pass.
+#pragma once
+#include <cuda_bf16.h>
+
+#include "ptx.cuh"
+#include "state.cuh"
+
+namespace dvt {
+
+enum XKind : int32_t { X_ROWS = 0, X_EMBED = 1 };
+enum Epi : int32_t { EPI_STORE = 0, EPI_DGF = 1, EPI_RESID = 2, EPI_SWIGLU = 3, EPI_LMHEAD = 4 };
+
+constexpr int kRowsPerStageMax = 4;
+
+struct GemvGroup {
+  const void* w[3];      // up to three matrices sharing K and X
+  int32_t rows[3];
+  int32_t n_mat;
+  int32_t paired;        // 1: the CTA's row range applies to each matrix (gate/up)
+  int32_t xkind;
+  int32_t x_from_dyn;    // X_ROWS: source rows are the caller's hidden_feats
+  const float* xsrc;     // X_ROWS: fp32 rows
+  int64_t xld;           //         row stride in floats
+  const int32_t* xidx;   //         source row of each m (NULL: m)
+  const void* embed;     // X_EMBED: [vocab, K] in the storage dtype
+  const int32_t* tokens; //          token of each m
+  const void* gain;      // RMSNorm gain [K] (storage dtype) or NULL: no norm
+  int32_t out_off;       // EPI_STORE: offset added to the output column
+};
+
+struct GemvParams {
+  GemvGroup g[2];        // blockIdx.y selects the group (DGF projections use two)
+  const StepDyn* dyn;
+  int32_t K, M;
+  int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
+  int32_t epi;
+  float eps;
+  float* out;            // STORE/SWIGLU: [M, out_ld]; DGF/RESID: residual stream rows x [M, out_ld]
+  int64_t out_ld;
+  const float* hbuf;     // DGF: [M, 2d] = [h1 || h2]
+  const void* bias;      // DGF: gate bias [d]
+  int32_t d;
+  int32_t b;             // LMHEAD: candidates kept per row
+  int32_t vocab;
+  float* cand_val;       // LMHEAD: [kMaxRows][grid][kMaxBranch]
+  int32_t* cand_id;
+  float* stat;           // LMHEAD: [kMaxRows][grid][2] = (max, sum exp)
+  float* tap;            // LMHEAD: optional logits tap rows [M, vocab]
+};
+
+template <typename WT>
+struct Unit;  // one 16-byte unit of a weight row as fp32 pairs
+template <>
+struct Unit<__nv_bfloat16> {
+  static constexpr int EPU = 8;
+  __device__ static __forceinline__ void unpack(const uint4& w, float2 (&f)[4]) {
+    f[0] = bf16x2_to_f32x2(w.x);
+    f[1] = bf16x2_to_f32x2(w.y);
+    f[2] = bf16x2_to_f32x2(w.z);
+    f[3] = bf16x2_to_f32x2(w.w);
+  }
+};
+template <>
+struct Unit<float> {
+  static constexpr int EPU = 4;
+  __device__ static __forceinline__ void unpack(const uint4& w, float2 (&f)[2]) {
+    f[0] = make_float2(__uint_as_float(w.x), __uint_as_float(w.y));
+    f[1] = make_float2(__uint_as_float(w.z), __uint_as_float(w.w));
+  }
+};
+
+struct RowRange {  // the CTA's share of the group's rows, as a list of "virtual rows"
+  int32_t cnt;     // virtual rows of this CTA
+  int32_t n0, cr;  // paired: first row and rows per matrix
+  int64_t g0;      // linearised: first global row
+};
+
+__device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int nct) {
+  RowRange r;
+  if (G.paired) {
+    r.n0 = static_cast<int32_t>(static_cast<int64_t>(c) * G.rows[0] / nct);
+    const int32_t n1 = static_cast<int32_t>(static_cast<int64_t>(c + 1) * G.rows[0] / nct);
+    r.cr = n1 - r.n0;
+    r.cnt = r.cr * G.n_mat;
+    r.g0 = 0;
+  } else {
+    int64_t tot = 0;
+    for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
+    r.g0 = static_cast<int64_t>(c) * tot / nct;
+    const int64_t g1 = static_cast<int64_t>(c + 1) * tot / nct;
+    r.cnt = static_cast<int32_t>(g1 - r.g0);
+    r.n0 = 0;
+    r.cr = 0;
+  }
+  return r;
+}
+
+// virtual row v -> matrix j, row n within it
+__device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& rr, int v, int& j,
+                                           int& n) {
+  if (G.paired) {
+    j = v / rr.cr;
+    n = rr.n0 + (v - j * rr.cr);
+  } else {
+    int64_t g = rr.g0 + v;
+    j = 0;
+    if (g >= G.rows[0]) {
+      g -= G.rows[0];
+      j = 1;
+      if (g >= G.rows[1]) {
+        g -= G.rows[1];
+        j = 2;
+      }
+    }
+    n = static_cast<int32_t>(g);
+  }
+}
+
+__device__ __forceinline__ float sigmoidf_acc(float z) { return 1.0f / (1.0f + expf(-z)); }
+
+// strict order of LM-head candidates: logit descending, token id ascending (reading A7)
+__device__ __forceinline__ bool cand_before(float va, int ia, float vb, int ib) {
+  return va > vb || (va == vb && ia < ib);
+}
+
+template <typename WT, int MT, int NI>
+__global__ void __launch_bounds__(kThreads, 1) k_gemv(const GemvParams p) {
+  constexpr int EPU = Unit<WT>::EPU;
+  constexpr int PAIRS = EPU / 2;
+  constexpr int R = kRowsPerStageMax;
+  constexpr int V = R * MT;
+  extern __shared__ __align__(128) uint8_t smem[];
+
+  const GemvGroup& G = p.g[blockIdx.y];
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nct = gridDim.x, c = blockIdx.x;
+  const int NS = p.n_stages, RS = p.rows_per_stage;
+
+  uint8_t* ring = smem;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + static_cast<size_t>(NS) * p.stage_bytes);
+  uint64_t* empty = full + 8;
+  float* part = reinterpret_cast<float*>(empty + 8);  // [2][warps][V]
+  float* rstd_s = part + 2 * kConsumerWarps * V;      // [4]
+  float* red_s = rstd_s + 4;                          // [warps][4]
+  float* res = red_s + kConsumerWarps * 4;            // [cnt][MT]
+
+  const RowRange rr = cta_rows(G, c, nct);
+  const int spp = (rr.cnt + RS - 1) / RS;  // stages per pass over the CTA's rows
+  const int m_tiles = (p.M + MT - 1) / MT;
+  const int U = p.row_bytes >> 4;          // 16-byte units per row
+
+  if (tid == 0) {
+    for (int s = 0; s < NS; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], kConsumerWarps);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+  pdl_launch_dependents();
+
+  if (warp == kConsumerWarps) {
+    // ---------------- producer: stream this CTA's rows, once per m-tile -----
+    const uint64_t pol = l2_policy_evict_first();
+    int it = 0;
+    for (int mt = 0; mt < m_tiles; ++mt) {
+      for (int s = 0; s < spp; ++s, ++it) {
+        const int slot = it % NS;
+        if (it >= NS) mbar_wait(&empty[slot], ((it / NS) & 1) ^ 1);
+        const int nr = min(RS, rr.cnt - s * RS);
+        if (lane == 0) mbar_arrive_expect_tx(&full[slot], static_cast<uint32_t>(nr) * p.row_bytes);
+        __syncwarp();
+        if (lane < nr) {
+          int j, n;
+          locate_row(G, rr, s * RS + lane, j, n);
+          const uint8_t* src = static_cast<const uint8_t*>(G.w[j]) + static_cast<size_t>(n) * p.row_bytes;
+          bulk_g2s(ring + static_cast<size_t>(slot) * p.stage_bytes + static_cast<size_t>(lane) * p.row_bytes,
+                   src, p.row_bytes, &full[slot], pol);
+        }
+      }
+    }
+    return;
+  }
+
+  // ---------------- consumers -------------------------------------------------
+  pdl_wait();  // activations of the previous kernel are visible from here on
+  const StepDyn* dyn = p.dyn;
+  const bool normed = G.gain != nullptr;
+
+  for (int mt = 0; mt < m_tiles; ++mt) {
+    const int m0 = mt * MT;
+    // X slice of this thread: units tid, tid+256, ... of K, MT rows, fp32 pairs
+    float2 xx[MT][NI][PAIRS];
+    float ss[MT];
+#pragma unroll
+    for (int m = 0; m < MT; ++m) {
+      ss[m] = 0.f;
+      const int mm = m0 + m;
+      const bool mvalid = mm < p.M;
+      const float* xrow = nullptr;
+      const WT* erow = nullptr;
+      if (mvalid) {
+        if (G.xkind == X_ROWS) {
+          const float* base = G.x_from_dyn ? dyn->feats : G.xsrc;
+          const int64_t ri = G.xidx ? G.xidx[mm] : mm;
+          xrow = base + ri * G.xld;
+        } else {
+          erow = static_cast<const WT*>(G.embed) + static_cast<size_t>(G.tokens[mm]) * p.K;
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < NI; ++i) {
+        const int u = tid + i * kConsumerThreads;
+        float xv[EPU];
+#pragma unroll
+        for (int e = 0; e < EPU; ++e) xv[e] = 0.f;
+        if (mvalid && u < U) {
+          if (xrow) {
+#pragma unroll
+            for (int q = 0; q < EPU / 4; ++q) {
+              const float4 t4 = *reinterpret_cast<const float4*>(xrow + static_cast<size_t>(u) * EPU + q * 4);
+              xv[q * 4 + 0] = t4.x; xv[q * 4 + 1] = t4.y; xv[q * 4 + 2] = t4.z; xv[q * 4 + 3] = t4.w;
+            }
+          } else {
+            const uint4 w = *reinterpret_cast<const uint4*>(erow + static_cast<size_t>(u) * EPU);
+            float2 f[PAIRS];
+            Unit<WT>::unpack(w, f);
+#pragma unroll
+            for (int q = 0; q < PAIRS; ++q) { xv[2 * q] = f[q].x; xv[2 * q + 1] = f[q].y; }
+          }
+          if (normed) {
+#pragma unroll
+            for (int e = 0; e < EPU; ++e) ss[m] = fmaf(xv[e], xv[e], ss[m]);
+            const uint4 gw = *reinterpret_cast<const uint4*>(static_cast<const WT*>(G.gain) + static_cast<size_t>(u) * EPU);
+            float2 gf[PAIRS];
+            Unit<WT>::unpack(gw, gf);
+#pragma unroll
+            for (int q = 0; q < PAIRS; ++q) { xv[2 * q] *= gf[q].x; xv[2 * q + 1] *= gf[q].y; }
+          }
+        }
+#pragma unroll
+        for (int q = 0; q < PAIRS; ++q) xx[m][i][q] = make_float2(xv[2 * q], xv[2 * q + 1]);
+      }
+    }
+    if (normed) {  // RMSNorm: y = x / sqrt(mean(x^2) + eps) * g; 1/rms is applied to the results
+#pragma unroll
+      for (int m = 0; m < MT; ++m) {
+        const float t = warp_sum(ss[m]);
+        if (lane == 0) red_s[warp * 4 + m] = t;
+      }
+      consumer_sync();
+      if (tid < MT) {
+        float t = 0.f;
+        for (int w = 0; w < kConsumerWarps; ++w) t += red_s[w * 4 + tid];
+        rstd_s[tid] = 1.0f / sqrtf(t / static_cast<float>(p.K) + p.eps);
+      }
+      // visibility of rstd_s is ordered by the consumer_sync()s of the stage loop / epilogue
+    }
+
+    // ---- stream the rows ---------------------------------------------------
+    for (int s = 0; s < spp; ++s) {
+      const int it = mt * spp + s;
+      const int slot = it % NS;
+      const int nr = min(RS, rr.cnt - s * RS);
+      mbar_wait(&full[slot], (it / NS) & 1);
+      const uint8_t* sb = ring + static_cast<size_t>(slot) * p.stage_bytes;
+      float2 acc[R][MT];
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int m = 0; m < MT; ++m) acc[r][m] = make_float2(0.f, 0.f);
+#pragma unroll
+      for (int i = 0; i < NI; ++i) {
+        const int u = tid + i * kConsumerThreads;
+        if (u < U) {
+#pragma unroll
+          for (int r = 0; r < R; ++r) {
+            if (r < nr) {
+              const uint4 w = *reinterpret_cast<const uint4*>(sb + static_cast<size_t>(r) * p.row_bytes + (static_cast<size_t>(u) << 4));
+              float2 wf[PAIRS];
+              Unit<WT>::unpack(w, wf);
+#pragma unroll
+              for (int q = 0; q < PAIRS; ++q)
+#pragma unroll
+                for (int m = 0; m < MT; ++m) ffma2(acc[r][m], wf[q], xx[m][i][q]);
+            }
+          }
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[slot]);  // the stage's bytes are in registers now
+
+      float v[V];
+#pragma unroll
+      for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int m = 0; m < MT; ++m) v[r * MT + m] = acc[r][m].x + acc[r][m].y;
+      const float tot = warp_reduce_transpose<V>(v, lane);
+      float* pb = part + (it & 1) * (kConsumerWarps * V);
+      if ((lane & (32 / V - 1)) == 0) pb[warp * V + lane / (32 / V)] = tot;
+      consumer_sync();
+      if (tid < nr * MT) {  // fixed-order sum over the warps: deterministic
+        float t = 0.f;
+#pragma unroll
+        for (int w = 0; w < kConsumerWarps; ++w) t += pb[w * V + tid];
+        res[(s * RS) * MT + tid] = t;
+      }
+    }
+    consumer_sync();
+
+    // ---- fused epilogue over the CTA's results -------------------------------
+    const int nres = rr.cnt * MT;
+    if (normed) {
+      for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rstd_s[idx % MT];
+      consumer_sync();
+    }
+    if (p.epi == EPI_STORE) {
+      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
+        const int v2 = idx / MT, mm = m0 + idx % MT;
+        if (mm < p.M) p.out[mm * p.out_ld + G.out_off + rr.g0 + v2] = res[idx];
+      }
+    } else if (p.epi == EPI_DGF) {
+      // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
+      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
+        const int mm = m0 + idx % MT;
+        const int64_t n = rr.g0 + idx / MT;
+        if (mm < p.M) {
+          float bz;
+          if (sizeof(WT) == 2) bz = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[n]);
+          else bz = static_cast<const float*>(p.bias)[n];
+          const float g = sigmoidf_acc(res[idx] + bz);
+          const float h1 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + n];
+          const float h2 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + p.d + n];
+          p.out[mm * p.out_ld + n] = g * h1 + (1.0f - g) * h2;
+        }
+      }
+    } else if (p.epi == EPI_RESID) {
+      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
+        const int mm = m0 + idx % MT;
+        const int64_t n = rr.g0 + idx / MT;
+        if (mm < p.M) p.out[mm * p.out_ld + n] += res[idx];
+      }
+    } else if (p.epi == EPI_SWIGLU) {
+      // act = SiLU(Wgate n) * (Wup n); gate rows are virtual rows [0, cr), up rows [cr, 2cr)
+      for (int idx = tid; idx < rr.cr * MT; idx += kConsumerThreads) {
+        const int r = idx / MT, m = idx % MT, mm = m0 + m;
+        if (mm < p.M) {
+          const float gv = res[r * MT + m], uv = res[(rr.cr + r) * MT + m];
+          p.out[mm * p.out_ld + rr.n0 + r] = gv * sigmoidf_acc(gv) * uv;
+        }
+      }
+    } else {  // EPI_LMHEAD: logits of rows [g0, g0 + cnt) of the vocabulary
+      if (p.tap) {
+        for (int idx = tid; idx < nres; idx += kConsumerThreads) {
+          const int mm = m0 + idx % MT;
+          if (mm < p.M) p.tap[static_cast<int64_t>(mm) * p.vocab + rr.g0 + idx / MT] = res[idx];
+        }
+      }
+      if (warp < MT && m0 + warp < p.M) {
+        const int m = warp, mm = m0 + warp;
+        float mx = -INFINITY;
+        for (int v2 = lane; v2 < rr.cnt; v2 += 32) mx = fmaxf(mx, res[v2 * MT + m]);
+        mx = warp_max(mx);
+        float se = 0.f;
+        for (int v2 = lane; v2 < rr.cnt; v2 += 32) se += expf(res[v2 * MT + m] - mx);
+        se = warp_sum(se);
+        const int64_t pc = static_cast<int64_t>(mm) * nct + c;
+        if (lane == 0) { p.stat[pc * 2] = mx; p.stat[pc * 2 + 1] = se; }
+        // local top-b: b rounds of "best candidate strictly after the previous pick"
+        float lv = INFINITY; int li = -1;
+        for (int jb = 0; jb < p.b; ++jb) {
+          float bv = -INFINITY; int bi = 0x7fffffff;
+          for (int v2 = lane; v2 < rr.cnt; v2 += 32) {
+            const float val = res[v2 * MT + m];
+            const int id = static_cast<int>(rr.g0) + v2;
+            if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+          }
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) {
+            const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+            if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+          }
+          if (lane == 0) { p.cand_val[pc * kMaxBranch + jb] = bv; p.cand_id[pc * kMaxBranch + jb] = bi; }
+          lv = bv; li = bi;
+        }
+      }
+    }
+    consumer_sync();  // res is reused by the next m-tile
+  }
+}
+
+}  // namespace dvt

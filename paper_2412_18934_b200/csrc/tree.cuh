@@ -1,0 +1,331 @@
+// tree.cuh -- the integer side of the draft step:
+//   S0  per-step set-up: level-0 row tables, rotary table
+//   S7  merge of the LM-head partial top-b lists, log-softmax normaliser,
+//       cumulative log-probability scores ("global acceptance probability"),
+//       pool append, frontier selection, next level's row tables / ancestor masks
+//   S8  final rerank to the top-gamma candidates, emitted in pool order
+//   S9  KV commit of the accepted path
+// Orders (reading A7): candidates of a row by (logit desc, token id asc);
+// nodes by (cumulative score desc, pool index asc). Everything here is
+// rank-by-counting on strict total orders, hence bit-exact by construction.
+#pragma once
+#include "gemv.cuh"
+#include "ptx.cuh"
+#include "state.cuh"
+
+namespace dvt {
+
+struct Pool {  // device arrays of capacity pool_cap
+  int32_t* token;
+  int32_t* parent;  // pool index or -1 (child of the root)
+  int32_t* depth;   // 1-based level
+  float* cum;       // sum of natural-log probabilities root -> node (reading A9)
+  int32_t* row;     // step row that forwarded the node, or -1
+};
+
+// ---- S0 ---------------------------------------------------------------------
+// grid = n_new + depth - 1 CTAs (one rotary-table row each) x 64 threads.
+__global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, RowTables* rt0,
+                             float2* rope, const double* inv_freq, int half, int vocab) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const int r = blockIdx.x, n_new = dynv.n_new;
+  // rotary angles in fp64: pos * theta^(-2i/dh) reaches thousands of radians
+  const int pos = r < n_new ? dynv.L + r : dynv.Lp + (r - n_new);
+  for (int i = threadIdx.x; i < half; i += blockDim.x) {
+    double s, c;
+    sincos(static_cast<double>(pos) * inv_freq[i], &s, &c);
+    rope[static_cast<size_t>(r) * half + i] = make_float2(static_cast<float>(c), static_cast<float>(s));
+  }
+  if (r == 0) {
+    if (threadIdx.x == 0) {
+      *dyn = dynv;
+      ts->status = 0;
+      ts->pool_size = 0;
+      ts->n_out = 0;
+    }
+    __syncthreads();
+    for (int m = threadIdx.x; m < n_new; m += blockDim.x) {
+      int t = dynv.tokens[m];
+      if (t < 0 || t >= vocab) {
+        t = min(max(t, 0), vocab - 1);
+        atomicOr(&ts->status, 1);
+      }
+      rt0->token[m] = t;
+      rt0->src[m] = m;
+      rt0->slot[m] = m;  // cache row L + m
+      rt0->pool[m] = -1;
+      for (int w = 0; w < kMaskWords; ++w) {  // causal among the level-0 rows: bits 0..m
+        const int lo = w * 32;
+        rt0->mask[m][w] = m >= lo + 31 ? 0xffffffffu : (m < lo ? 0u : (0xffffffffu >> (31 - (m - lo))));
+      }
+    }
+  }
+}
+
+// dgf_proj == 0: h1 = f, h2 = e (W1 = W2 = identity). grid-stride over M * 2d.
+template <typename WT>
+__global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, int64_t xld,
+                         const RowTables* rt, int use_idx, const WT* embed, float* hbuf, int M, int d) {
+  pdl_launch_dependents();
+  pdl_wait();
+  const float* base = from_dyn ? dyn->feats : xsrc;
+  for (int64_t idx = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; idx < static_cast<int64_t>(M) * 2 * d;
+       idx += static_cast<int64_t>(gridDim.x) * blockDim.x) {
+    const int m = static_cast<int>(idx / (2 * d)), k = static_cast<int>(idx % (2 * d));
+    float v;
+    if (k < d) v = base[static_cast<int64_t>(use_idx ? rt->src[m] : m) * xld + k];
+    else {
+      const WT e = embed[static_cast<size_t>(rt->token[m]) * d + (k - d)];
+      if (sizeof(WT) == 2) v = __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(&e));
+      else v = *reinterpret_cast<const float*>(&e);
+    }
+    hbuf[idx] = v;
+  }
+}
+
+// ---- S7 / S8 -----------------------------------------------------------------
+struct TreeLevelParams {
+  const StepDyn* dyn;
+  TreeState* ts;
+  Pool pool;
+  uint32_t* treemask;      // [kMaxTreeSlots][kMaskWords] ancestor mask of each tree row
+  // LM-head partials of this level's rows ...
+  const float* cand_val;
+  const int32_t* cand_id;
+  const float* stat;
+  int32_t nct;
+  // ... or (replay) caller-supplied lists
+  const int32_t* rp_tokens;
+  const float* rp_logp;
+  int32_t rp_maxb, rp_row0;
+  int32_t M, b;            // rows expanded at this level, children kept per row
+  int32_t level;           // 0-based; children get depth level + 1
+  int32_t pool_begin;      // pool index of this level's first child
+  int32_t M_next;          // rows of the next level (0: this is the last level)
+  int32_t next_row0;       // step row of the next level's first row
+  int32_t next_t0;         // tree-row index (= new-region slot) of the next level's first row
+  int32_t n_new;           // step rows before the first tree row; root row = n_new - 1
+  const RowTables* cur;
+  RowTables* next;
+  // final rerank (last level only)
+  int32_t gamma, pool_total;
+  int32_t* out_pool_idx;   // [gamma] pool index of each emitted candidate (for kv_commit)
+  int32_t* o_ids;          // explicit outputs (replay); NULL: take them from dyn
+  float* o_scores;
+  int32_t* o_parents;
+  int32_t* o_depths;
+  int32_t* o_n;
+};
+
+__device__ __forceinline__ bool node_before(const float* cum, int a, int b) {
+  const float ca = cum[a], cb = cum[b];
+  return ca > cb || (ca == cb && a < b);
+}
+
+constexpr int kTreeThreads = 256;
+constexpr int kPoolSmem = 4352;  // >= kMaxBranch + kMaxTreeSlots * kMaxBranch + slack
+
+__global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelParams p) {
+  __shared__ float s_cum[kPoolSmem];
+  __shared__ int32_t s_new[kPoolSmem];
+  __shared__ int32_t s_cnt[kTreeThreads + 1];
+  pdl_launch_dependents();
+  pdl_wait();
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const Pool& P = p.pool;
+
+  // ---- phase A: children of each expanded row --------------------------------
+  for (int m = warp; m < p.M; m += kTreeThreads / 32) {
+    const int parent = p.cur->pool[m];
+    const float pcum = parent < 0 ? 0.f : P.cum[parent];
+    const int base = p.pool_begin + m * p.b;
+    if (p.rp_tokens) {
+      if (lane < p.b) {
+        const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
+        P.token[base + lane] = p.rp_tokens[o];
+        P.parent[base + lane] = parent;
+        P.depth[base + lane] = p.level + 1;
+        P.cum[base + lane] = pcum + p.rp_logp[o];
+        P.row[base + lane] = -1;
+      }
+      continue;
+    }
+    // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order
+    const float* st = p.stat + static_cast<size_t>(m) * p.nct * 2;
+    float mg = -INFINITY;
+    for (int c = lane; c < p.nct; c += 32) mg = fmaxf(mg, st[c * 2]);
+    mg = warp_max(mg);
+    float se = 0.f;
+    for (int c = lane; c < p.nct; c += 32) {
+      const float mc = st[c * 2];
+      se += (mc == -INFINITY) ? 0.f : st[c * 2 + 1] * expf(mc - mg);
+    }
+    se = warp_sum(se);
+    const float logz = mg + logf(se);
+    // global top-b of the row: b rounds of "best candidate strictly after the previous pick"
+    const float* cv = p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
+    const int32_t* ci = p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
+    float lv = INFINITY;
+    int li = -1;
+    for (int jb = 0; jb < p.b; ++jb) {
+      float bv = -INFINITY;
+      int bi = 0x7fffffff;
+      for (int c = lane; c < p.nct; c += 32) {
+        for (int j = 0; j < p.b; ++j) {
+          const float val = cv[c * kMaxBranch + j];
+          const int id = ci[c * kMaxBranch + j];
+          if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+        }
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+      }
+      if (lane == 0) {
+        P.token[base + jb] = bi;
+        P.parent[base + jb] = parent;
+        P.depth[base + jb] = p.level + 1;
+        P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
+        P.row[base + jb] = -1;
+      }
+      lv = bv;
+      li = bi;
+    }
+  }
+  __syncthreads();
+
+  // ---- phase B: frontier of the next level = top-M_next children by score -----
+  const int n = p.M * p.b;
+  if (p.M_next > 0) {
+    for (int i = tid; i < n; i += kTreeThreads) s_cum[i] = P.cum[p.pool_begin + i];
+    __syncthreads();
+    for (int i = tid; i < n; i += kTreeThreads) {
+      int rank = 0;
+      for (int j = 0; j < n; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
+      if (rank < p.M_next) {
+        const int node = p.pool_begin + i, r = rank;
+        const int parent = P.parent[node];
+        const int t = p.next_t0 + r;  // tree-row index = new-region slot
+        p.next->token[r] = P.token[node];
+        p.next->src[r] = parent < 0 ? p.n_new - 1 : P.row[parent];
+        p.next->slot[r] = t;
+        p.next->pool[r] = node;
+        P.row[node] = p.next_row0 + r;
+        for (int w = 0; w < kMaskWords; ++w) {
+          uint32_t mk = parent < 0 ? 0u : p.treemask[(P.row[parent] - p.n_new) * kMaskWords + w];
+          if ((t >> 5) == w) mk |= 1u << (t & 31);
+          p.treemask[t * kMaskWords + w] = mk;
+          p.next->mask[r][w] = mk;
+        }
+      }
+    }
+    return;
+  }
+
+  // ---- phase C (last level): S8, top-gamma of the whole pool, pool order ------
+  const int Pn = p.pool_total;
+  for (int i = tid; i < Pn; i += kTreeThreads) s_cum[i] = P.cum[i];
+  __syncthreads();
+  const int n_keep = min(p.gamma, Pn);
+  for (int i = tid; i < Pn; i += kTreeThreads) {
+    int rank = 0;
+    for (int j = 0; j < Pn; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
+    s_new[i] = rank < n_keep ? 1 : 0;
+  }
+  __syncthreads();
+  // exclusive prefix count of the keep flags: contiguous chunk per thread
+  const int chunk = (Pn + kTreeThreads - 1) / kTreeThreads;
+  const int lo = min(Pn, tid * chunk), hi = min(Pn, lo + chunk);
+  int cnt = 0;
+  for (int i = lo; i < hi; ++i) cnt += s_new[i];
+  s_cnt[tid + 1] = cnt;
+  __syncthreads();
+  if (tid == 0) {
+    s_cnt[0] = 0;
+    for (int i = 1; i <= kTreeThreads; ++i) s_cnt[i] += s_cnt[i - 1];
+  }
+  __syncthreads();
+  int run = s_cnt[tid];
+  for (int i = lo; i < hi; ++i) {
+    const int k = s_new[i];
+    s_new[i] = k ? run : -1;  // output index of node i, or -1
+    run += k;
+  }
+  __syncthreads();
+  const StepDyn* dyn = p.dyn;
+  int32_t* o_ids = p.o_ids ? p.o_ids : dyn->out_ids;
+  float* o_scores = p.o_ids ? p.o_scores : dyn->out_scores;
+  int32_t* o_parents = p.o_ids ? p.o_parents : dyn->out_parents;
+  int32_t* o_depths = p.o_ids ? p.o_depths : dyn->out_depths;
+  int32_t* o_n = p.o_ids ? p.o_n : dyn->out_n;
+  for (int i = tid; i < Pn; i += kTreeThreads) {
+    const int o = s_new[i];
+    if (o < 0) continue;
+    const int parent = P.parent[i];
+    o_ids[o] = P.token[i];
+    o_scores[o] = s_cum[i];
+    o_parents[o] = parent < 0 ? -1 : s_new[parent];  // kept set is ancestor-closed (A7)
+    if (o_depths) o_depths[o] = P.depth[i];
+    p.out_pool_idx[o] = i;
+  }
+  if (tid == 0) {
+    *o_n = n_keep;
+    p.ts->n_out = n_keep;
+    p.ts->pool_size = Pn;
+  }
+}
+
+// ---- S9 ------------------------------------------------------------------------
+struct CommitPath {
+  int32_t n;
+  int32_t idx[kMaxDepth + 1];
+};
+
+// Validates the accepted path against the last step's output (root first, each
+// entry a child of the previous one) and lists the tree rows to move.
+__global__ void k_commit_plan(const CommitPath path, TreeState* ts, Pool pool, const int32_t* out_pool_idx,
+                              int n_new) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  int err = 0, n_mv = 0;
+  bool run = true;
+  int prev = -1;
+  for (int i = 0; i < path.n && !err; ++i) {
+    const int o = path.idx[i];
+    if (o < 0 || o >= ts->n_out) { err = 1; break; }
+    const int node = out_pool_idx[o];
+    if (pool.parent[node] != prev) { err = 1; break; }
+    prev = node;
+    const int row = pool.row[node];
+    if (run && row >= 0) ts->commit_src[n_mv++] = row - n_new;
+    else run = false;
+  }
+  ts->commit_err = err;
+  ts->commit_n = err ? 0 : n_mv;
+}
+
+// grid = (n_layers * Hkv, 2): moves the committed rows of one (layer, kv-head) of
+// K (y = 0) or V (y = 1): cache row Lp + src[i] -> Lp + i. All sources are read
+// before any destination is written (src[i] >= i, ranges may overlap).
+__global__ void k_commit_move(const TreeState* ts, void* kc, void* vc, int capacity, int Lp, int row_bytes) {
+  extern __shared__ __align__(16) uint8_t sm[];
+  const int n = ts->commit_n;
+  if (ts->commit_err || n == 0) return;
+  uint8_t* base = static_cast<uint8_t*>(blockIdx.y ? vc : kc) +
+                  static_cast<size_t>(blockIdx.x) * capacity * row_bytes;
+  const int units = row_bytes / 16;
+  for (int idx = threadIdx.x; idx < n * units; idx += blockDim.x) {
+    const int i = idx / units, u = idx % units;
+    reinterpret_cast<uint4*>(sm)[idx] =
+        *reinterpret_cast<const uint4*>(base + static_cast<size_t>(Lp + ts->commit_src[i]) * row_bytes + u * 16);
+  }
+  __syncthreads();
+  for (int idx = threadIdx.x; idx < n * units; idx += blockDim.x) {
+    const int i = idx / units, u = idx % units;
+    *reinterpret_cast<uint4*>(base + static_cast<size_t>(Lp + i) * row_bytes + u * 16) = reinterpret_cast<uint4*>(sm)[idx];
+  }
+}
+
+}  // namespace dvt

@@ -1,0 +1,73 @@
+"""CPU-side checks of the boundary: libdovetail_draft.so builds for sm_100a, loads, and
+exports every symbol include/dovetail.h declares; the ctypes structs match the header's
+layout; without a usable device the entry points fail loudly (no fallback)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+import torch
+
+from paper_2412_18934_b200 import binding, build
+from paper_2412_18934_b200.configs import CONFIGS
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return binding.load()
+
+
+def _declared():
+    src = open(os.path.join(ROOT, "include", "dovetail.h")).read()
+    return sorted(set(re.findall(r"\b(dovetail_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(lib):
+    names = _declared()
+    assert set(names) == set(binding.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+
+
+def test_struct_layouts_match_header():
+    # sizes implied by include/dovetail.h (LP64): 7 int32 + 2 float + 7 int32; 9 pointers; ...
+    assert C.sizeof(binding.ConfigT) == 16 * 4
+    assert C.sizeof(binding.LayerWeightsT) == 9 * 8
+    assert C.sizeof(binding.WeightsT) == 8 * 8
+    assert C.sizeof(binding.KVCacheT) == 24
+    assert C.sizeof(binding.TreeSpecT) == 4 * (1 + 16 + 16 + 1)
+    assert C.sizeof(binding.DraftOutT) == 5 * 8
+
+
+def test_null_arguments_are_rejected(lib):
+    assert lib.dovetail_draft_init(None, None, None) == binding.EINVAL
+    assert lib.dovetail_draft_step(None, None, None, 1, None, None, None, None) == binding.EINVAL
+    assert lib.dovetail_kv_commit(None, None, None, 0, 0, None, None) == binding.EINVAL
+    assert lib.dovetail_last_launch_count(None) == 0
+    assert lib.dovetail_forward_bytes(None, 0) == 0
+    assert b"null" in lib.dovetail_last_error(None)
+    lib.dovetail_draft_destroy(None)
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-device behaviour")
+def test_no_device_means_error_not_fallback(lib):
+    """With no sm_100 device dovetail_draft_init returns DOVETAIL_ECUDA: nothing computes on the CPU."""
+    cfg = CONFIGS["c1"]
+    c = binding.config_t(cfg)
+    dummy = C.c_void_p(16)  # never dereferenced: the device check comes first
+    layers = (binding.LayerWeightsT * cfg.n_layers)(*[binding.LayerWeightsT(*[16] * 9) for _ in range(cfg.n_layers)])
+    w = binding.WeightsT(16, 16, 16, 16, 16, layers, None, 16)
+    out = C.c_void_p()
+    rc = lib.dovetail_draft_init(C.byref(w), C.byref(c), C.byref(out))
+    assert rc == binding.ECUDA and not out.value
+    assert lib.dovetail_last_error(None)
+
+
+def test_binding_refuses_missing_library(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libdovetail_draft.so")
+    with pytest.raises(FileNotFoundError):
+        binding.load()

@@ -1,0 +1,111 @@
+"""-m gpu: the CUDA draft step (through the C ABI) against the fp64 oracle, element by
+element on the same seeded inputs. Small shapes span several tiles and ragged tails
+(rows per CTA, K not a multiple of 256 units, prefix not a multiple of the attention
+stage); the BASELINE.json configs run at full size."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+from parity import compare, make_case, run_gpu, run_oracle
+from paper_2412_18934_b200 import binding
+from paper_2412_18934_b200.configs import BF16, CONFIGS, F32, DraftConfig, TreeSpec, c4_sweep, paper_preset
+
+pytestmark = pytest.mark.gpu
+
+
+def small_cfg(**kw) -> DraftConfig:
+    base = dict(name="small", hidden=192, n_q_heads=4, n_kv_heads=2, head_dim=64, n_layers=2, ffn=344,
+                vocab=1000, dtype=F32, prefix=70, feat_scale=1.0, rope_theta=1e4,
+                tree=TreeSpec(3, (3, 2, 2), (0, 4, 5), 9), seed=11)
+    base.update(kw)
+    return DraftConfig(**base)
+
+
+def _boost(case, lm=40.0, emb=20.0):
+    """Spread the toy distributions so that the top-k decisions are far from ties."""
+    case.top["lm_head"] = (case.top["lm_head"].float() * lm).to(case.top["lm_head"].dtype)
+    case.top["embed"] = (case.top["embed"].float() * emb).to(case.top["embed"].dtype)
+    return case
+
+
+def _run(case, **kw):
+    h, kv, gpu = run_gpu(case, **kw)
+    ora = run_oracle(case)
+    s = compare(case, gpu, ora)
+    print({k: (f"{v:.3e}" if isinstance(v, float) else v) for k, v in s.items()})
+    binding.dovetail_draft_destroy(h)
+    return s, gpu, ora
+
+
+@pytest.mark.parametrize("dtype", [F32, BF16])
+@pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "no_first_norm_final_norm", "n_new5",
+                                     "no_prefix", "long_prefix", "wide"])
+def test_step_parity_small(dtype, variant):
+    kw, n_new, prefix = dict(dtype=dtype), 1, None
+    if variant == "mha_dh128":
+        kw.update(hidden=256, n_q_heads=2, n_kv_heads=2, head_dim=128)
+    elif variant == "mqa":
+        kw.update(n_q_heads=4, n_kv_heads=1)
+    elif variant == "no_proj":
+        kw.update(dgf_proj=0)
+    elif variant == "no_first_norm_final_norm":
+        kw.update(first_layer_input_norm=0, final_norm=1)
+    elif variant == "n_new5":
+        n_new = 5
+    elif variant == "no_prefix":
+        prefix = 0
+    elif variant == "long_prefix":
+        prefix, n_new = 333, 2
+    elif variant == "wide":  # rows per level 1, 6, 12: several m-tiles in every GEMV, query tiles in attention
+        kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
+    s, gpu, ora = _run(case)
+    assert s["same_tree"] or s["oracle_min_margin"] < 1e-2
+    if dtype == F32:
+        assert s["logit_max_abs_err"] < 1e-4
+
+
+def test_config_c1_tiny_fp32():
+    """BASELINE.json configs[0]: hidden 256, 4 x 64, 2 layers, FFN 688, vocab 1024, prefix 64, 14-token tree."""
+    cfg = CONFIGS["c1"]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case)
+    assert gpu["n_out"] == 14
+    assert s["logit_max_abs_err"] < 1e-4
+
+
+def test_paper_preset_tree_small_model():
+    """PAPER.md:184 server setting: width 10, depth 7, 16 candidates (on a small model)."""
+    cfg = small_cfg(dtype=BF16, tree=paper_preset(True))
+    case = _boost(make_case(cfg, n_new=3))
+    s, gpu, ora = _run(case)
+    assert gpu["n_out"] == 16
+
+
+def test_determinism_run_to_run():
+    cfg = small_cfg(dtype=BF16)
+    case = _boost(make_case(cfg, n_new=2))
+    _, _, a = run_gpu(case)
+    _, _, b = run_gpu(case)
+    for key in ("token_ids", "scores", "parents", "hhat", "logits", "k", "v"):
+        assert np.array_equal(a[key], b[key]), key
+
+
+@pytest.mark.parametrize("name", ["c2", "c3", "c5"])
+def test_full_size_configs(name):
+    """BASELINE.json configs[1], [2] (headline) and [4] at full size, in the launch
+    configuration bench.py times. The oracle runs the whole step in fp64 on the host."""
+    cfg = CONFIGS[name]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case)
+    assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
+
+
+def test_c4_sweep_point():
+    """BASELINE.json configs[3]: one point of the sweep (1 layer, 4 rows per level, prefix 2048)."""
+    cfg = [c for c in c4_sweep() if c.name == "c4_l1_g32"][0]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case)
+    assert gpu["n_out"] == 32

@@ -1,0 +1,182 @@
+"""-m gpu: the integer path on its own (S7, S8, S9) and the ABI's error behaviour.
+
+dovetail_tree_replay is fed per-row top-b lists and must reproduce the oracle's
+bookkeeping bit for bit (P10). Log-probabilities are drawn on a 1/1024 grid so that
+every cumulative sum is exact in fp32 and fp64 alike; exact ties are frequent."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from parity import make_case, run_gpu, run_oracle
+from paper_2412_18934_b200 import binding
+from paper_2412_18934_b200.configs import BF16, F32, TreeSpec, paper_preset
+from test_gpu_parity import _boost, small_cfg
+
+pytestmark = pytest.mark.gpu
+
+
+def _lists(tree: TreeSpec, rng, vocab=50, grid=1024, spread=3000):
+    rows = 1 + tree.tree_rows()
+    maxb = max(tree.branch)
+    toks = np.zeros((rows, maxb), np.int32)
+    lp = np.zeros((rows, maxb), np.float32)
+    for r in range(rows):
+        t = rng.choice(vocab, size=maxb, replace=False)
+        v = -rng.integers(0, spread, size=maxb).astype(np.float64) / grid
+        order = np.lexsort((t, -v))  # logp desc, token asc: the order the LM-head stage emits
+        toks[r], lp[r] = t[order], v[order]
+    return toks, lp
+
+
+@pytest.fixture(scope="module")
+def handle():
+    cfg = small_cfg(dtype=F32)
+    case = make_case(cfg, n_new=1)
+    h = binding.dovetail_draft_init(case.top, case.layers, cfg)
+    yield h
+    binding.dovetail_draft_destroy(h)
+
+
+TREES = [
+    TreeSpec(1, (4,), (0,), 3),
+    TreeSpec(3, (2, 2, 2), (0, 0, 0), 14),
+    TreeSpec(4, (3, 2, 2, 2), (0, 0, 0, 0), 10),
+    TreeSpec(5, (2,) * 5, (0, 2, 2, 2, 2), 16),
+    TreeSpec(5, (4,) * 5, (0, 4, 4, 4, 4), 32),
+    TreeSpec(6, (1,) * 6, (0, 1, 1, 1, 1, 1), 6),
+    TreeSpec(3, (8, 5, 3), (0, 6, 64), 200),
+    paper_preset(True),
+    paper_preset(False),
+    TreeSpec(4, (32, 32, 32, 32), (0, 64, 32, 32), 100),
+]
+
+
+@pytest.mark.parametrize("ti", range(len(TREES)))
+@pytest.mark.parametrize("spread", [3000, 6])  # 6: almost everything ties
+def test_tree_replay_bit_exact(handle, ti, spread):
+    tree = TREES[ti]
+    rng = np.random.default_rng(100 + ti)
+    toks, lp = _lists(tree, rng, vocab=max(64, max(tree.branch) + 5), spread=spread)
+    ora = oracle.tree_replay(tree.depth, tree.branch, tree.beam, tree.gamma, toks, lp.astype(np.float64))
+    P = tree.pool_size()
+    dev = "cuda"
+    pool = dict(token=torch.zeros(P, dtype=torch.int32, device=dev), parent=torch.zeros(P, dtype=torch.int32, device=dev),
+                depth=torch.zeros(P, dtype=torch.int32, device=dev), cum=torch.zeros(P, dtype=torch.float32, device=dev),
+                size=torch.zeros(1, dtype=torch.int32, device=dev))
+    out = binding.dovetail_tree_replay(handle, tree, torch.from_numpy(toks).to(dev), torch.from_numpy(lp).to(dev),
+                                       pool=pool)
+    torch.cuda.synchronize()
+    n = int(out["n_out"].item())
+    assert n == ora["n_out"] == min(tree.gamma, P)
+    assert int(pool["size"].item()) == P
+    assert np.array_equal(pool["token"].cpu().numpy(), ora["pool_token"])
+    assert np.array_equal(pool["parent"].cpu().numpy(), ora["pool_parent"])
+    assert np.array_equal(pool["depth"].cpu().numpy(), ora["pool_depth"])
+    assert np.array_equal(pool["cum"].cpu().numpy().astype(np.float64), ora["pool_cum"])  # sums are exact on the grid
+    assert np.array_equal(out["token_ids"][:n].cpu().numpy(), ora["token_ids"])
+    assert np.array_equal(out["parents"][:n].cpu().numpy(), ora["parents"])
+    assert np.array_equal(out["depths"][:n].cpu().numpy(), ora["depths"])
+    assert np.array_equal(out["scores"][:n].cpu().numpy().astype(np.float64), ora["scores"])
+
+
+def test_kv_commit_modes():
+    """P9 / O9: mode 0 leaves the cache alone and a repeated step reproduces itself; mode 1 moves
+    the accepted nodes' rows exactly as the oracle's memmove does."""
+    cfg = small_cfg(dtype=BF16)
+    case = _boost(make_case(cfg, n_new=2))
+    h, kv, gpu = run_gpu(case)
+    ora = run_oracle(case)
+    assert np.array_equal(gpu["token_ids"], ora["token_ids"]) and np.array_equal(gpu["parents"], ora["parents"])
+    # deepest accepted chain: follow parents from the deepest output node
+    leaf = int(np.argmax(gpu["depths"]))
+    path = [leaf]
+    while gpu["parents"][path[-1]] >= 0:
+        path.append(int(gpu["parents"][path[-1]]))
+    path = path[::-1]
+    Lp = kv.committed_len
+    assert Lp == case.L + 2
+    # bad paths: EINVAL, cache untouched
+    before_k = kv.k.clone()
+    for bad in ([path[-1]], path[::-1] if len(path) > 1 else [99], [0, 0]):
+        with pytest.raises(binding.DovetailError) as ei:
+            binding.dovetail_kv_commit(h, kv, bad, mode=1)
+        assert ei.value.code == binding.EINVAL
+        assert torch.equal(before_k, kv.k) and kv.committed_len == Lp
+    n = binding.dovetail_kv_commit(h, kv, path, mode=1)
+    torch.cuda.synchronize()
+    # oracle: tree rows of the accepted nodes (pool_row - n_new), leading forwarded run
+    keep_idx = _kept_pool_indices(ora)
+    rows = [int(ora["pool_row"][keep_idx[i]]) for i in path]
+    tree_rows = [r - 2 if r >= 0 else -1 for r in rows]
+    kc, vc = gpu["k"].copy(), gpu["v"].copy()
+    moved = oracle.kv_commit(_ocfg(cfg), kc, vc, case.capacity, Lp, tree_rows, 1)
+    assert n == moved and kv.committed_len == Lp + moved
+    from helpers import kv_np
+    assert np.array_equal(kv_np(kv.k), kc) and np.array_equal(kv_np(kv.v), vc)
+    # a second commit without a new step is refused
+    with pytest.raises(binding.DovetailError):
+        binding.dovetail_kv_commit(h, kv, path, mode=1)
+    binding.dovetail_draft_destroy(h)
+
+    # mode 0: step, discard, step again with the same inputs -> identical results
+    h, kv, a = run_gpu(case)
+    assert binding.dovetail_kv_commit(h, kv, path, mode=0) == 0
+    kv.committed_len = case.L
+    out = binding.dovetail_draft_step(h, case.feats, case.tokens, kv, case.tree)
+    torch.cuda.synchronize()
+    n2 = int(out["n_out"].item())
+    assert np.array_equal(out["token_ids"][:n2].cpu().numpy(), a["token_ids"])
+    assert np.array_equal(out["scores"][:n2].cpu().numpy(), a["scores"])
+    binding.dovetail_draft_destroy(h)
+
+
+def _ocfg(cfg):
+    from helpers import ocfg
+    return ocfg(cfg)
+
+
+def _kept_pool_indices(ora):
+    """Pool index of each emitted candidate: the top-gamma by (score desc, index asc), in pool order."""
+    cum = ora["pool_cum"]
+    order = np.lexsort((np.arange(len(cum)), -cum))
+    return np.sort(order[:ora["n_out"]])
+
+
+def test_error_paths():
+    cfg = small_cfg(dtype=F32)
+    case = make_case(cfg, n_new=1)
+    h = binding.dovetail_draft_init(case.top, case.layers, cfg, max_rows=8, max_tree_slots=16, max_branch=4)
+    kv = binding.KVCache(case.k.clone(), case.v.clone(), case.L)
+    good = TreeSpec(2, (2, 2), (0, 0), 4)
+
+    def code(fn):
+        with pytest.raises(binding.DovetailError) as ei:
+            fn()
+        return ei.value.code
+
+    step = lambda tree, kvc=kv, f=case.feats, t=case.tokens: binding.dovetail_draft_step(h, f, t, kvc, tree)
+    assert code(lambda: step(TreeSpec(0, (), (), 1))) == binding.EINVAL                 # depth
+    assert code(lambda: step(TreeSpec(2, (5, 2), (0, 0), 4))) == binding.EINVAL          # branch > max_branch
+    assert code(lambda: step(TreeSpec(2, (2, 2), (0, 0), 0))) == binding.EINVAL          # gamma
+    assert code(lambda: step(TreeSpec(4, (4, 4, 4, 4), (0, 0, 0, 0), 4))) == binding.EINVAL  # rows > max_rows
+    assert code(lambda: step(TreeSpec(6, (2,) * 6, (0, 0, 0, 4, 4, 4), 4))) == binding.EINVAL  # > max_tree_slots
+    many = torch.zeros((9, cfg.hidden), device="cuda")
+    assert code(lambda: step(good, f=many, t=torch.zeros(9, dtype=torch.int32, device="cuda"))) == binding.EINVAL
+    small = binding.KVCache(case.k.clone(), case.v.clone(), case.capacity - 1)
+    assert code(lambda: step(good, kvc=small)) == binding.ECAPACITY
+    assert small.committed_len == case.capacity - 1 and kv.committed_len == case.L    # nothing advanced
+    assert "capacity" in binding.dovetail_last_error(h)
+    assert code(lambda: binding.dovetail_kv_commit(h, kv, [0], mode=0)) == binding.EINVAL  # no step yet
+    out = step(good)
+    torch.cuda.synchronize()
+    assert int(out["n_out"].item()) == 4 and kv.committed_len == case.L + 1
+    assert binding.dovetail_last_launch_count(h) > 0
+    assert binding.dovetail_forward_bytes(h, case.L) == cfg.forward_bytes(case.L)
+    binding.dovetail_draft_destroy(h)
+    # init-time validation
+    bad = small_cfg(dtype=F32, head_dim=32, hidden=128)
+    c2 = make_case(bad, n_new=1)
+    with pytest.raises(binding.DovetailError) as ei:
+        binding.dovetail_draft_init(c2.top, c2.layers, bad)
+    assert ei.value.code == binding.EINVAL
