@@ -218,6 +218,20 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree,
  * Borrowed until replaced. */
 int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat);
 
+/* Optional per-kernel timing, for the roofline report (off by default). When
+ * enabled, dovetail_draft_step brackets every kernel launch with CUDA events on
+ * cuda_stream (this serialises the launches: programmatic dependent launch
+ * cannot overlap across an event, so the step itself runs slower). After the
+ * stream has been synchronised by the caller, dovetail_profile_read adds up the
+ * last step's launches by kind:
+ *   kind 0 step set-up, 1 DGF projections, 2 DGF gate, 3 QKV, 4 tree attention,
+ *   5 O-proj, 6 gate/up, 7 down, 8 LM head, 9 tree bookkeeping, 10 h fill.
+ * ms, launches, bytes: host arrays of DOVETAIL_N_KINDS entries; bytes are the
+ * algorithmic HBM bytes of the kind's launches (weights, prefix K/V). */
+#define DOVETAIL_N_KINDS 11
+int dovetail_draft_set_profile(dovetail_draft_t* h, int32_t enable);
+int dovetail_profile_read(dovetail_draft_t* h, float* ms, int32_t* launches, int64_t* bytes);
+
 /* Number of kernel launches the last dovetail_draft_step enqueued. */
 int dovetail_last_launch_count(const dovetail_draft_t* h);
 

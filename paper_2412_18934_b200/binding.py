@@ -17,7 +17,8 @@ MAX_DEPTH, MAX_LAYERS = 16, 16
 OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "dovetail_tree_replay",
-           "dovetail_draft_set_taps", "dovetail_last_launch_count", "dovetail_forward_bytes",
+           "dovetail_draft_set_taps", "dovetail_draft_set_profile", "dovetail_profile_read",
+           "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 
 
@@ -85,6 +86,10 @@ def load() -> C.CDLL:
                                              C.c_int32, C.POINTER(DraftOutT)] + [C.c_void_p] * 6
         lib.dovetail_draft_set_taps.restype = C.c_int
         lib.dovetail_draft_set_taps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.dovetail_draft_set_profile.restype = C.c_int
+        lib.dovetail_draft_set_profile.argtypes = [C.c_void_p, C.c_int32]
+        lib.dovetail_profile_read.restype = C.c_int
+        lib.dovetail_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
         lib.dovetail_last_launch_count.restype = C.c_int
         lib.dovetail_last_launch_count.argtypes = [C.c_void_p]
         lib.dovetail_forward_bytes.restype = C.c_int64
@@ -240,6 +245,24 @@ def dovetail_tree_replay(h: Draft, tree: TreeSpec, cand_tokens, cand_logp, out: 
 def dovetail_draft_set_taps(h: Draft, logits=None, hhat=None):
     h.taps = (logits, hhat)
     _check(load().dovetail_draft_set_taps(h.ptr, _dp(logits), _dp(hhat)), h.ptr)
+
+
+N_KINDS = 11
+KIND_NAMES = ("step_begin", "dgf_proj", "dgf_gate", "qkv", "tree_attention", "o_proj", "gate_up", "down",
+              "lm_head", "tree_level", "h_fill")
+
+
+def dovetail_draft_set_profile(h: Draft, enable: bool):
+    _check(load().dovetail_draft_set_profile(h.ptr, 1 if enable else 0), h.ptr)
+
+
+def dovetail_profile_read(h: Draft) -> Dict[str, Dict]:
+    """Per-kind totals of the last (profiled, synchronised) step: ms, launches, algorithmic bytes."""
+    ms = (C.c_float * N_KINDS)()
+    n = (C.c_int32 * N_KINDS)()
+    b = (C.c_int64 * N_KINDS)()
+    _check(load().dovetail_profile_read(h.ptr, ms, n, b), h.ptr)
+    return {KIND_NAMES[k]: dict(ms=ms[k], launches=n[k], bytes=b[k]) for k in range(N_KINDS)}
 
 
 def dovetail_last_launch_count(h: Draft) -> int:

@@ -71,6 +71,14 @@ struct dovetail_draft {
   int last_n_new = 0, last_depth = 0, last_gamma = 0;
   int last_launches = 0;
   int launches = 0;
+  // optional per-kernel timing
+  bool profile = false;
+  int cur_kind = 0;
+  int64_t cur_bytes = 0;
+  std::vector<cudaEvent_t> ev;       // 2 per launch
+  std::vector<int> ev_kind;
+  std::vector<int64_t> ev_bytes;
+  int ev_used = 0;
   char err[512] = "no error";
 };
 
@@ -102,7 +110,22 @@ cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 bl
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   ++h->launches;
-  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+  if (!h->profile) return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+  // profiling: bracket the launch with events (serialises the kernels)
+  const int i = h->ev_used++;
+  while (static_cast<int>(h->ev.size()) < 2 * (i + 1)) {
+    cudaEvent_t e;
+    cudaError_t r = cudaEventCreate(&e);
+    if (r != cudaSuccess) return r;
+    h->ev.push_back(e);
+  }
+  if (static_cast<int>(h->ev_kind.size()) <= i) { h->ev_kind.resize(i + 1); h->ev_bytes.resize(i + 1); }
+  h->ev_kind[i] = h->cur_kind;
+  h->ev_bytes[i] = h->cur_bytes;
+  cudaEventRecord(h->ev[2 * i], st);
+  cudaError_t r = cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+  cudaEventRecord(h->ev[2 * i + 1], st);
+  return r;
 }
 
 using GemvKernel = void (*)(const GemvParams);
@@ -183,8 +206,12 @@ GemvShape gemv_shape(int K, int es, int M, int res_rows) {
 int div_up(int a, int b) { return (a + b - 1) / b; }
 
 // Enqueue one GEMV: group list, K, M rows, epilogue.
-int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, int ctas_per_group) {
+int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, int ctas_per_group, int kind) {
   int res_rows = 0;
+  h->cur_kind = kind;
+  h->cur_bytes = 0;
+  for (int g = 0; g < n_groups; ++g)
+    for (int j = 0; j < p.g[g].n_mat; ++j) h->cur_bytes += static_cast<int64_t>(p.g[g].rows[j]) * p.K * h->es;
   for (int g = 0; g < n_groups; ++g) {
     const GemvGroup& G = p.g[g];
     int r;
@@ -268,6 +295,7 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
   if (h->ts_host) cudaFreeHost(h->ts_host);
+  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
 }
 
 }  // namespace
@@ -413,6 +441,9 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
   dv.out_parents = out->parents;
   dv.out_depths = out->depths;
   dv.out_n = out->n_out;
+  h->ev_used = 0;
+  h->cur_kind = 0;
+  h->cur_bytes = 0;
   e = launch(h, k_step_begin, dim3(n_new + tree->depth - 1), dim3(64), 0, st, dv, h->dyn, h->ts, h->rt, h->rope,
              static_cast<const double*>(h->inv_freq), half, V);
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
@@ -445,10 +476,12 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
       p.epi = EPI_STORE;
       p.out = h->hbuf;
       p.out_ld = 2 * d;
-      rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)));
+      rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)), 1);
       if (rc) return rc;
     } else {
       const int blocks = std::min(nsm, div_up(M * 2 * d, 256));
+      h->cur_kind = 10;
+      h->cur_bytes = 0;
       if (bf16)
         e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
                    static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
@@ -473,7 +506,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
       p.hbuf = h->hbuf;
       p.bias = h->w.dgf_bg;
       p.d = d;
-      rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+      rc = run_gemv(h, st, p, 1, std::min(nsm, d), 2);
       if (rc) return rc;
     }
 
@@ -493,7 +526,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         p.epi = EPI_STORE;
         p.out = h->qkv;
         p.out_ld = ldq;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq));
+        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq), 3);
         if (rc) return rc;
       }
       {  // S2 (RoPE, KV append) + S3 tree attention
@@ -522,6 +555,8 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
         const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
                             static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
+        h->cur_kind = 4;
+        h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
         e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
         if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "attention launch failed: %s", cudaGetErrorString(e));
       }
@@ -534,7 +569,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 5);
         if (rc) return rc;
       }
       {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
@@ -550,7 +585,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         p.epi = EPI_SWIGLU;
         p.out = h->act;
         p.out_ld = F;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, F));
+        rc = run_gemv(h, st, p, 1, std::min(nsm, F), 6);
         if (rc) return rc;
       }
       {  // S5b: x += Wdown act
@@ -562,7 +597,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d));
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 7);
         if (rc) return rc;
       }
     }
@@ -583,7 +618,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
       p.cand_id = h->cand_id;
       p.stat = h->stat;
       p.tap = h->tap_logits ? h->tap_logits + static_cast<size_t>(lp.row0 + (l == 0 ? n_new - 1 : 0)) * V : nullptr;
-      rc = run_gemv(h, st, p, 1, lm_ctas);
+      rc = run_gemv(h, st, p, 1, lm_ctas, 8);
       if (rc) return rc;
     }
     {  // S7 (+ S8 after the last level)
@@ -610,6 +645,8 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
       t.gamma = tree->gamma;
       t.pool_total = pool_total;
       t.out_pool_idx = h->out_pool_idx;
+      h->cur_kind = 9;
+      h->cur_bytes = 0;
       e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
       if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
     }
@@ -675,15 +712,16 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, 
   int tree_rows = 0, pool_total = 0;
   int rc = validate_tree(h, tree, 1, plan, tree_rows, pool_total);
   if (rc != DOVETAIL_OK) return rc;
-  int need_rows = 1 + tree_rows - (tree->depth > 1 ? 0 : 0);
-  // rows consumed: the root and every forwarded row of levels 1 .. D-1
-  need_rows = 1;
+  int need_rows = 1;  // rows consumed: the root and every forwarded row of levels 1 .. D-1
   for (int l = 1; l < tree->depth; ++l) need_rows += plan[l].rows;
   int maxb = 0;
   for (int l = 0; l < tree->depth; ++l) maxb = std::max(maxb, tree->branch[l]);
   if (n_rows < need_rows || max_b < maxb) return fail(h, DOVETAIL_EINVAL, "replay needs %d rows of %d candidates", need_rows, maxb);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   h->launches = 0;
+  h->ev_used = 0;
+  h->cur_kind = 9;
+  h->cur_bytes = 0;
   cudaError_t e = cudaMemsetAsync(h->rt, 0xff, sizeof(RowTables), st);  // level-0 row: pool = -1
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "memset failed: %s", cudaGetErrorString(e));
   int row = 0;
@@ -743,6 +781,28 @@ int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat) {
 }
 
 int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
+
+int dovetail_draft_set_profile(dovetail_draft_t* h, int32_t enable) {
+  if (!h) return DOVETAIL_EINVAL;
+  h->profile = enable != 0;
+  h->ev_used = 0;
+  return DOVETAIL_OK;
+}
+
+int dovetail_profile_read(dovetail_draft_t* h, float* ms, int32_t* launches, int64_t* bytes) {
+  if (!h || !ms || !launches || !bytes) return h ? fail(h, DOVETAIL_EINVAL, "null argument") : DOVETAIL_EINVAL;
+  for (int k = 0; k < DOVETAIL_N_KINDS; ++k) { ms[k] = 0.f; launches[k] = 0; bytes[k] = 0; }
+  for (int i = 0; i < h->ev_used; ++i) {
+    float t = 0.f;
+    cudaError_t e = cudaEventElapsedTime(&t, h->ev[2 * i], h->ev[2 * i + 1]);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "profile read failed (synchronise the stream first): %s", cudaGetErrorString(e));
+    const int k = h->ev_kind[i];
+    ms[k] += t;
+    launches[k] += 1;
+    bytes[k] += h->ev_bytes[i];
+  }
+  return DOVETAIL_OK;
+}
 
 int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
   if (!h) return 0;
