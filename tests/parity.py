@@ -116,6 +116,11 @@ def bf16_ulp_diff(a: np.ndarray, b: np.ndarray) -> np.ndarray:
     return np.abs(key(a) - key(b))
 
 
+def bf16_bits_to_f64(a: np.ndarray) -> np.ndarray:
+    """uint16 bf16 bit patterns widened exactly."""
+    return (a.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
+
+
 def compare(case: Case, gpu: dict, ora: dict, log=print) -> dict:
     """Element-by-element comparison. Returns a summary dict; raises AssertionError on a
     mismatch that the stated tolerances do not allow."""
@@ -159,12 +164,22 @@ def compare(case: Case, gpu: dict, ora: dict, log=print) -> dict:
         assert np.array_equal(g[:, :, :case.L], o[:, :, :case.L]), f"{name} prefix modified"
         used = case.L + rows
         if g.dtype == np.uint16:
-            ulp = bf16_ulp_diff(g[:, :, case.L:used], o[:, :, case.L:used])
+            gs, os_ = g[:, :, case.L:used], o[:, :, case.L:used]
+            ulp = bf16_ulp_diff(gs, os_)
             summary[f"{name}_rows_off_by_1ulp"] = int((ulp == 1).sum())
-            # stored values are fp32 results rounded to bf16: a 1e-6 difference before rounding can
-            # move a value across a rounding boundary, never further than one ulp
-            assert ulp.max() <= 1, f"{name} cache rows differ by {ulp.max()} bf16 ulps"
-            assert (ulp == 1).mean() < 0.02, f"{name}: {(ulp == 1).mean():.3%} of stored values off by one ulp"
+            # Stored values are fp32 results rounded to bf16. The fp32 accumulation differs from the
+            # oracle's fp64 by at most KV_ABS before rounding (K <= 13824 terms of magnitude <= 1e-1,
+            # 2^-24 relative each, summed in a fixed tree), which can move a value across one rounding
+            # boundary: allowed difference = one bf16 ulp of the larger magnitude + KV_ABS. (Counting
+            # ulps alone is meaningless next to zero, where one ulp is far below KV_ABS.)
+            KV_ABS = 3e-5
+            gf, of = bf16_bits_to_f64(gs), bf16_bits_to_f64(os_)
+            mag = np.maximum(np.abs(gf), np.abs(of))
+            one_ulp = np.exp2(np.floor(np.log2(np.maximum(mag, 1e-30))) - 7)
+            bad = np.abs(gf - of) > one_ulp + KV_ABS
+            assert not bad.any(), (f"{name} cache rows differ beyond one bf16 ulp + {KV_ABS}: "
+                                   f"{int(bad.sum())} values, worst {np.abs(gf - of).max():.3e}")
+            assert (ulp != 0).mean() < 0.02, f"{name}: {(ulp != 0).mean():.3%} of stored values differ"
         else:
             np.testing.assert_allclose(g[:, :, case.L:used], o[:, :, case.L:used], **tol)
         assert np.array_equal(g[:, :, used:], o[:, :, used:]), f"{name} rows past the step modified"
