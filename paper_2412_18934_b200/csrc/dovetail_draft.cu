@@ -10,6 +10,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -17,6 +18,7 @@
 #include "../../include/dovetail.h"
 #include "attention.cuh"
 #include "gemv.cuh"
+#include "gemv_mma.cuh"
 #include "state.cuh"
 #include "tree.cuh"
 
@@ -73,6 +75,7 @@ struct dovetail_draft {
   int launches = 0;
   // optional per-kernel timing
   bool profile = false;
+  bool force_fma = false;  // DOVETAIL_FORCE_FMA=1: bf16 GEMVs on the FMA kernel (for A/B measurements)
   int cur_kind = 0;
   int64_t cur_bytes = 0;
   std::vector<cudaEvent_t> ev;       // 2 per launch
@@ -141,6 +144,13 @@ GemvKernel pick_gemv(int MT, int NI) {
   return k_gemv<WT, 2, 7>;
 }
 
+GemvKernel pick_gemv_mma(int NT) {
+  if (NT == 1) return k_gemv_mma<1, 4>;
+  if (NT == 2) return k_gemv_mma<2, 4>;
+  if (NT == 4) return k_gemv_mma<4, 4>;
+  return k_gemv_mma<8, 2>;
+}
+
 using AttnKernel = void (*)(const AttnParams);
 
 template <typename WT, int DH>
@@ -162,6 +172,7 @@ cudaError_t set_max_smem_all() {
     cudaError_t r = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
     if (r != cudaSuccess) e = r;
   };
+  for (int nt = 1; nt <= 8; nt *= 2) set(reinterpret_cast<const void*>(pick_gemv_mma(nt)));
   const int mts[3] = {1, 2, 4};
   for (int mt : mts) {
     set(reinterpret_cast<const void*>(pick_gemv<__nv_bfloat16>(mt, 3)));
@@ -205,9 +216,48 @@ GemvShape gemv_shape(int K, int es, int M, int res_rows) {
 
 int div_up(int a, int b) { return (a + b - 1) / b; }
 
+// Geometry of the tensor-core GEMV (gemv_mma.cuh) for a [*, K] bf16 matrix, M draft rows and
+// at most max_cnt rows per CTA.
+struct MmaShape {
+  int NT, RBMAX, S, ncols, PC, RS, KC, KP, seg_stride, bs_stride, stage_bytes, n_stages, smem;
+  bool ok;
+};
+
+MmaShape mma_shape(int K, int M, int max_cnt) {
+  MmaShape s{};
+  s.ok = K % 32 == 0 && M >= 1 && M <= kMmaMaxM && max_cnt >= 1;
+  if (!s.ok) return s;
+  auto nt_for = [](int cols) { int t = (cols + 7) / 8, r = 1; while (r < t) r *= 2; return r; };
+  const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
+  s.S = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
+  s.NT = nt2;
+  if (s.NT > 8) { s.ok = false; return s; }
+  s.RBMAX = s.NT == 8 ? 2 : 4;
+  s.ncols = M * s.S;
+  s.PC = (s.ncols + 1) & ~1;
+  s.RS = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
+  while (kConsumerWarps * s.RS * s.PC * 4 > 32768 && s.RS > 16) s.RS -= 16;
+  const int target = 32768 / (s.RS * 2);
+  s.KC = target >= 1024 ? 1024 : (target >= 512 ? 512 : 256);
+  s.KC = std::min(s.KC, (K + 63) / 64 * 64);
+  int kpmax = (65536 / s.ncols / 2) / s.KC * s.KC;
+  if (kpmax < s.KC) kpmax = s.KC;
+  const int n_panels = div_up(K, kpmax);
+  s.KP = div_up(div_up(K, n_panels), s.KC) * s.KC;
+  s.seg_stride = s.KC * 2 + 16;
+  s.bs_stride = s.KP * 2 + 16;
+  s.stage_bytes = s.RS * s.seg_stride;
+  int fixed = 128 + 4 * kMmaMaxM + s.ncols * s.bs_stride + 16 + kConsumerWarps * s.RS * s.PC * 4 + max_cnt * M * 4;
+  fixed = (fixed + 15) / 16 * 16;
+  s.n_stages = std::min(8, (kSmemMax - fixed - 64) / s.stage_bytes);
+  if (s.n_stages < 2) s.ok = false;
+  s.smem = s.n_stages * s.stage_bytes + fixed;
+  return s;
+}
+
 // Enqueue one GEMV: group list, K, M rows, epilogue.
 int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, int ctas_per_group, int kind) {
-  int res_rows = 0;
+  int res_rows = 0, max_cnt = 0;
   h->cur_kind = kind;
   h->cur_bytes = 0;
   for (int g = 0; g < n_groups; ++g)
@@ -222,6 +272,32 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
       r = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group) + 1;
     }
     if (r > res_rows) res_rows = r;
+    int mc;
+    if (G.paired) mc = G.n_mat * div_up(G.rows[0], ctas_per_group);
+    else {
+      long tot = 0;
+      for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
+      mc = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group);
+    }
+    if (mc > max_cnt) max_cnt = mc;
+  }
+  p.dyn = h->dyn;
+  if (h->es == 2 && !h->force_fma) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
+    const MmaShape ms = mma_shape(p.K, p.M, max_cnt);
+    if (ms.ok) {
+      p.rows_per_stage = ms.RS;
+      p.n_stages = ms.n_stages;
+      p.stage_bytes = ms.stage_bytes;
+      p.row_bytes = p.K * 2;
+      p.kc = ms.KC;
+      p.kp = ms.KP;
+      p.split = ms.S;
+      p.seg_stride = ms.seg_stride;
+      p.bs_stride = ms.bs_stride;
+      cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
+      return DOVETAIL_OK;
+    }
   }
   const GemvShape s = gemv_shape(p.K, h->es, p.M, res_rows);
   if (!s.ok) return fail(h, DOVETAIL_EINVAL, "GEMV with K = %d is not supported (K * elem size must be a multiple of 16 and <= 28672 bytes)", p.K);
@@ -343,6 +419,10 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   h->layers.assign(w->layers, w->layers + c.n_layers);
   h->w.layers = h->layers.data();
   h->num_sms = prop.multiProcessorCount;
+  {
+    const char* ev = getenv("DOVETAIL_FORCE_FMA");
+    h->force_fma = ev && ev[0] == '1';
+  }
   h->es = es;
   h->dq = dq;
   h->dkv = dkv;

@@ -51,6 +51,8 @@ struct GemvParams {
   const StepDyn* dyn;
   int32_t K, M;
   int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
+  // k_gemv_mma only: K-chunk per stage, K-panel of the B store, split ways, strides (bytes)
+  int32_t kc, kp, split, seg_stride, bs_stride;
   int32_t epi;
   float eps;
   float* out;            // STORE/SWIGLU: [M, out_ld]; DGF/RESID: residual stream rows x [M, out_ld]
