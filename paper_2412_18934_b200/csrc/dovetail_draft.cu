@@ -238,7 +238,7 @@ MmaShape mma_shape(int K, int M, int max_cnt) {
   s.RS = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
   while (kConsumerWarps * s.RS * s.PC * 4 > 32768 && s.RS > 16) s.RS -= 16;
   const int target = 32768 / (s.RS * 2);
-  s.KC = target >= 1024 ? 1024 : (target >= 512 ? 512 : 256);
+  s.KC = target >= 1024 ? 1024 : 512;
   s.KC = std::min(s.KC, (K + 63) / 64 * 64);
   int kpmax = (65536 / s.ncols / 2) / s.KC * s.KC;
   if (kpmax < s.KC) kpmax = s.KC;
@@ -247,7 +247,7 @@ MmaShape mma_shape(int K, int M, int max_cnt) {
   s.seg_stride = s.KC * 2 + 16;
   s.bs_stride = s.KP * 2 + 16;
   s.stage_bytes = s.RS * s.seg_stride;
-  int fixed = 128 + 4 * kMmaMaxM + s.ncols * s.bs_stride + 16 + kConsumerWarps * s.RS * s.PC * 4 + max_cnt * M * 4;
+  int fixed = 128 + 16 + (4 + 8 + 4 * kConsumerWarps) * kMmaMaxM + s.ncols * s.bs_stride + 16 + kConsumerWarps * s.RS * s.PC * 4 + max_cnt * M * 4;
   fixed = (fixed + 15) / 16 * 16;
   s.n_stages = std::min(8, (kSmemMax - fixed - 64) / s.stage_bytes);
   if (s.n_stages < 2) s.ok = false;

@@ -66,6 +66,7 @@ struct GemvParams {
   int32_t* cand_id;
   float* stat;           // LMHEAD: [kMaxRows][grid][2] = (max, sum exp)
   float* tap;            // LMHEAD: optional logits tap rows [M, vocab]
+  unsigned long long* trace;  // DVT_TRACE builds only
 };
 
 template <typename WT>

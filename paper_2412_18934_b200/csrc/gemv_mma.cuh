@@ -39,6 +39,15 @@
 
 namespace dvt {
 
+#ifdef DVT_TRACE  // microbenchmark builds only: per-CTA time stamps (ns) at the phases of the kernel
+#define DVT_STAMP(i) do { if ((threadIdx.x & 31) == 0 && p.trace) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[(static_cast<size_t>(blockIdx.x) * 12 + (threadIdx.x >> 5)) * 8 + (i)] = t_; } } while (0)
+#else
+#define DVT_STAMP(i) do { } while (0)
+#endif
+
+#ifndef DVT_GATE_SLOT
+#define DVT_GATE_SLOT 1
+#endif
 constexpr int kMmaMaxM = 32;
 // A 1-D bulk copy costs its issuing warp ~35 ns whatever its size (measured: one producer warp
 // moves 2.4 TB/s chip-wide with 512-byte copies, four move 7.2 TB/s), so four warps produce.
@@ -78,20 +87,25 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
   uint8_t* ring = smem;
   uint64_t* full = reinterpret_cast<uint64_t*>(smem + static_cast<size_t>(NS) * p.stage_bytes);
   uint64_t* empty = full + 8;
-  float* rstd_s = reinterpret_cast<float*>(empty + 8);  // [32]
-  uint8_t* bstore = reinterpret_cast<uint8_t*>(rstd_s + kMmaMaxM);  // [ncols][bs_stride] + 16 zero bytes
+  uint64_t* xbar = empty + 8;  // consumers have issued their activation loads
+  float* rstd_s = reinterpret_cast<float*>(xbar + 2);  // [32]
+  const void** xptr_s = reinterpret_cast<const void**>(rstd_s + kMmaMaxM);  // [32] source row of each m
+  float* ss_part = reinterpret_cast<float*>(xptr_s + kMmaMaxM);  // [warps][32] sum of squares
+  uint8_t* bstore = reinterpret_cast<uint8_t*>(ss_part + kConsumerWarps * kMmaMaxM);  // [ncols][bs_stride] + 16 zero bytes
   float* part = reinterpret_cast<float*>(bstore + static_cast<size_t>(ncols) * p.bs_stride + 16);  // [warps][RS][PC]
   float* res = part + static_cast<size_t>(kConsumerWarps) * RS * PC;  // [cnt][M]
 
   const RowRange rr = cta_rows(G, c, nct);
   const int n_sb = (rr.cnt + RS - 1) / RS;
   const int n_panels = (K + KP - 1) / KP;
+  DVT_STAMP(0);
 
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) {
       mbar_init(&full[s], kMmaProducerWarps);
       mbar_init(&empty[s], kConsumerWarps);
     }
+    mbar_init(xbar, kConsumerWarps);
     mbar_fence_init();
   }
   __syncthreads();
@@ -117,6 +131,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
         }
         for (int k0 = k_begin; k0 < k_end; k0 += KC) {
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+          // The activation loads of the consumers must not queue behind a ring full of weights on
+          // this SM's return path (measured: 5 us instead of 1 us): only the first stage is
+          // prefetched before the consumers have issued them.
+          if (round == 0 && slot == DVT_GATE_SLOT) mbar_wait(xbar, 0);
           const uint32_t segb = static_cast<uint32_t>(min(KC, k_end - k0)) * 2u;
           if (lane == 0) mbar_arrive_expect_tx(&full[slot], static_cast<uint32_t>(my_rows) * segb);
           __syncwarp();
@@ -126,46 +144,28 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
         }
       }
     }
+    DVT_STAMP(1);
     return;
   }
 
   // ---------------- consumers -------------------------------------------------
-  pdl_wait();  // activations of the previous kernel are visible from here on
+  pdl_wait();
+  DVT_STAMP(1);  // activations of the previous kernel are visible from here on
   const StepDyn* dyn = p.dyn;
   const bool normed = G.gain != nullptr;
   const __nv_bfloat16* gain = static_cast<const __nv_bfloat16*>(G.gain);
 
-  auto x_row = [&](int m, const float*& xrow, const __nv_bfloat16*& erow) {
-    xrow = nullptr;
-    erow = nullptr;
-    if (G.xkind == X_ROWS) {
+  const bool x_embed = G.xkind != X_ROWS;
+  if (tid < M && (x_embed || G.x_from_dyn || G.xidx)) {  // source row of each draft row (fp32 rows, or bf16 embedding rows)
+    if (!x_embed) {
       const float* base = G.x_from_dyn ? dyn->feats : G.xsrc;
-      const int64_t ri = G.xidx ? G.xidx[m] : m;
-      xrow = base + ri * G.xld;
+      const int64_t ri = G.xidx ? G.xidx[tid] : tid;
+      xptr_s[tid] = base + ri * G.xld;
     } else {
-      erow = static_cast<const __nv_bfloat16*>(G.embed) + static_cast<size_t>(G.tokens[m]) * K;
-    }
-  };
-  auto x_pair = [&](const float* xrow, const __nv_bfloat16* erow, int k) -> float2 {
-    if (xrow) return *reinterpret_cast<const float2*>(xrow + k);
-    return bf16x2_to_f32x2(*reinterpret_cast<const uint32_t*>(erow + k));
-  };
-
-  if (normed) {  // RMSNorm: y = x / sqrt(mean(x^2) + eps) * g; 1/rms is applied to the results
-    for (int m = warp; m < M; m += kConsumerWarps) {
-      const float* xrow;
-      const __nv_bfloat16* erow;
-      x_row(m, xrow, erow);
-      float ss = 0.f;
-      for (int k = lane * 2; k < K; k += 64) {
-        const float2 v = x_pair(xrow, erow, k);
-        ss = fmaf(v.x, v.x, ss);
-        ss = fmaf(v.y, v.y, ss);
-      }
-      ss = warp_sum(ss);
-      if (lane == 0) rstd_s[m] = 1.0f / sqrtf(ss / static_cast<float>(K) + p.eps);
+      xptr_s[tid] = static_cast<const __nv_bfloat16*>(G.embed) + static_cast<size_t>(G.tokens[tid]) * K;
     }
   }
+  ss_part[tid] = 0.f;  // kConsumerWarps * kMmaMaxM == kConsumerThreads
   if (tid < 4) reinterpret_cast<uint32_t*>(bstore + static_cast<size_t>(ncols) * p.bs_stride)[tid] = 0u;
 
   // per-lane ldmatrix address pieces
@@ -187,34 +187,96 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
     const int kp_pairs = (k_end - k_begin) >> 1;
     // ---- split activations of this panel -> B store ---------------------------
     consumer_sync();  // every warp is done with the previous panel's B store
-    for (int m = 0; m < M; ++m) {
-      const float* xrow;
-      const __nv_bfloat16* erow;
-      x_row(m, xrow, erow);
-      uint8_t* col0 = bstore + static_cast<size_t>(m * S) * p.bs_stride;
-      for (int kp = tid; kp < kp_pairs; kp += kConsumerThreads) {
-        const int k = k_begin + 2 * kp;
-        float2 v = x_pair(xrow, erow, k);
-        if (normed) {
-          const float2 g = bf16x2_to_f32x2(*reinterpret_cast<const uint32_t*>(gain + k));
-          v.x *= g.x;
-          v.y *= g.y;
+    {
+      // Item idx = m * K8 + j covers k = k_begin + 8 j .. + 7 of row m: two 16-byte loads of
+      // activations (one of gains), one 16-byte store per split column. The loads of a round are
+      // issued before any is used (one L2 round trip per round of IB items per thread).
+      constexpr int IB = 6;
+      const int K8 = kp_pairs >> 2;
+      const int n_items = M * K8;
+      const bool direct = !x_embed && !G.x_from_dyn && !G.xidx;  // rows of a dense fp32 matrix
+      bool signalled = pn > 0;
+      for (int base = 0; base < n_items; base += kConsumerThreads * IB) {
+        float4 va[IB], vb[IB];
+        uint4 gq[IB];
+        int mi[IB], ji[IB];
+#pragma unroll
+        for (int i = 0; i < IB; ++i) {
+          const int idx = base + i * kConsumerThreads + tid;
+          const bool valid = idx < n_items;
+          const int m = valid ? idx / K8 : M;
+          const int j = idx - m * K8;
+          mi[i] = m;
+          ji[i] = j;
+          va[i] = vb[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+          gq[i] = make_uint4(0u, 0u, 0u, 0u);
+          if (valid) {
+            const int k = k_begin + 8 * j;
+            if (!x_embed) {
+              const float* xr = direct ? G.xsrc + static_cast<int64_t>(m) * G.xld : static_cast<const float*>(xptr_s[m]);
+              va[i] = __ldg(reinterpret_cast<const float4*>(xr + k));
+              vb[i] = __ldg(reinterpret_cast<const float4*>(xr + k + 4));
+            } else {
+              const uint4 e = __ldg(reinterpret_cast<const uint4*>(static_cast<const __nv_bfloat16*>(xptr_s[m]) + k));
+              const float2 e0 = bf16x2_to_f32x2(e.x), e1 = bf16x2_to_f32x2(e.y), e2 = bf16x2_to_f32x2(e.z), e3 = bf16x2_to_f32x2(e.w);
+              va[i] = make_float4(e0.x, e0.y, e1.x, e1.y);
+              vb[i] = make_float4(e2.x, e2.y, e3.x, e3.y);
+            }
+            if (normed) gq[i] = __ldg(reinterpret_cast<const uint4*>(gain + k));
+          }
         }
-        uint32_t h = pack_bf16x2_rn(v.x, v.y);
-        *reinterpret_cast<uint32_t*>(col0 + 4 * kp) = h;
-        float2 r = bf16x2_to_f32x2(h);
-        r.x = v.x - r.x;
-        r.y = v.y - r.y;
-        h = pack_bf16x2_rn(r.x, r.y);
-        *reinterpret_cast<uint32_t*>(col0 + p.bs_stride + 4 * kp) = h;
-        if (S == 3) {
-          const float2 r1 = bf16x2_to_f32x2(h);
-          h = pack_bf16x2_rn(r.x - r1.x, r.y - r1.y);
-          *reinterpret_cast<uint32_t*>(col0 + 2 * p.bs_stride + 4 * kp) = h;
+        if (!signalled) {  // loads are in flight: let the producers fill the ring
+          __syncwarp();
+          if (lane == 0) mbar_arrive(xbar);
+          signalled = true;
         }
+#pragma unroll
+        for (int i = 0; i < IB; ++i) {
+          float x[8] = {va[i].x, va[i].y, va[i].z, va[i].w, vb[i].x, vb[i].y, vb[i].z, vb[i].w};
+          const int m = mi[i];
+          if (normed) {
+            float ssq = 0.f;
+#pragma unroll
+            for (int e = 0; e < 8; ++e) ssq = fmaf(x[e], x[e], ssq);
+            // segmented sum over the rows present in this warp's 32 items (usually one)
+            const int m_lo = __shfl_sync(0xffffffffu, m, 0), m_hi = min(__shfl_sync(0xffffffffu, m, 31), M - 1);
+            for (int mm = m_lo; mm <= m_hi; ++mm) {
+              const float t = warp_sum(m == mm ? ssq : 0.f);
+              if (lane == 0) ss_part[warp * kMmaMaxM + mm] += t;
+            }
+            const uint32_t gwv[4] = {gq[i].x, gq[i].y, gq[i].z, gq[i].w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const float2 g = bf16x2_to_f32x2(gwv[e]);
+              x[2 * e] *= g.x;
+              x[2 * e + 1] *= g.y;
+            }
+          }
+          if (m < M) {
+            uint32_t h0[4], h1[4], h2[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              h0[e] = pack_bf16x2_rn(x[2 * e], x[2 * e + 1]);
+              const float2 f0 = bf16x2_to_f32x2(h0[e]);
+              const float rx = x[2 * e] - f0.x, ry = x[2 * e + 1] - f0.y;
+              h1[e] = pack_bf16x2_rn(rx, ry);
+              const float2 f1 = bf16x2_to_f32x2(h1[e]);
+              h2[e] = pack_bf16x2_rn(rx - f1.x, ry - f1.y);
+            }
+            uint8_t* col0 = bstore + static_cast<size_t>(m * S) * p.bs_stride + 16 * ji[i];
+            *reinterpret_cast<uint4*>(col0) = make_uint4(h0[0], h0[1], h0[2], h0[3]);
+            *reinterpret_cast<uint4*>(col0 + p.bs_stride) = make_uint4(h1[0], h1[1], h1[2], h1[3]);
+            if (S == 3) *reinterpret_cast<uint4*>(col0 + 2 * p.bs_stride) = make_uint4(h2[0], h2[1], h2[2], h2[3]);
+          }
+        }
+      }
+      if (!signalled) {
+        __syncwarp();
+        if (lane == 0) mbar_arrive(xbar);
       }
     }
     consumer_sync();
+    if (pn == 0) DVT_STAMP(2);
 
     for (int sb = 0; sb < n_sb; ++sb) {
       const int v0 = sb * RS, nr = min(RS, rr.cnt - v0);
@@ -230,6 +292,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       for (int k0 = k_begin; k0 < k_end; k0 += KC) {
         const int n_units = min(KC, k_end - k0) >> 5;  // 32 k per unit
         mbar_wait(&full[slot], round & 1);
+        if (round == 0 && slot == 0) DVT_STAMP(3);
         const uint32_t sbase = ring_u + static_cast<uint32_t>(slot) * p.stage_bytes + a_lane;
         for (int u = warp; u < n_units; u += kConsumerWarps) {
           uint32_t b[NT][4];
@@ -290,9 +353,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
     }
   }
 
+  DVT_STAMP(4);
   // ---- fused epilogue over the CTA's results: res[v * M + m] ---------------------
   const int nres = rr.cnt * M;
-  if (normed) {
+  if (normed) {  // RMSNorm: y = x / sqrt(mean(x^2) + eps) * g; 1/rms is applied to the results
+    if (tid < M) {
+      float t = 0.f;
+      for (int w = 0; w < kConsumerWarps; ++w) t += ss_part[w * kMmaMaxM + tid];
+      rstd_s[tid] = 1.0f / sqrtf(t / static_cast<float>(K) + p.eps);
+    }
+    consumer_sync();
     for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rstd_s[idx % M];
     consumer_sync();
   }
@@ -360,6 +430,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       }
     }
   }
+  DVT_STAMP(5);
 }
 
 }  // namespace dvt
