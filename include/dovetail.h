@@ -218,6 +218,23 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree,
  * Borrowed until replaced. */
 int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat);
 
+/* Optional teacher forcing for parity tests; all pointers NULL (the default) disables it.
+ * A draft step feeds every level with the previous levels' results (the parent's output
+ * hidden state, and the ancestors' K/V rows), so a rounding-level difference
+ * at level 0 is amplified level by level (x3 per level on the 13B-shaped random-weight
+ * model) and an element-wise comparison of deep rows would measure that amplification,
+ * not the arithmetic. With forcing, after every level the step
+ *   1. copies the K/V rows it has just computed for that level into tap_k / tap_v
+ *      (the hhat tap of dovetail_draft_set_taps is likewise taken per level), then
+ *   2. overwrites those cache rows with the rows of force_k / force_v and the level's
+ *      rows of its hidden-state buffer with the rows of force_hhat,
+ * so that each level is computed from the caller's (the oracle's) state.
+ *   force_hhat     : dev fp32 [rows of the step, d], step-row order (as the hhat tap)
+ *   force_k/v, tap_k/v : dev, same dtype, layout and capacity as the KV cache of the step
+ * Borrowed until replaced. The copies serialise the stream between levels. */
+int dovetail_draft_set_forcing(dovetail_draft_t* h, const float* force_hhat, const void* force_k,
+                               const void* force_v, void* tap_k, void* tap_v);
+
 /* Optional per-kernel timing, for the roofline report (off by default). When
  * enabled, dovetail_draft_step brackets every kernel launch with CUDA events on
  * cuda_stream (this serialises the launches: programmatic dependent launch

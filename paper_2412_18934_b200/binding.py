@@ -17,7 +17,7 @@ MAX_DEPTH, MAX_LAYERS = 16, 16
 OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "dovetail_tree_replay",
-           "dovetail_draft_set_taps", "dovetail_draft_set_profile", "dovetail_profile_read",
+           "dovetail_draft_set_taps", "dovetail_draft_set_forcing", "dovetail_draft_set_profile", "dovetail_profile_read",
            "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 
@@ -86,6 +86,8 @@ def load() -> C.CDLL:
                                              C.c_int32, C.POINTER(DraftOutT)] + [C.c_void_p] * 6
         lib.dovetail_draft_set_taps.restype = C.c_int
         lib.dovetail_draft_set_taps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.dovetail_draft_set_forcing.restype = C.c_int
+        lib.dovetail_draft_set_forcing.argtypes = [C.c_void_p] + [C.c_void_p] * 5
         lib.dovetail_draft_set_profile.restype = C.c_int
         lib.dovetail_draft_set_profile.argtypes = [C.c_void_p, C.c_int32]
         lib.dovetail_profile_read.restype = C.c_int
@@ -245,6 +247,13 @@ def dovetail_tree_replay(h: Draft, tree: TreeSpec, cand_tokens, cand_logp, out: 
 def dovetail_draft_set_taps(h: Draft, logits=None, hhat=None):
     h.taps = (logits, hhat)
     _check(load().dovetail_draft_set_taps(h.ptr, _dp(logits), _dp(hhat)), h.ptr)
+
+
+def dovetail_draft_set_forcing(h: Draft, force_hhat=None, force_k=None, force_v=None, tap_k=None, tap_v=None):
+    """Teacher forcing for parity tests (include/dovetail.h); all None disables it."""
+    h.forcing = (force_hhat, force_k, force_v, tap_k, tap_v)  # keep the tensors alive
+    _check(load().dovetail_draft_set_forcing(h.ptr, _dp(force_hhat), _dp(force_k), _dp(force_v), _dp(tap_k), _dp(tap_v)),
+           h.ptr)
 
 
 N_KINDS = 11

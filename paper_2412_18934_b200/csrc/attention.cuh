@@ -20,6 +20,12 @@
 
 namespace dvt {
 
+#ifdef DVT_TRACE  // microbenchmark builds only
+#define DVT_ASTAMP(i) do { if (threadIdx.x == 0 && p.trace) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 8 + (i)] = t_; } } while (0)
+#else
+#define DVT_ASTAMP(i) do { } while (0)
+#endif
+
 constexpr int kAttnStagePos = 32;  // positions per ring stage
 
 struct AttnParams {
@@ -37,6 +43,7 @@ struct AttnParams {
   float* ws;               // partials [Hkv][n_chunks][qv_cap][dh + 2]
   int32_t qv_cap;
   int32_t* counters;       // [Hkv], zero between launches
+  unsigned long long* trace;  // DVT_TRACE builds only
 };
 
 struct SoftState {  // running (max, sum) of one query vector
@@ -113,10 +120,12 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     }
     mbar_fence_init();
   }
+  DVT_ASTAMP(0);
   __syncthreads();
   pdl_launch_dependents();
   pdl_wait();  // q/k/v of this level and the step's dynamic state are visible
 
+  DVT_ASTAMP(1);
   const StepDyn* dyn = p.dyn;
   const int Lbase = p.level0 ? dyn->L : dyn->Lp;
   const int cap = dyn->capacity;
@@ -177,6 +186,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     }
     __threadfence_block();
     consumer_sync();
+    DVT_ASTAMP(2);
   }
 
   for (int qt = 0; qt < n_qt; ++qt) {
@@ -204,6 +214,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
         for (int e = 0; e < EPU; ++e) q[t][e] = 0.f;
       }
     }
+    DVT_ASTAMP(3);
     float mrun[QT], lrun[QT], o[QT][EPU];
 #pragma unroll
     for (int t = 0; t < QT; ++t) {
@@ -260,6 +271,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       if (lane == 0) mbar_arrive(&empty[slot]);
     }
 
+    DVT_ASTAMP(4);
     // ---- the new region: earlier rows of this step, masked per row ------------
     if (c == 0) {
       for (int j0 = 0; j0 < p.new_cnt; j0 += NG) {
@@ -287,6 +299,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       }
     }
 
+    DVT_ASTAMP(5);
     // ---- merge the row groups of the warp, then the warps ---------------------
 #pragma unroll
     for (int t = 0; t < QT; ++t) {
@@ -332,6 +345,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     consumer_sync();  // wsm is reused by the next query tile
   }
 
+  DVT_ASTAMP(6);
   if (n_chunks > 1) {
     // the last CTA of this kv-head to arrive merges all chunks in chunk order
     __threadfence();
@@ -363,6 +377,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       if (tid == 0) p.counters[hk] = 0;
     }
   }
+  DVT_ASTAMP(7);
 }
 
 }  // namespace dvt

@@ -68,6 +68,12 @@ struct dovetail_draft {
   // taps (borrowed)
   float* tap_logits = nullptr;
   float* tap_hhat = nullptr;
+  // teacher forcing for parity tests (borrowed)
+  const float* force_hhat = nullptr;
+  const void* force_k = nullptr;
+  const void* force_v = nullptr;
+  void* tap_k = nullptr;
+  void* tap_v = nullptr;
   // last step
   bool have_step = false;
   int last_n_new = 0, last_depth = 0, last_gamma = 0;
@@ -730,11 +736,26 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
       e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
       if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
     }
-  }
-  if (h->tap_hhat) {
-    e = cudaMemcpyAsync(h->tap_hhat, h->hhat, static_cast<size_t>(n_new + tree_rows) * d * sizeof(float),
-                        cudaMemcpyDeviceToDevice, st);
-    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap copy failed: %s", cudaGetErrorString(e));
+    // parity-test hooks: taps of this level's results, then teacher forcing (dovetail.h)
+    e = cudaSuccess;
+    const size_t xoff = static_cast<size_t>(lp.row0) * d, xbytes = static_cast<size_t>(M) * d * sizeof(float);
+    if (h->tap_hhat) e = cudaMemcpyAsync(h->tap_hhat + xoff, h->hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
+    if (h->force_hhat && e == cudaSuccess)
+      e = cudaMemcpyAsync(h->hhat + xoff, h->force_hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
+    {
+      const size_t pitch = static_cast<size_t>(kv->capacity) * dh * h->es, width = static_cast<size_t>(M) * dh * h->es;
+      const size_t off = static_cast<size_t>(l == 0 ? L : Lp + lp.t0) * dh * h->es, height = static_cast<size_t>(c.n_layers) * c.n_kv_heads;
+      auto cp2 = [&](void* dst, const void* src) {
+        if (dst && src && e == cudaSuccess)
+          e = cudaMemcpy2DAsync(static_cast<uint8_t*>(dst) + off, pitch, static_cast<const uint8_t*>(src) + off, pitch, width, height,
+                                cudaMemcpyDeviceToDevice, st);
+      };
+      cp2(h->tap_k, kv->k);
+      cp2(h->tap_v, kv->v);
+      cp2(kv->k, h->force_k);
+      cp2(kv->v, h->force_v);
+    }
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap / forcing copy failed: %s", cudaGetErrorString(e));
   }
   e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
@@ -857,6 +878,17 @@ int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat) {
   if (!h) return DOVETAIL_EINVAL;
   h->tap_logits = logits;
   h->tap_hhat = hhat;
+  return DOVETAIL_OK;
+}
+
+int dovetail_draft_set_forcing(dovetail_draft_t* h, const float* force_hhat, const void* force_k, const void* force_v,
+                               void* tap_k, void* tap_v) {
+  if (!h) return DOVETAIL_EINVAL;
+  h->force_hhat = force_hhat;
+  h->force_k = force_k;
+  h->force_v = force_v;
+  h->tap_k = tap_k;
+  h->tap_v = tap_v;
   return DOVETAIL_OK;
 }
 

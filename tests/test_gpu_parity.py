@@ -31,11 +31,19 @@ def _boost(case, lm=40.0, emb=20.0):
 
 
 def _run(case, **kw):
-    h, kv, gpu = run_gpu(case, **kw)
+    """Free-running step (discrete outputs, level-0 values) and teacher-forced step (every row, element by
+    element) against the oracle."""
     ora = run_oracle(case)
+    h, kv, free = run_gpu(case, **kw)
+    s_free = compare(case, free, ora)
+    binding.dovetail_draft_destroy(h)
+    h, kv, gpu = run_gpu(case, force=ora, **kw)
     s = compare(case, gpu, ora)
+    s["free_same_tree"] = s_free["same_tree"]
+    s["free_deep_rows_logit_viol"] = s_free.get("deep_rows_logit_viol")
     print({k: (f"{v:.3e}" if isinstance(v, float) else v) for k, v in s.items()})
     binding.dovetail_draft_destroy(h)
+    s["same_tree"] = s["same_tree"] and s_free["same_tree"]
     return s, gpu, ora
 
 
