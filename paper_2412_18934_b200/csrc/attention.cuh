@@ -43,6 +43,11 @@ struct AttnParams {
   float* ws;               // partials [Hkv][n_chunks][qv_cap][dh + 2]
   int32_t qv_cap;
   int32_t* counters;       // [Hkv], zero between launches
+  // k_tree_attention_mma: the cache of this step as launch arguments, so that the producers can
+  // stream the prefix before griddepcontrol.wait (the prefix does not depend on this level)
+  const void* kc;
+  const void* vc;
+  int32_t cap, Lbase;
   unsigned long long* trace;  // DVT_TRACE builds only
 };
 

@@ -1,0 +1,489 @@
+// attention_mma.cuh -- tensor-core tree attention for bf16 caches (S2 append + S3,
+// PAPER.md:94): same contract as k_tree_attention (attention.cuh), same grid
+// (n_chunks, Hkv), same partial / merge protocol, but the per-position work runs on
+// mma.sync.m16n8k16 the way flash-decoding kernels do:
+//
+//   S = Q K^T : A = 16 query vectors (rows of the level x q-heads of the GQA group,
+//               zero padded) x head_dim, B = K rows as stored ([position][d] is the
+//               "col" operand as it is);
+//   O += P V  : A = P (the S accumulators re-used as the A fragment), B = V rows
+//               through ldmatrix.trans.
+// Neither the fp32 queries nor the probabilities are rounded to bf16: both are split
+// into a bf16 head and a bf16 remainder (two mma per tile, 16 mantissa bits), the
+// softmax statistics and the accumulators are fp32.
+//
+// CTA = 4 consumer warps + 2 producer warps, <= 2 CTAs per SM. The producers copy
+// blocks of 64 positions (K and V rows, 16-byte cp.async with an XOR swizzle of the
+// 16-byte chunk index by position & 7, which makes every ldmatrix conflict free; a
+// 1-D bulk copy cannot swizzle) into a 3-deep ring signalled by mbarriers; each
+// consumer warp owns one 16-position tile of every block and its own online-softmax
+// state; warps, then chunks, are merged in fixed order (deterministic).
+#pragma once
+#include <cuda_bf16.h>
+
+#include "attention.cuh"
+#include "gemv_mma.cuh"
+#include "ptx.cuh"
+#include "state.cuh"
+
+namespace dvt {
+
+constexpr int kAmWarps = 4;                       // consumer warps
+constexpr int kAmConsumers = kAmWarps * 32;       // 128
+constexpr int kAmProducers = 64;                  // two producer warps
+constexpr int kAmThreads = kAmConsumers + kAmProducers;
+constexpr int kAmBlockPos = 64;                   // positions per ring block
+constexpr int kAmStages = 3;
+constexpr int kAmQRows = 16;                      // query vectors per pass
+
+__device__ __forceinline__ void am_consumer_sync() {
+  asm volatile("bar.sync 2, %0;" ::"n"(kAmConsumers) : "memory");
+}
+
+__device__ __forceinline__ void ldsm_x4_trans(uint32_t (&r)[4], uint32_t addr) {
+  asm volatile("ldmatrix.sync.aligned.m8n8.x4.trans.shared.b16 {%0, %1, %2, %3}, [%4];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+               : "r"(addr)
+               : "memory");
+}
+
+// 16-byte async copy global -> shared; src_bytes = 0 writes zeros without reading.
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+}
+// arrives on the mbarrier once all prior cp.async of this thread have landed
+__device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// ---- thread-block cluster: the chunks of one kv-head merge through distributed shared memory
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+  return r;
+}
+// all threads of all CTAs of the cluster; release / acquire over shared::cluster
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ float ld_dsmem_f32(uint32_t local_addr, uint32_t rank) {
+  uint32_t ra;
+  float v;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(local_addr), "r"(rank));
+  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(ra) : "memory");
+  return v;
+}
+
+// byte offset of 16-byte chunk `ch` of row `r` in a swizzled [rows][ROWB] tile
+template <int ROWB>
+__device__ __forceinline__ uint32_t am_swz(int r, int ch) {
+  return static_cast<uint32_t>(r) * ROWB + static_cast<uint32_t>((ch ^ (r & 7)) << 4);
+}
+
+constexpr size_t am_smem_bytes(int DH) {
+  // q hi + lo tiles, ring of (K, V) blocks (the merge scratch aliases it), barriers
+  return static_cast<size_t>(2 * kAmQRows * DH * 2) + static_cast<size_t>(kAmStages) * 2 * kAmBlockPos * DH * 2 + 128;
+}
+
+template <int DH>
+__global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const AttnParams p) {
+  using WT = __nv_bfloat16;
+  constexpr int ROWB = DH * 2;            // bytes of one K (or V) row
+  constexpr int CPR = ROWB / 16;          // 16-byte chunks per row
+  constexpr int KS = DH / 16;             // k-steps of S = Q K^T
+  constexpr int DN = DH / 8;              // 8-wide d tiles of O
+  constexpr int PB = kAmBlockPos;
+  constexpr int BLK_BYTES = 2 * PB * ROWB;
+  constexpr int HALF = DH / 2;
+  constexpr int WSTR = DH + 2;            // partial record: o[DH], m, l
+  extern __shared__ __align__(128) uint8_t smem[];
+  uint8_t* q_hi = smem;                   // [16][ROWB] swizzled bf16 heads of the rotated, scaled queries
+  uint8_t* q_lo = q_hi + kAmQRows * ROWB; // remainders
+  uint8_t* ring = q_lo + kAmQRows * ROWB;
+  uint64_t* full = reinterpret_cast<uint64_t*>(ring + kAmStages * BLK_BYTES);
+  uint64_t* empty = full + 4;
+  uint64_t* tailbar = empty + 4;
+  int* flag_s = reinterpret_cast<int*>(tailbar + 1);
+  // The warp-merge scratch and this CTA's record alias the ring: when they are written every block of
+  // the pass has been consumed, and the producers resume only after the pass's second cluster barrier.
+  float* wsm = reinterpret_cast<float*>(ring);  // [warps][QR][WSTR]
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int c = blockIdx.x, hk = blockIdx.y, n_chunks = gridDim.x;
+  const int grp = p.Hq / p.Hkv;
+  const int qv_tot = p.M * grp;
+  const int n_pass = (qv_tot + kAmQRows - 1) / kAmQRows;
+  const int QR = min(kAmQRows, qv_tot);  // rows of the warp-merge scratch
+  float* crec = wsm + static_cast<size_t>(kAmWarps) * QR * WSTR;  // [QR][WSTR] this CTA's record, read by the cluster leader
+  // chunks [group * CS, (group + 1) * CS) of a kv-head form a cluster (CS = 1 without the launch attribute)
+  const int CS = static_cast<int>(cluster_nctarank()), crank = static_cast<int>(cluster_ctarank());
+  const int n_groups = n_chunks / CS, group = c / CS;
+  const int dq = p.Hq * DH, dkv = p.Hkv * DH, ldq = dq + 2 * dkv;
+
+  if (tid == 0) {
+    for (int s = 0; s < kAmStages; ++s) {
+      mbar_init(&full[s], kAmProducers);
+      mbar_init(&empty[s], kAmWarps);
+    }
+    mbar_init(tailbar, kAmConsumers);
+    mbar_fence_init();
+  }
+  DVT_ASTAMP(0);
+  __syncthreads();
+  pdl_launch_dependents();
+
+  const int Lbase = p.Lbase, cap = p.cap;
+  const WT* kc = static_cast<const WT*>(p.kc) + (static_cast<size_t>(p.layer) * p.Hkv + hk) * cap * DH;
+  const WT* vc = static_cast<const WT*>(p.vc) + (static_cast<size_t>(p.layer) * p.Hkv + hk) * cap * DH;
+  int pch = (Lbase + n_chunks - 1) / n_chunks;
+  pch = (pch + PB - 1) / PB * PB;
+  const int p_begin = min(Lbase, c * pch), p_end = min(Lbase, p_begin + pch);
+  const int n_blk = (p_end - p_begin + PB - 1) / PB;
+  const int n_tail = c == 0 ? (p.new_cnt + PB - 1) / PB : 0;  // the new region, chunk 0 only
+  const int nb = n_blk + n_tail;
+
+  if (warp >= kAmWarps) {
+    // ---------------- producers ---------------------------------------------------
+    const int ptid = tid - kAmConsumers;
+    int slot = 0, round = 0;
+    bool tail_ready = false;
+    for (int pass = 0; pass < n_pass; ++pass) {
+      for (int b = 0; b < nb; ++b) {
+        int pos0, cnt;
+        if (b < n_blk) {
+          pos0 = p_begin + b * PB;
+          cnt = min(PB, p_end - pos0);
+        } else {
+          if (!tail_ready) {  // this level's rows are appended by the consumers first
+            mbar_wait(tailbar, 0);
+            tail_ready = true;
+          }
+          pos0 = Lbase + (b - n_blk) * PB;
+          cnt = min(PB, p.new_cnt - (b - n_blk) * PB);
+        }
+        if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+        const uint32_t kdst = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vdst = kdst + PB * ROWB;
+        const uint8_t* ksrc = reinterpret_cast<const uint8_t*>(kc + static_cast<size_t>(pos0) * DH);
+        const uint8_t* vsrc = reinterpret_cast<const uint8_t*>(vc + static_cast<size_t>(pos0) * DH);
+#pragma unroll 4
+        for (int i = ptid; i < PB * CPR; i += kAmProducers) {
+          const int r = i / CPR, ch = i % CPR;
+          const bool valid = r < cnt;  // rows past the end are zero filled (0 * stale NaN would poison P V)
+          const size_t so = valid ? static_cast<size_t>(r) * ROWB + ch * 16 : 0;
+          const uint32_t d = am_swz<ROWB>(r, ch);
+          cp_async16(kdst + d, ksrc + so, valid ? 16u : 0u);
+          cp_async16(vdst + d, vsrc + so, valid ? 16u : 0u);
+        }
+        cp_async_arrive(&full[slot]);
+        if (++slot == kAmStages) { slot = 0; ++round; }
+      }
+      cluster_sync_all();  // the two cluster barriers of the pass (see the consumers)
+      cluster_sync_all();
+    }
+    return;
+  }
+
+  // ---------------- consumers -----------------------------------------------------
+  pdl_wait();  // q/k/v of this level and the row tables are visible from here on
+  DVT_ASTAMP(1);
+  const RowTables* rows = p.rows;
+  const int g = lane >> 2, tq = lane & 3;
+  const float scale = 1.0f / sqrtf(static_cast<float>(DH));
+
+  // S2: append this level's K/V rows of kv-head hk (chunk 0 only). K is rotated (half-split
+  // pairing (i, i + dh/2), reading A3) and both are rounded to the cache dtype, as the oracle
+  // stores them; the new region is then attended from the cache like the prefix.
+  if (c == 0) {
+    WT* kcw = const_cast<WT*>(kc);
+    WT* vcw = const_cast<WT*>(vc);
+    for (int idx = tid; idx < p.M * HALF; idx += kAmConsumers) {
+      const int m = idx / HALF, i = idx % HALF;
+      const float* kr = p.qkv + static_cast<size_t>(m) * ldq + dq + hk * DH;
+      const float2 cs = p.rope[static_cast<size_t>(p.rope_row0 + (p.rope_per_row ? m : 0)) * HALF + i];
+      const float a = kr[i], b = kr[i + HALF];
+      WT* dst = kcw + static_cast<size_t>(Lbase + rows->slot[m]) * DH;
+      store_cache(dst + i, a * cs.x - b * cs.y);
+      store_cache(dst + i + HALF, b * cs.x + a * cs.y);
+    }
+    for (int idx = tid; idx < p.M * DH; idx += kAmConsumers) {
+      const int m = idx / DH, i = idx % DH;
+      const float* vr = p.qkv + static_cast<size_t>(m) * ldq + dq + dkv + hk * DH;
+      store_cache(vcw + static_cast<size_t>(Lbase + rows->slot[m]) * DH + i, vr[i]);
+    }
+    __threadfence();
+    mbar_arrive(tailbar);
+    DVT_ASTAMP(2);
+  }
+
+  int slot = 0, round = 0;
+  for (int pass = 0; pass < n_pass; ++pass) {
+    const int qv0 = pass * kAmQRows;
+    const int nq = min(kAmQRows, qv_tot - qv0);  // query vectors of this pass
+    // ---- rotated, scaled queries -> bf16 head + remainder tiles ------------------
+    for (int idx = tid; idx < kAmQRows * HALF; idx += kAmConsumers) {
+      const int r = idx / HALF, i = idx % HALF;
+      float x0 = 0.f, x1 = 0.f;
+      if (r < nq) {
+        const int qv = qv0 + r, m = qv / grp, hq = hk * grp + qv % grp;
+        const float* qr = p.qkv + static_cast<size_t>(m) * ldq + hq * DH;
+        const float2 cs = p.rope[static_cast<size_t>(p.rope_row0 + (p.rope_per_row ? m : 0)) * HALF + i];
+        const float a = qr[i], b = qr[i + HALF];
+        x0 = (a * cs.x - b * cs.y) * scale;
+        x1 = (b * cs.x + a * cs.y) * scale;
+      }
+      const float xs[2] = {x0, x1};
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const int d = i + h * HALF;
+        const uint32_t off = am_swz<ROWB>(r, d >> 3) + (d & 7) * 2;
+        const uint16_t hi = f32_to_bf16_rn(xs[h]);
+        const float rem = xs[h] - __uint_as_float(static_cast<uint32_t>(hi) << 16);
+        *reinterpret_cast<uint16_t*>(q_hi + off) = hi;
+        *reinterpret_cast<uint16_t*>(q_lo + off) = f32_to_bf16_rn(rem);
+      }
+    }
+    am_consumer_sync();
+    DVT_ASTAMP(3);
+
+    // rows of this thread's accumulators: g and g + 8; their draft rows for the tail masks
+    int mrow[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int r = g + 8 * h;
+      mrow[h] = r < nq ? (qv0 + r) / grp : -1;
+    }
+    float mrun[2] = {-INFINITY, -INFINITY}, lrun[2] = {0.f, 0.f};
+    float o[DN][4];
+#pragma unroll
+    for (int t = 0; t < DN; ++t)
+#pragma unroll
+      for (int e = 0; e < 4; ++e) o[t][e] = 0.f;
+
+    // per-lane ldmatrix row / chunk pieces
+    const int a_row = (lane & 7) + ((lane >> 3) & 1) * 8, a_ch = lane >> 4;          // A: q tiles
+    const int k_row = (lane & 7) + (lane >> 4) * 8, k_ch = (lane >> 3) & 1;          // B of S: K rows
+    const int v_row = (lane & 7) + ((lane >> 3) & 1) * 8, v_ch = lane >> 4;          // B of PV: V rows (.trans)
+
+    for (int b = 0; b < nb; ++b) {
+      const bool tail = b >= n_blk;
+      const int cnt = tail ? min(PB, p.new_cnt - (b - n_blk) * PB) : min(PB, p_end - (p_begin + b * PB));
+      mbar_wait(&full[slot], round & 1);
+      const int t0 = warp * 16;  // this warp's tile of the block
+      if (t0 < cnt) {
+        const uint32_t kb = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vb = kb + PB * ROWB;
+        float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+#pragma unroll
+        for (int ks = 0; ks < KS; ++ks) {
+          uint32_t ah[4], al[4], kf[4];
+          ldsm_x4(ah, smem_u32(q_hi) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
+          ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
+          ldsm_x4(kf, kb + am_swz<ROWB>(t0 + k_row, ks * 2 + k_ch));
+          mma_bf16_16816(s[0], ah, kf[0], kf[1]);
+          mma_bf16_16816(s[0], al, kf[0], kf[1]);
+          mma_bf16_16816(s[1], ah, kf[2], kf[3]);
+          mma_bf16_16816(s[1], al, kf[2], kf[3]);
+        }
+        // masks: positions past the block's end, padded query rows, and (new region) the
+        // ancestor mask of the row
+        float mx[2] = {-INFINITY, -INFINITY};
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int h = e >> 1, pos = t0 + nt * 8 + 2 * tq + (e & 1);
+            bool ok = pos < cnt && mrow[h] >= 0;
+            if (ok && tail) {
+              const int j = (b - n_blk) * PB + pos;
+              ok = (rows->mask[mrow[h]][j >> 5] >> (j & 31)) & 1u;
+            }
+            s[nt][e] = ok ? s[nt][e] : -INFINITY;
+            mx[h] = fmaxf(mx[h], s[nt][e]);
+          }
+        float corr[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
+          mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
+          const float mn = fmaxf(mrun[h], mx[h]);
+          corr[h] = (mrun[h] == -INFINITY) ? 0.f : expf(mrun[h] - mn);
+          mrun[h] = mn;
+          lrun[h] *= corr[h];
+        }
+        uint32_t ph[4], pl[4];  // P as the A fragment of P V: head and remainder
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const float p0 = (s[nt][2 * h] == -INFINITY) ? 0.f : expf(s[nt][2 * h] - mrun[h]);
+            const float p1 = (s[nt][2 * h + 1] == -INFINITY) ? 0.f : expf(s[nt][2 * h + 1] - mrun[h]);
+            lrun[h] += p0 + p1;
+            const uint32_t hi = pack_bf16x2_rn(p0, p1);
+            const float2 hf = bf16x2_to_f32x2(hi);
+            ph[nt * 2 + h] = hi;
+            pl[nt * 2 + h] = pack_bf16x2_rn(p0 - hf.x, p1 - hf.y);
+          }
+#pragma unroll
+        for (int t = 0; t < DN; ++t) {
+          o[t][0] *= corr[0];
+          o[t][1] *= corr[0];
+          o[t][2] *= corr[1];
+          o[t][3] *= corr[1];
+        }
+#pragma unroll
+        for (int t = 0; t < DN; t += 2) {
+          uint32_t vf[4];
+          ldsm_x4_trans(vf, vb + am_swz<ROWB>(t0 + v_row, t + v_ch));
+          mma_bf16_16816(o[t], ph, vf[0], vf[1]);
+          mma_bf16_16816(o[t], pl, vf[0], vf[1]);
+          mma_bf16_16816(o[t + 1], ph, vf[2], vf[3]);
+          mma_bf16_16816(o[t + 1], pl, vf[2], vf[3]);
+        }
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[slot]);
+      if (++slot == kAmStages) { slot = 0; ++round; }
+    }
+    DVT_ASTAMP(5);
+    am_consumer_sync();  // every warp is done with the ring: the merge scratch aliases it
+
+    // ---- merge the four warps (fixed order), then hand the chunk's partial on ------
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 1);
+      lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 2);
+      const int r = g + 8 * h;
+      if (r < nq) {
+        float* w = wsm + (static_cast<size_t>(warp) * QR + r) * WSTR;
+#pragma unroll
+        for (int t = 0; t < DN; ++t)
+          *reinterpret_cast<float2*>(w + t * 8 + 2 * tq) = make_float2(o[t][2 * h], o[t][2 * h + 1]);
+        if (tq == 0) { w[DH] = mrun[h]; w[DH + 1] = lrun[h]; }
+      }
+    }
+    am_consumer_sync();
+    for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
+      const int r = idx / DH, dd = idx % DH;
+      const int qv = qv0 + r;
+      float mm = -INFINITY;
+      for (int w = 0; w < kAmWarps; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
+      float ll = 0.f, oo = 0.f;
+      for (int w = 0; w < kAmWarps; ++w) {
+        const float* rr = wsm + (w * QR + r) * WSTR;
+        const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
+        ll += rr[DH + 1] * cw;
+        oo += rr[dd] * cw;
+      }
+      float* rr = crec + static_cast<size_t>(r) * WSTR;
+      rr[dd] = oo;
+      if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
+    }
+    // ---- merge the chunks of the cluster in rank order through distributed shared memory ----
+    cluster_sync_all();  // every CTA's record is complete and visible cluster-wide
+    if (crank == 0) {
+      const uint32_t crec_u = smem_u32(crec);
+      for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
+        const int r = idx / DH, dd = idx % DH;
+        const int qv = qv0 + r;
+        const uint32_t ra = crec_u + static_cast<uint32_t>(r * WSTR) * 4;
+        float mk[8], lk[8], ok[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          mk[k] = -INFINITY;
+          lk[k] = 0.f;
+          ok[k] = 0.f;
+          if (k < CS) {
+            mk[k] = ld_dsmem_f32(ra + DH * 4, k);
+            lk[k] = ld_dsmem_f32(ra + (DH + 1) * 4, k);
+            ok[k] = ld_dsmem_f32(ra + dd * 4, k);
+          }
+        }
+        float mm = -INFINITY;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) mm = fmaxf(mm, mk[k]);
+        float ll = 0.f, oo = 0.f;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          const float cw = (mk[k] == -INFINITY) ? 0.f : expf(mk[k] - mm);
+          ll += lk[k] * cw;
+          oo += ok[k] * cw;
+        }
+        if (n_groups == 1) {
+          const int m = qv / grp, hq = hk * grp + qv % grp;
+          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+        } else {
+          float* rr = p.ws + ((static_cast<size_t>(hk) * n_groups + group) * p.qv_cap + qv) * WSTR;
+          rr[dd] = oo;
+          if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
+        }
+      }
+    }
+    cluster_sync_all();  // the leader has read the records: they (and the query tiles) may be reused
+  }
+  DVT_ASTAMP(6);
+
+  if (n_groups > 1 && crank == 0) {
+    // the last cluster leader of this kv-head to arrive merges all groups in group order
+    __threadfence();
+    am_consumer_sync();
+    if (tid == 0) {
+      const int old = atomicAdd(&p.counters[hk], 1);
+      *flag_s = (old == n_groups - 1);
+    }
+    am_consumer_sync();
+    if (*flag_s) {
+      __threadfence();
+      // All blocks have been consumed, so the ring is free: the partial records are staged through
+      // it with independent loads (one L2 round trip) instead of a chain of dependent ones.
+      float* stg = reinterpret_cast<float*>(ring);
+      const int rec = n_groups * WSTR;                       // floats of one query vector's records
+      const int G = max(1, (kAmStages * BLK_BYTES / 4) / rec);  // query vectors per group
+      for (int q0 = 0; q0 < qv_tot; q0 += G) {
+        const int gq = min(G, qv_tot - q0);
+        const int n_el = gq * rec;
+        for (int base = 0; base < n_el; base += kAmConsumers * 8) {
+          float v[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int e = base + i * kAmConsumers + tid;
+            v[i] = 0.f;
+            if (e < n_el) {
+              const int q = e / rec, rem = e - q * rec, cc = rem / WSTR, w = rem - cc * WSTR;
+              v[i] = __ldcg(p.ws + ((static_cast<size_t>(hk) * n_groups + cc) * p.qv_cap + q0 + q) * WSTR + w);
+            }
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int e = base + i * kAmConsumers + tid;
+            if (e < n_el) stg[e] = v[i];
+          }
+        }
+        am_consumer_sync();
+        for (int idx = tid; idx < gq * DH; idx += kAmConsumers) {
+          const int q = idx / DH, dd = idx % DH, qv = q0 + q;
+          const float* base = stg + q * rec;
+          float mm = -INFINITY;
+          for (int cc = 0; cc < n_groups; ++cc) mm = fmaxf(mm, base[cc * WSTR + DH]);
+          float ll = 0.f, oo = 0.f;
+          for (int cc = 0; cc < n_groups; ++cc) {
+            const float* rr = base + cc * WSTR;
+            const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
+            ll += rr[DH + 1] * cw;
+            oo += rr[dd] * cw;
+          }
+          const int m = qv / grp, hq = hk * grp + qv % grp;
+          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+        }
+        am_consumer_sync();
+      }
+      if (tid == 0) p.counters[hk] = 0;
+    }
+  }
+  DVT_ASTAMP(7);
+}
+
+}  // namespace dvt

@@ -17,6 +17,7 @@
 
 #include "../../include/dovetail.h"
 #include "attention.cuh"
+#include "attention_mma.cuh"
 #include "gemv.cuh"
 #include "gemv_mma.cuh"
 #include "state.cuh"
@@ -106,18 +107,22 @@ int fail(dovetail_draft* h, int code, const char* fmt, ...) {
 // serialization attribute so that its prologue / weight prefetch overlaps the
 // tail of its predecessor; the kernels call griddepcontrol.wait themselves.
 template <typename... KArgs, typename... Args>
-cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
-                   cudaStream_t st, Args... args) {
+cudaError_t launch_c(dovetail_draft* h, int cluster_x, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                     cudaStream_t st, Args... args) {
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid;
   cfg.blockDim = block;
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = 1;
+  attr[1].id = cudaLaunchAttributeClusterDimension;  // thread-block cluster along x (attention chunks)
+  attr[1].val.clusterDim.x = cluster_x;
+  attr[1].val.clusterDim.y = 1;
+  attr[1].val.clusterDim.z = 1;
   cfg.attrs = attr;
-  cfg.numAttrs = 1;
+  cfg.numAttrs = cluster_x > 1 ? 2 : 1;
   ++h->launches;
   if (!h->profile) return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
   // profiling: bracket the launch with events (serialises the kernels)
@@ -135,6 +140,12 @@ cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 bl
   cudaError_t r = cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
   cudaEventRecord(h->ev[2 * i + 1], st);
   return r;
+}
+
+template <typename... KArgs, typename... Args>
+cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
+                   cudaStream_t st, Args... args) {
+  return launch_c(h, 1, kern, grid, block, smem, st, args...);
 }
 
 using GemvKernel = void (*)(const GemvParams);
@@ -179,6 +190,8 @@ cudaError_t set_max_smem_all() {
     if (r != cudaSuccess) e = r;
   };
   for (int nt = 1; nt <= 8; nt *= 2) set(reinterpret_cast<const void*>(pick_gemv_mma(nt)));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<64>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<128>));
   const int mts[3] = {1, 2, 4};
   for (int mt : mts) {
     set(reinterpret_cast<const void*>(pick_gemv<__nv_bfloat16>(mt, 3)));
@@ -635,15 +648,34 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
         a.qv_cap = h->qv_cap;
         a.counters = h->attn_cnt;
         const int Lbase = l == 0 ? L : Lp;
-        int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
         const int qv_tot = M * grp;
-        const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
-        const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
-        const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
-                            static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
         h->cur_kind = 4;
         h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
-        e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
+        if (bf16 && !h->force_fma) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
+          a.kc = kv->k;
+          a.vc = kv->v;
+          a.cap = kv->capacity;
+          a.Lbase = Lbase;
+          const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
+          int n_chunks = std::min(h->attn_chunks_cap, n_blocks), cs;
+          if (n_chunks <= 8) {
+            n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
+            cs = n_chunks;
+          } else {
+            n_chunks = n_chunks / 8 * 8;
+            cs = 8;
+          }
+          const size_t smem = am_smem_bytes(dh);
+          e = launch_c(h, cs, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
+                       dim3(kAmThreads), smem, st, a);
+        } else {
+          int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
+          const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
+          const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
+          const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
+                              static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
+          e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
+        }
         if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "attention launch failed: %s", cudaGetErrorString(e));
       }
       {  // S4: x += Wo o
