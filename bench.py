@@ -11,7 +11,7 @@ draft; it fits one GPU). Prints ONE JSON line (rank 0).
   value      draft tokens/s (gamma candidates per step / step time), inputs resident in HBM
   e2e        the same through the C ABI with HOST inputs and outputs: per step an H2D copy of
              (hidden_feats, tokens) from pinned memory and a D2H read of the candidates
-  roofline   the weight-streaming GEMV kernel (k_gemv, > 95 % of the bytes): algorithmic
+  roofline   the weight-streaming GEMV kernel (k_gemv_mma, > 95 % of the bytes): algorithmic
              bytes per launch / its mean launch duration (CUDA events around every launch,
              taken in a separate instrumented pass over the same steps), against the
              measured HBM copy bandwidth of MEASURED_PEAKS.json
@@ -272,7 +272,7 @@ def main():
                 traffic = json.load(open(tp)).get(cfg.name, {}).get("k_gemv_dram_bytes_per_launch")
             except Exception:
                 traffic = None
-        roof = {"bound": "hbm", "kernel": "k_gemv (all weight-streaming GEMV launches of the step)",
+        roof = {"bound": "hbm", "kernel": "k_gemv_mma (bf16) / k_gemv (fp32): all weight-streaming GEMV launches of the step",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
                 "traffic": traffic, "bytes_per_launch": g_b / g_n if g_n else 0, "us_per_launch": g_ms / g_n * 1e3 if g_n else 0,
                 "launches_per_step": g_n // kp, "gemv_share_of_step_time": g_ms / tot_ms if tot_ms else None,
@@ -286,7 +286,7 @@ def main():
     peak, peak_src = peaks()
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 accumulate over bf16 weights" if cfg.dtype == 1 else "f32", "data": "synthetic",
+            "dtype": "bf16 weights and KV cache, f32 activations and accumulation" if cfg.dtype == 1 else "f32", "data": "synthetic",
             "config": config, "draft_step_us": step_ms * 1e3, "forward_us": step_ms * 1e3 / tree.depth,
             "step_hbm_gbs": step_bytes / (step_ms * 1e-3) / 1e9,
             "step_frac_of_measured_peak": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
