@@ -177,7 +177,7 @@ def main():
         return
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU path)"
-    from paper_2412_18934_b200 import binding
+    from paper_2412_18934_b200 import binding, replicas
     binding.load()  # fail loudly if the library is missing
     torch.cuda.set_device(local)
     if world > 1:
@@ -223,11 +223,7 @@ def main():
         e1.record(stream)
         torch.cuda.synchronize()
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms, _ = replicas.job_time_and_work(e0.elapsed_time(e1), 0.0, device="cuda")  # max over ranks
         return ms
 
     for _ in range(W):
