@@ -127,73 +127,119 @@ constexpr int kTreeThreads = 256;
 constexpr int kPoolSmem = 4352;  // >= kMaxBranch + kMaxTreeSlots * kMaxBranch + slack
 
 __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelParams p) {
-  __shared__ float s_cum[kPoolSmem];
-  __shared__ int32_t s_new[kPoolSmem];
+  // phase A stages candidate lists (3 x kCandSmem words); phases B / C reuse the space for the pool scores
+  constexpr int kCandSmem = 3072;
+  static_assert(3 * kCandSmem >= 2 * kPoolSmem, "shared staging too small for the pool");
+  __shared__ float s_raw[3 * kCandSmem];
   __shared__ int32_t s_cnt[kTreeThreads + 1];
+  float* s_cum = s_raw;
+  int32_t* s_new = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);
   pdl_launch_dependents();
   pdl_wait();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const Pool& P = p.pool;
 
   // ---- phase A: children of each expanded row --------------------------------
-  for (int m = warp; m < p.M; m += kTreeThreads / 32) {
-    const int parent = p.cur->pool[m];
-    const float pcum = parent < 0 ? 0.f : P.cum[parent];
-    const int base = p.pool_begin + m * p.b;
-    if (p.rp_tokens) {
-      if (lane < p.b) {
-        const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
-        P.token[base + lane] = p.rp_tokens[o];
-        P.parent[base + lane] = parent;
-        P.depth[base + lane] = p.level + 1;
-        P.cum[base + lane] = pcum + p.rp_logp[o];
-        P.row[base + lane] = -1;
-      }
-      continue;
-    }
-    // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order
-    const float* st = p.stat + static_cast<size_t>(m) * p.nct * 2;
-    float mg = -INFINITY;
-    for (int c = lane; c < p.nct; c += 32) mg = fmaxf(mg, st[c * 2]);
-    mg = warp_max(mg);
-    float se = 0.f;
-    for (int c = lane; c < p.nct; c += 32) {
-      const float mc = st[c * 2];
-      se += (mc == -INFINITY) ? 0.f : st[c * 2 + 1] * expf(mc - mg);
-    }
-    se = warp_sum(se);
-    const float logz = mg + logf(se);
-    // global top-b of the row: b rounds of "best candidate strictly after the previous pick"
-    const float* cv = p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
-    const int32_t* ci = p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
-    float lv = INFINITY;
-    int li = -1;
-    for (int jb = 0; jb < p.b; ++jb) {
-      float bv = -INFINITY;
-      int bi = 0x7fffffff;
-      for (int c = lane; c < p.nct; c += 32) {
-        for (int j = 0; j < p.b; ++j) {
-          const float val = cv[c * kMaxBranch + j];
-          const int id = ci[c * kMaxBranch + j];
-          if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+  // The per-CTA top-b lists and softmax statistics of a group of rows are first brought into
+  // shared memory with independent loads (one L2 round trip); each row is then merged by one warp.
+  float* s_cv = s_raw;
+  int32_t* s_ci = reinterpret_cast<int32_t*>(s_raw + kCandSmem);
+  float* s_st = s_raw + 2 * kCandSmem;
+  const int per_row = p.rp_tokens ? 0 : p.nct * p.b;
+  int G = per_row > 0 ? min(kCandSmem / per_row, (kCandSmem / 2) / max(p.nct, 1)) : 0;  // rows per group
+  G = min(G, p.M);
+  for (int g0 = 0; g0 < p.M; g0 += max(G, 1)) {
+    const int gr = G > 0 ? min(G, p.M - g0) : 0;
+    if (gr > 0) {
+      const int n_c = gr * per_row;
+      for (int base = 0; base < n_c; base += kTreeThreads * 4) {
+        float v[4];
+        int id[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int idx = base + i * kTreeThreads + tid;
+          v[i] = 0.f;
+          id[i] = 0;
+          if (idx < n_c) {
+            const int mc = idx / p.b, j = idx - mc * p.b;  // mc = (row in group) * nct + cta
+            const size_t o = (static_cast<size_t>(g0) * p.nct + mc) * kMaxBranch + j;
+            v[i] = p.cand_val[o];
+            id[i] = p.cand_id[o];
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const int idx = base + i * kTreeThreads + tid;
+          if (idx < n_c) { s_cv[idx] = v[i]; s_ci[idx] = id[i]; }
         }
       }
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-      }
-      if (lane == 0) {
-        P.token[base + jb] = bi;
-        P.parent[base + jb] = parent;
-        P.depth[base + jb] = p.level + 1;
-        P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
-        P.row[base + jb] = -1;
-      }
-      lv = bv;
-      li = bi;
+      for (int idx = tid; idx < gr * p.nct * 2; idx += kTreeThreads) s_st[idx] = p.stat[static_cast<size_t>(g0) * p.nct * 2 + idx];
+      __syncthreads();
     }
+    const int m_end = G > 0 ? g0 + gr : p.M;
+    for (int m = g0 + warp; m < m_end; m += kTreeThreads / 32) {
+      const int parent = p.cur->pool[m];
+      const float pcum = parent < 0 ? 0.f : P.cum[parent];
+      const int base = p.pool_begin + m * p.b;
+      if (p.rp_tokens) {
+        if (lane < p.b) {
+          const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
+          P.token[base + lane] = p.rp_tokens[o];
+          P.parent[base + lane] = parent;
+          P.depth[base + lane] = p.level + 1;
+          P.cum[base + lane] = pcum + p.rp_logp[o];
+          P.row[base + lane] = -1;
+        }
+        continue;
+      }
+      // candidates and statistics of this row: shared memory (grouped) or global (lists too long)
+      const float* st = gr > 0 ? s_st + (m - g0) * p.nct * 2 : p.stat + static_cast<size_t>(m) * p.nct * 2;
+      const float* cv = gr > 0 ? s_cv + (m - g0) * per_row : p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
+      const int32_t* ci = gr > 0 ? s_ci + (m - g0) * per_row : p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
+      const int cstride = gr > 0 ? p.b : kMaxBranch;
+      // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order
+      float mg = -INFINITY;
+      for (int c = lane; c < p.nct; c += 32) mg = fmaxf(mg, st[c * 2]);
+      mg = warp_max(mg);
+      float se = 0.f;
+      for (int c = lane; c < p.nct; c += 32) {
+        const float mc = st[c * 2];
+        se += (mc == -INFINITY) ? 0.f : st[c * 2 + 1] * expf(mc - mg);
+      }
+      se = warp_sum(se);
+      const float logz = mg + logf(se);
+      // global top-b of the row: b rounds of "best candidate strictly after the previous pick"
+      float lv = INFINITY;
+      int li = -1;
+      for (int jb = 0; jb < p.b; ++jb) {
+        float bv = -INFINITY;
+        int bi = 0x7fffffff;
+        for (int c = lane; c < p.nct; c += 32) {
+          for (int j = 0; j < p.b; ++j) {
+            const float val = cv[c * cstride + j];
+            const int id = ci[c * cstride + j];
+            if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+          }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+          if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) {
+          P.token[base + jb] = bi;
+          P.parent[base + jb] = parent;
+          P.depth[base + jb] = p.level + 1;
+          P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
+          P.row[base + jb] = -1;
+        }
+        lv = bv;
+        li = bi;
+      }
+    }
+    if (G == 0) break;     // ungrouped: the loop above covered every row
+    __syncthreads();       // the group's staging is reused
   }
   __syncthreads();
 
