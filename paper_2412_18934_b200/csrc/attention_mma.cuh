@@ -140,10 +140,13 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   const int Lbase = p.Lbase, cap = p.cap;
   const WT* kc = static_cast<const WT*>(p.kc) + (static_cast<size_t>(p.layer) * p.Hkv + hk) * cap * DH;
   const WT* vc = static_cast<const WT*>(p.vc) + (static_cast<size_t>(p.layer) * p.Hkv + hk) * cap * DH;
-  int pch = (Lbase + n_chunks - 1) / n_chunks;
-  pch = (pch + PB - 1) / PB * PB;
-  const int p_begin = min(Lbase, c * pch), p_end = min(Lbase, p_begin + pch);
-  const int n_blk = (p_end - p_begin + PB - 1) / PB;
+  // blocks of PB positions are dealt to the chunks; the spare ones go to the LAST chunks because
+  // chunk 0 also attends the new region
+  const int n_blocks = (Lbase + PB - 1) / PB, bbase = n_blocks / n_chunks, brem = n_blocks % n_chunks;
+  const int b_begin = c * bbase + max(0, c - (n_chunks - brem));
+  const int b_end = b_begin + bbase + (c >= n_chunks - brem ? 1 : 0);
+  const int p_begin = min(Lbase, b_begin * PB), p_end = min(Lbase, b_end * PB);
+  const int n_blk = b_end - b_begin;
   const int n_tail = c == 0 ? (p.new_cnt + PB - 1) / PB : 0;  // the new region, chunk 0 only
   const int nb = n_blk + n_tail;
 
@@ -276,7 +279,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       const int t0 = warp * 16;  // this warp's tile of the block
       if (t0 < cnt) {
         const uint32_t kb = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vb = kb + PB * ROWB;
+        // four independent accumulation chains (head / remainder x two position tiles): a dependent
+        // HMMA chain of 16 per tile was the longest latency of the block
         float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+        float sl[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
 #pragma unroll
         for (int ks = 0; ks < KS; ++ks) {
           uint32_t ah[4], al[4], kf[4];
@@ -284,10 +290,14 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
           ldsm_x4(kf, kb + am_swz<ROWB>(t0 + k_row, ks * 2 + k_ch));
           mma_bf16_16816(s[0], ah, kf[0], kf[1]);
-          mma_bf16_16816(s[0], al, kf[0], kf[1]);
+          mma_bf16_16816(sl[0], al, kf[0], kf[1]);
           mma_bf16_16816(s[1], ah, kf[2], kf[3]);
-          mma_bf16_16816(s[1], al, kf[2], kf[3]);
+          mma_bf16_16816(sl[1], al, kf[2], kf[3]);
         }
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt)
+#pragma unroll
+          for (int e = 0; e < 4; ++e) s[nt][e] += sl[nt][e];
         // masks: positions past the block's end, padded query rows, and (new region) the
         // ancestor mask of the row
         float mx[2] = {-INFINITY, -INFINITY};
