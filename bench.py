@@ -140,7 +140,10 @@ def main():
 
     import torch
     from paper_2412_18934_b200.configs import CONFIGS
-    cfg = CONFIGS[a.config]
+    from paper_2412_18934_b200.configs import c4_sweep
+    all_cfgs = dict(CONFIGS)
+    all_cfgs.update({c.name: c for c in c4_sweep()})  # BASELINE.json configs[3]: c4_l{layers}_g{gamma}
+    cfg = all_cfgs[a.config]
     tree = cfg.tree
     config = {"workload": f"{cfg.name}: hidden {cfg.hidden}, {cfg.n_q_heads}q/{cfg.n_kv_heads}kv x {cfg.head_dim}, "
                           f"{cfg.n_layers} layers, ffn {cfg.ffn}, vocab {cfg.vocab}, prefix {cfg.prefix}, "

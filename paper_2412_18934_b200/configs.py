@@ -111,6 +111,12 @@ def c4_sweep() -> List[DraftConfig]:
         for k, gamma in ((1, 4), (2, 8), (2, 16), (4, 32)):
             out.append(replace(_C3, name=f"c4_l{layers}_g{gamma}", n_layers=layers, prefix=2048,
                                tree=TreeSpec(5, (k,) * 5, (0,) + (k,) * 4, gamma), seed=1237))
+    # forward-level form: one tree level of M rows (a depth-2 tree whose root keeps M children), so that
+    # step time - level-0 forward = one forward at tree width M
+    for layers in (1, 4):
+        for m in (4, 8, 16, 32):
+            out.append(replace(_C3, name=f"c4_l{layers}_m{m}", n_layers=layers, prefix=2048,
+                               tree=TreeSpec(2, (m, 2), (0, m), 16), seed=1237))
     return out
 
 

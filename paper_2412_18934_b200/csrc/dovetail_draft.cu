@@ -302,19 +302,28 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
   }
   p.dyn = h->dyn;
   if (h->es == 2 && !h->force_fma) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
-    const MmaShape ms = mma_shape(p.K, p.M, max_cnt);
-    if (ms.ok) {
-      p.rows_per_stage = ms.RS;
-      p.n_stages = ms.n_stages;
-      p.stage_bytes = ms.stage_bytes;
-      p.row_bytes = p.K * 2;
-      p.kc = ms.KC;
-      p.kp = ms.KP;
-      p.split = ms.S;
-      p.seg_stride = ms.seg_stride;
-      p.bs_stride = ms.bs_stride;
-      cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
-      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
+    // Levels wider than 16 rows run in chunks of <= 16 rows (the weights are streamed once per chunk):
+    // beyond 32 B columns the split activations no longer fit next to a useful ring.
+    const int Mtot = p.M, chunk = Mtot > 16 ? 16 : Mtot;
+    if (mma_shape(p.K, chunk, max_cnt).ok) {
+      for (int m0 = 0; m0 < Mtot; m0 += chunk) {
+        const int mc = std::min(chunk, Mtot - m0);
+        const MmaShape ms = mma_shape(p.K, mc, max_cnt);
+        p.M = mc;
+        p.m0 = m0;
+        p.rows_per_stage = ms.RS;
+        p.n_stages = ms.n_stages;
+        p.stage_bytes = ms.stage_bytes;
+        p.row_bytes = p.K * 2;
+        p.kc = ms.KC;
+        p.kp = ms.KP;
+        p.split = ms.S;
+        p.seg_stride = ms.seg_stride;
+        p.bs_stride = ms.bs_stride;
+        if (m0 > 0) h->cur_bytes = 0;  // the algorithmic bytes are counted once
+        cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
+        if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
+      }
       return DOVETAIL_OK;
     }
   }

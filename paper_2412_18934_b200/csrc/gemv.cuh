@@ -53,6 +53,7 @@ struct GemvParams {
   int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
   // k_gemv_mma only: K-chunk per stage, K-panel of the B store, split ways, strides (bytes)
   int32_t kc, kp, split, seg_stride, bs_stride;
+  int32_t m0;            // k_gemv_mma: first draft row of this launch (levels wider than 16 rows run in row chunks)
   int32_t epi;
   float eps;
   float* out;            // STORE/SWIGLU: [M, out_ld]; DGF/RESID: residual stream rows x [M, out_ld]

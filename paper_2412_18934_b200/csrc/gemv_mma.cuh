@@ -159,10 +159,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
   if (tid < M && (x_embed || G.x_from_dyn || G.xidx)) {  // source row of each draft row (fp32 rows, or bf16 embedding rows)
     if (!x_embed) {
       const float* base = G.x_from_dyn ? dyn->feats : G.xsrc;
-      const int64_t ri = G.xidx ? G.xidx[tid] : tid;
+      const int64_t ri = G.xidx ? G.xidx[p.m0 + tid] : p.m0 + tid;
       xptr_s[tid] = base + ri * G.xld;
     } else {
-      xptr_s[tid] = static_cast<const __nv_bfloat16*>(G.embed) + static_cast<size_t>(G.tokens[tid]) * K;
+      xptr_s[tid] = static_cast<const __nv_bfloat16*>(G.embed) + static_cast<size_t>(G.tokens[p.m0 + tid]) * K;
     }
   }
   ss_part[tid] = 0.f;  // kConsumerWarps * kMmaMaxM == kConsumerThreads
@@ -213,7 +213,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
           if (valid) {
             const int k = k_begin + 8 * j;
             if (!x_embed) {
-              const float* xr = direct ? G.xsrc + static_cast<int64_t>(m) * G.xld : static_cast<const float*>(xptr_s[m]);
+              const float* xr = direct ? G.xsrc + static_cast<int64_t>(p.m0 + m) * G.xld : static_cast<const float*>(xptr_s[m]);
               va[i] = __ldg(reinterpret_cast<const float4*>(xr + k));
               vb[i] = __ldg(reinterpret_cast<const float4*>(xr + k + 4));
             } else {
@@ -369,7 +369,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
   if (p.epi == EPI_STORE) {
     for (int idx = tid; idx < nres; idx += kConsumerThreads) {
       const int v2 = idx / M, mm = idx - v2 * M;
-      p.out[mm * p.out_ld + G.out_off + rr.g0 + v2] = res[idx];
+      p.out[(p.m0 + mm) * p.out_ld + G.out_off + rr.g0 + v2] = res[idx];
     }
   } else if (p.epi == EPI_DGF) {
     // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
@@ -378,27 +378,27 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       const int64_t n = rr.g0 + v2;
       const float bz = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[n]);
       const float g = sigmoidf_acc(res[idx] + bz);
-      const float h1 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + n];
-      const float h2 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + p.d + n];
-      p.out[mm * p.out_ld + n] = g * h1 + (1.0f - g) * h2;
+      const float h1 = p.hbuf[static_cast<int64_t>(p.m0 + mm) * 2 * p.d + n];
+      const float h2 = p.hbuf[static_cast<int64_t>(p.m0 + mm) * 2 * p.d + p.d + n];
+      p.out[(p.m0 + mm) * p.out_ld + n] = g * h1 + (1.0f - g) * h2;
     }
   } else if (p.epi == EPI_RESID) {
     for (int idx = tid; idx < nres; idx += kConsumerThreads) {
       const int v2 = idx / M, mm = idx - v2 * M;
-      p.out[mm * p.out_ld + rr.g0 + v2] += res[idx];
+      p.out[(p.m0 + mm) * p.out_ld + rr.g0 + v2] += res[idx];
     }
   } else if (p.epi == EPI_SWIGLU) {
     // act = SiLU(Wgate n) * (Wup n); gate rows are virtual rows [0, cr), up rows [cr, 2cr)
     for (int idx = tid; idx < rr.cr * M; idx += kConsumerThreads) {
       const int r = idx / M, mm = idx - r * M;
       const float gv = res[r * M + mm], uv = res[(rr.cr + r) * M + mm];
-      p.out[mm * p.out_ld + rr.n0 + r] = gv * sigmoidf_acc(gv) * uv;
+      p.out[(p.m0 + mm) * p.out_ld + rr.n0 + r] = gv * sigmoidf_acc(gv) * uv;
     }
   } else {  // EPI_LMHEAD: logits of rows [g0, g0 + cnt) of the vocabulary
     if (p.tap) {
       for (int idx = tid; idx < nres; idx += kConsumerThreads) {
         const int v2 = idx / M, mm = idx - v2 * M;
-        p.tap[static_cast<int64_t>(mm) * p.vocab + rr.g0 + v2] = res[idx];
+        p.tap[static_cast<int64_t>(p.m0 + mm) * p.vocab + rr.g0 + v2] = res[idx];
       }
     }
     for (int m = warp; m < M; m += kConsumerWarps) {
@@ -408,7 +408,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       float se = 0.f;
       for (int v2 = lane; v2 < rr.cnt; v2 += 32) se += expf(res[v2 * M + m] - mx);
       se = warp_sum(se);
-      const int64_t pc = static_cast<int64_t>(m) * nct + c;
+      const int64_t pc = static_cast<int64_t>(p.m0 + m) * nct + c;
       if (lane == 0) { p.stat[pc * 2] = mx; p.stat[pc * 2 + 1] = se; }
       // local top-b: b rounds of "best candidate strictly after the previous pick"
       float lv = INFINITY; int li = -1;

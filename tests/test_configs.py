@@ -49,7 +49,7 @@ def test_baseline_config_trees():
     for c in ("c3", "c5"):
         assert CONFIGS[c].tree.rows_per_level() == [1, 2, 2, 2, 2] and CONFIGS[c].tree.pool_size() == 18
         assert CONFIGS[c].tree.gamma == 16
-    assert len(c4_sweep()) == 16
+    assert len(c4_sweep()) == 16 + 8  # step-level sweep + forward-level (one level of M rows) sweep
 
 
 def test_algorithmic_bytes_per_forward():

@@ -49,7 +49,7 @@ def _run(case, **kw):
 
 @pytest.mark.parametrize("dtype", [F32, BF16])
 @pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "no_first_norm_final_norm", "n_new5",
-                                     "no_prefix", "long_prefix", "wide"])
+                                     "no_prefix", "long_prefix", "wide", "very_wide"])
 def test_step_parity_small(dtype, variant):
     kw, n_new, prefix = dict(dtype=dtype), 1, None
     if variant == "mha_dh128":
@@ -68,6 +68,8 @@ def test_step_parity_small(dtype, variant):
         prefix, n_new = 333, 2
     elif variant == "wide":  # rows per level 1, 6, 12: several m-tiles in every GEMV, query tiles in attention
         kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    elif variant == "very_wide":  # 20 rows in one level: the GEMVs run in row chunks of 16 + 4
+        kw.update(tree=TreeSpec(2, (20, 2), (0, 20), 24))
     case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
     s, gpu, ora = _run(case)
     assert s["same_tree"] or s["oracle_min_margin"] < 1e-2
