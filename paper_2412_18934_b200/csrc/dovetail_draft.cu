@@ -254,23 +254,39 @@ MmaShape mma_shape(int K, int M, int max_cnt) {
   s.RBMAX = s.NT == 8 ? 2 : 4;
   s.ncols = M * s.S;
   s.PC = (s.ncols + 1) & ~1;
-  s.RS = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
-  while (kConsumerWarps * s.RS * s.PC * 4 > 32768 && s.RS > 16) s.RS -= 16;
-  const int target = 32768 / (s.RS * 2);
-  s.KC = target >= 1024 ? 1024 : 512;
-  s.KC = std::min(s.KC, (K + 63) / 64 * 64);
-  int kpmax = (65536 / s.ncols / 2) / s.KC * s.KC;
-  if (kpmax < s.KC) kpmax = s.KC;
-  const int n_panels = div_up(K, kpmax);
-  s.KP = div_up(div_up(K, n_panels), s.KC) * s.KC;
-  s.seg_stride = s.KC * 2 + 16;
-  s.bs_stride = s.KP * 2 + 16;
-  s.stage_bytes = s.RS * s.seg_stride;
-  int fixed = 128 + 16 + (4 + 8 + 4 * kConsumerWarps) * kMmaMaxM + s.ncols * s.bs_stride + 16 + kConsumerWarps * s.RS * s.PC * 4 + max_cnt * M * 4;
-  fixed = (fixed + 15) / 16 * 16;
-  s.n_stages = std::min(8, (kSmemMax - fixed - 64) / s.stage_bytes);
-  if (s.n_stages < 2) s.ok = false;
-  s.smem = s.n_stages * s.stage_bytes + fixed;
+  // Rows per stage, K-chunk and B-store budget: the first candidate that leaves a ring of >= 3 stages or
+  // >= 120 KB (else the deepest ring found). Wide levels need the smaller stages: their B store and partial
+  // buffers take most of the shared memory.
+  const int rs_max = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
+  MmaShape best{};
+  for (int rs = rs_max; rs >= 16; rs -= 16) {
+    if (kConsumerWarps * rs * s.PC * 4 > 32768 && rs > 16) continue;
+    for (int kc0 : {512, 256}) {
+      for (int bbudget : {65536, 49152, 32768}) {
+        MmaShape c = s;
+        c.RS = rs;
+        c.KC = (rs * 2 * kc0 <= 16384) ? 1024 : kc0;
+        c.KC = std::min(c.KC, (K + 63) / 64 * 64);
+        int kpmax = (bbudget / c.ncols / 2) / c.KC * c.KC;
+        if (kpmax < c.KC) kpmax = c.KC;
+        const int n_panels = div_up(K, kpmax);
+        c.KP = div_up(div_up(K, n_panels), c.KC) * c.KC;
+        c.seg_stride = c.KC * 2 + 16;
+        c.bs_stride = c.KP * 2 + 16;
+        c.stage_bytes = c.RS * c.seg_stride;
+        int fixed = 128 + 16 + (4 + 8 + 4 * kConsumerWarps) * kMmaMaxM + c.ncols * c.bs_stride + 16 +
+                    kConsumerWarps * c.RS * c.PC * 4 + max_cnt * M * 4;
+        fixed = (fixed + 15) / 16 * 16;
+        c.n_stages = std::min(8, (kSmemMax - fixed - 64) / c.stage_bytes);
+        c.smem = c.n_stages * c.stage_bytes + fixed;
+        c.ok = c.n_stages >= 2;
+        if (!c.ok) continue;
+        if (c.n_stages >= 3 || c.n_stages * c.stage_bytes >= 120 * 1024) return c;  // two 66 KB stages stream as well as four 33 KB ones
+        if (!best.ok || c.n_stages * c.stage_bytes > best.n_stages * best.stage_bytes) best = c;
+      }
+    }
+  }
+  s = best;
   return s;
 }
 
