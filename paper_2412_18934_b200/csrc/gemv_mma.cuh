@@ -45,9 +45,6 @@ namespace dvt {
 #define DVT_STAMP(i) do { } while (0)
 #endif
 
-#ifndef DVT_GATE_SLOT
-#define DVT_GATE_SLOT 1
-#endif
 constexpr int kMmaMaxM = 32;
 // A 1-D bulk copy costs its issuing warp ~35 ns whatever its size (measured: one producer warp
 // moves 2.4 TB/s chip-wide with 512-byte copies, four move 7.2 TB/s), so four warps produce.
@@ -131,10 +128,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
         }
         for (int k0 = k_begin; k0 < k_end; k0 += KC) {
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
-          // The activation loads of the consumers must not queue behind a ring full of weights on
-          // this SM's return path (measured: 5 us instead of 1 us): only the first stage is
-          // prefetched before the consumers have issued them.
-          if (round == 0 && slot == DVT_GATE_SLOT) mbar_wait(xbar, 0);
+          // Only the first stage is requested before the consumers have issued their activation
+          // loads, so that those do not queue behind a ring full of weights on this SM's return
+          // path (a precaution: measured neutral once the loads were batched into one round).
+          if (round == 0 && slot == 1) mbar_wait(xbar, 0);
           const uint32_t segb = static_cast<uint32_t>(min(KC, k_end - k0)) * 2u;
           if (lane == 0) mbar_arrive_expect_tx(&full[slot], static_cast<uint32_t>(my_rows) * segb);
           __syncwarp();
