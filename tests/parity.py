@@ -18,29 +18,7 @@ from paper_2412_18934_b200.configs import BF16, DraftConfig, TreeSpec
 TOL = {BF16: dict(rtol=2e-2, atol=1e-2), 0: dict(rtol=1e-4, atol=1e-4)}
 
 
-@dataclass
-class Case:
-    cfg: DraftConfig
-    top: Dict
-    layers: list
-    k: torch.Tensor
-    v: torch.Tensor
-    feats: torch.Tensor
-    tokens: torch.Tensor
-    L: int
-    capacity: int
-    tree: TreeSpec
-
-
-def make_case(cfg: DraftConfig, n_new: int = 1, prefix: Optional[int] = None, tree: Optional[TreeSpec] = None,
-              slack: int = 8, device="cuda") -> Case:
-    tree = tree or cfg.tree
-    L = cfg.prefix if prefix is None else prefix
-    cap = L + n_new + tree.tree_rows() + slack
-    top, layers = synth.make_weights(cfg, device=device)
-    k, v = synth.make_kv(cfg, cap, L, device=device)
-    feats, tokens = synth.make_inputs(cfg, n_new, device=device)
-    return Case(cfg, top, layers, k, v, feats, tokens, L, cap, tree)
+from paper_2412_18934_b200.cases import Case, make_case  # noqa: F401  (re-exported for the tests)
 
 
 def _kv_torch(a: np.ndarray, like: torch.Tensor) -> torch.Tensor:
