@@ -300,18 +300,24 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           for (int e = 0; e < 4; ++e) s[nt][e] += sl[nt][e];
         // masks: positions past the block's end, padded query rows, and (new region) the
         // ancestor mask of the row
+        // (a full prefix block needs none: padded query rows are zero vectors, their scores are 0 and
+        // their results are never read)
         float mx[2] = {-INFINITY, -INFINITY};
+        const bool need_mask = tail || cnt < PB;  // uniform over the CTA
 #pragma unroll
         for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            const int h = e >> 1, pos = t0 + nt * 8 + 2 * tq + (e & 1);
-            bool ok = pos < cnt && mrow[h] >= 0;
-            if (ok && tail) {
-              const int j = (b - n_blk) * PB + pos;
-              ok = (rows->mask[mrow[h]][j >> 5] >> (j & 31)) & 1u;
+            const int h = e >> 1;
+            if (need_mask) {
+              const int pos = t0 + nt * 8 + 2 * tq + (e & 1);
+              bool ok = pos < cnt && mrow[h] >= 0;
+              if (ok && tail) {
+                const int j = (b - n_blk) * PB + pos;
+                ok = (rows->mask[mrow[h]][j >> 5] >> (j & 31)) & 1u;
+              }
+              s[nt][e] = ok ? s[nt][e] : -INFINITY;
             }
-            s[nt][e] = ok ? s[nt][e] : -INFINITY;
             mx[h] = fmaxf(mx[h], s[nt][e]);
           }
         float corr[2];
@@ -320,7 +326,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
           mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
           const float mn = fmaxf(mrun[h], mx[h]);
-          corr[h] = (mrun[h] == -INFINITY) ? 0.f : expf(mrun[h] - mn);
+          corr[h] = (mrun[h] == -INFINITY) ? 0.f : __expf(mrun[h] - mn);
           mrun[h] = mn;
           lrun[h] *= corr[h];
         }
@@ -329,20 +335,23 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
         for (int nt = 0; nt < 2; ++nt)
 #pragma unroll
           for (int h = 0; h < 2; ++h) {
-            const float p0 = (s[nt][2 * h] == -INFINITY) ? 0.f : expf(s[nt][2 * h] - mrun[h]);
-            const float p1 = (s[nt][2 * h + 1] == -INFINITY) ? 0.f : expf(s[nt][2 * h + 1] - mrun[h]);
+            // ex2.approx of the difference to the running maximum (<= 0): relative error ~1e-6
+            const float p0 = (s[nt][2 * h] == -INFINITY) ? 0.f : __expf(s[nt][2 * h] - mrun[h]);
+            const float p1 = (s[nt][2 * h + 1] == -INFINITY) ? 0.f : __expf(s[nt][2 * h + 1] - mrun[h]);
             lrun[h] += p0 + p1;
             const uint32_t hi = pack_bf16x2_rn(p0, p1);
             const float2 hf = bf16x2_to_f32x2(hi);
             ph[nt * 2 + h] = hi;
             pl[nt * 2 + h] = pack_bf16x2_rn(p0 - hf.x, p1 - hf.y);
           }
+        if (__any_sync(0xffffffffu, corr[0] != 1.f || corr[1] != 1.f)) {  // the maximum rarely moves after the first tiles
 #pragma unroll
-        for (int t = 0; t < DN; ++t) {
-          o[t][0] *= corr[0];
-          o[t][1] *= corr[0];
-          o[t][2] *= corr[1];
-          o[t][3] *= corr[1];
+          for (int t = 0; t < DN; ++t) {
+            o[t][0] *= corr[0];
+            o[t][1] *= corr[0];
+            o[t][2] *= corr[1];
+            o[t][3] *= corr[1];
+          }
         }
 #pragma unroll
         for (int t = 0; t < DN; t += 2) {
