@@ -682,13 +682,21 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
           a.cap = kv->capacity;
           a.Lbase = Lbase;
           const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
-          int n_chunks = std::min(h->attn_chunks_cap, n_blocks), cs;
+          // Chunks per kv-head (measured on C2 / C3 / C5): at least two 64-position blocks per chunk (a CTA's
+          // fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one cluster of 8
+          // no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
+          int n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2)), cs;
           if (n_chunks <= 8) {
             n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
             cs = n_chunks;
           } else {
-            n_chunks = n_chunks / 8 * 8;
+            n_chunks = std::max(8, std::min(n_chunks, 200 / c.n_kv_heads) / 8 * 8);
             cs = 8;
+          }
+          if (const char* ev = getenv("DOVETAIL_ATTN_CHUNKS")) {  // measurement override
+            n_chunks = std::max(1, std::min(atoi(ev), n_blocks));
+            cs = n_chunks <= 8 ? n_chunks : 8;
+            n_chunks = n_chunks / cs * cs;
           }
           const size_t smem = am_smem_bytes(dh);
           e = launch_c(h, cs, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
