@@ -403,10 +403,12 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     }
     // ---- merge the chunks of the cluster in rank order through distributed shared memory ----
     cluster_sync_all();  // every CTA's record is complete and visible cluster-wide
-    if (crank == 0) {
+    {  // every rank merges its slice of the head dimension (the work of the merge is spread over the cluster)
       const uint32_t crec_u = smem_u32(crec);
-      for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
-        const int r = idx / DH, dd = idx % DH;
+      const int slice = (DH + CS - 1) / CS;
+      for (int idx = tid; idx < nq * slice; idx += kAmConsumers) {
+        const int r = idx / slice, dd = crank * slice + idx % slice;
+        if (dd >= DH) continue;
         const int qv = qv0 + r;
         const uint32_t ra = crec_u + static_cast<uint32_t>(r * WSTR) * 4;
         float mk[8], lk[8], ok[8];
@@ -440,8 +442,9 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
         }
       }
+      if (n_groups > 1) __threadfence();  // the group's partial is complete in global memory before the leader counts in
     }
-    cluster_sync_all();  // the leader has read the records: they (and the query tiles) may be reused
+    cluster_sync_all();  // every rank has read the records: they (and the query tiles) may be reused
   }
   DVT_ASTAMP(6);
 
