@@ -49,7 +49,7 @@ def _run(case, **kw):
 
 @pytest.mark.parametrize("dtype", [F32, BF16])
 @pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "no_first_norm_final_norm", "n_new5",
-                                     "no_prefix", "long_prefix", "wide", "very_wide"])
+                                     "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch"])
 def test_step_parity_small(dtype, variant):
     kw, n_new, prefix = dict(dtype=dtype), 1, None
     if variant == "mha_dh128":
@@ -70,6 +70,10 @@ def test_step_parity_small(dtype, variant):
         kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
     elif variant == "very_wide":  # 20 rows in one level: the GEMVs run in row chunks of 16 + 4
         kw.update(tree=TreeSpec(2, (20, 2), (0, 20), 24))
+    elif variant == "n_new33":  # level 0 of 33 rows: GEMV row chunks 16 + 16 + 1, several attention query passes
+        n_new = 33
+    elif variant == "max_branch":  # 32 children of the root, all forwarded: b = max_branch, a 32-row level
+        kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
     case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
     s, gpu, ora = _run(case)
     assert s["same_tree"] or s["oracle_min_margin"] < 1e-2
