@@ -264,7 +264,7 @@ def main():
         tot_ms = sum(v["ms"] for v in agg.values())
         achieved = (g_b / g_n) / (g_ms / g_n * 1e-3) / 1e9 if g_n else 0.0
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        tp = os.path.join(ROOT, "profiles", "traffic.json.txt")
         if os.path.exists(tp):
             try:
                 traffic = json.load(open(tp)).get(cfg.name, {}).get("k_gemv_dram_bytes_per_launch")
