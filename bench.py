@@ -267,7 +267,11 @@ def main():
         tp = os.path.join(ROOT, "profiles", "traffic.json.txt")
         if os.path.exists(tp):
             try:
-                traffic = json.load(open(tp)).get(cfg.name, {}).get("k_gemv_dram_bytes_per_launch")
+                t = json.load(open(tp)).get(cfg.name, {})
+                # the ncu capture covers 8 launches; scale its DRAM bytes / algorithmic bytes ratio to the
+                # mean launch of the whole step so that traffic is comparable with bytes_per_launch
+                if t.get("k_gemv_dram_bytes_per_launch") and t.get("captured_algorithmic_bytes_per_launch") and g_n:
+                    traffic = (g_b / g_n) * t["k_gemv_dram_bytes_per_launch"] / t["captured_algorithmic_bytes_per_launch"]
             except Exception:
                 traffic = None
         roof = {"bound": "hbm", "kernel": "k_gemv_mma (bf16) / k_gemv (fp32): all weight-streaming GEMV launches of the step",
