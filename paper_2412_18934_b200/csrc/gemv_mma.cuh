@@ -130,7 +130,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
           // Only the first stage is requested before the consumers have issued their activation
           // loads, so that those do not queue behind a ring full of weights on this SM's return
-          // path (a precaution: measured neutral once the loads were batched into one round).
+          // path. Measured on the c3 step: gate before stage 1: 3080 us; before stage 0: 3125 us;
+          // before stage 2: 3106 us; no gate: 3107 us.
           if (round == 0 && slot == 1) mbar_wait(xbar, 0);
           const uint32_t segb = static_cast<uint32_t>(min(KC, k_end - k0)) * 2u;
           if (lane == 0) mbar_arrive_expect_tx(&full[slot], static_cast<uint32_t>(my_rows) * segb);
