@@ -1,29 +1,35 @@
 #!/usr/bin/env python
 """bench.py -- draft-step throughput of the B200-native Dovetail draft model.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c3|c1|c2|c5|c4_...|all] [--impl ours|reference]
 
-One "step" is one dovetail_draft_step: D forwards of the draft model over the levels of
-the draft tree plus the final rerank (all rows of SURVEY.md 8a), on synthetic seeded
-inputs shaped like BASELINE.json's headline workload (configs[2], the Llama-2-13B-shaped
-draft; it fits one GPU). Prints ONE JSON line (rank 0).
+One "step" is one dovetail_draft_step: D forwards of the draft model over the levels of the draft tree plus
+the final rerank (all rows of SURVEY.md 8a), on synthetic seeded inputs shaped like BASELINE.json's headline
+workload (configs[2], the Llama-2-13B-shaped draft; it fits one GPU). Prints ONE JSON line (rank 0);
+`--config all` prints one line per configuration (C1, C2, C3, C5 and the C4 sweep), headline last.
 
-  value      draft tokens/s (gamma candidates per step / step time), inputs resident in HBM
-  e2e        the same through the C ABI with HOST inputs and outputs: per step an H2D copy of
-             (hidden_feats, tokens) from pinned memory and a D2H read of the candidates
-  roofline   the weight-streaming GEMV kernel (k_gemv_mma, > 95 % of the bytes): algorithmic
-             bytes per launch / its mean launch duration (CUDA events around every launch,
-             taken in a separate instrumented pass over the same steps), against the
-             measured HBM copy bandwidth of MEASURED_PEAKS.json
-  cpu_baseline  the fp64 oracle, as it stands, on the host cores (rank 0, N = 1)
+  value        draft tokens/s (gamma candidates per step / step time), inputs resident in HBM; the K timed
+               steps are bracketed by one pair of CUDA events on the launching stream
+  e2e          the same through the C ABI with HOST inputs and outputs: per step an H2D copy of
+               (hidden_feats, tokens) from pinned memory and a D2H read of the candidates
+  roofline     the weight-streaming GEMV launches (k_gemv_mma, > 95 % of the bytes): algorithmic bytes per
+               launch / mean launch duration. Durations come from %globaltimer stamps every kernel writes at
+               its first CTA's start and last CTA's end (dovetail_trace_*, include/dovetail_hooks.h) -- the
+               launches keep their programmatic-dependent-launch overlap -- taken as each launch's EXCLUSIVE
+               time (clipped to start at the end of the launches before it), so that the kinds add up to at
+               most the step, and scaled to the event-timed ms_per_step. Peaks: the measured copy bandwidth of
+               MEASURED_PEAKS.json, the read-only streaming ceilings measured in this run
+               (dovetail_probe_stream), and the 8 TB/s nominal figure BASELINE.json's 70 % bar refers to.
+  cpu_baseline the fp64 oracle, as it stands, on the host cores (all cores and one thread; rank 0, N = 1)
 
-N > 1: independent replicas, one process per GPU (a batch-1 draft step is a sequential
-chain and does not shard); value sums the replicas, time is the
-max over ranks.
+N > 1: independent replicas, one process per GPU (a batch-1 draft step is a sequential chain and does not
+shard); value sums the replicas, time is the max over ranks. Without torchrun,
+`--gpus N` re-launches itself under torch.distributed.run with N ranks.
 """
 import argparse
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -34,14 +40,16 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FALLBACK_HBM_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+NOMINAL_HBM_GBS = 8000.0   # BASELINE.json north_star: "HBM bytes at about 8 TB/s"
 METRIC, UNIT = "draft_tokens_per_s_batch1", "tokens/s"
+GEMV_KINDS = ("dgf_proj", "dgf_gate", "qkv", "o_proj", "gate_up", "down", "lm_head")
 
 
 def peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         try:
-            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs: read+write copy)"
         except Exception:
             pass
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
@@ -95,25 +103,41 @@ class ClockSampler:
 
 
 def dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
+def set_omp_threads(n: int):
+    """The oracle's OpenMP loops take their thread count from libgomp; nothing of oracle/ is touched."""
+    import ctypes
+    try:
+        ctypes.CDLL("libgomp.so.1").omp_set_num_threads(int(n))
+        return True
+    except Exception:
+        return False
 
 
 def oracle_sample(case, full_step: bool):
-    """Time the oracle on a bounded sample of the workload. Returns (seconds per whole step
-    (extrapolated when sampled), description, cores)."""
+    """Time the oracle on a bounded sample of the workload. Returns (seconds per whole step (extrapolated when
+    sampled), description)."""
     sys.path.insert(0, os.path.join(ROOT, "tests"))
     from parity import run_oracle
     from paper_2412_18934_b200.configs import TreeSpec
     import dataclasses
-    cores = len(os.sched_getaffinity(0))
     tree = case.tree
     if full_step:
         t0 = time.perf_counter()
         run_oracle(case, dump=False)
-        return time.perf_counter() - t0, "one whole draft step (all D forwards + rerank)", cores
+        return time.perf_counter() - t0, "one whole draft step (all D forwards + rerank)"
     # one level-0 forward + LM head + top-k = 1 of the step's row-forwards
     sub = dataclasses.replace(case, tree=TreeSpec(1, (tree.branch[0],), (0,), tree.branch[0]))
     t0 = time.perf_counter()
@@ -121,70 +145,68 @@ def oracle_sample(case, full_step: bool):
     dt = time.perf_counter() - t0
     row_forwards = sum(tree.rows_per_level(case.tokens.shape[0]))
     return dt * row_forwards, (f"one level-0 row-forward (DGF + {case.cfg.n_layers} layers + LM head + top-k), "
-                               f"scaled x{row_forwards} row-forwards of the step"), cores
+                               f"scaled x{row_forwards} row-forwards of the step")
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="c3")
-    ap.add_argument("--n-new", type=int, default=1)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-profile-pass", action="store_true")
-    a = ap.parse_args()
-    rank, world, local = dist_env()
-    K, W = a.steps, max(a.warmup, 3)
+def _to_host(case):
+    import dataclasses
+    hc = lambda t: None if t is None else t.detach().cpu()
+    return dataclasses.replace(case, top={k: hc(v) for k, v in case.top.items()},
+                               layers=[{k: hc(v) for k, v in l.items()} for l in case.layers],
+                               k=case.k.cpu(), v=case.v.cpu(), feats=case.feats.cpu(), tokens=case.tokens.cpu())
 
-    import torch
-    from paper_2412_18934_b200.configs import CONFIGS
-    from paper_2412_18934_b200.configs import c4_sweep
-    all_cfgs = dict(CONFIGS)
-    all_cfgs.update({c.name: c for c in c4_sweep()})  # BASELINE.json configs[3]: c4_l{layers}_g{gamma}
-    cfg = all_cfgs[a.config]
+
+def all_configs():
+    from paper_2412_18934_b200.configs import CONFIGS, c4_sweep, depth_sweep
+    cfgs = {c.name: c for c in CONFIGS.values()}
+    cfgs.update({k: v for k, v in CONFIGS.items()})
+    cfgs.update({c.name: c for c in c4_sweep()})
+    cfgs.update({c.name: c for c in depth_sweep()})
+    return cfgs
+
+
+def workload(cfg, n_new, world):
     tree = cfg.tree
-    config = {"workload": f"{cfg.name}: hidden {cfg.hidden}, {cfg.n_q_heads}q/{cfg.n_kv_heads}kv x {cfg.head_dim}, "
-                          f"{cfg.n_layers} layers, ffn {cfg.ffn}, vocab {cfg.vocab}, prefix {cfg.prefix}, "
-                          f"tree D{tree.depth} branch {list(tree.branch)} beam {list(tree.beam)} gamma {tree.gamma}, "
-                          f"n_new {a.n_new}",
-              "batch": 1, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
-              "l2": "inputs larger than L2 (every forward streams > 1 GB of weights)"}
-    from paper_2412_18934_b200.cases import make_case  # seeded inputs only; the oracle is imported by its own legs
+    return {"workload": f"{cfg.name}: hidden {cfg.hidden}, {cfg.n_q_heads}q/{cfg.n_kv_heads}kv x {cfg.head_dim}, "
+                        f"{cfg.n_layers} layers, ffn {cfg.ffn}, vocab {cfg.vocab}, prefix {cfg.prefix}, fusion {cfg.fusion_name}, "
+                        f"tree D{tree.depth} branch {list(tree.branch)} beam {list(tree.beam)} gamma {tree.gamma}, "
+                        f"n_new {n_new}",
+            "batch": 1, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+            "l2": "inputs larger than L2 (every forward streams its weights, > 1 GB on the 7B / 13B shapes, once)"}
 
-    if a.impl == "reference":
-        # the oracle, as it stands, on the host cores; rank 0 alone
-        if rank != 0:
-            return
-        dev = "cuda" if torch.cuda.is_available() else "cpu"
-        case = make_case(cfg, n_new=a.n_new, device=dev)
-        case = _to_host(case)
-        t_probe, _, cores = oracle_sample(case, full_step=False)
-        full = t_probe * (K + W) < 150.0
-        for _ in range(W if full else min(W, 3)):
-            oracle_sample(case, full)
-        ts = []
-        for _ in range(K):
-            t, sample, cores = oracle_sample(case, full)
-            ts.append(t)
-        step_s = sum(ts) / len(ts)
-        val = tree.gamma / step_s
-        line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": 0, "steps": K, "warmup": W,
-                "ms_per_step": step_s * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f64", "data": "synthetic", "config": config,
-                "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
-                "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
-        print(json.dumps(line))
-        return
 
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU path)"
+def reference_line(a, cfg):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 alone."""
+    import torch
+    from paper_2412_18934_b200.cases import make_case
+    K, W = a.steps, max(a.warmup, 3)
+    case = _to_host(make_case(cfg, n_new=a.n_new, device="cuda" if torch.cuda.is_available() else "cpu"))
+    cores = len(os.sched_getaffinity(0))
+    t_probe, _ = oracle_sample(case, full_step=False)
+    full = t_probe * (K + W) < 150.0
+    for _ in range(W if full else min(W, 3)):
+        oracle_sample(case, full)
+    ts = []
+    for _ in range(K):
+        t, sample = oracle_sample(case, full)
+        ts.append(t)
+    step_s = sum(ts) / len(ts)
+    val = cfg.tree.gamma / step_s
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": 0, "steps": K, "warmup": W,
+            "ms_per_step": step_s * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload(cfg, a.n_new, 1),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "cpu_model": cpu_model()},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+
+
+def bench_one(a, cfg, rank, world, local, dist):
+    import dataclasses
+    import torch
     from paper_2412_18934_b200 import binding, replicas
-    binding.load()  # fail loudly if the library is missing
-    torch.cuda.set_device(local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2412_18934_b200.cases import make_case  # seeded inputs only; the oracle is imported by its own legs
+    K, W = a.steps, max(a.warmup, 3)
+    tree = cfg.tree
 
     def barrier():
         if world > 1:
@@ -196,9 +218,9 @@ def main():
     out = binding.alloc_out(tree.gamma)
     stream = torch.cuda.current_stream()
 
-    def step_device():
+    def step_device(hh=h):
         kv.committed_len = case.L  # untimed bookkeeping: discard the tree rows (kv_commit mode 0 semantics)
-        binding.dovetail_draft_step(h, case.feats, case.tokens, kv, tree, out)
+        binding.dovetail_draft_step(hh, case.feats, case.tokens, kv, tree, out)
 
     # host-side buffers of the end-to-end path
     feats_h = case.feats.cpu().pin_memory()
@@ -242,80 +264,214 @@ def main():
     launches = binding.dovetail_last_launch_count(h) * K
     n_out = int(out["n_out"].item())
     assert n_out == min(tree.gamma, tree.pool_size()), "the step did not produce its candidates"
+    binding.dovetail_draft_status(h)
+    step_ms = ms / K
+    step_bytes = tree.depth * binding.dovetail_forward_bytes(h, case.L + a.n_new)
+    peak, peak_src = peaks()
 
-    # instrumented pass: CUDA events around every launch of the same steps
-    roof = None
-    if not a.no_profile_pass:
-        peak, peak_src = peaks()
-        binding.dovetail_draft_set_profile(h, True)
-        agg = {}
-        kp = min(K, 20)
+    # ---- distribution over individually timed replays (median of >= 200 after >= 20 warm-ups)
+    R = a.replays
+    dist_us = None
+    if R > 0 and world == 1:
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(R)]
+        for _ in range(20):
+            step_device()
+        for e0, e1 in ev:
+            e0.record(stream)
+            step_device()
+            e1.record(stream)
+        torch.cuda.synchronize()
+        ts = sorted(e0.elapsed_time(e1) * 1e3 for e0, e1 in ev)
+        dist_us = {"replays": R, "median": ts[R // 2], "p10": ts[R // 10], "p90": ts[(9 * R) // 10], "min": ts[0]}
+
+    # ---- per-kernel device time: globaltimer stamps, PDL overlap kept --------------------------------
+    roof, per_level = None, None
+    if not a.no_trace:
+        binding.dovetail_trace_enable(h, True)
+        kp = min(max(K, 5), 20)
+        agg, lv, step_tr = {}, {}, []
+        for _ in range(3):
+            step_device()
         for _ in range(kp):
             step_device()
             torch.cuda.synchronize()
-            for kind, r in binding.dovetail_profile_read(h).items():
-                g = agg.setdefault(kind, dict(ms=0.0, launches=0, bytes=0))
-                g["ms"] += r["ms"]; g["launches"] += r["launches"]; g["bytes"] += r["bytes"]
-        binding.dovetail_draft_set_profile(h, False)
-        gemv = ("dgf_proj", "dgf_gate", "qkv", "o_proj", "gate_up", "down", "lm_head")
-        g_ms = sum(agg[k]["ms"] for k in gemv)
-        g_n = sum(agg[k]["launches"] for k in gemv)
-        g_b = sum(agg[k]["bytes"] for k in gemv)
-        tot_ms = sum(v["ms"] for v in agg.values())
-        achieved = (g_b / g_n) / (g_ms / g_n * 1e-3) / 1e9 if g_n else 0.0
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json.txt")
+            t = binding.dovetail_trace_read(h)
+            step_tr.append(t["step_us"])
+            for name, r in t["kinds"].items():
+                g = agg.setdefault(name, dict(busy_us=0.0, excl_us=0.0, launches=0, bytes=0))
+                for f in g:
+                    g[f] += r[f]
+            for l, r in t["levels"].items():
+                lv[l] = lv.get(l, 0.0) + r["excl_us"]
+        binding.dovetail_trace_enable(h, False)
+        tot_excl = sum(v["excl_us"] for v in agg.values())
+        step_tr_us = sum(step_tr) / kp
+        scale = (step_ms * 1e3) / (tot_excl / kp) if tot_excl else 0.0  # trace pass -> event-timed step
+        g_excl = sum(agg[k]["excl_us"] for k in GEMV_KINDS) / kp * scale
+        g_n = sum(agg[k]["launches"] for k in GEMV_KINDS) // kp
+        g_b = sum(agg[k]["bytes"] for k in GEMV_KINDS) / kp
+        achieved = g_b / (g_excl * 1e-6) / 1e9 if g_excl else 0.0
+        by_kind = {}
+        for name, v in agg.items():
+            if not v["launches"]:
+                continue
+            us = v["excl_us"] / kp * scale
+            by_kind[name] = {"us_per_step": round(us, 2), "launches_per_step": v["launches"] // kp,
+                             "us_per_launch": round(us / (v["launches"] / kp), 2),
+                             "busy_us_per_launch": round(v["busy_us"] / v["launches"], 2),
+                             "gbs": round(v["bytes"] / kp / (us * 1e-6) / 1e9, 1) if v["bytes"] and us else None,
+                             "frac_of_measured_peak": round(v["bytes"] / kp / (us * 1e-6) / 1e9 / peak, 3) if v["bytes"] and us else None}
+        per_level = [round(lv[l] / kp * scale, 2) for l in sorted(lv)]
+        # read-only streaming ceilings, same run, same device buffers (the largest weight matrix set: > L2)
+        ceil = {}
+        if world == 1:
+            big = max((t for l in case.layers for t in (l["wgate"], l["wup"], l["wdown"])), key=lambda t: t.numel())
+            pool = torch.empty(max(1 << 30, big.numel() * big.element_size()), dtype=torch.uint8, device="cuda")
+            pool.random_(0, 255)
+            for name, mode, seg in (("stream_sum_ldg128", 0, 0), ("stream_bulk_1k", 1, 1024), ("stream_bulk_2k", 1, 2048)):
+                best = 0.0
+                for it in range(6):
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    binding.dovetail_probe_stream(h, pool, mode, seg)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    if it >= 1:
+                        best = max(best, pool.numel() / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+                ceil[name] = round(best, 1)
+            del pool
+        read_ceiling = max(ceil.values()) if ceil else None
+        traffic, traffic_src = None, None
+        tp = os.path.join(ROOT, "profiles", "r2_traffic.json.txt")
         if os.path.exists(tp):
             try:
-                t = json.load(open(tp)).get(cfg.name, {})
-                # the ncu capture covers 8 launches; scale its DRAM bytes / algorithmic bytes ratio to the
-                # mean launch of the whole step so that traffic is comparable with bytes_per_launch
-                if t.get("k_gemv_dram_bytes_per_launch") and t.get("captured_algorithmic_bytes_per_launch") and g_n:
-                    traffic = (g_b / g_n) * t["k_gemv_dram_bytes_per_launch"] / t["captured_algorithmic_bytes_per_launch"]
+                t = json.load(open(tp)).get(cfg.name)
+                if t:  # DRAM bytes per GEMV launch of a committed ncu --set full capture of this very command
+                    traffic, traffic_src = t["dram_bytes_per_gemv_launch"], t["source"]
             except Exception:
                 traffic = None
-        roof = {"bound": "hbm", "kernel": "k_gemv_mma (bf16) / k_gemv (fp32): all weight-streaming GEMV launches of the step",
+        roof = {"bound": "hbm",
+                "kernel": "k_gemv_mma (bf16) / k_gemv (fp32): all weight-streaming GEMV launches of the step",
                 "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
-                "traffic": traffic, "bytes_per_launch": g_b / g_n if g_n else 0, "us_per_launch": g_ms / g_n * 1e3 if g_n else 0,
-                "launches_per_step": g_n // kp, "gemv_share_of_step_time": g_ms / tot_ms if tot_ms else None,
-                "by_kind_us_per_step": {k: round(v["ms"] / kp * 1e3, 2) for k, v in agg.items() if v["launches"]},
-                "note": "instrumented pass serialises the launches (no programmatic-dependent-launch overlap)"}
+                "traffic": traffic, "traffic_source": traffic_src,
+                "bytes_per_launch": g_b / g_n if g_n else 0, "us_per_launch": g_excl / g_n if g_n else 0,
+                "launches_per_step": g_n, "gemv_share_of_step_time": g_excl / (step_ms * 1e3) if step_ms else None,
+                "frac_of_8tbs_nominal": achieved / NOMINAL_HBM_GBS,
+                "read_only_ceilings_gbs": ceil, "frac_of_read_only_ceiling": achieved / read_ceiling if read_ceiling else None,
+                "by_kind": by_kind, "kinds_sum_us": round(sum(v["us_per_step"] for v in by_kind.values()), 2),
+                "trace_step_us": round(step_tr_us, 2),
+                "how": "globaltimer stamps per launch (first CTA start, last CTA end), exclusive time per launch, "
+                       "scaled so that the kinds add up to the event-timed step; PDL overlap kept"}
 
-    step_bytes = tree.depth * binding.dovetail_forward_bytes(h, case.L + a.n_new)
-    step_ms = ms / K
     value = world * tree.gamma * K / (ms * 1e-3)
     e2e_val = world * tree.gamma * K / (ms_e2e * 1e-3)
-    peak, peak_src = peaks()
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16 weights and KV cache, f32 activations and accumulation" if cfg.dtype == 1 else "f32", "data": "synthetic",
-            "config": config, "draft_step_us": step_ms * 1e3, "forward_us": step_ms * 1e3 / tree.depth,
+            "dtype": "bf16 weights and KV cache, f32 activations and accumulation" if cfg.dtype == 1 else "f32",
+            "data": "synthetic", "config": workload(cfg, a.n_new, world),
+            "draft_step_us": step_ms * 1e3, "draft_step_us_replays": dist_us,
+            "forward_us": step_ms * 1e3 / tree.depth, "forward_us_per_level": per_level,
+            "forwards_per_s": tree.depth / (step_ms * 1e-3),
             "step_hbm_gbs": step_bytes / (step_ms * 1e-3) / 1e9,
             "step_frac_of_measured_peak": step_bytes / (step_ms * 1e-3) / 1e9 / peak,
-            "step_frac_of_8tbs_nominal": step_bytes / (step_ms * 1e-3) / 1e9 / 8000.0,
+            "step_frac_of_8tbs_nominal": step_bytes / (step_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
             "algorithmic_bytes_per_step": step_bytes,
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e / K,
                     "h2d_bytes_per_step": feats_h.numel() * 4 + tok_h.numel() * 4,
                     "d2h_bytes_per_step": sum(v.numel() * v.element_size() for v in out_h.values())},
             "gpu_launches": launches, "clocks": clk, "roofline": roof}
+
+    # ---- reading A1 "report both": the same step with dgf_proj = 0 (W1 = W2 = I) ----------------------------
+    if a.both_dgf and world == 1 and cfg.dgf_proj == 1 and cfg.fusion == 0:
+        cfg0 = dataclasses.replace(cfg, dgf_proj=0)
+        top0 = dict(case.top, dgf_w1=None, dgf_w2=None)
+        h0 = binding.dovetail_draft_init(top0, case.layers, cfg0)
+        for _ in range(W):
+            step_device(h0)
+        ms0 = timed(lambda: step_device(h0), K)
+        b0 = tree.depth * binding.dovetail_forward_bytes(h0, case.L + a.n_new)
+        line["dgf_proj0"] = {"ms_per_step": ms0 / K, "value": tree.gamma * K / (ms0 * 1e-3),
+                             "step_frac_of_measured_peak": b0 / (ms0 / K * 1e-3) / 1e9 / peak,
+                             "step_frac_of_8tbs_nominal": b0 / (ms0 / K * 1e-3) / 1e9 / NOMINAL_HBM_GBS}
+        binding.dovetail_draft_destroy(h0)
+
     if rank == 0 and world == 1 and not a.no_cpu_baseline:
         hc = _to_host(case)
-        t, sample, cores = oracle_sample(hc, full_step=True)
-        line["cpu_baseline"] = {"value": tree.gamma / t, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": sample, "seconds_per_step": t}
-    if rank == 0:
-        print(json.dumps(line))
+        cores = len(os.sched_getaffinity(0))
+        t_all, sample_all = oracle_sample(hc, full_step=True)
+        one = None
+        if set_omp_threads(1):
+            t1, sample1 = oracle_sample(hc, full_step=False)
+            one = {"seconds_per_step": t1, "value": tree.gamma / t1, "sample": sample1}
+            set_omp_threads(cores)
+        line["cpu_baseline"] = {"value": tree.gamma / t_all, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": sample_all, "seconds_per_step": t_all, "cpu_model": cpu_model(),
+                                "one_thread": one,
+                                "paper_context": "PAPER.md:70 T_D = 7.2 ms per forward (5 blocks, RTX 2080 SUPER, fp16); "
+                                                 "PAPER.md:9 1.79x-10.1x end-to-end speedups (context only)"}
     binding.dovetail_draft_destroy(h)
+    return line
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="c3")
+    ap.add_argument("--n-new", type=int, default=1)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--replays", type=int, default=200)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-trace", action="store_true")
+    ap.add_argument("--no-both-dgf", dest="both_dgf", action="store_false")
+    a = ap.parse_args()
+    rank, world, local = dist_env()
+
+    if a.impl == "reference":
+        if rank != 0:
+            return
+        print(json.dumps(reference_line(a, all_configs()[a.config if a.config != "all" else "c3"])))
+        return
+
+    if "WORLD_SIZE" not in os.environ and a.gpus > 1:
+        # not under torchrun: spawn the N replica ranks ourselves
+        s = socket.socket()
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+        s.close()
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={a.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
+    if a.gpus != world:
+        sys.exit(f"bench.py: --gpus {a.gpus} disagrees with WORLD_SIZE={world} of the launcher")
+
+    import torch
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU path)"
+    from paper_2412_18934_b200 import binding
+    binding.load()  # fail loudly if the library is missing
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfgs = all_configs()
+    if a.config == "all":
+        names = ["c1", "c2", "c5"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
+    else:
+        names = [a.config]
+    for i, name in enumerate(names):
+        last = i == len(names) - 1
+        if not last:  # the sweep lines carry the step numbers only
+            aa = argparse.Namespace(**vars(a))
+            aa.no_cpu_baseline, aa.both_dgf, aa.replays = True, False, 0
+        else:
+            aa = a
+        line = bench_one(aa, cfgs[name], rank, world, local, dist)
+        if rank == 0:
+            print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
-
-
-def _to_host(case):
-    import dataclasses
-    hc = lambda t: None if t is None else t.detach().cpu()
-    return dataclasses.replace(case, top={k: hc(v) for k, v in case.top.items()},
-                               layers=[{k: hc(v) for k, v in l.items()} for l in case.layers],
-                               k=case.k.cpu(), v=case.v.cpu(), feats=case.feats.cpu(), tokens=case.tokens.cpu())
 
 
 if __name__ == "__main__":

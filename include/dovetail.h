@@ -51,6 +51,16 @@ typedef enum {
 
 typedef enum { DOVETAIL_F32 = 0, DOVETAIL_BF16 = 1 } dovetail_dtype_t;
 
+/* Fusion of the target's hidden feature f with the token embedding e.
+ *   DGF           the paper's Dynamic Gating Fusion: h1 = W1 f, h2 = W2 e,
+ *                 g = sigmoid(Wg [h1 || h2] + bg), x = g * h1 + (1 - g) * h2.
+ *   CONCAT_LINEAR the EAGLE-2 fusion DGF replaces ("simply concatenates the two and maps
+ *                 them to the hidden state dimension through a single linear transformation",
+ *                 PAPER.md:104; ablation row "w/o both", Table 6):
+ *                 x = Wfc [f || e] + bfc, with Wfc [d, 2d] passed as dgf_wg and bfc [d] as
+ *                 dgf_bg; dgf_w1 / dgf_w2 are ignored (dgf_proj must be 0). */
+typedef enum { DOVETAIL_FUSION_DGF = 0, DOVETAIL_FUSION_CONCAT_LINEAR = 1 } dovetail_fusion_t;
+
 /* Model shape. The block is the LLaMA-family decoder layer of the paper's
  * target models: pre-RMSNorm, rotary embedding with half-split
  * pairing (i, i + head_dim/2), grouped-query attention, SiLU-gated FFN, no
@@ -72,6 +82,7 @@ typedef struct {
   int32_t max_rows;     /* largest n_new and largest beam[] a step may use (<= 64)   */
   int32_t max_tree_slots; /* largest sum over tree levels of forwarded rows (<= 128) */
   int32_t max_branch;   /* largest branch[] a step may use (<= 32)                   */
+  int32_t fusion;       /* dovetail_fusion_t: how the feature and the embedding are fused */
 } dovetail_config_t;
 
 /* Device pointers to one decoder layer's weights. */
@@ -170,7 +181,11 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
  * Ties: top-k within a row by (logit desc, token id asc); frontier and final
  * selection by (cumulative score desc, pool index asc).
  * Errors: EINVAL (null pointers, n_new out of range, bad tree spec),
- * ECAPACITY, ECUDA. On error nothing was enqueued and kv is untouched. */
+ * ECAPACITY, ECUDA. Every shape of the step (tree plan, GEMV and attention
+ * geometry of every level) is checked before the first launch: on EINVAL /
+ * ECAPACITY nothing was enqueued and kv is untouched. A token id outside
+ * [0, vocab) cannot be seen without reading device memory: the step clamps it,
+ * raises a device-side flag and dovetail_draft_status() reports EINVAL. */
 int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens,
                         int32_t n_new, dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree,
                         const dovetail_draft_out_t* out, void* cuda_stream);
@@ -209,45 +224,15 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree,
                          int32_t* pool_parent, int32_t* pool_depth, float* pool_cum,
                          int32_t* pool_size, void* cuda_stream);
 
-/* Optional taps for parity tests; pass NULL to disable (the default).
- *   logits : dev fp32 [max rows of a step, V]; row r of the step (level-0 rows
- *            first, then tree rows in cache-slot order) receives the LM-head
- *            logits of that row (level 0: only the last row is computed).
- *   hhat   : dev fp32 [max rows of a step, d]; the draft's output hidden state
- *            of each row.
- * Borrowed until replaced. */
-int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat);
-
-/* Optional teacher forcing for parity tests; all pointers NULL (the default) disables it.
- * A draft step feeds every level with the previous levels' results (the parent's output
- * hidden state, and the ancestors' K/V rows), so a rounding-level difference
- * at level 0 is amplified level by level (x3 per level on the 13B-shaped random-weight
- * model) and an element-wise comparison of deep rows would measure that amplification,
- * not the arithmetic. With forcing, after every level the step
- *   1. copies the K/V rows it has just computed for that level into tap_k / tap_v
- *      (the hhat tap of dovetail_draft_set_taps is likewise taken per level), then
- *   2. overwrites those cache rows with the rows of force_k / force_v and the level's
- *      rows of its hidden-state buffer with the rows of force_hhat,
- * so that each level is computed from the caller's (the oracle's) state.
- *   force_hhat     : dev fp32 [rows of the step, d], step-row order (as the hhat tap)
- *   force_k/v, tap_k/v : dev, same dtype, layout and capacity as the KV cache of the step
- * Borrowed until replaced. The copies serialise the stream between levels. */
-int dovetail_draft_set_forcing(dovetail_draft_t* h, const float* force_hhat, const void* force_k,
-                               const void* force_v, void* tap_k, void* tap_v);
-
-/* Optional per-kernel timing, for the roofline report (off by default). When
- * enabled, dovetail_draft_step brackets every kernel launch with CUDA events on
- * cuda_stream (this serialises the launches: programmatic dependent launch
- * cannot overlap across an event, so the step itself runs slower). After the
- * stream has been synchronised by the caller, dovetail_profile_read adds up the
- * last step's launches by kind:
- *   kind 0 step set-up, 1 DGF projections, 2 DGF gate, 3 QKV, 4 tree attention,
- *   5 O-proj, 6 gate/up, 7 down, 8 LM head, 9 tree bookkeeping, 10 h fill.
- * ms, launches, bytes: host arrays of DOVETAIL_N_KINDS entries; bytes are the
- * algorithmic HBM bytes of the kind's launches (weights, prefix K/V). */
-#define DOVETAIL_N_KINDS 11
-int dovetail_draft_set_profile(dovetail_draft_t* h, int32_t enable);
-int dovetail_profile_read(dovetail_draft_t* h, float* ms, int32_t* launches, int64_t* bytes);
+/* Result of the device-side input checks of the steps enqueued so far on this
+ * handle (the step consumes the accepted tokens; a token id outside
+ * [0, vocab) has no embedding row). dovetail_draft_step itself never
+ * synchronises, so the check is reported here: the call synchronises
+ * cuda_stream, reads the device-side status word and clears it.
+ * Returns OK, EINVAL (a token id of a step since the last call was out of
+ * range: that step gathered a clamped embedding row and its candidates are
+ * meaningless) or ECUDA. */
+int dovetail_draft_status(dovetail_draft_t* h, void* cuda_stream);
 
 /* Number of kernel launches the last dovetail_draft_step enqueued. */
 int dovetail_last_launch_count(const dovetail_draft_t* h);

@@ -11,6 +11,7 @@ from .oracle import (  # noqa: F401
     build,
     dgf,
     forward,
+    fusion_linear,
     kv_commit,
     lm_head,
     log_softmax,

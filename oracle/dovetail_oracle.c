@@ -32,6 +32,7 @@ typedef struct {
   int32_t hidden, n_q_heads, n_kv_heads, head_dim, n_layers, ffn, vocab;
   double rope_theta, rms_eps;
   int32_t dtype, dgf_proj, first_layer_input_norm, final_norm;
+  int32_t fusion; /* 0: Dynamic Gating Fusion (the paper's); 1: concat + one Linear (the EAGLE-2 baseline, "w/o both") */
 } orc_config_t;
 
 typedef struct {
@@ -144,6 +145,19 @@ void orc_dgf(const orc_config_t* c, const orc_weights_t* w, const double* f, int
   free(e); free(h); free(z);
 }
 
+/* The fusion DGF replaces ("simply concatenates the two and maps them to the hidden
+ * state dimension through a single linear transformation"; Table 6 row "w/o both"):
+ * x = Wfc [f || e] + bfc, Wfc [d, 2d] and bfc [d] in the dgf_wg / dgf_bg slots (reading A17: hidden
+ * state first, as in DGF's [h1 || h2]; with bias, the 2d^2 + d count of SURVEY.md P1). */
+void orc_fusion_linear(const orc_config_t* c, const orc_weights_t* w, const double* f, int token, double* x) {
+  int d = c->hidden, dt = c->dtype;
+  double* h = (double*)malloc(sizeof(double) * 2 * d);
+  for (int i = 0; i < d; ++i) { h[i] = f[i]; h[d + i] = ld(w->embed, (size_t)token * d + i, dt); }
+  orc_matvec(w->dgf_wg, dt, d, 2 * d, h, x);
+  for (int i = 0; i < d; ++i) x[i] += ld(w->dgf_bg, i, dt);
+  free(h);
+}
+
 /* Attention of one row (O4): q [Hq*dh] already rotated; the row may attend the
  * cache slots listed in allowed[0..n_allowed). K (post-RoPE) and V are read
  * from the cache of this layer as stored. out [Hq*dh]. GQA: q-head h uses
@@ -232,7 +246,10 @@ static void forward_rows(const orc_config_t* c, const orc_weights_t* w, void* kc
   double* ga = (double*)malloc(sizeof(double) * F);
   double* up = (double*)malloc(sizeof(double) * F);
 
-  for (int r = 0; r < R; ++r) orc_dgf(c, w, feats + (size_t)r * d, tokens[r], x + (size_t)r * d);
+  for (int r = 0; r < R; ++r) {
+    if (c->fusion == 1) orc_fusion_linear(c, w, feats + (size_t)r * d, tokens[r], x + (size_t)r * d);
+    else orc_dgf(c, w, feats + (size_t)r * d, tokens[r], x + (size_t)r * d);
+  }
 
   for (int l = 0; l < c->n_layers; ++l) {
     const orc_layer_t* L = &w->layers[l];

@@ -34,7 +34,7 @@ class _Cfg(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("hidden", "n_q_heads", "n_kv_heads", "head_dim", "n_layers", "ffn", "vocab")] + \
                [("rope_theta", C.c_double), ("rms_eps", C.c_double)] + \
-               [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm")]
+               [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm", "fusion")]
 
 
 class _Layer(C.Structure):
@@ -73,11 +73,12 @@ class OracleConfig:
     dgf_proj: int = 1
     first_layer_input_norm: int = 1
     final_norm: int = 0
+    fusion: int = 0  # 0 DGF; 1 concat + Linear, the EAGLE-2 baseline
 
     def c(self) -> _Cfg:
         return _Cfg(self.hidden, self.n_q_heads, self.n_kv_heads, self.head_dim, self.n_layers,
                     self.ffn, self.vocab, float(self.rope_theta), float(self.rms_eps), self.dtype,
-                    self.dgf_proj, self.first_layer_input_norm, self.final_norm)
+                    self.dgf_proj, self.first_layer_input_norm, self.final_norm, self.fusion)
 
 
 def _np(a):
@@ -161,6 +162,14 @@ def dgf(cfg: OracleConfig, w: OracleWeights, f: np.ndarray, token: int) -> np.nd
     x = np.empty(cfg.hidden, dtype=np.float64)
     cc, cw = cfg.c(), w.c()
     _load().orc_dgf(C.byref(cc), C.byref(cw), _ptr(f), C.c_int(int(token)), _ptr(x))
+    return x
+
+
+def fusion_linear(cfg: OracleConfig, w: OracleWeights, f: np.ndarray, token: int) -> np.ndarray:
+    f = np.ascontiguousarray(f, dtype=np.float64)
+    x = np.empty(cfg.hidden, dtype=np.float64)
+    cc, cw = cfg.c(), w.c()
+    _load().orc_fusion_linear(C.byref(cc), C.byref(cw), _ptr(f), C.c_int(int(token)), _ptr(x))
     return x
 
 

@@ -16,10 +16,12 @@ MAX_DEPTH, MAX_LAYERS = 16, 16
 
 OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
+# include/dovetail.h
 EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "dovetail_tree_replay",
-           "dovetail_draft_set_taps", "dovetail_draft_set_forcing", "dovetail_draft_set_profile", "dovetail_profile_read",
-           "dovetail_last_launch_count", "dovetail_forward_bytes",
+           "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
+# include/dovetail_hooks.h (test and measurement hooks)
+HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream")
 
 
 class DovetailError(RuntimeError):
@@ -32,7 +34,7 @@ class ConfigT(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("hidden", "n_q_heads", "n_kv_heads", "head_dim", "n_layers", "ffn", "vocab")] + \
                [("rope_theta", C.c_float), ("rms_eps", C.c_float)] + \
                [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm",
-                                         "max_rows", "max_tree_slots", "max_branch")]
+                                         "max_rows", "max_tree_slots", "max_branch", "fusion")]
 
 
 LAYER_KEYS = ("g_attn", "wq", "wk", "wv", "wo", "g_ffn", "wgate", "wup", "wdown")
@@ -61,6 +63,14 @@ class DraftOutT(C.Structure):
                 ("depths", C.c_void_p), ("n_out", C.c_void_p)]
 
 
+HOOK_FIELDS = ("tap_logits", "tap_hhat", "tap_k", "tap_v", "tap_pool_token", "tap_pool_cum",
+               "force_hhat", "force_k", "force_v", "force_pool_token", "force_pool_cum")
+
+
+class HooksT(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in HOOK_FIELDS]
+
+
 _lib = None
 
 
@@ -84,14 +94,17 @@ def load() -> C.CDLL:
         lib.dovetail_tree_replay.restype = C.c_int
         lib.dovetail_tree_replay.argtypes = [C.c_void_p, C.POINTER(TreeSpecT), C.c_void_p, C.c_void_p, C.c_int32,
                                              C.c_int32, C.POINTER(DraftOutT)] + [C.c_void_p] * 6
-        lib.dovetail_draft_set_taps.restype = C.c_int
-        lib.dovetail_draft_set_taps.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
-        lib.dovetail_draft_set_forcing.restype = C.c_int
-        lib.dovetail_draft_set_forcing.argtypes = [C.c_void_p] + [C.c_void_p] * 5
-        lib.dovetail_draft_set_profile.restype = C.c_int
-        lib.dovetail_draft_set_profile.argtypes = [C.c_void_p, C.c_int32]
-        lib.dovetail_profile_read.restype = C.c_int
-        lib.dovetail_profile_read.argtypes = [C.c_void_p, C.POINTER(C.c_float), C.POINTER(C.c_int32), C.POINTER(C.c_int64)]
+        lib.dovetail_hooks_set.restype = C.c_int
+        lib.dovetail_hooks_set.argtypes = [C.c_void_p, C.POINTER(HooksT)]
+        lib.dovetail_draft_status.restype = C.c_int
+        lib.dovetail_draft_status.argtypes = [C.c_void_p, C.c_void_p]
+        lib.dovetail_trace_enable.restype = C.c_int
+        lib.dovetail_trace_enable.argtypes = [C.c_void_p, C.c_int32]
+        lib.dovetail_trace_read.restype = C.c_int
+        lib.dovetail_trace_read.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int64),
+                                            C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
+        lib.dovetail_probe_stream.restype = C.c_int
+        lib.dovetail_probe_stream.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_void_p]
         lib.dovetail_last_launch_count.restype = C.c_int
         lib.dovetail_last_launch_count.argtypes = [C.c_void_p]
         lib.dovetail_forward_bytes.restype = C.c_int64
@@ -107,7 +120,7 @@ def load() -> C.CDLL:
 def config_t(cfg: DraftConfig, max_rows: int = 64, max_tree_slots: int = 128, max_branch: int = 32) -> ConfigT:
     return ConfigT(cfg.hidden, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.n_layers, cfg.ffn, cfg.vocab,
                    float(cfg.rope_theta), float(cfg.rms_eps), cfg.dtype, cfg.dgf_proj,
-                   cfg.first_layer_input_norm, cfg.final_norm, max_rows, max_tree_slots, max_branch)
+                   cfg.first_layer_input_norm, cfg.final_norm, max_rows, max_tree_slots, max_branch, cfg.fusion)
 
 
 def tree_spec_t(tree: TreeSpec) -> TreeSpecT:
@@ -139,7 +152,7 @@ class Draft:
 
     def __init__(self, ptr: int, cfg: DraftConfig, keep):
         self.ptr, self.cfg, self._keep = ptr, cfg, keep
-        self.taps = None
+        self.hooks = None
 
     def close(self):
         if self.ptr:
@@ -157,7 +170,7 @@ class KVCache:
     """dovetail_kv_cache_t over two torch tensors [n_layers][n_kv_heads][capacity][head_dim]."""
 
     def __init__(self, k, v, committed_len: int):
-        assert k.shape == v.shape and k.dim() == 4
+        assert k.shape == v.shape and k.dim() == 4 and k.dtype == v.dtype
         self.k, self.v = k, v
         self.c = KVCacheT(_dp(k), _dp(v), k.shape[2], committed_len)
 
@@ -210,8 +223,20 @@ def _out_t(out: Dict) -> DraftOutT:
 def dovetail_draft_step(h: Draft, hidden_feats, tokens, kv: KVCache, tree: TreeSpec, out: Optional[Dict] = None,
                         stream=None) -> Dict:
     """Enqueues one draft step; returns the device output buffers (asynchronous)."""
+    import torch
+    # the ABI takes raw pointers: a wrong dtype or shape would be silently reinterpreted
+    d, cdt = h.cfg.hidden, (torch.bfloat16 if h.cfg.dtype == BF16 else torch.float32)
+    if hidden_feats.dtype != torch.float32 or hidden_feats.dim() != 2 or hidden_feats.shape[1] != d:
+        raise TypeError(f"hidden_feats must be float32 [n_new, {d}], got {hidden_feats.dtype} {tuple(hidden_feats.shape)}")
+    if tokens.dtype != torch.int32 or tokens.dim() != 1 or tokens.shape[0] != hidden_feats.shape[0]:
+        raise TypeError(f"tokens must be int32 [n_new = {hidden_feats.shape[0]}], got {tokens.dtype} {tuple(tokens.shape)}")
+    if kv.k.dtype != cdt or kv.k.shape[0] != h.cfg.n_layers or kv.k.shape[1] != h.cfg.n_kv_heads or kv.k.shape[3] != h.cfg.head_dim:
+        raise TypeError(f"KV cache must be {cdt} [n_layers, n_kv_heads, capacity, head_dim], got {kv.k.dtype} {tuple(kv.k.shape)}")
     if out is None:
         out = alloc_out(tree.gamma, hidden_feats.device)
+    for name, dt in (("token_ids", torch.int32), ("scores", torch.float32), ("parents", torch.int32), ("n_out", torch.int32)):
+        if out[name].dtype != dt or out[name].numel() < (1 if name == "n_out" else tree.gamma):
+            raise TypeError(f"out[{name!r}] must be {dt} with room for gamma = {tree.gamma} entries")
     t = tree_spec_t(tree)
     o = _out_t(out)
     rc = load().dovetail_draft_step(h.ptr, _dp(hidden_feats), _dp(tokens), int(tokens.shape[0]), C.byref(kv.c),
@@ -244,16 +269,22 @@ def dovetail_tree_replay(h: Draft, tree: TreeSpec, cand_tokens, cand_logp, out: 
     return out
 
 
-def dovetail_draft_set_taps(h: Draft, logits=None, hhat=None):
-    h.taps = (logits, hhat)
-    _check(load().dovetail_draft_set_taps(h.ptr, _dp(logits), _dp(hhat)), h.ptr)
+def dovetail_hooks_set(h: Draft, **hooks):
+    """Test hooks (include/dovetail_hooks.h): keyword = field of dovetail_hooks_t, value = device tensor.
+    No keywords removes every hook."""
+    unknown = set(hooks) - set(HOOK_FIELDS)
+    assert not unknown, f"unknown hook fields {unknown}"
+    h.hooks = dict(hooks)  # keep the tensors alive
+    if not hooks:
+        _check(load().dovetail_hooks_set(h.ptr, None), h.ptr)
+        return
+    t = HooksT(*[_dp(hooks.get(n)) for n in HOOK_FIELDS])
+    _check(load().dovetail_hooks_set(h.ptr, C.byref(t)), h.ptr)
 
 
-def dovetail_draft_set_forcing(h: Draft, force_hhat=None, force_k=None, force_v=None, tap_k=None, tap_v=None):
-    """Teacher forcing for parity tests (include/dovetail.h); all None disables it."""
-    h.forcing = (force_hhat, force_k, force_v, tap_k, tap_v)  # keep the tensors alive
-    _check(load().dovetail_draft_set_forcing(h.ptr, _dp(force_hhat), _dp(force_k), _dp(force_v), _dp(tap_k), _dp(tap_v)),
-           h.ptr)
+def dovetail_draft_status(h: Draft, stream=None):
+    """Synchronises the stream; raises DovetailError(EINVAL) if a step saw a token id outside [0, vocab)."""
+    _check(load().dovetail_draft_status(h.ptr, _stream(stream)), h.ptr)
 
 
 N_KINDS = 11
@@ -261,17 +292,44 @@ KIND_NAMES = ("step_begin", "dgf_proj", "dgf_gate", "qkv", "tree_attention", "o_
               "lm_head", "tree_level", "h_fill")
 
 
-def dovetail_draft_set_profile(h: Draft, enable: bool):
-    _check(load().dovetail_draft_set_profile(h.ptr, 1 if enable else 0), h.ptr)
+def dovetail_trace_enable(h: Draft, enable: bool):
+    _check(load().dovetail_trace_enable(h.ptr, 1 if enable else 0), h.ptr)
 
 
-def dovetail_profile_read(h: Draft) -> Dict[str, Dict]:
-    """Per-kind totals of the last (profiled, synchronised) step: ms, launches, algorithmic bytes."""
-    ms = (C.c_float * N_KINDS)()
-    n = (C.c_int32 * N_KINDS)()
-    b = (C.c_int64 * N_KINDS)()
-    _check(load().dovetail_profile_read(h.ptr, ms, n, b), h.ptr)
-    return {KIND_NAMES[k]: dict(ms=ms[k], launches=n[k], bytes=b[k]) for k in range(N_KINDS)}
+def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
+    """Device time of the last traced, synchronised step from the per-launch globaltimer stamps (the
+    launches keep their PDL overlap). Returns step_us (first start to last end), per-kind and per-level
+    busy_us (sum of end - start) and excl_us (each launch clipped to start no earlier than the end of the
+    launches before it, so that kinds / levels add up to at most the step), launches and algorithmic bytes."""
+    kind = (C.c_int32 * cap)()
+    level = (C.c_int32 * cap)()
+    nbytes = (C.c_int64 * cap)()
+    t0 = (C.c_uint64 * cap)()
+    t1 = (C.c_uint64 * cap)()
+    n = C.c_int32(0)
+    _check(load().dovetail_trace_read(h.ptr, cap, kind, level, nbytes, t0, t1, C.byref(n)), h.ptr)
+    kinds = {name: dict(busy_us=0.0, excl_us=0.0, launches=0, bytes=0) for name in KIND_NAMES}
+    levels: Dict[int, Dict] = {}
+    first, last, prev_end = None, 0, 0
+    for i in range(n.value):
+        a, b = t0[i], t1[i]
+        if a == 2 ** 64 - 1 or b == 0 or b < a:  # the launch did not stamp
+            continue
+        first = a if first is None else min(first, a)
+        last = max(last, b)
+        c0 = max(a, prev_end)
+        prev_end = max(prev_end, b)
+        for rec in (kinds[KIND_NAMES[kind[i]]], levels.setdefault(level[i], dict(busy_us=0.0, excl_us=0.0, launches=0, bytes=0))):
+            rec["busy_us"] += (b - a) * 1e-3
+            rec["excl_us"] += max(0, b - c0) * 1e-3
+            rec["launches"] += 1
+            rec["bytes"] += nbytes[i]
+    return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
+
+
+def dovetail_probe_stream(h: Draft, buf, mode: int, seg: int = 1024, stream=None):
+    """Read-only streaming ceiling probe (include/dovetail_hooks.h) over a device tensor; asynchronous."""
+    _check(load().dovetail_probe_stream(h.ptr, _dp(buf), buf.numel() * buf.element_size(), mode, seg, _stream(stream)), h.ptr)
 
 
 def dovetail_last_launch_count(h: Draft) -> int:

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdovetail_draft.so")
 SOURCES = ["dovetail_draft.cu"]
-HEADERS = ["ptx.cuh", "state.cuh", "gemv.cuh", "gemv_mma.cuh", "attention.cuh", "attention_mma.cuh", "tree.cuh"]
+HEADERS = ["ptx.cuh", "state.cuh", "gemv.cuh", "gemv_mma.cuh", "attention.cuh", "attention_mma.cuh", "tree.cuh", "stream_probe.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 
@@ -29,7 +29,7 @@ def _stale() -> bool:
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in SOURCES + HEADERS]
-    deps.append(os.path.join(os.path.dirname(_HERE), "include", "dovetail.h"))
+    deps += [os.path.join(os.path.dirname(_HERE), "include", f) for f in ("dovetail.h", "dovetail_hooks.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -48,6 +48,7 @@ class DraftConfig:
     dgf_proj: int = 1
     first_layer_input_norm: int = 1
     final_norm: int = 0
+    fusion: int = 0           # 0: DGF; 1: concat + one Linear 2d -> d, the EAGLE-2 baseline
     prefix: int = 64          # committed KV length L of the workload
     feat_scale: float = 1.0   # features ~ N(0,1) * feat_scale
     tree: TreeSpec = field(default_factory=lambda: TreeSpec(1, (1,), (0,), 1))
@@ -57,12 +58,16 @@ class DraftConfig:
     def esize(self) -> int:
         return 4 if self.dtype == F32 else 2
 
+    @property
+    def fusion_name(self) -> str:
+        return "concat+linear (EAGLE-2 baseline)" if self.fusion == 1 else ("DGF" if self.dgf_proj else "DGF without projections")
+
     def weight_params(self) -> Dict[str, int]:
         """Parameter counts by group; the draft's learnable parameters exclude
         the embedding and the LM head, which are the target's (Table 6)."""
         d, F = self.hidden, self.ffn
         dq, dkv = self.n_q_heads * self.head_dim, self.n_kv_heads * self.head_dim
-        dgf = (2 * d * d if self.dgf_proj else 0) + 2 * d * d + d
+        dgf = (2 * d * d if (self.dgf_proj and self.fusion == 0) else 0) + 2 * d * d + d
         layer = d * dq + 2 * d * dkv + dq * d + 3 * d * F + 2 * d
         return dict(dgf=dgf, layer=layer, layers=layer * self.n_layers, lm_head=self.vocab * d,
                     final_norm=d if self.final_norm else 0)
@@ -117,6 +122,17 @@ def c4_sweep() -> List[DraftConfig]:
         for m in (4, 8, 16, 32):
             out.append(replace(_C3, name=f"c4_l{layers}_m{m}", n_layers=layers, prefix=2048,
                                tree=TreeSpec(2, (m, 2), (0, m), 16), seed=1237))
+    return out
+
+
+def depth_sweep() -> List[DraftConfig]:
+    """The ablation's shape (Table 6, Table 7 :373-383) as a latency-vs-depth sweep on the
+    7B-shaped draft: the EAGLE-2 baseline (concat + Linear, 1 block, "w/o both"), then DGF with 1 ... 6 blocks
+    ("w/ DGF", "w/ DGF + 1" ... "+ 5"), prefix 512, the paper's 16-candidate server tree shape of C3."""
+    tree = TreeSpec(5, (2,) * 5, (0, 2, 2, 2, 2), 16)
+    out = [replace(_C2, name="depth_eagle2_l1", n_layers=1, fusion=1, dgf_proj=0, tree=tree, seed=1239)]
+    for layers in range(1, 7):
+        out.append(replace(_C2, name=f"depth_dgf_l{layers}", n_layers=layers, tree=tree, seed=1239))
     return out
 
 

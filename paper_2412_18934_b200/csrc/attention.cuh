@@ -20,11 +20,6 @@
 
 namespace dvt {
 
-#ifdef DVT_TRACE  // microbenchmark builds only
-#define DVT_ASTAMP(i) do { if (threadIdx.x == 0 && p.trace) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[(static_cast<size_t>(blockIdx.y) * gridDim.x + blockIdx.x) * 8 + (i)] = t_; } } while (0)
-#else
-#define DVT_ASTAMP(i) do { } while (0)
-#endif
 
 constexpr int kAttnStagePos = 32;  // positions per ring stage
 
@@ -48,7 +43,8 @@ struct AttnParams {
   const void* kc;
   const void* vc;
   int32_t cap, Lbase;
-  unsigned long long* trace;  // DVT_TRACE builds only
+  int32_t Lsafe;           // committed_len at step entry: rows below it are never written by the step
+  unsigned long long* trace;  // dovetail_trace_*: {first CTA start, last CTA end} of this launch, or NULL
 };
 
 struct SoftState {  // running (max, sum) of one query vector
@@ -125,12 +121,10 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     }
     mbar_fence_init();
   }
-  DVT_ASTAMP(0);
   __syncthreads();
   pdl_launch_dependents();
+  trace_begin(p.trace);
   pdl_wait();  // q/k/v of this level and the step's dynamic state are visible
-
-  DVT_ASTAMP(1);
   const StepDyn* dyn = p.dyn;
   const int Lbase = p.level0 ? dyn->L : dyn->Lp;
   const int cap = dyn->capacity;
@@ -191,7 +185,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     }
     __threadfence_block();
     consumer_sync();
-    DVT_ASTAMP(2);
   }
 
   for (int qt = 0; qt < n_qt; ++qt) {
@@ -219,7 +212,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
         for (int e = 0; e < EPU; ++e) q[t][e] = 0.f;
       }
     }
-    DVT_ASTAMP(3);
     float mrun[QT], lrun[QT], o[QT][EPU];
 #pragma unroll
     for (int t = 0; t < QT; ++t) {
@@ -275,8 +267,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       __syncwarp();
       if (lane == 0) mbar_arrive(&empty[slot]);
     }
-
-    DVT_ASTAMP(4);
     // ---- the new region: earlier rows of this step, masked per row ------------
     if (c == 0) {
       for (int j0 = 0; j0 < p.new_cnt; j0 += NG) {
@@ -303,8 +293,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
         update(kf, vf, ok);
       }
     }
-
-    DVT_ASTAMP(5);
     // ---- merge the row groups of the warp, then the warps ---------------------
 #pragma unroll
     for (int t = 0; t < QT; ++t) {
@@ -349,8 +337,6 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
     }
     consumer_sync();  // wsm is reused by the next query tile
   }
-
-  DVT_ASTAMP(6);
   if (n_chunks > 1) {
     // the last CTA of this kv-head to arrive merges all chunks in chunk order
     __threadfence();
@@ -382,7 +368,7 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       if (tid == 0) p.counters[hk] = 0;
     }
   }
-  DVT_ASTAMP(7);
+  trace_end(p.trace);
 }
 
 }  // namespace dvt

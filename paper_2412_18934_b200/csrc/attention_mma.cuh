@@ -108,7 +108,8 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   uint64_t* full = reinterpret_cast<uint64_t*>(ring + kAmStages * BLK_BYTES);
   uint64_t* empty = full + 4;
   uint64_t* tailbar = empty + 4;
-  int* flag_s = reinterpret_cast<int*>(tailbar + 1);
+  uint64_t* gatebar = tailbar + 1;  // a consumer has passed griddepcontrol.wait
+  int* flag_s = reinterpret_cast<int*>(gatebar + 1);
   // The warp-merge scratch and this CTA's record alias the ring: when they are written every block of
   // the pass has been consumed, and the producers resume only after the pass's second cluster barrier.
   float* wsm = reinterpret_cast<float*>(ring);  // [warps][QR][WSTR]
@@ -131,11 +132,12 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       mbar_init(&empty[s], kAmWarps);
     }
     mbar_init(tailbar, kAmConsumers);
+    mbar_init(gatebar, 1);
     mbar_fence_init();
   }
-  DVT_ASTAMP(0);
   __syncthreads();
   pdl_launch_dependents();
+  trace_begin(p.trace);
 
   const int Lbase = p.Lbase, cap = p.cap;
   const WT* kc = static_cast<const WT*>(p.kc) + (static_cast<size_t>(p.layer) * p.Hkv + hk) * cap * DH;
@@ -153,14 +155,23 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   if (warp >= kAmWarps) {
     // ---------------- producers ---------------------------------------------------
     const int ptid = tid - kAmConsumers;
+    // Invariant: before griddepcontrol.wait only cache rows below p.Lsafe -- the
+    // prefix committed before this step, which no kernel of the step writes -- may be read. Rows
+    // [Lsafe, Lbase) of a tree level were appended by this step's level-0 kernels, several launches
+    // back; programmatic dependent launch orders a kernel only against its immediate predecessor and
+    // only after the wait, so blocks that reach past Lsafe are gated on a consumer having waited.
     int slot = 0, round = 0;
-    bool tail_ready = false;
+    bool tail_ready = false, gate_open = false;
     for (int pass = 0; pass < n_pass; ++pass) {
       for (int b = 0; b < nb; ++b) {
         int pos0, cnt;
         if (b < n_blk) {
           pos0 = p_begin + b * PB;
           cnt = min(PB, p_end - pos0);
+          if (!gate_open && pos0 + cnt > p.Lsafe) {
+            mbar_wait(gatebar, 0);
+            gate_open = true;
+          }
         } else {
           if (!tail_ready) {  // this level's rows are appended by the consumers first
             mbar_wait(tailbar, 0);
@@ -193,7 +204,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
 
   // ---------------- consumers -----------------------------------------------------
   pdl_wait();  // q/k/v of this level and the row tables are visible from here on
-  DVT_ASTAMP(1);
+  if (tid == 0) mbar_arrive(gatebar);
   const RowTables* rows = p.rows;
   const int g = lane >> 2, tq = lane & 3;
   const float scale = 1.0f / sqrtf(static_cast<float>(DH));
@@ -220,7 +231,6 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     }
     __threadfence();
     mbar_arrive(tailbar);
-    DVT_ASTAMP(2);
   }
 
   int slot = 0, round = 0;
@@ -251,7 +261,6 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       }
     }
     am_consumer_sync();
-    DVT_ASTAMP(3);
 
     // rows of this thread's accumulators: g and g + 8; their draft rows for the tail masks
     int mrow[2];
@@ -367,7 +376,6 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       if (lane == 0) mbar_arrive(&empty[slot]);
       if (++slot == kAmStages) { slot = 0; ++round; }
     }
-    DVT_ASTAMP(5);
     am_consumer_sync();  // every warp is done with the ring: the merge scratch aliases it
 
     // ---- merge the four warps (fixed order), then hand the chunk's partial on ------
@@ -446,7 +454,6 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     }
     cluster_sync_all();  // every rank has read the records: they (and the query tiles) may be reused
   }
-  DVT_ASTAMP(6);
 
   if (n_groups > 1 && crank == 0) {
     // the last cluster leader of this kv-head to arrive merges all groups in group order
@@ -505,7 +512,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       if (tid == 0) p.counters[hk] = 0;
     }
   }
-  DVT_ASTAMP(7);
+  trace_end(p.trace);
 }
 
 }  // namespace dvt

@@ -10,17 +10,18 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
 
 #include "../../include/dovetail.h"
+#include "../../include/dovetail_hooks.h"
 #include "attention.cuh"
 #include "attention_mma.cuh"
 #include "gemv.cuh"
 #include "gemv_mma.cuh"
 #include "state.cuh"
+#include "stream_probe.cuh"
 #include "tree.cuh"
 
 using namespace dvt;
@@ -66,29 +67,26 @@ struct dovetail_draft {
   uint32_t* treemask = nullptr;
   int32_t* out_pool_idx = nullptr;
   TreeState* ts_host = nullptr;  // pinned
-  // taps (borrowed)
-  float* tap_logits = nullptr;
-  float* tap_hhat = nullptr;
-  // teacher forcing for parity tests (borrowed)
-  const float* force_hhat = nullptr;
-  const void* force_k = nullptr;
-  const void* force_v = nullptr;
-  void* tap_k = nullptr;
-  void* tap_v = nullptr;
+  // test / measurement hooks (dovetail_hooks.h); never set in a plain step
+  dovetail_hooks_t hooks{};
+  bool hooks_on = false;
   // last step
   bool have_step = false;
   int last_n_new = 0, last_depth = 0, last_gamma = 0;
   int last_launches = 0;
   int launches = 0;
-  // optional per-kernel timing
-  bool profile = false;
-  bool force_fma = false;  // DOVETAIL_FORCE_FMA=1: bf16 GEMVs on the FMA kernel (for A/B measurements)
+  bool dry = false;  // shape-checking pass of dovetail_draft_step: nothing is launched
+  // per-launch time stamps (dovetail_trace_*)
+  bool trace_on = false;
+  unsigned long long* trace_buf = nullptr;  // device [kMaxTraceLaunches][2]
+  unsigned long long* trace_host = nullptr; // pinned
   int cur_kind = 0;
   int64_t cur_bytes = 0;
-  std::vector<cudaEvent_t> ev;       // 2 per launch
-  std::vector<int> ev_kind;
-  std::vector<int64_t> ev_bytes;
-  int ev_used = 0;
+  int cur_level = 0;
+  float* probe_sink = nullptr;
+  std::vector<int> tr_kind, tr_level;
+  std::vector<int64_t> tr_bytes;
+  int tr_used = 0;
   char err[512] = "no error";
 };
 
@@ -106,46 +104,53 @@ int fail(dovetail_draft* h, int code, const char* fmt, ...) {
 // ---- launch helper: every kernel is launched with the programmatic-stream-
 // serialization attribute so that its prologue / weight prefetch overlaps the
 // tail of its predecessor; the kernels call griddepcontrol.wait themselves.
+constexpr int kMaxTraceLaunches = 4096;
+
+// Time-stamp slot of the launch about to be made (NULL unless tracing); records its kind / bytes.
+unsigned long long* trace_slot(dovetail_draft* h) {
+  if (!h->trace_on || h->dry || h->launches >= kMaxTraceLaunches) return nullptr;
+  const int i = h->launches;
+  if (static_cast<int>(h->tr_kind.size()) <= i) { h->tr_kind.resize(i + 1); h->tr_level.resize(i + 1); h->tr_bytes.resize(i + 1); }
+  h->tr_kind[i] = h->cur_kind;
+  h->tr_level[i] = h->cur_level;
+  h->tr_bytes[i] = h->cur_bytes;
+  h->tr_used = i + 1;
+  return h->trace_buf + 2 * static_cast<size_t>(i);
+}
+
 template <typename... KArgs, typename... Args>
-cudaError_t launch_c(dovetail_draft* h, int cluster_x, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
-                     cudaStream_t st, Args... args) {
+cudaError_t launch_c(dovetail_draft* h, int cluster_x, bool pdl, void (*kern)(KArgs...), dim3 grid, dim3 block,
+                     size_t smem, cudaStream_t st, Args... args) {
+  if (h->dry) return cudaSuccess;
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = grid;
   cfg.blockDim = block;
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cudaLaunchAttribute attr[2];
-  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  attr[0].val.programmaticStreamSerializationAllowed = 1;
-  attr[1].id = cudaLaunchAttributeClusterDimension;  // thread-block cluster along x (attention chunks)
-  attr[1].val.clusterDim.x = cluster_x;
-  attr[1].val.clusterDim.y = 1;
-  attr[1].val.clusterDim.z = 1;
-  cfg.attrs = attr;
-  cfg.numAttrs = cluster_x > 1 ? 2 : 1;
-  ++h->launches;
-  if (!h->profile) return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
-  // profiling: bracket the launch with events (serialises the kernels)
-  const int i = h->ev_used++;
-  while (static_cast<int>(h->ev.size()) < 2 * (i + 1)) {
-    cudaEvent_t e;
-    cudaError_t r = cudaEventCreate(&e);
-    if (r != cudaSuccess) return r;
-    h->ev.push_back(e);
+  int na = 0;
+  if (pdl) {
+    attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
   }
-  if (static_cast<int>(h->ev_kind.size()) <= i) { h->ev_kind.resize(i + 1); h->ev_bytes.resize(i + 1); }
-  h->ev_kind[i] = h->cur_kind;
-  h->ev_bytes[i] = h->cur_bytes;
-  cudaEventRecord(h->ev[2 * i], st);
-  cudaError_t r = cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
-  cudaEventRecord(h->ev[2 * i + 1], st);
-  return r;
+  if (cluster_x > 1) {  // thread-block cluster along x (attention chunks)
+    attr[na].id = cudaLaunchAttributeClusterDimension;
+    attr[na].val.clusterDim.x = cluster_x;
+    attr[na].val.clusterDim.y = 1;
+    attr[na].val.clusterDim.z = 1;
+    ++na;
+  }
+  cfg.attrs = attr;
+  cfg.numAttrs = na;
+  ++h->launches;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
 }
 
 template <typename... KArgs, typename... Args>
 cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem,
                    cudaStream_t st, Args... args) {
-  return launch_c(h, 1, kern, grid, block, smem, st, args...);
+  return launch_c(h, 1, true, kern, grid, block, smem, st, args...);
 }
 
 using GemvKernel = void (*)(const GemvParams);
@@ -317,7 +322,7 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
     if (mc > max_cnt) max_cnt = mc;
   }
   p.dyn = h->dyn;
-  if (h->es == 2 && !h->force_fma) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
+  if (h->es == 2) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
     // Levels wider than 16 rows run in chunks of <= 16 rows (the weights are streamed once per chunk):
     // beyond 32 B columns the split activations no longer fit next to a useful ring.
     const int Mtot = p.M, chunk = Mtot > 16 ? 16 : Mtot;
@@ -337,6 +342,7 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
         p.seg_stride = ms.seg_stride;
         p.bs_stride = ms.bs_stride;
         if (m0 > 0) h->cur_bytes = 0;  // the algorithmic bytes are counted once
+        p.trace = trace_slot(h);
         cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
         if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
       }
@@ -351,6 +357,7 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
   p.row_bytes = s.row_bytes;
   p.dyn = h->dyn;
   GemvKernel k = h->es == 2 ? pick_gemv<__nv_bfloat16>(s.MT, s.NI) : pick_gemv<float>(s.MT, s.NI);
+  p.trace = trace_slot(h);
   cudaError_t e = launch(h, k, dim3(ctas_per_group, n_groups), dim3(kThreads), s.smem, st, p);
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
@@ -415,7 +422,320 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
   if (h->ts_host) cudaFreeHost(h->ts_host);
-  for (cudaEvent_t e : h->ev) cudaEventDestroy(e);
+  cudaFree(h->trace_buf);
+  cudaFree(h->probe_sink);
+  if (h->trace_host) cudaFreeHost(h->trace_host);
+}
+
+// Test hooks of one level (dovetail_hooks.h): taps of what the level computed, then teacher forcing.
+int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* kv, const LevelPlan& lp, int l, int L,
+                int Lp) {
+  const dovetail_config_t& c = h->cfg;
+  const dovetail_hooks_t& k = h->hooks;
+  const int d = c.hidden, dh = c.head_dim, M = lp.rows;
+  cudaError_t e = cudaSuccess;
+  const size_t xoff = static_cast<size_t>(lp.row0) * d, xbytes = static_cast<size_t>(M) * d * sizeof(float);
+  if (k.tap_hhat) e = cudaMemcpyAsync(k.tap_hhat + xoff, h->hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
+  if (k.force_hhat && e == cudaSuccess)
+    e = cudaMemcpyAsync(h->hhat + xoff, k.force_hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
+  const size_t pitch = static_cast<size_t>(kv->capacity) * dh * h->es, width = static_cast<size_t>(M) * dh * h->es;
+  const size_t off = static_cast<size_t>(l == 0 ? L : Lp + lp.t0) * dh * h->es;
+  const size_t height = static_cast<size_t>(c.n_layers) * c.n_kv_heads;
+  auto cp2 = [&](void* dst, const void* src) {
+    if (dst && src && e == cudaSuccess)
+      e = cudaMemcpy2DAsync(static_cast<uint8_t*>(dst) + off, pitch, static_cast<const uint8_t*>(src) + off, pitch, width,
+                            height, cudaMemcpyDeviceToDevice, st);
+  };
+  cp2(k.tap_k, kv->k);
+  cp2(k.tap_v, kv->v);
+  cp2(kv->k, k.force_k);
+  cp2(kv->v, k.force_v);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap / forcing copy failed: %s", cudaGetErrorString(e));
+  return DOVETAIL_OK;
+}
+
+// Enqueues (or, with h->dry, only shape-checks) the kernels of one draft step.
+int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, const int32_t* tokens, int n_new,
+                 dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree, const dovetail_draft_out_t* out,
+                 const std::vector<LevelPlan>& plan, int pool_total) {
+  const dovetail_config_t& c = h->cfg;
+  const int L = kv->committed_len, Lp = L + n_new;
+  int rc = DOVETAIL_OK;
+  h->launches = 0;
+  const int d = c.hidden, F = c.ffn, V = c.vocab, dh = c.head_dim, half = dh / 2;
+  const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
+  const int grp = c.n_q_heads / c.n_kv_heads;
+  const bool bf16 = c.dtype == DOVETAIL_BF16;
+  cudaError_t e;
+
+  // S0: per-step state, level-0 row tables, rotary table
+  StepDyn dv{};
+  dv.feats = hidden_feats;
+  dv.tokens = tokens;
+  dv.kc = kv->k;
+  dv.vc = kv->v;
+  dv.capacity = kv->capacity;
+  dv.L = L;
+  dv.n_new = n_new;
+  dv.Lp = Lp;
+  dv.out_ids = out->token_ids;
+  dv.out_scores = out->scores;
+  dv.out_parents = out->parents;
+  dv.out_depths = out->depths;
+  dv.out_n = out->n_out;
+  h->cur_kind = 0;
+  h->cur_bytes = 0;
+  h->cur_level = 0;
+  if (h->trace_on && !h->dry) {  // start = ~0 (atomicMin), end = 0 (atomicMax)
+    e = cudaMemsetAsync(h->trace_buf, 0, sizeof(unsigned long long) * 2 * kMaxTraceLaunches, st);
+    if (e == cudaSuccess) e = cudaMemset2DAsync(h->trace_buf, 16, 0xff, 8, kMaxTraceLaunches, st);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "trace reset failed: %s", cudaGetErrorString(e));
+  }
+  // k_step_begin is launched WITHOUT programmatic serialization: it starts only once everything
+  // enqueued before the step has completed, which is what lets later kernels read the committed
+  // prefix (cache rows < L) before their griddepcontrol.wait.
+  e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(64), 0, st, dv, h->dyn, h->ts, h->rt,
+               h->rope, static_cast<const double*>(h->inv_freq), half, V, trace_slot(h));
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+
+  for (int l = 0; l < tree->depth; ++l) {
+    const LevelPlan& lp = plan[l];
+    const int M = lp.rows;
+    h->cur_level = l;
+    RowTables* cur = h->rt + (l & 1);
+    RowTables* nxt = h->rt + ((l + 1) & 1);
+    float* x = h->hhat + static_cast<size_t>(lp.row0) * d;  // residual stream rows of this level
+
+    // S0 + S1: gather, DGF projections h1 = W1 f, h2 = W2 e (PAPER.md:104)
+    if (c.dgf_proj) {
+      GemvParams p{};
+      p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
+      p.g[0].w[0] = h->w.dgf_w1;
+      p.g[0].rows[0] = d;
+      p.g[0].n_mat = 1;
+      p.g[0].out_off = 0;
+      p.g[1] = GemvGroup{};
+      p.g[1].xkind = X_EMBED;
+      p.g[1].embed = h->w.embed;
+      p.g[1].tokens = cur->token;
+      p.g[1].w[0] = h->w.dgf_w2;
+      p.g[1].rows[0] = d;
+      p.g[1].n_mat = 1;
+      p.g[1].out_off = d;
+      p.K = d;
+      p.M = M;
+      p.epi = EPI_STORE;
+      p.out = h->hbuf;
+      p.out_ld = 2 * d;
+      rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)), 1);
+      if (rc) return rc;
+    } else {
+      const int blocks = std::min(nsm, div_up(M * 2 * d, 256));
+      h->cur_kind = 10;
+      h->cur_bytes = 0;
+      if (bf16)
+        e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
+                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
+                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d, trace_slot(h));
+      else
+        e = launch(h, k_fill_h<float>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
+                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
+                   static_cast<const float*>(h->w.embed), h->hbuf, M, d, trace_slot(h));
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+    }
+    {  // S1: gate, sigmoid, blend; or the single Linear of the EAGLE-2 fusion (:104)
+      GemvParams p{};
+      p.g[0] = rows_group(h->hbuf, 2 * d, nullptr, 0, nullptr);
+      p.g[0].w[0] = h->w.dgf_wg;
+      p.g[0].rows[0] = d;
+      p.g[0].n_mat = 1;
+      p.K = 2 * d;
+      p.M = M;
+      p.epi = c.fusion == DOVETAIL_FUSION_CONCAT_LINEAR ? EPI_STORE : EPI_DGF;
+      p.out = x;
+      p.out_ld = d;
+      p.hbuf = h->hbuf;
+      p.bias = h->w.dgf_bg;
+      p.d = d;
+      rc = run_gemv(h, st, p, 1, std::min(nsm, d), 2);
+      if (rc) return rc;
+    }
+
+    for (int ly = 0; ly < c.n_layers; ++ly) {
+      const dovetail_layer_weights_t& W = h->layers[ly];
+      {  // S2: RMSNorm + Q, K, V projections (PAPER.md:110-112)
+        GemvParams p{};
+        const void* gain = (ly == 0 && !c.first_layer_input_norm) ? nullptr : W.g_attn;
+        p.g[0] = rows_group(x, d, nullptr, 0, gain);
+        p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq;
+        p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv;
+        p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv;
+        p.g[0].n_mat = 3;
+        p.K = d;
+        p.M = M;
+        p.eps = c.rms_eps;
+        p.epi = EPI_STORE;
+        p.out = h->qkv;
+        p.out_ld = ldq;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq), 3);
+        if (rc) return rc;
+      }
+      {  // S2 (RoPE, KV append) + S3 tree attention
+        AttnParams a{};
+        a.dyn = h->dyn;
+        a.qkv = h->qkv;
+        a.obuf = h->obuf;
+        a.rows = cur;
+        a.rope = h->rope;
+        a.rope_row0 = l == 0 ? 0 : n_new + l - 1;
+        a.rope_per_row = l == 0 ? 1 : 0;
+        a.M = M;
+        a.Hq = c.n_q_heads;
+        a.Hkv = c.n_kv_heads;
+        a.layer = ly;
+        a.level0 = l == 0 ? 1 : 0;
+        a.new_cnt = l == 0 ? n_new : lp.t0 + M;
+        a.n_stages = kAttnStages;
+        a.ws = h->attn_ws;
+        a.qv_cap = h->qv_cap;
+        a.counters = h->attn_cnt;
+        const int Lbase = l == 0 ? L : Lp;
+        const int qv_tot = M * grp;
+        h->cur_kind = 4;
+        h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
+        a.trace = trace_slot(h);
+        if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
+          a.kc = kv->k;
+          a.vc = kv->v;
+          a.cap = kv->capacity;
+          a.Lbase = Lbase;
+          a.Lsafe = L;
+          const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
+          // Chunks per kv-head (measured on C2 / C3 / C5): at least two 64-position blocks per chunk (a CTA's
+          // fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one cluster of 8
+          // no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
+          int n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2)), cs;
+          if (n_chunks <= 8) {
+            n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
+            cs = n_chunks;
+          } else {
+            n_chunks = std::max(8, std::min(n_chunks, 200 / c.n_kv_heads) / 8 * 8);
+            cs = 8;
+          }
+          const size_t smem = am_smem_bytes(dh);
+          e = launch_c(h, cs, true, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
+                       dim3(kAmThreads), smem, st, a);
+        } else {
+          int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
+          const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
+          const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
+          const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
+                              static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
+          e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
+        }
+        if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "attention launch failed: %s", cudaGetErrorString(e));
+      }
+      {  // S4: x += Wo o
+        GemvParams p{};
+        p.g[0] = rows_group(h->obuf, dq, nullptr, 0, nullptr);
+        p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        p.K = dq;
+        p.M = M;
+        p.epi = EPI_RESID;
+        p.out = x;
+        p.out_ld = d;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 5);
+        if (rc) return rc;
+      }
+      {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
+        GemvParams p{};
+        p.g[0] = rows_group(x, d, nullptr, 0, W.g_ffn);
+        p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F;
+        p.g[0].w[1] = W.wup; p.g[0].rows[1] = F;
+        p.g[0].n_mat = 2;
+        p.g[0].paired = 1;
+        p.K = d;
+        p.M = M;
+        p.eps = c.rms_eps;
+        p.epi = EPI_SWIGLU;
+        p.out = h->act;
+        p.out_ld = F;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, F), 6);
+        if (rc) return rc;
+      }
+      {  // S5b: x += Wdown act
+        GemvParams p{};
+        p.g[0] = rows_group(h->act, F, nullptr, 0, nullptr);
+        p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        p.K = F;
+        p.M = M;
+        p.epi = EPI_RESID;
+        p.out = x;
+        p.out_ld = d;
+        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 7);
+        if (rc) return rc;
+      }
+    }
+
+    const int lm_ctas = std::min(nsm, V);
+    {  // S6: LM head + per-CTA top-b + softmax statistics. Level 0: the last row seeds the tree.
+      GemvParams p{};
+      const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
+      p.g[0] = rows_group(xs, d, nullptr, 0, c.final_norm ? h->w.g_final : nullptr);
+      p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1;
+      p.K = d;
+      p.M = lp.rows_lm;
+      p.eps = c.rms_eps;
+      p.epi = EPI_LMHEAD;
+      p.b = tree->branch[l];
+      p.vocab = V;
+      p.cand_val = h->cand_val;
+      p.cand_id = h->cand_id;
+      p.stat = h->stat;
+      p.tap = h->hooks.tap_logits ? h->hooks.tap_logits + static_cast<size_t>(lp.row0 + (l == 0 ? n_new - 1 : 0)) * V : nullptr;
+      rc = run_gemv(h, st, p, 1, lm_ctas, 8);
+      if (rc) return rc;
+    }
+    {  // S7 (+ S8 after the last level)
+      TreeLevelParams t{};
+      t.dyn = h->dyn;
+      t.ts = h->ts;
+      t.pool = h->pool;
+      t.treemask = h->treemask;
+      t.cand_val = h->cand_val;
+      t.cand_id = h->cand_id;
+      t.stat = h->stat;
+      t.nct = lm_ctas;
+      t.M = lp.rows_lm;
+      t.b = tree->branch[l];
+      t.level = l;
+      t.pool_begin = lp.pool_begin;
+      const bool last = l + 1 == tree->depth;
+      t.M_next = last ? 0 : plan[l + 1].rows;
+      t.next_row0 = last ? 0 : plan[l + 1].row0;
+      t.next_t0 = last ? 0 : plan[l + 1].t0;
+      t.n_new = n_new;
+      t.cur = cur;
+      t.next = nxt;
+      t.gamma = tree->gamma;
+      t.pool_total = pool_total;
+      t.out_pool_idx = h->out_pool_idx;
+      t.tap_token = h->hooks.tap_pool_token;
+      t.tap_cum = h->hooks.tap_pool_cum;
+      t.force_token = h->hooks.force_pool_token;
+      t.force_cum = h->hooks.force_pool_cum;
+      h->cur_kind = 9;
+      h->cur_bytes = 0;
+      t.trace = trace_slot(h);
+      e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
+    }
+    if (h->hooks_on && !h->dry) {
+      rc = level_hooks(h, st, kv, lp, l, L, Lp);
+      if (rc) return rc;
+    }
+  }
+  return DOVETAIL_OK;
 }
 
 }  // namespace
@@ -429,7 +749,9 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   if (c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.n_q_heads % c.n_kv_heads != 0 ||
       (c.head_dim != 64 && c.head_dim != 128) || c.n_layers < 1 || c.n_layers > DOVETAIL_MAX_LAYERS ||
       c.ffn < 8 || c.vocab < 1 || !(c.rope_theta > 0.f) || !(c.rms_eps >= 0.f) ||
-      (c.dtype != DOVETAIL_F32 && c.dtype != DOVETAIL_BF16))
+      (c.dtype != DOVETAIL_F32 && c.dtype != DOVETAIL_BF16) ||
+      (c.fusion != DOVETAIL_FUSION_DGF && c.fusion != DOVETAIL_FUSION_CONCAT_LINEAR) ||
+      (c.fusion == DOVETAIL_FUSION_CONCAT_LINEAR && c.dgf_proj))
     return fail(nullptr, DOVETAIL_EINVAL, "bad model shape");
   if (c.max_rows < 1 || c.max_rows > kMaxRows || c.max_tree_slots < 0 || c.max_tree_slots > kMaxTreeSlots ||
       c.max_branch < 1 || c.max_branch > kMaxBranch)
@@ -463,10 +785,6 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   h->layers.assign(w->layers, w->layers + c.n_layers);
   h->w.layers = h->layers.data();
   h->num_sms = prop.multiProcessorCount;
-  {
-    const char* ev = getenv("DOVETAIL_FORCE_FMA");
-    h->force_fma = ev && ev[0] == '1';
-  }
   h->es = es;
   h->dq = dq;
   h->dkv = dkv;
@@ -543,286 +861,15 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
     return fail(h, DOVETAIL_ECAPACITY, "KV cache too small: %d committed + %d new + %d tree rows > capacity %d", L, n_new, tree_rows, kv->capacity);
 
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  h->launches = 0;
-  const int d = c.hidden, F = c.ffn, V = c.vocab, dh = c.head_dim, half = dh / 2;
-  const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
-  const int grp = c.n_q_heads / c.n_kv_heads;
-  const bool bf16 = c.dtype == DOVETAIL_BF16;
-  cudaError_t e;
-
-  // S0: per-step state, level-0 row tables, rotary table
-  StepDyn dv{};
-  dv.feats = hidden_feats;
-  dv.tokens = tokens;
-  dv.kc = kv->k;
-  dv.vc = kv->v;
-  dv.capacity = kv->capacity;
-  dv.L = L;
-  dv.n_new = n_new;
-  dv.Lp = Lp;
-  dv.out_ids = out->token_ids;
-  dv.out_scores = out->scores;
-  dv.out_parents = out->parents;
-  dv.out_depths = out->depths;
-  dv.out_n = out->n_out;
-  h->ev_used = 0;
-  h->cur_kind = 0;
-  h->cur_bytes = 0;
-  e = launch(h, k_step_begin, dim3(n_new + tree->depth - 1), dim3(64), 0, st, dv, h->dyn, h->ts, h->rt, h->rope,
-             static_cast<const double*>(h->inv_freq), half, V);
-  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
-
-  for (int l = 0; l < tree->depth; ++l) {
-    const LevelPlan& lp = plan[l];
-    const int M = lp.rows;
-    RowTables* cur = h->rt + (l & 1);
-    RowTables* nxt = h->rt + ((l + 1) & 1);
-    float* x = h->hhat + static_cast<size_t>(lp.row0) * d;  // residual stream rows of this level
-
-    // S0 + S1: gather, DGF projections h1 = W1 f, h2 = W2 e (PAPER.md:104)
-    if (c.dgf_proj) {
-      GemvParams p{};
-      p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
-      p.g[0].w[0] = h->w.dgf_w1;
-      p.g[0].rows[0] = d;
-      p.g[0].n_mat = 1;
-      p.g[0].out_off = 0;
-      p.g[1] = GemvGroup{};
-      p.g[1].xkind = X_EMBED;
-      p.g[1].embed = h->w.embed;
-      p.g[1].tokens = cur->token;
-      p.g[1].w[0] = h->w.dgf_w2;
-      p.g[1].rows[0] = d;
-      p.g[1].n_mat = 1;
-      p.g[1].out_off = d;
-      p.K = d;
-      p.M = M;
-      p.epi = EPI_STORE;
-      p.out = h->hbuf;
-      p.out_ld = 2 * d;
-      rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)), 1);
-      if (rc) return rc;
-    } else {
-      const int blocks = std::min(nsm, div_up(M * 2 * d, 256));
-      h->cur_kind = 10;
-      h->cur_bytes = 0;
-      if (bf16)
-        e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
-                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
-                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d);
-      else
-        e = launch(h, k_fill_h<float>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
-                   static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
-                   static_cast<const float*>(h->w.embed), h->hbuf, M, d);
-      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
-    }
-    {  // S1: gate, sigmoid, blend
-      GemvParams p{};
-      p.g[0] = rows_group(h->hbuf, 2 * d, nullptr, 0, nullptr);
-      p.g[0].w[0] = h->w.dgf_wg;
-      p.g[0].rows[0] = d;
-      p.g[0].n_mat = 1;
-      p.K = 2 * d;
-      p.M = M;
-      p.epi = EPI_DGF;
-      p.out = x;
-      p.out_ld = d;
-      p.hbuf = h->hbuf;
-      p.bias = h->w.dgf_bg;
-      p.d = d;
-      rc = run_gemv(h, st, p, 1, std::min(nsm, d), 2);
-      if (rc) return rc;
-    }
-
-    for (int ly = 0; ly < c.n_layers; ++ly) {
-      const dovetail_layer_weights_t& W = h->layers[ly];
-      {  // S2: RMSNorm + Q, K, V projections (PAPER.md:110-112)
-        GemvParams p{};
-        const void* gain = (ly == 0 && !c.first_layer_input_norm) ? nullptr : W.g_attn;
-        p.g[0] = rows_group(x, d, nullptr, 0, gain);
-        p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq;
-        p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv;
-        p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv;
-        p.g[0].n_mat = 3;
-        p.K = d;
-        p.M = M;
-        p.eps = c.rms_eps;
-        p.epi = EPI_STORE;
-        p.out = h->qkv;
-        p.out_ld = ldq;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq), 3);
-        if (rc) return rc;
-      }
-      {  // S2 (RoPE, KV append) + S3 tree attention
-        AttnParams a{};
-        a.dyn = h->dyn;
-        a.qkv = h->qkv;
-        a.obuf = h->obuf;
-        a.rows = cur;
-        a.rope = h->rope;
-        a.rope_row0 = l == 0 ? 0 : n_new + l - 1;
-        a.rope_per_row = l == 0 ? 1 : 0;
-        a.M = M;
-        a.Hq = c.n_q_heads;
-        a.Hkv = c.n_kv_heads;
-        a.layer = ly;
-        a.level0 = l == 0 ? 1 : 0;
-        a.new_cnt = l == 0 ? n_new : lp.t0 + M;
-        a.n_stages = kAttnStages;
-        a.ws = h->attn_ws;
-        a.qv_cap = h->qv_cap;
-        a.counters = h->attn_cnt;
-        const int Lbase = l == 0 ? L : Lp;
-        const int qv_tot = M * grp;
-        h->cur_kind = 4;
-        h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
-        if (bf16 && !h->force_fma) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
-          a.kc = kv->k;
-          a.vc = kv->v;
-          a.cap = kv->capacity;
-          a.Lbase = Lbase;
-          const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
-          // Chunks per kv-head (measured on C2 / C3 / C5): at least two 64-position blocks per chunk (a CTA's
-          // fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one cluster of 8
-          // no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
-          int n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2)), cs;
-          if (n_chunks <= 8) {
-            n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
-            cs = n_chunks;
-          } else {
-            n_chunks = std::max(8, std::min(n_chunks, 200 / c.n_kv_heads) / 8 * 8);
-            cs = 8;
-          }
-          if (const char* ev = getenv("DOVETAIL_ATTN_CHUNKS")) {  // measurement override
-            n_chunks = std::max(1, std::min(atoi(ev), n_blocks));
-            cs = n_chunks <= 8 ? n_chunks : 8;
-            n_chunks = n_chunks / cs * cs;
-          }
-          const size_t smem = am_smem_bytes(dh);
-          e = launch_c(h, cs, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
-                       dim3(kAmThreads), smem, st, a);
-        } else {
-          int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
-          const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
-          const int stage_bytes = 2 * kAttnStagePos * dh * h->es;
-          const size_t smem = static_cast<size_t>(kAttnStages) * stage_bytes + 128 +
-                              static_cast<size_t>(kConsumerWarps) * QT * (dh + 2) * 4 + 16;
-          e = launch(h, pick_attn(c.dtype, dh, QT), dim3(n_chunks, c.n_kv_heads), dim3(kThreads), smem, st, a);
-        }
-        if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "attention launch failed: %s", cudaGetErrorString(e));
-      }
-      {  // S4: x += Wo o
-        GemvParams p{};
-        p.g[0] = rows_group(h->obuf, dq, nullptr, 0, nullptr);
-        p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
-        p.K = dq;
-        p.M = M;
-        p.epi = EPI_RESID;
-        p.out = x;
-        p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 5);
-        if (rc) return rc;
-      }
-      {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
-        GemvParams p{};
-        p.g[0] = rows_group(x, d, nullptr, 0, W.g_ffn);
-        p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F;
-        p.g[0].w[1] = W.wup; p.g[0].rows[1] = F;
-        p.g[0].n_mat = 2;
-        p.g[0].paired = 1;
-        p.K = d;
-        p.M = M;
-        p.eps = c.rms_eps;
-        p.epi = EPI_SWIGLU;
-        p.out = h->act;
-        p.out_ld = F;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, F), 6);
-        if (rc) return rc;
-      }
-      {  // S5b: x += Wdown act
-        GemvParams p{};
-        p.g[0] = rows_group(h->act, F, nullptr, 0, nullptr);
-        p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
-        p.K = F;
-        p.M = M;
-        p.epi = EPI_RESID;
-        p.out = x;
-        p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 7);
-        if (rc) return rc;
-      }
-    }
-
-    const int lm_ctas = std::min(nsm, V);
-    {  // S6: LM head + per-CTA top-b + softmax statistics. Level 0: the last row seeds the tree.
-      GemvParams p{};
-      const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
-      p.g[0] = rows_group(xs, d, nullptr, 0, c.final_norm ? h->w.g_final : nullptr);
-      p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1;
-      p.K = d;
-      p.M = lp.rows_lm;
-      p.eps = c.rms_eps;
-      p.epi = EPI_LMHEAD;
-      p.b = tree->branch[l];
-      p.vocab = V;
-      p.cand_val = h->cand_val;
-      p.cand_id = h->cand_id;
-      p.stat = h->stat;
-      p.tap = h->tap_logits ? h->tap_logits + static_cast<size_t>(lp.row0 + (l == 0 ? n_new - 1 : 0)) * V : nullptr;
-      rc = run_gemv(h, st, p, 1, lm_ctas, 8);
-      if (rc) return rc;
-    }
-    {  // S7 (+ S8 after the last level)
-      TreeLevelParams t{};
-      t.dyn = h->dyn;
-      t.ts = h->ts;
-      t.pool = h->pool;
-      t.treemask = h->treemask;
-      t.cand_val = h->cand_val;
-      t.cand_id = h->cand_id;
-      t.stat = h->stat;
-      t.nct = lm_ctas;
-      t.M = lp.rows_lm;
-      t.b = tree->branch[l];
-      t.level = l;
-      t.pool_begin = lp.pool_begin;
-      const bool last = l + 1 == tree->depth;
-      t.M_next = last ? 0 : plan[l + 1].rows;
-      t.next_row0 = last ? 0 : plan[l + 1].row0;
-      t.next_t0 = last ? 0 : plan[l + 1].t0;
-      t.n_new = n_new;
-      t.cur = cur;
-      t.next = nxt;
-      t.gamma = tree->gamma;
-      t.pool_total = pool_total;
-      t.out_pool_idx = h->out_pool_idx;
-      h->cur_kind = 9;
-      h->cur_bytes = 0;
-      e = launch(h, k_tree_level, dim3(1), dim3(kTreeThreads), 0, st, t);
-      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
-    }
-    // parity-test hooks: taps of this level's results, then teacher forcing (dovetail.h)
-    e = cudaSuccess;
-    const size_t xoff = static_cast<size_t>(lp.row0) * d, xbytes = static_cast<size_t>(M) * d * sizeof(float);
-    if (h->tap_hhat) e = cudaMemcpyAsync(h->tap_hhat + xoff, h->hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
-    if (h->force_hhat && e == cudaSuccess)
-      e = cudaMemcpyAsync(h->hhat + xoff, h->force_hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
-    {
-      const size_t pitch = static_cast<size_t>(kv->capacity) * dh * h->es, width = static_cast<size_t>(M) * dh * h->es;
-      const size_t off = static_cast<size_t>(l == 0 ? L : Lp + lp.t0) * dh * h->es, height = static_cast<size_t>(c.n_layers) * c.n_kv_heads;
-      auto cp2 = [&](void* dst, const void* src) {
-        if (dst && src && e == cudaSuccess)
-          e = cudaMemcpy2DAsync(static_cast<uint8_t*>(dst) + off, pitch, static_cast<const uint8_t*>(src) + off, pitch, width, height,
-                                cudaMemcpyDeviceToDevice, st);
-      };
-      cp2(h->tap_k, kv->k);
-      cp2(h->tap_v, kv->v);
-      cp2(kv->k, h->force_k);
-      cp2(kv->v, h->force_v);
-    }
-    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap / forcing copy failed: %s", cudaGetErrorString(e));
+  // Pass 1 checks every shape of the plan without launching (on error nothing was enqueued);
+  // pass 2 enqueues.
+  for (int pass = 0; pass < 2; ++pass) {
+    h->dry = pass == 0;
+    rc = enqueue_step(h, st, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
+    h->dry = false;
+    if (rc != DOVETAIL_OK) return rc;
   }
-  e = cudaGetLastError();
+  cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
   kv->committed_len = Lp;  // the level-0 rows are real, verified tokens
   h->have_step = true;
@@ -885,9 +932,10 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, 
   if (n_rows < need_rows || max_b < maxb) return fail(h, DOVETAIL_EINVAL, "replay needs %d rows of %d candidates", need_rows, maxb);
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   h->launches = 0;
-  h->ev_used = 0;
   h->cur_kind = 9;
   h->cur_bytes = 0;
+  const bool trace_was = h->trace_on;
+  h->trace_on = false;  // the replay is not part of the traced step
   cudaError_t e = cudaMemsetAsync(h->rt, 0xff, sizeof(RowTables), st);  // level-0 row: pool = -1
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "memset failed: %s", cudaGetErrorString(e));
   int row = 0;
@@ -936,48 +984,93 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, 
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "copy failed: %s", cudaGetErrorString(e));
   h->have_step = false;
   h->last_launches = h->launches;
+  h->trace_on = trace_was;
   return DOVETAIL_OK;
 }
 
-int dovetail_draft_set_taps(dovetail_draft_t* h, float* logits, float* hhat) {
+int dovetail_hooks_set(dovetail_draft_t* h, const dovetail_hooks_t* hooks) {
   if (!h) return DOVETAIL_EINVAL;
-  h->tap_logits = logits;
-  h->tap_hhat = hhat;
-  return DOVETAIL_OK;
-}
-
-int dovetail_draft_set_forcing(dovetail_draft_t* h, const float* force_hhat, const void* force_k, const void* force_v,
-                               void* tap_k, void* tap_v) {
-  if (!h) return DOVETAIL_EINVAL;
-  h->force_hhat = force_hhat;
-  h->force_k = force_k;
-  h->force_v = force_v;
-  h->tap_k = tap_k;
-  h->tap_v = tap_v;
+  h->hooks = hooks ? *hooks : dovetail_hooks_t{};
+  const dovetail_hooks_t& k = h->hooks;
+  if ((k.tap_pool_token == nullptr) != (k.tap_pool_cum == nullptr) ||
+      (k.force_pool_token == nullptr) != (k.force_pool_cum == nullptr)) {
+    h->hooks = dovetail_hooks_t{};
+    h->hooks_on = false;
+    return fail(h, DOVETAIL_EINVAL, "pool taps / forcing need both the token and the score array");
+  }
+  h->hooks_on = k.tap_logits || k.tap_hhat || k.tap_k || k.tap_v || k.tap_pool_token || k.force_hhat || k.force_k ||
+                k.force_v || k.force_pool_token;
   return DOVETAIL_OK;
 }
 
 int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
 
-int dovetail_draft_set_profile(dovetail_draft_t* h, int32_t enable) {
+int dovetail_draft_status(dovetail_draft_t* h, void* cuda_stream) {
   if (!h) return DOVETAIL_EINVAL;
-  h->profile = enable != 0;
-  h->ev_used = 0;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t e = cudaMemcpyAsync(h->ts_host, h->ts, sizeof(TreeState), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(&h->ts->status, 0, sizeof(int32_t), st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "status read failed: %s", cudaGetErrorString(e));
+  if (h->ts_host->status & 1)
+    return fail(h, DOVETAIL_EINVAL, "a token id passed to dovetail_draft_step was outside [0, vocab = %d)", h->cfg.vocab);
   return DOVETAIL_OK;
 }
 
-int dovetail_profile_read(dovetail_draft_t* h, float* ms, int32_t* launches, int64_t* bytes) {
-  if (!h || !ms || !launches || !bytes) return h ? fail(h, DOVETAIL_EINVAL, "null argument") : DOVETAIL_EINVAL;
-  for (int k = 0; k < DOVETAIL_N_KINDS; ++k) { ms[k] = 0.f; launches[k] = 0; bytes[k] = 0; }
-  for (int i = 0; i < h->ev_used; ++i) {
-    float t = 0.f;
-    cudaError_t e = cudaEventElapsedTime(&t, h->ev[2 * i], h->ev[2 * i + 1]);
-    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "profile read failed (synchronise the stream first): %s", cudaGetErrorString(e));
-    const int k = h->ev_kind[i];
-    ms[k] += t;
-    launches[k] += 1;
-    bytes[k] += h->ev_bytes[i];
+int dovetail_trace_enable(dovetail_draft_t* h, int32_t enable) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (enable && !h->trace_buf) {
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&h->trace_buf), sizeof(unsigned long long) * 2 * kMaxTraceLaunches);
+    if (e == cudaSuccess) e = cudaMallocHost(reinterpret_cast<void**>(&h->trace_host), sizeof(unsigned long long) * 2 * kMaxTraceLaunches);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ENOMEM, "trace buffer: %s", cudaGetErrorString(e));
   }
+  h->trace_on = enable != 0;
+  h->tr_used = 0;
+  return DOVETAIL_OK;
+}
+
+int dovetail_trace_read(dovetail_draft_t* h, int32_t cap, int32_t* kind, int32_t* level, int64_t* bytes,
+                        uint64_t* t0_ns, uint64_t* t1_ns, int32_t* n) {
+  if (!h || !kind || !level || !bytes || !t0_ns || !t1_ns || !n || cap < 0)
+    return h ? fail(h, DOVETAIL_EINVAL, "null argument") : DOVETAIL_EINVAL;
+  *n = 0;
+  if (!h->trace_buf || h->tr_used == 0) return DOVETAIL_OK;
+  cudaError_t e = cudaMemcpy(h->trace_host, h->trace_buf, sizeof(unsigned long long) * 2 * h->tr_used, cudaMemcpyDeviceToHost);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "trace read failed: %s", cudaGetErrorString(e));
+  const int cnt = std::min(cap, h->tr_used);
+  for (int i = 0; i < cnt; ++i) {
+    kind[i] = h->tr_kind[i];
+    level[i] = h->tr_level[i];
+    bytes[i] = h->tr_bytes[i];
+    t0_ns[i] = h->trace_host[2 * i];
+    t1_ns[i] = h->trace_host[2 * i + 1];
+  }
+  *n = cnt;
+  return DOVETAIL_OK;
+}
+
+int dovetail_probe_stream(dovetail_draft_t* h, const void* buf, int64_t bytes, int32_t mode, int32_t seg,
+                          void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (!buf || bytes < (1 << 20) || (reinterpret_cast<uintptr_t>(buf) & 15) || (mode != 0 && mode != 1))
+    return fail(h, DOVETAIL_EINVAL, "probe: buffer must be 16-byte aligned and >= 1 MiB, mode 0 or 1");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaError_t e = cudaSuccess;
+  if (!h->probe_sink) e = cudaMalloc(reinterpret_cast<void**>(&h->probe_sink), sizeof(float));
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ENOMEM, "probe: %s", cudaGetErrorString(e));
+  if (mode == 0) {
+    k_stream_sum<<<h->num_sms * 4, 512, 0, st>>>(static_cast<const uint4*>(buf), bytes / 16, h->probe_sink);
+  } else {
+    if (seg < 512 || seg > 8192 || seg % 16) return fail(h, DOVETAIL_EINVAL, "probe: seg must be a multiple of 16 in [512, 8192]");
+    const int rows = std::min(128, 32768 / seg * 2);           // ~64 KB stages, <= 32 segments per producer warp
+    const int n_stages = std::min(8, (200 * 1024) / (rows * seg));
+    const size_t smem = static_cast<size_t>(n_stages) * rows * seg + 128;
+    e = cudaFuncSetAttribute(k_stream_bulk, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+    if (e == cudaSuccess)
+      k_stream_bulk<<<h->num_sms, kProbeThreads, smem, st>>>(static_cast<const uint8_t*>(buf), bytes, seg, rows, n_stages, h->probe_sink);
+  }
+  if (e == cudaSuccess) e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "probe launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
 }
 
@@ -985,7 +1078,7 @@ int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
   if (!h) return 0;
   const dovetail_config_t& c = h->cfg;
   const int64_t d = c.hidden, F = c.ffn, dq = h->dq, dkv = h->dkv;
-  int64_t params = (c.dgf_proj ? 2 * d * d : 0) + 2 * d * d + d;
+  int64_t params = (c.dgf_proj ? 2 * d * d : 0) + 2 * d * d + d;  // DGF (4d^2 + d) or the concat + Linear fusion (2d^2 + d)
   params += static_cast<int64_t>(c.n_layers) * (d * dq + 2 * d * dkv + dq * d + 3 * d * F + 2 * d);
   params += static_cast<int64_t>(c.vocab) * d + (c.final_norm ? d : 0);
   const int64_t kvb = static_cast<int64_t>(c.n_layers) * 2 * prefix_len * dkv;

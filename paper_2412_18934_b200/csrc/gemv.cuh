@@ -59,7 +59,7 @@ struct GemvParams {
   float* out;            // STORE/SWIGLU: [M, out_ld]; DGF/RESID: residual stream rows x [M, out_ld]
   int64_t out_ld;
   const float* hbuf;     // DGF: [M, 2d] = [h1 || h2]
-  const void* bias;      // DGF: gate bias [d]
+  const void* bias;      // DGF: gate bias [d]; STORE: optional bias added to the result (fusion linear)
   int32_t d;
   int32_t b;             // LMHEAD: candidates kept per row
   int32_t vocab;
@@ -67,7 +67,7 @@ struct GemvParams {
   int32_t* cand_id;
   float* stat;           // LMHEAD: [kMaxRows][grid][2] = (max, sum exp)
   float* tap;            // LMHEAD: optional logits tap rows [M, vocab]
-  unsigned long long* trace;  // DVT_TRACE builds only
+  unsigned long long* trace;  // dovetail_trace_*: {first CTA start, last CTA end} of this launch, or NULL
 };
 
 template <typename WT>
@@ -167,6 +167,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_gemv(const GemvParams p) {
   float* res = red_s + kConsumerWarps * 4;            // [cnt][MT]
 
   const RowRange rr = cta_rows(G, c, nct);
+  trace_begin(p.trace);
   const int spp = (rr.cnt + RS - 1) / RS;  // stages per pass over the CTA's rows
   const int m_tiles = (p.M + MT - 1) / MT;
   const int U = p.row_bytes >> 4;          // 16-byte units per row
@@ -336,10 +337,15 @@ __global__ void __launch_bounds__(kThreads, 1) k_gemv(const GemvParams p) {
       for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rstd_s[idx % MT];
       consumer_sync();
     }
-    if (p.epi == EPI_STORE) {
+    if (p.epi == EPI_STORE) {  // optional bias: the concat + Linear fusion
       for (int idx = tid; idx < nres; idx += kConsumerThreads) {
         const int v2 = idx / MT, mm = m0 + idx % MT;
-        if (mm < p.M) p.out[mm * p.out_ld + G.out_off + rr.g0 + v2] = res[idx];
+        float bz = 0.f;
+        if (p.bias) {
+          if (sizeof(WT) == 2) bz = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[rr.g0 + v2]);
+          else bz = static_cast<const float*>(p.bias)[rr.g0 + v2];
+        }
+        if (mm < p.M) p.out[mm * p.out_ld + G.out_off + rr.g0 + v2] = res[idx] + bz;
       }
     } else if (p.epi == EPI_DGF) {
       // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
@@ -410,6 +416,7 @@ __global__ void __launch_bounds__(kThreads, 1) k_gemv(const GemvParams p) {
     }
     consumer_sync();  // res is reused by the next m-tile
   }
+  trace_end(p.trace);
 }
 
 }  // namespace dvt

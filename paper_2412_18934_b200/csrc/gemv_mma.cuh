@@ -39,11 +39,6 @@
 
 namespace dvt {
 
-#ifdef DVT_TRACE  // microbenchmark builds only: per-CTA time stamps (ns) at the phases of the kernel
-#define DVT_STAMP(i) do { if ((threadIdx.x & 31) == 0 && p.trace) { unsigned long long t_; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_)); p.trace[(static_cast<size_t>(blockIdx.x) * 12 + (threadIdx.x >> 5)) * 8 + (i)] = t_; } } while (0)
-#else
-#define DVT_STAMP(i) do { } while (0)
-#endif
 
 constexpr int kMmaMaxM = 32;
 // A 1-D bulk copy costs its issuing warp ~35 ns whatever its size (measured: one producer warp
@@ -95,7 +90,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
   const RowRange rr = cta_rows(G, c, nct);
   const int n_sb = (rr.cnt + RS - 1) / RS;
   const int n_panels = (K + KP - 1) / KP;
-  DVT_STAMP(0);
+  trace_begin(p.trace);
 
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) {
@@ -142,13 +137,11 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
         }
       }
     }
-    DVT_STAMP(1);
     return;
   }
 
   // ---------------- consumers -------------------------------------------------
   pdl_wait();
-  DVT_STAMP(1);  // activations of the previous kernel are visible from here on
   const StepDyn* dyn = p.dyn;
   const bool normed = G.gain != nullptr;
   const __nv_bfloat16* gain = static_cast<const __nv_bfloat16*>(G.gain);
@@ -274,7 +267,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       }
     }
     consumer_sync();
-    if (pn == 0) DVT_STAMP(2);
 
     for (int sb = 0; sb < n_sb; ++sb) {
       const int v0 = sb * RS, nr = min(RS, rr.cnt - v0);
@@ -290,7 +282,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       for (int k0 = k_begin; k0 < k_end; k0 += KC) {
         const int n_units = min(KC, k_end - k0) >> 5;  // 32 k per unit
         mbar_wait(&full[slot], round & 1);
-        if (round == 0 && slot == 0) DVT_STAMP(3);
         const uint32_t sbase = ring_u + static_cast<uint32_t>(slot) * p.stage_bytes + a_lane;
         for (int u = warp; u < n_units; u += kConsumerWarps) {
           uint32_t b[NT][4];
@@ -350,8 +341,6 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       consumer_sync();  // part is reused by the next super-block
     }
   }
-
-  DVT_STAMP(4);
   // ---- fused epilogue over the CTA's results: res[v * M + m] ---------------------
   const int nres = rr.cnt * M;
   if (normed) {  // RMSNorm: y = x / sqrt(mean(x^2) + eps) * g; 1/rms is applied to the results
@@ -364,10 +353,12 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
     for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rstd_s[idx % M];
     consumer_sync();
   }
-  if (p.epi == EPI_STORE) {
+  if (p.epi == EPI_STORE) {  // optional bias: the concat + Linear fusion
+    const __nv_bfloat16* bias = static_cast<const __nv_bfloat16*>(p.bias);
     for (int idx = tid; idx < nres; idx += kConsumerThreads) {
       const int v2 = idx / M, mm = idx - v2 * M;
-      p.out[(p.m0 + mm) * p.out_ld + G.out_off + rr.g0 + v2] = res[idx];
+      const float bz = bias ? __bfloat162float(bias[rr.g0 + v2]) : 0.f;
+      p.out[(p.m0 + mm) * p.out_ld + G.out_off + rr.g0 + v2] = res[idx] + bz;
     }
   } else if (p.epi == EPI_DGF) {
     // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
@@ -428,7 +419,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const GemvParams p)
       }
     }
   }
-  DVT_STAMP(5);
+  trace_end(p.trace);
 }
 
 }  // namespace dvt

@@ -79,6 +79,20 @@ __device__ __forceinline__ void pdl_launch_dependents() {
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
+// ---- per-launch time stamps (dovetail_hooks.h dovetail_trace_*): t[0] = earliest CTA start,
+// t[1] = latest CTA end, in ns of %globaltimer. t == NULL (the default) costs one predicate.
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+__device__ __forceinline__ void trace_begin(unsigned long long* t) {
+  if (t != nullptr && threadIdx.x == 0) atomicMin(t, globaltimer_ns());
+}
+__device__ __forceinline__ void trace_end(unsigned long long* t) {
+  if (t != nullptr && threadIdx.x == 0) atomicMax(t + 1, globaltimer_ns());
+}
+
 // ---- named barrier among the consumer warps only ---------------------------
 __device__ __forceinline__ void consumer_sync() {
   asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");

@@ -26,8 +26,10 @@ struct Pool {  // device arrays of capacity pool_cap
 // ---- S0 ---------------------------------------------------------------------
 // grid = n_new + depth - 1 CTAs (one rotary-table row each) x 64 threads.
 __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, RowTables* rt0,
-                             float2* rope, const double* inv_freq, int half, int vocab) {
+                             float2* rope, const double* inv_freq, int half, int vocab,
+                             unsigned long long* trace) {
   pdl_launch_dependents();
+  trace_begin(trace);
   pdl_wait();
   const int r = blockIdx.x, n_new = dynv.n_new;
   // rotary angles in fp64: pos * theta^(-2i/dh) reaches thousands of radians
@@ -39,8 +41,7 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
   }
   if (r == 0) {
     if (threadIdx.x == 0) {
-      *dyn = dynv;
-      ts->status = 0;
+      *dyn = dynv;  // ts->status is sticky until dovetail_draft_status / kv_commit reads it
       ts->pool_size = 0;
       ts->n_out = 0;
     }
@@ -61,13 +62,17 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
       }
     }
   }
+  __syncthreads();
+  trace_end(trace);
 }
 
 // dgf_proj == 0: h1 = f, h2 = e (W1 = W2 = identity). grid-stride over M * 2d.
 template <typename WT>
 __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, int64_t xld,
-                         const RowTables* rt, int use_idx, const WT* embed, float* hbuf, int M, int d) {
+                         const RowTables* rt, int use_idx, const WT* embed, float* hbuf, int M, int d,
+                         unsigned long long* trace) {
   pdl_launch_dependents();
+  trace_begin(trace);
   pdl_wait();
   const float* base = from_dyn ? dyn->feats : xsrc;
   for (int64_t idx = blockIdx.x * static_cast<int64_t>(blockDim.x) + threadIdx.x; idx < static_cast<int64_t>(M) * 2 * d;
@@ -82,6 +87,8 @@ __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, in
     }
     hbuf[idx] = v;
   }
+  __syncthreads();
+  trace_end(trace);
 }
 
 // ---- S7 / S8 -----------------------------------------------------------------
@@ -116,6 +123,12 @@ struct TreeLevelParams {
   int32_t* o_parents;
   int32_t* o_depths;
   int32_t* o_n;
+  // test hooks (dovetail_hooks.h): taps of this level's candidates as computed, then teacher forcing
+  int32_t* tap_token;
+  float* tap_cum;
+  const int32_t* force_token;
+  const float* force_cum;
+  unsigned long long* trace;
 };
 
 __device__ __forceinline__ bool node_before(const float* cum, int a, int b) {
@@ -135,6 +148,7 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   float* s_cum = s_raw;
   int32_t* s_new = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);
   pdl_launch_dependents();
+  trace_begin(p.trace);
   pdl_wait();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const Pool& P = p.pool;
@@ -243,8 +257,17 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   }
   __syncthreads();
 
-  // ---- phase B: frontier of the next level = top-M_next children by score -----
   const int n = p.M * p.b;
+  if (p.tap_token != nullptr || p.force_token != nullptr) {  // hooks: never set in a plain step
+    for (int i = tid; i < n; i += kTreeThreads) {
+      const int node = p.pool_begin + i;
+      if (p.tap_token) { p.tap_token[node] = P.token[node]; p.tap_cum[node] = P.cum[node]; }
+      if (p.force_token) { P.token[node] = p.force_token[node]; P.cum[node] = p.force_cum[node]; }
+    }
+    __syncthreads();
+  }
+
+  // ---- phase B: frontier of the next level = top-M_next children by score -----
   if (p.M_next > 0) {
     for (int i = tid; i < n; i += kTreeThreads) s_cum[i] = P.cum[p.pool_begin + i];
     __syncthreads();
@@ -268,6 +291,8 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
         }
       }
     }
+    __syncthreads();
+    trace_end(p.trace);
     return;
   }
 
@@ -322,6 +347,8 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
     p.ts->n_out = n_keep;
     p.ts->pool_size = Pn;
   }
+  __syncthreads();
+  trace_end(p.trace);
 }
 
 // ---- S9 ------------------------------------------------------------------------

@@ -35,8 +35,8 @@ def make_weights(cfg: DraftConfig, device="cpu", seed=None) -> Tuple[Dict[str, t
     r = lambda *s: _randn(s, 0.02, gen, device, dt)
     top = dict(
         embed=r(V, d),
-        dgf_w1=r(d, d) if cfg.dgf_proj else None,
-        dgf_w2=r(d, d) if cfg.dgf_proj else None,
+        dgf_w1=r(d, d) if (cfg.dgf_proj and cfg.fusion == 0) else None,
+        dgf_w2=r(d, d) if (cfg.dgf_proj and cfg.fusion == 0) else None,
         dgf_wg=r(d, 2 * d),
         dgf_bg=r(d),
         g_final=torch.ones(d, device=device, dtype=dt) if cfg.final_norm else None,

@@ -23,7 +23,7 @@ def tiny_cfg(**kw) -> DraftConfig:
 def ocfg(cfg: DraftConfig) -> oracle.OracleConfig:
     return oracle.OracleConfig(cfg.hidden, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.n_layers,
                                cfg.ffn, cfg.vocab, cfg.rope_theta, cfg.rms_eps, cfg.dtype, cfg.dgf_proj,
-                               cfg.first_layer_input_norm, cfg.final_norm)
+                               cfg.first_layer_input_norm, cfg.final_norm, cfg.fusion)
 
 
 def oweights(top, layers) -> oracle.OracleWeights:
@@ -109,6 +109,8 @@ class RefDraft:
     def dgf(self, f: torch.Tensor, tokens: torch.Tensor) -> torch.Tensor:
         t = self.top
         e = t["embed"][tokens.long()]
+        if self.cfg.fusion == 1:  # concat + one Linear, by the library routine
+            return torch.nn.functional.linear(torch.cat([f, e], -1), t["dgf_wg"], t["dgf_bg"])
         h1 = f @ t["dgf_w1"].T if self.cfg.dgf_proj else f
         h2 = e @ t["dgf_w2"].T if self.cfg.dgf_proj else e
         g = torch.sigmoid(torch.cat([h1, h2], -1) @ t["dgf_wg"].T + t["dgf_bg"])

@@ -2,23 +2,63 @@
 
 The CUDA path is called through the C ABI (binding.py); the oracle through
 oracle/. Inputs are generated once (on the GPU when there is one) and the very
-same stored values are handed to both sides."""
-from dataclasses import dataclass
-from typing import Dict, Optional
+same stored values are handed to both sides.
+
+Two runs of the same step are compared with the oracle:
+
+  free     the plain step. Discrete outputs (token ids, parents, depths, n_out, committed_len)
+           must be identical; logits, hidden states and scores of EVERY row must meet
+           BASELINE.json's tolerance. A discrete difference is excused only by the LOCAL tie
+           rule below, and then only the rows computed before the divergence are compared.
+  forced   teacher forcing (include/dovetail_hooks.h): after every level the
+           hidden states, K/V rows and candidates are replaced by the oracle's, so each
+           level's arithmetic is compared in isolation: every row at the tolerance AND at a
+           much tighter observed-accuracy bound, stored K/V rows against a fixed bound, and
+           the per-row top-b decisions one by one.
+
+Local tie rule (reading A13): where the GPU's and the oracle's decision differ -- a row's
+k-th best token, the w-th frontier node of a level, the gamma-th candidate -- the ORACLE's
+own margin between the two alternatives at that very decision (its logits of the two tokens
+of that row / its scores of the two nodes) must be below the logit tolerance. A near-tie
+anywhere else excuses nothing.
+"""
+from typing import Optional
 
 import numpy as np
 import torch
 
 import oracle
-from helpers import kv_np, np_to_f64, ocfg, oweights
-from paper_2412_18934_b200 import binding, synth
-from paper_2412_18934_b200.configs import BF16, DraftConfig, TreeSpec
+from helpers import kv_np, ocfg, oweights
+from paper_2412_18934_b200 import binding
+from paper_2412_18934_b200.configs import BF16
 
 # BASELINE.json north_star: logits within 2e-2 relative / 1e-2 absolute in bf16, 1e-4 in fp32.
 TOL = {BF16: dict(rtol=2e-2, atol=1e-2), 0: dict(rtol=1e-4, atol=1e-4)}
 
+# Observed-accuracy bounds of the teacher-forced run, so that a loss of accumulation accuracy cannot hide under
+# the 1e-2 of the stated tolerance (DESIGN.md section 6 gives the measured figures; these are ~3-4x above them):
+#   logits        |err| <= max(2e-4, 2.5e-5 x max|logit|)   (C3: 82 x 2.5e-5 = 2e-3; an fp32 dot product of
+#                 K = d terms errs by ~eps sqrt(K) x the logit scale, and inherits the hidden state's error)
+#   hidden state  |err| <= 5e-5 x max|hhat|                  (fp32 accumulation through <= 8 blocks)
+FORCED_LOGIT_REL = {BF16: 2.5e-5, 0: 2.5e-6}
+FORCED_LOGIT_FLOOR = {BF16: 2e-4, 0: 1e-4}
+FORCED_HHAT_REL = {BF16: 5e-5, 0: 5e-6}
 
-from paper_2412_18934_b200.cases import Case, make_case  # noqa: F401  (re-exported for the tests)
+# Stored bf16 K/V rows of the teacher-forced run: a stored value may differ from the oracle's by one bf16 ulp
+# (the fp32 value sat next to a rounding boundary) plus KV_PRE, a FIXED bound on the fp32-vs-fp64 difference
+# before rounding: a K/V entry is W . norm(x) with |entry| <~ 6.5 on these models, and the fp32 forward of one
+# level errs by <= 1.5e-5 relative (the hidden-state bound above is 5e-5 of the largest element): 6.5 x 1.5e-5 = 1e-4.
+KV_PRE = {BF16: 1e-4}
+
+# Free-running step, levels whose rows cannot meet the stated tolerance because the synthetic model amplifies
+# any perturbation from level to level (DESIGN.md section 6): the GPU's error at level l may be at most
+# SENS_K x (its own level-0 error / the oracle's level-0 response) x the oracle's level-l response to a
+# relative SENS_ETA perturbation of the step's input features -- i.e. the error grows no faster than the
+# model's own sensitivity, measured with the oracle alone.
+SENS_ETA = 1e-6
+SENS_K = 4.0
+
+from paper_2412_18934_b200.cases import Case, make_case  # noqa: F401,E402  (re-exported for the tests)
 
 
 def _kv_torch(a: np.ndarray, like: torch.Tensor) -> torch.Tensor:
@@ -32,32 +72,38 @@ def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: i
             force: Optional[dict] = None):
     """One step through the C ABI. Returns (handle, kv, dict of host arrays).
 
-    force = an oracle result: teacher forcing (include/dovetail.h) -- every level is computed from the
-    oracle's hidden states and K/V rows of the earlier levels; the returned hhat / k / v are the values the
+    force = an oracle result: teacher forcing -- every level is computed from the oracle's hidden states,
+    K/V rows and candidates of the earlier levels; the returned hhat / k / v / pool arrays are the values the
     GPU computed (tapped before they were overwritten)."""
     cfg, tree = case.cfg, case.tree
     h = binding.dovetail_draft_init(case.top, case.layers, cfg, max_rows, max_tree_slots, max_branch)
     k, v = case.k.clone(), case.v.clone()
     kv = binding.KVCache(k, v, case.L)
-    tap_k = tap_v = None
-    if force is not None:
-        tap_k, tap_v = case.k.clone(), case.v.clone()
-        fh = torch.from_numpy(np.ascontiguousarray(force["row_hhat"], dtype=np.float32)).to(k.device)
-        binding.dovetail_draft_set_forcing(h, fh, _kv_torch(force["k"], k), _kv_torch(force["v"], v), tap_k, tap_v)
+    hooks = {}
     n_new = case.tokens.shape[0]
     rows = n_new + tree.tree_rows()
-    tl = th = None
-    if taps:
-        tl = torch.zeros((rows, cfg.vocab), dtype=torch.float32, device="cuda")
-        th = torch.zeros((rows, cfg.hidden), dtype=torch.float32, device="cuda")
-        binding.dovetail_draft_set_taps(h, tl, th)
+    P = tree.pool_size()
+    if taps or force is not None:
+        hooks["tap_logits"] = torch.zeros((rows, cfg.vocab), dtype=torch.float32, device="cuda")
+        hooks["tap_hhat"] = torch.zeros((rows, cfg.hidden), dtype=torch.float32, device="cuda")
+        hooks["tap_pool_token"] = torch.full((P,), -1, dtype=torch.int32, device="cuda")
+        hooks["tap_pool_cum"] = torch.zeros((P,), dtype=torch.float32, device="cuda")
+    if force is not None:
+        hooks["tap_k"], hooks["tap_v"] = case.k.clone(), case.v.clone()
+        hooks["force_hhat"] = torch.from_numpy(np.ascontiguousarray(force["row_hhat"], dtype=np.float32)).to(k.device)
+        hooks["force_k"], hooks["force_v"] = _kv_torch(force["k"], k), _kv_torch(force["v"], v)
+        hooks["force_pool_token"] = torch.from_numpy(np.ascontiguousarray(force["pool_token"], dtype=np.int32)).to(k.device)
+        hooks["force_pool_cum"] = torch.from_numpy(force["pool_cum"].astype(np.float32)).to(k.device)
+    if hooks:
+        binding.dovetail_hooks_set(h, **hooks)
     out = binding.dovetail_draft_step(h, case.feats, case.tokens, kv, tree)
-    torch.cuda.synchronize()
+    binding.dovetail_draft_status(h)  # synchronises; raises on a bad token id
     n = int(out["n_out"].item())
+    g = lambda name: None if name not in hooks else hooks[name].cpu().numpy()
     res = dict(token_ids=out["token_ids"][:n].cpu().numpy(), scores=out["scores"][:n].cpu().numpy(),
                parents=out["parents"][:n].cpu().numpy(), depths=out["depths"][:n].cpu().numpy(), n_out=n,
-               logits=None if tl is None else tl.cpu().numpy(), hhat=None if th is None else th.cpu().numpy(),
-               k=kv_np(k if tap_k is None else tap_k), v=kv_np(v if tap_v is None else tap_v), forced=force is not None,
+               logits=g("tap_logits"), hhat=g("tap_hhat"), pool_token=g("tap_pool_token"), pool_cum=g("tap_pool_cum"),
+               k=kv_np(hooks.get("tap_k", k)), v=kv_np(hooks.get("tap_v", v)), forced=force is not None,
                committed_len=kv.committed_len, launches=binding.dovetail_last_launch_count(h))
     return h, kv, res
 
@@ -70,38 +116,6 @@ def run_oracle(case: Case, dump: bool = True):
                       case.tree.branch, case.tree.beam, case.tree.gamma, dump=dump)
     res["k"], res["v"] = kc, vc
     return res
-
-
-def oracle_margins(case: Case, ora: dict) -> float:
-    """Smallest decision margin of the oracle's tree search, in log-prob units: the gap at
-    every per-row top-b boundary, every frontier boundary and the gamma boundary. A GPU/oracle
-    difference in the discrete outputs is a legitimate tie only if this is below tolerance."""
-    tree, n_new = case.tree, case.tokens.shape[0]
-    gaps = []
-    rows = [n_new - 1] + list(range(n_new, ora["total_rows"]))
-    rpl = tree.rows_per_level(n_new)
-    level_of = {n_new - 1: 0}
-    r = n_new
-    for l in range(1, tree.depth):
-        for _ in range(rpl[l]):
-            level_of[r] = l
-            r += 1
-    for row in rows:
-        lg = np.sort(ora["row_logits"][row])[::-1]
-        b = tree.branch[level_of[row]]
-        if b < len(lg):
-            gaps.append(lg[b - 1] - lg[b])
-        gaps.extend(np.abs(np.diff(lg[:b])).tolist())
-    depth, cum = ora["pool_depth"], ora["pool_cum"]
-    for l in range(1, tree.depth):
-        c = np.sort(cum[depth == l])[::-1]
-        m = rpl[l]
-        if m < len(c):
-            gaps.append(c[m - 1] - c[m])
-    c = np.sort(cum)[::-1]
-    if tree.gamma < len(c):
-        gaps.append(c[tree.gamma - 1] - c[tree.gamma])
-    return float(min(gaps)) if gaps else float("inf")
 
 
 def bf16_ulp_diff(a: np.ndarray, b: np.ndarray) -> np.ndarray:
@@ -117,78 +131,241 @@ def bf16_bits_to_f64(a: np.ndarray) -> np.ndarray:
     return (a.astype(np.uint32) << 16).view(np.float32).astype(np.float64)
 
 
-def compare(case: Case, gpu: dict, ora: dict, log=print) -> dict:
-    """Element-by-element comparison. Returns a summary dict; raises AssertionError on a
-    mismatch that the stated tolerances do not allow."""
+def level_layout(case: Case):
+    """Step rows of each level, and for each level the (first pool index, rows expanded, branch)."""
+    tree, n_new = case.tree, case.tokens.shape[0]
+    rpl = tree.rows_per_level(n_new)
+    rows, r = [list(range(n_new))], n_new
+    for l in range(1, tree.depth):
+        rows.append(list(range(r, r + rpl[l])))
+        r += rpl[l]
+    pools, pb = [], 0
+    for l in range(tree.depth):
+        m = 1 if l == 0 else rpl[l]
+        pools.append((pb, m, tree.branch[l]))
+        pb += m * tree.branch[l]
+    return rows, pools
+
+
+def _order(cum: np.ndarray, idx: np.ndarray) -> np.ndarray:
+    """Indices idx sorted by the strict node order (score desc, pool index asc) (reading A7)."""
+    return idx[np.lexsort((idx, -cum[idx]))]
+
+
+def first_divergence(case: Case, gpu: dict, ora: dict):
+    """Walks the decisions of the tree search in the order they are taken and returns None when the GPU took
+    every one as the oracle did, else (level, what, oracle's margin at that decision). Decisions: the
+    children of every expanded row (tokens, rank by rank), then the level's frontier, ..., the final gamma
+    selection. GPU decisions are re-derived from its tapped candidates with the same strict orders (the
+    bookkeeping kernels themselves are bit-exact by test_gpu_tree.py)."""
+    tree, n_new = case.tree, case.tokens.shape[0]
+    rows, pools = level_layout(case)
+    gt, gc = gpu["pool_token"], gpu["pool_cum"].astype(np.float64)
+    ot, oc, orow = ora["pool_token"], ora["pool_cum"], ora["pool_row"]
+    lm_row_of_level = [[n_new - 1]] + rows[1:]
+    for l in range(tree.depth):
+        pb, m, b = pools[l]
+        for r in range(m):
+            lrow = lm_row_of_level[l][r]
+            for j in range(b):
+                i = pb + r * b + j
+                if gt[i] != ot[i]:
+                    lg = ora["row_logits"][lrow]
+                    return l, f"row {lrow} child {j}: gpu token {gt[i]} vs oracle {ot[i]}", float(abs(lg[ot[i]] - lg[gt[i]]))
+        if l + 1 < tree.depth:
+            w = len(rows[l + 1])
+            idx = np.arange(pb, pb + m * b)
+            fo, fg = _order(oc, idx)[:w], _order(gc, idx)[:w]
+            if not np.array_equal(fo, fg):
+                p = int(np.argmax(fo != fg))
+                return l, f"frontier of level {l + 1} rank {p}: gpu node {fg[p]} vs oracle {fo[p]}", float(abs(oc[fo[p]] - oc[fg[p]]))
+    P = len(ot)
+    n_keep = min(tree.gamma, P)
+    idx = np.arange(P)
+    so, sg = np.sort(_order(oc, idx)[:n_keep]), np.sort(_order(gc, idx)[:n_keep])
+    if not np.array_equal(so, sg):
+        a, bb = np.setdiff1d(so, sg), np.setdiff1d(sg, so)
+        return tree.depth, f"gamma selection: gpu keeps {bb} vs oracle {a}", float(np.max(np.abs(oc[a][:, None] - oc[bb][None, :])))
+    return None
+
+
+def oracle_sensitivity(case: Case, ora: dict):
+    """Per-level response (max |delta logit|, max |delta hhat|) of the ORACLE to a relative SENS_ETA perturbation
+    of the input features; None for levels at or after the first level whose candidates change."""
+    import dataclasses
+    g = torch.Generator(device="cpu")
+    g.manual_seed(4242)
+    sign = (torch.randint(0, 2, case.feats.shape, generator=g).float() * 2 - 1).to(case.feats.device)
+    pert = dataclasses.replace(case, feats=(case.feats.double() * (1.0 + SENS_ETA * sign.double())).float())
+    op = run_oracle(pert)
+    rows, pools = level_layout(case)
+    n_new = case.tokens.shape[0]
+    out, ok = [], True
+    for l, rr in enumerate(rows):
+        pb, m, b = pools[l]
+        lm = [n_new - 1] if l == 0 else rr
+        out.append((float(np.abs(op["row_logits"][lm] - ora["row_logits"][lm]).max()),
+                    float(np.abs(op["row_hhat"][rr] - ora["row_hhat"][rr]).max())) if ok else None)
+        ok = ok and np.array_equal(op["pool_token"][pb:pb + m * b], ora["pool_token"][pb:pb + m * b]) and \
+            np.array_equal(np.argsort(-op["pool_cum"][pb:pb + m * b], kind="stable"), np.argsort(-ora["pool_cum"][pb:pb + m * b], kind="stable"))
+    return out
+
+
+def error_table(case: Case, gpu: dict, ora: dict) -> list:
+    """Per level: max |logit error|, max |hidden-state error| of the level's rows."""
+    rows, _ = level_layout(case)
+    n_new = case.tokens.shape[0]
+    tab = []
+    for l, rr in enumerate(rows):
+        lm = [n_new - 1] if l == 0 else rr
+        tab.append(dict(level=l, rows=len(rr),
+                        logit=float(np.abs(gpu["logits"][lm] - ora["row_logits"][lm]).max()),
+                        hhat=float(np.abs(gpu["hhat"][rr] - ora["row_hhat"][rr]).max())))
+    return tab
+
+
+def compare(case: Case, gpu: dict, ora: dict, log=print, tight: bool = False) -> dict:
+    """Element-by-element comparison of one run (free or forced) with the oracle. Returns a summary dict;
+    raises AssertionError on a mismatch that the stated tolerances do not allow.
+
+    tight: also hold the forced run to the observed-accuracy bounds above (the full-size configurations; on toy
+    models with a few cached positions one bf16 rounding flip of a row's own stored K/V entry -- reading A12 --
+    moves the attention output by 2^-9 of it, which is above those bounds and below the stated tolerance)."""
     cfg, tree = case.cfg, case.tree
     tol = TOL[cfg.dtype]
+    forced = bool(gpu.get("forced", False))
     n_new = case.tokens.shape[0]
-    rows = ora["total_rows"]
-    summary = {}
-    # hidden states of every step row
-    hh_err = np.abs(gpu["hhat"][:rows] - ora["row_hhat"][:rows])
-    hh_ref = np.abs(ora["row_hhat"][:rows]).max()
-    summary["hhat_max_abs_err"] = float(hh_err.max())
-    summary["hhat_scale"] = float(hh_ref)
-    # logits of the rows whose LM head ran (last level-0 row, then all tree rows)
-    lm_rows = [n_new - 1] + list(range(n_new, rows))
-    gl, ol = gpu["logits"][lm_rows], ora["row_logits"][lm_rows]
-    summary["logit_max_abs_err"] = float(np.abs(gl - ol).max())
-    margin = oracle_margins(case, ora)
-    summary["oracle_min_margin"] = margin
+    n_rows = ora["total_rows"]
+    rows, pools = level_layout(case)
+    tab = error_table(case, gpu, ora)
+    summary = dict(forced=forced, per_level=tab, hhat_scale=float(np.abs(ora["row_hhat"][:n_rows]).max()),
+                   logit_max_abs_err=max(t["logit"] for t in tab), hhat_max_abs_err=max(t["hhat"] for t in tab))
+    log(("forced" if forced else "free  ") + " per-level max abs error  " +
+        "  ".join(f"L{t['level']}: logit {t['logit']:.2e} hhat {t['hhat']:.2e}" for t in tab))
+
+    # ---- discrete outputs ------------------------------------------------------------------------
     same_tree = (gpu["n_out"] == ora["n_out"] and np.array_equal(gpu["token_ids"], ora["token_ids"])
                  and np.array_equal(gpu["parents"], ora["parents"]) and np.array_equal(gpu["depths"], ora["depths"]))
     summary["same_tree"] = bool(same_tree)
-    if not same_tree:
-        # ids may differ only where the oracle's own decision gap is below tolerance (logged tie)
-        assert margin < tol["atol"], (
-            f"discrete outputs differ but the oracle's smallest decision margin is {margin:.3e}: "
-            f"gpu ids {gpu['token_ids']} parents {gpu['parents']} vs oracle {ora['token_ids']} {ora['parents']}")
-        log(f"TIE logged: oracle margin {margin:.3e} < {tol['atol']}; discrete outputs differ, "
-            f"value comparisons restricted to the level-0 rows")
-        lm_rows = [n_new - 1]
-        np.testing.assert_allclose(gpu["logits"][lm_rows], ora["row_logits"][lm_rows], **tol)
-        np.testing.assert_allclose(gpu["hhat"][:n_new], ora["row_hhat"][:n_new], **tol)
+    summary["tie"] = None
+    div = first_divergence(case, gpu, ora)
+    last_level = tree.depth  # levels [0, last_level) are comparable row by row
+    if forced:
+        # the candidates were forced to the oracle's after every level: the outputs follow from the oracle's
+        # pool through the (bit-exact) bookkeeping and must be identical
+        assert same_tree, (f"forced run: outputs differ from the oracle's although the pool was forced: gpu ids "
+                           f"{gpu['token_ids']} parents {gpu['parents']} vs {ora['token_ids']} {ora['parents']}")
+        # every row's own top-b decision is still the GPU's: check each one locally
+        gt, ot = gpu["pool_token"], ora["pool_token"]
+        lm_rows = [[n_new - 1]] + rows[1:]
+        n_ties = 0
+        for l in range(tree.depth):
+            pb, m, b = pools[l]
+            for r in range(m):
+                lg = ora["row_logits"][lm_rows[l][r]]
+                for j in range(b):
+                    i = pb + r * b + j
+                    if gt[i] != ot[i]:
+                        margin = float(abs(lg[ot[i]] - lg[gt[i]]))
+                        assert margin < tol["atol"], (f"level {l} row {lm_rows[l][r]} child {j}: gpu token {gt[i]} vs oracle "
+                                                      f"{ot[i]}, oracle margin {margin:.3e} is not a tie")
+                        n_ties += 1
+                        log(f"TIE logged (forced run): level {l} row {lm_rows[l][r]} child {j}, oracle margin {margin:.3e}")
+        summary["tie"] = n_ties or None
+    elif not same_tree or div is not None:
+        assert div is not None, (f"outputs differ but every decision re-derived from the GPU's candidates matches the "
+                                 f"oracle's: bookkeeping bug? gpu ids {gpu['token_ids']} parents {gpu['parents']} vs oracle "
+                                 f"{ora['token_ids']} {ora['parents']}")
+        level, what, margin = div
+        assert margin < tol["atol"], (f"first differing decision (level {level}, {what}) has oracle margin {margin:.3e} "
+                                      f">= {tol['atol']}: not a tie")
+        log(f"TIE logged (free run): level {level}, {what}; oracle margin {margin:.3e} < {tol['atol']}; "
+            f"rows of levels > {level} are not comparable in this run")
+        summary["tie"] = (level, what, margin)
+        last_level = min(tree.depth, level + 1)
+    else:
+        assert gpu["committed_len"] == ora["committed_len"]
+
+    # ---- values: every comparable row at the stated tolerance ----------------------------------------
+    def within(g, o):
+        return bool(np.all(np.abs(g - o) <= tol["atol"] + tol["rtol"] * np.abs(o)))
+
+    summary["sensitivity_bound_levels"] = []
+    sens = None
+    for l in range(last_level):
+        lm = [n_new - 1] if l == 0 else rows[l]
+        gl, ol = gpu["logits"][lm], ora["row_logits"][lm]
+        gh, oh = gpu["hhat"][rows[l]], ora["row_hhat"][rows[l]]
+        if within(gl, ol) and within(gh, oh):
+            continue
+        # level 0 and every level of a forced run are computed from the caller's / the oracle's state: no excuse
+        assert not forced and l > 0, (f"level {l}: logits / hidden states outside rtol {tol['rtol']} atol {tol['atol']}: "
+                                     f"max abs err logit {tab[l]['logit']:.3e} hhat {tab[l]['hhat']:.3e}")
+        if sens is None:
+            sens = oracle_sensitivity(case, ora)
+        assert sens[l] is not None and sens[0][0] > 0 and sens[0][1] > 0, f"level {l}: no sensitivity bound available"
+        b_logit = SENS_K * tab[0]["logit"] / sens[0][0] * sens[l][0]
+        b_hhat = SENS_K * tab[0]["hhat"] / sens[0][1] * sens[l][1]
+        log(f"free   level {l}: outside the stated tolerance (logit err {tab[l]['logit']:.3e}, hhat err {tab[l]['hhat']:.3e}); "
+            f"sensitivity bound logit {b_logit:.3e} hhat {b_hhat:.3e} (oracle response to a {SENS_ETA:g} input perturbation: "
+            f"level 0 {sens[0][0]:.3e} / {sens[0][1]:.3e}, level {l} {sens[l][0]:.3e} / {sens[l][1]:.3e})")
+        assert tab[l]["logit"] <= b_logit and tab[l]["hhat"] <= b_hhat, (
+            f"level {l}: free-running error (logit {tab[l]['logit']:.3e}, hhat {tab[l]['hhat']:.3e}) grows faster than the "
+            f"model's own sensitivity allows (bounds {b_logit:.3e}, {b_hhat:.3e})")
+        summary["sensitivity_bound_levels"].append(l)
+    if same_tree and not summary["sensitivity_bound_levels"]:
+        np.testing.assert_allclose(gpu["scores"], ora["scores"], **tol)
+    # candidates whose token agrees: cumulative log-probability
+    n_pool = sum(m * b for (_, m, b) in pools[:last_level])
+    agree = gpu["pool_token"][:n_pool] == ora["pool_token"][:n_pool]
+    if not summary["sensitivity_bound_levels"]:
+        np.testing.assert_allclose(gpu["pool_cum"][:n_pool][agree], ora["pool_cum"][:n_pool][agree], **tol)
+    if not forced:
         return summary
-    assert gpu["committed_len"] == ora["committed_len"]
-    if not gpu.get("forced", False):
-        # Free-running step: every level consumes the previous levels' results, so rounding-level
-        # differences are amplified level by level (DESIGN.md "Parity and teacher forcing"). The
-        # element-wise bar applies to the rows computed from the caller's inputs (level 0); deeper rows
-        # are held to it in the teacher-forced run. Discrete outputs are identical (checked above).
-        lm0 = [n_new - 1]
-        np.testing.assert_allclose(gpu["logits"][lm0], ora["row_logits"][lm0], **tol)
-        np.testing.assert_allclose(gpu["hhat"][:n_new], ora["row_hhat"][:n_new], **tol)
-        summary["deep_rows_logit_viol"] = int((np.abs(gl - ol) > tol["atol"] + tol["rtol"] * np.abs(ol)).sum())
-        return summary
-    np.testing.assert_allclose(gl, ol, **tol)
-    np.testing.assert_allclose(gpu["hhat"][:rows], ora["row_hhat"][:rows], **tol)
-    np.testing.assert_allclose(gpu["scores"], ora["scores"], **tol)
-    # KV cache: rows the step appended (prefix must be untouched bit for bit)
+
+    # ---- forced run only: observed accuracy, stored K/V rows ---------------------------------------------
+    summary["logit_scale"] = float(np.abs(ora["row_logits"][[n_new - 1] + list(range(n_new, n_rows))]).max())
+    lbound = max(FORCED_LOGIT_FLOOR[cfg.dtype], FORCED_LOGIT_REL[cfg.dtype] * summary["logit_scale"])
+    assert not tight or summary["logit_max_abs_err"] <= lbound, (
+        f"teacher-forced logit error {summary['logit_max_abs_err']:.3e} > {lbound:.3e} (logit scale {summary['logit_scale']:.3e})")
+    assert not tight or summary["hhat_max_abs_err"] <= FORCED_HHAT_REL[cfg.dtype] * summary["hhat_scale"], (
+        f"teacher-forced hidden-state error {summary['hhat_max_abs_err']:.3e} > {FORCED_HHAT_REL[cfg.dtype]} x "
+        f"scale {summary['hhat_scale']:.3e}")
     for name in ("k", "v"):
         g, o = gpu[name], ora[name]
         assert np.array_equal(g[:, :, :case.L], o[:, :, :case.L]), f"{name} prefix modified"
-        used = case.L + rows
+        used = case.L + n_rows
         if g.dtype == np.uint16:
             gs, os_ = g[:, :, case.L:used], o[:, :, case.L:used]
             ulp = bf16_ulp_diff(gs, os_)
-            summary[f"{name}_rows_off_by_1ulp"] = int((ulp == 1).sum())
-            # Stored values are fp32 results rounded to bf16. Before rounding, the fp32 value differs
-            # from the oracle's fp64 one by the fp32 error of the forward up to that layer -- the same
-            # error the hidden states of this run show against the oracle (hhat_max_abs_err, itself
-            # held to the stated tolerance above); one matvec alone gives 3e-5 (K <= 13824 terms of
-            # magnitude <= 1e-1, 2^-24 relative each). That difference can move a value across one
-            # rounding boundary: allowed = one bf16 ulp of the larger magnitude + KV_ABS. (Counting
-            # ulps alone is meaningless next to zero, where one ulp is far below KV_ABS.)
-            KV_ABS = max(3e-5, 4.0 * summary["hhat_max_abs_err"])
             gf, of = bf16_bits_to_f64(gs), bf16_bits_to_f64(os_)
             mag = np.maximum(np.abs(gf), np.abs(of))
             one_ulp = np.exp2(np.floor(np.log2(np.maximum(mag, 1e-30))) - 7)
-            bad = np.abs(gf - of) > one_ulp + KV_ABS
-            assert not bad.any(), (f"{name} cache rows differ beyond one bf16 ulp + {KV_ABS}: "
-                                   f"{int(bad.sum())} values, worst {np.abs(gf - of).max():.3e}")
+            diff = np.abs(gf - of)
+            summary[f"{name}_stored_differ_frac"] = float((ulp != 0).mean())
+            summary[f"{name}_stored_max_abs_diff"] = float(diff.max())
+            bad = diff > one_ulp + KV_PRE[cfg.dtype]
+            assert not bad.any(), (f"{name} cache rows differ beyond one bf16 ulp + {KV_PRE[cfg.dtype]}: "
+                                   f"{int(bad.sum())} values, worst {diff.max():.3e}")
             assert (ulp != 0).mean() < 0.02, f"{name}: {(ulp != 0).mean():.3%} of stored values differ"
         else:
             np.testing.assert_allclose(g[:, :, case.L:used], o[:, :, case.L:used], **tol)
         assert np.array_equal(g[:, :, used:], o[:, :, used:]), f"{name} rows past the step modified"
     return summary
+
+
+def run_both(case: Case, log=print, tight: bool = False, **kw):
+    """Free-running and teacher-forced step against the oracle. Returns (summary of the forced run with the
+    free run's under 'free', forced gpu result, oracle result)."""
+    ora = run_oracle(case)
+    h, kv, free = run_gpu(case, **kw)
+    s_free = compare(case, free, ora, log=log)
+    binding.dovetail_draft_destroy(h)
+    h, kv, gpu = run_gpu(case, force=ora, **kw)
+    s = compare(case, gpu, ora, log=log, tight=tight)
+    binding.dovetail_draft_destroy(h)
+    s["free"] = s_free
+    brief = {k: (f"{v:.3e}" if isinstance(v, float) else v) for k, v in s.items() if k not in ("per_level", "free")}
+    log(f"forced: {brief}; free: same_tree {s_free['same_tree']} tie {s_free['tie']} "
+        f"logit err {s_free['logit_max_abs_err']:.3e} hhat err {s_free['hhat_max_abs_err']:.3e}")
+    return s, gpu, ora

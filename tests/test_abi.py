@@ -20,26 +20,37 @@ def lib():
     return binding.load()
 
 
-def _declared():
-    src = open(os.path.join(ROOT, "include", "dovetail.h")).read()
-    return sorted(set(re.findall(r"\b(dovetail_[a-z_]+)\s*\(", src)))
+def _declared(header):
+    src = open(os.path.join(ROOT, "include", header)).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)  # prototypes only, not the prose
+    return sorted(set(re.findall(r"\b(dovetail_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(lib):
-    names = _declared()
+    names = _declared("dovetail.h")
     assert set(names) == set(binding.EXPORTS)
-    for n in names:
+    hooks = _declared("dovetail_hooks.h")
+    assert set(hooks) == set(binding.HOOK_EXPORTS)
+    for n in names + hooks:
         assert getattr(lib, n) is not None
 
 
+def test_no_environment_variables_in_the_library():
+    """no env vars, no global state in the product."""
+    csrc = os.path.join(ROOT, "paper_2412_18934_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
 def test_struct_layouts_match_header():
-    # sizes implied by include/dovetail.h (LP64): 7 int32 + 2 float + 7 int32; 9 pointers; ...
-    assert C.sizeof(binding.ConfigT) == 16 * 4
+    # sizes implied by include/dovetail.h (LP64): 7 int32 + 2 float + 8 int32; 9 pointers; ...
+    assert C.sizeof(binding.ConfigT) == 17 * 4
     assert C.sizeof(binding.LayerWeightsT) == 9 * 8
     assert C.sizeof(binding.WeightsT) == 8 * 8
     assert C.sizeof(binding.KVCacheT) == 24
     assert C.sizeof(binding.TreeSpecT) == 4 * (1 + 16 + 16 + 1)
     assert C.sizeof(binding.DraftOutT) == 5 * 8
+    assert C.sizeof(binding.HooksT) == 11 * 8
 
 
 def test_null_arguments_are_rejected(lib):
@@ -47,6 +58,8 @@ def test_null_arguments_are_rejected(lib):
     assert lib.dovetail_draft_step(None, None, None, 1, None, None, None, None) == binding.EINVAL
     assert lib.dovetail_kv_commit(None, None, None, 0, 0, None, None) == binding.EINVAL
     assert lib.dovetail_last_launch_count(None) == 0
+    assert lib.dovetail_draft_status(None, None) == binding.EINVAL
+    assert lib.dovetail_hooks_set(None, None) == binding.EINVAL
     assert lib.dovetail_forward_bytes(None, 0) == 0
     assert b"null" in lib.dovetail_last_error(None)
     lib.dovetail_draft_destroy(None)

@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 import torch
 
-from parity import compare, make_case, run_gpu, run_oracle
+from parity import compare, make_case, run_both, run_gpu, run_oracle
 from paper_2412_18934_b200 import binding
 from paper_2412_18934_b200.configs import BF16, CONFIGS, F32, DraftConfig, TreeSpec, c4_sweep, paper_preset
 
@@ -31,24 +31,15 @@ def _boost(case, lm=40.0, emb=20.0):
 
 
 def _run(case, **kw):
-    """Free-running step (discrete outputs, level-0 values) and teacher-forced step (every row, element by
-    element) against the oracle."""
-    ora = run_oracle(case)
-    h, kv, free = run_gpu(case, **kw)
-    s_free = compare(case, free, ora)
-    binding.dovetail_draft_destroy(h)
-    h, kv, gpu = run_gpu(case, force=ora, **kw)
-    s = compare(case, gpu, ora)
-    s["free_same_tree"] = s_free["same_tree"]
-    s["free_deep_rows_logit_viol"] = s_free.get("deep_rows_logit_viol")
-    print({k: (f"{v:.3e}" if isinstance(v, float) else v) for k, v in s.items()})
-    binding.dovetail_draft_destroy(h)
-    s["same_tree"] = s["same_tree"] and s_free["same_tree"]
+    """Free-running step and teacher-forced step against the oracle (parity.run_both): every row of both
+    runs element by element; discrete outputs identical unless the oracle's margin AT the differing decision
+    is below tolerance."""
+    s, gpu, ora = run_both(case, **kw)
     return s, gpu, ora
 
 
 @pytest.mark.parametrize("dtype", [F32, BF16])
-@pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "no_first_norm_final_norm", "n_new5",
+@pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "fusion_linear", "no_first_norm_final_norm", "n_new5",
                                      "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch"])
 def test_step_parity_small(dtype, variant):
     kw, n_new, prefix = dict(dtype=dtype), 1, None
@@ -58,6 +49,8 @@ def test_step_parity_small(dtype, variant):
         kw.update(n_q_heads=4, n_kv_heads=1)
     elif variant == "no_proj":
         kw.update(dgf_proj=0)
+    elif variant == "fusion_linear":  # the EAGLE-2 fusion DGF replaces
+        kw.update(dgf_proj=0, fusion=1)
     elif variant == "no_first_norm_final_norm":
         kw.update(first_layer_input_norm=0, final_norm=1)
     elif variant == "n_new5":
@@ -76,7 +69,8 @@ def test_step_parity_small(dtype, variant):
         kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
     case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
     s, gpu, ora = _run(case)
-    assert s["same_tree"] or s["oracle_min_margin"] < 1e-2
+    assert s["same_tree"]  # forced run: always; the free run's tree may differ only by a logged local tie
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
     if dtype == F32:
         assert s["logit_max_abs_err"] < 1e-4
 
@@ -85,7 +79,7 @@ def test_config_c1_tiny_fp32():
     """BASELINE.json configs[0]: hidden 256, 4 x 64, 2 layers, FFN 688, vocab 1024, prefix 64, 14-token tree."""
     cfg = CONFIGS["c1"]
     case = make_case(cfg, n_new=1)
-    s, gpu, ora = _run(case)
+    s, gpu, ora = _run(case, tight=True)
     assert gpu["n_out"] == 14
     assert s["logit_max_abs_err"] < 1e-4
 
@@ -113,13 +107,29 @@ def test_full_size_configs(name):
     configuration bench.py times. The oracle runs the whole step in fp64 on the host."""
     cfg = CONFIGS[name]
     case = make_case(cfg, n_new=1)
-    s, gpu, ora = _run(case)
+    s, gpu, ora = _run(case, tight=True)
     assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
+    assert s["free"]["same_tree"], f"free-running tree differs from the oracle's: {s['free']['tie']}"
 
 
-def test_c4_sweep_point():
-    """BASELINE.json configs[3]: one point of the sweep (1 layer, 4 rows per level, prefix 2048)."""
-    cfg = [c for c in c4_sweep() if c.name == "c4_l1_g32"][0]
+@pytest.mark.parametrize("name", ["c4_l1_g32", "c4_l1_m8", "c4_l1_m16", "c4_l1_m32"])
+def test_c4_sweep_points(name):
+    """BASELINE.json configs[3] at full K (13B shape, prefix 2048): one step-level point (4 rows per level)
+    and the forward-level points with 8, 16 and 32 rows in one level."""
+    cfg = [c for c in c4_sweep() if c.name == name][0]
     case = make_case(cfg, n_new=1)
-    s, gpu, ora = _run(case)
-    assert gpu["n_out"] == 32
+    s, gpu, ora = _run(case, tight=True)
+    assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("name", ["depth_eagle2_l1", "depth_dgf_l1", "depth_dgf_l6"])
+def test_depth_sweep_ends(name):
+    """The ablation's shape (Table 6) at full size: the EAGLE-2 baseline (concat + Linear, one
+    block) and DGF with 1 and 6 blocks on the 7B-shaped draft."""
+    from paper_2412_18934_b200.configs import depth_sweep
+    cfg = [c for c in depth_sweep() if c.name == name][0]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case, tight=True)
+    assert gpu["n_out"] == 16
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None

@@ -173,6 +173,19 @@ def test_error_paths():
     assert int(out["n_out"].item()) == 4 and kv.committed_len == case.L + 1
     assert binding.dovetail_last_launch_count(h) > 0
     assert binding.dovetail_forward_bytes(h, case.L) == cfg.forward_bytes(case.L)
+    binding.dovetail_draft_status(h)  # a good step: OK
+    # a token id outside [0, vocab): the step cannot see it (device memory); dovetail_draft_status reports it
+    for bad_tok in (cfg.vocab, -1, 2 ** 30):
+        kv.committed_len = case.L
+        step(good, t=torch.tensor([bad_tok], dtype=torch.int32, device="cuda"))
+        assert code(lambda: binding.dovetail_draft_status(h)) == binding.EINVAL
+        assert "token id" in binding.dovetail_last_error(h)
+        binding.dovetail_draft_status(h)  # the flag is cleared by the read
+    # wrong dtypes never reach the raw-pointer ABI
+    with pytest.raises(TypeError):
+        step(good, f=case.feats.to(torch.bfloat16))
+    with pytest.raises(TypeError):
+        step(good, t=case.tokens.to(torch.int64))
     binding.dovetail_draft_destroy(h)
     # init-time validation
     bad = small_cfg(dtype=F32, head_dim=32, hidden=128)
@@ -180,3 +193,78 @@ def test_error_paths():
     with pytest.raises(binding.DovetailError) as ei:
         binding.dovetail_draft_init(c2.top, c2.layers, bad)
     assert ei.value.code == binding.EINVAL
+
+
+def test_two_steps_chained_through_commit_mode1():
+    """step -> kv_commit(mode 1) of the deepest accepted chain -> step again, against the oracle run on the
+    oracle's own committed cache: the moved rows, their rotary positions and committed_len are what the second
+    step's attention consumes (O9 then O2-O8)."""
+    from helpers import kv_np
+    from parity import compare
+    cfg = small_cfg(dtype=BF16, tree=TreeSpec(3, (3, 2, 2), (0, 3, 3), 8))
+    case = _boost(make_case(cfg, n_new=2, slack=40))
+    h, kv, gpu = run_gpu(case)
+    ora = run_oracle(case)
+    assert np.array_equal(gpu["token_ids"], ora["token_ids"]) and np.array_equal(gpu["parents"], ora["parents"])
+    leaf = int(np.argmax(gpu["depths"]))
+    path = [leaf]
+    while gpu["parents"][path[-1]] >= 0:
+        path.append(int(gpu["parents"][path[-1]]))
+    path = path[::-1]
+    Lp = kv.committed_len
+    moved = binding.dovetail_kv_commit(h, kv, path, mode=1)
+    keep_idx = _kept_pool_indices(ora)
+    tree_rows = [int(ora["pool_row"][keep_idx[i]]) - 2 if ora["pool_row"][keep_idx[i]] >= 0 else -1 for i in path]
+    okc, ovc = ora["k"], ora["v"]
+    assert oracle.kv_commit(_ocfg(cfg), okc, ovc, case.capacity, Lp, tree_rows, 1) == moved and moved >= 1
+    L2 = Lp + moved
+    assert kv.committed_len == L2
+    # second step: the accepted tokens' successors with fresh (seeded) target features; both sides start from
+    # their own committed cache
+    import dataclasses
+    from paper_2412_18934_b200 import synth
+    feats2, tokens2 = synth.make_inputs(cfg, 3, device="cuda", seed=99)
+    k2 = torch.from_numpy(okc.view(np.int16).copy()).view(torch.bfloat16).cuda()
+    v2 = torch.from_numpy(ovc.view(np.int16).copy()).view(torch.bfloat16).cuda()
+    case2 = dataclasses.replace(case, k=k2, v=v2, feats=feats2, tokens=tokens2, L=L2)
+    ora2 = run_oracle(case2)
+    rows2 = 3 + case.tree.tree_rows()
+    P = case.tree.pool_size()
+    hooks = dict(tap_logits=torch.zeros((rows2, cfg.vocab), device="cuda"), tap_hhat=torch.zeros((rows2, cfg.hidden), device="cuda"),
+                 tap_pool_token=torch.zeros(P, dtype=torch.int32, device="cuda"), tap_pool_cum=torch.zeros(P, device="cuda"))
+    binding.dovetail_hooks_set(h, **hooks)
+    out = binding.dovetail_draft_step(h, feats2, tokens2, kv, case.tree)  # the GPU's own cache, as committed
+    binding.dovetail_draft_status(h)
+    n = int(out["n_out"].item())
+    g2 = dict(token_ids=out["token_ids"][:n].cpu().numpy(), scores=out["scores"][:n].cpu().numpy(),
+              parents=out["parents"][:n].cpu().numpy(), depths=out["depths"][:n].cpu().numpy(), n_out=n,
+              logits=hooks["tap_logits"].cpu().numpy(), hhat=hooks["tap_hhat"].cpu().numpy(),
+              pool_token=hooks["tap_pool_token"].cpu().numpy(), pool_cum=hooks["tap_pool_cum"].cpu().numpy(),
+              k=kv_np(kv.k), v=kv_np(kv.v), forced=False, committed_len=kv.committed_len)
+    s2 = compare(case2, g2, ora2)
+    assert s2["same_tree"] and kv.committed_len == L2 + 3
+    binding.dovetail_draft_destroy(h)
+
+
+def test_trace_adds_up():
+    """dovetail_trace_*: per-kind exclusive device times add up to at most the step (the launches keep their
+    programmatic-dependent-launch overlap), every kind of the step is present, bytes = algorithmic bytes."""
+    cfg = small_cfg(dtype=BF16)
+    case = make_case(cfg, n_new=1)
+    h = binding.dovetail_draft_init(case.top, case.layers, cfg)
+    kv = binding.KVCache(case.k.clone(), case.v.clone(), case.L)
+    binding.dovetail_trace_enable(h, True)
+    out = binding.dovetail_draft_step(h, case.feats, case.tokens, kv, case.tree)
+    torch.cuda.synchronize()
+    t = binding.dovetail_trace_read(h)
+    kinds = t["kinds"]
+    n_launch = sum(k["launches"] for k in kinds.values())
+    assert n_launch == binding.dovetail_last_launch_count(h)
+    assert t["step_us"] > 0
+    assert sum(k["excl_us"] for k in kinds.values()) <= t["step_us"] * 1.0001
+    for name in ("step_begin", "dgf_proj", "dgf_gate", "qkv", "tree_attention", "o_proj", "gate_up", "down", "lm_head", "tree_level"):
+        assert kinds[name]["launches"] > 0 and kinds[name]["busy_us"] > 0, name
+    wbytes = sum(k["bytes"] for n, k in kinds.items() if n != "tree_attention")
+    assert wbytes == case.tree.depth * (cfg.forward_bytes(0) - (2 * cfg.n_layers + 1) * cfg.hidden * cfg.esize)  # all matrices; not the norm gains / gate bias
+    binding.dovetail_trace_enable(h, False)
+    binding.dovetail_draft_destroy(h)

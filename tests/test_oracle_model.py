@@ -78,6 +78,61 @@ def test_dgf_matches_torch_reference_random_weights():
         np.testing.assert_allclose(_dgf(cfg, top, layers, f[i].numpy(), int(toks[i])), want[i], rtol=1e-12)
 
 
+# ---- the fusion DGF replaces: concat + one Linear (Table 6 "w/o both") ----------
+
+def _fl(cfg, top, layers, f, tok):
+    return oracle.fusion_linear(ocfg(cfg), oweights(top, layers), f, tok)
+
+
+def test_fusion_linear_selectors_pin_concat_order_and_bias():
+    """Wfc = [I | 0] returns the feature, [0 | I] the embedding (hidden state first, reading A17), Wfc = 0 the
+    bias -- bit for bit."""
+    cfg = tiny_cfg(dgf_proj=0, fusion=1)
+    d = cfg.hidden
+    top, layers = synth.make_weights(cfg)
+    f = np.random.default_rng(5).normal(size=d)
+    e = top["embed"][4].double().numpy()
+    eye, zero = torch.eye(d), torch.zeros(d, d)
+    t = dict(top, dgf_wg=torch.cat([eye, zero], 1), dgf_bg=torch.zeros(d))
+    np.testing.assert_array_equal(_fl(cfg, t, layers, f, 4), f)
+    t = dict(top, dgf_wg=torch.cat([zero, eye], 1), dgf_bg=torch.zeros(d))
+    np.testing.assert_array_equal(_fl(cfg, t, layers, f, 4), e)
+    b = torch.randn(d, generator=torch.Generator().manual_seed(1))
+    t = dict(top, dgf_wg=torch.zeros(d, 2 * d), dgf_bg=b)
+    np.testing.assert_array_equal(_fl(cfg, t, layers, f, 4), b.double().numpy())
+
+
+def test_fusion_linear_matches_torch_linear_and_the_hf_stack():
+    """x = Wfc [f || e] + b against torch.nn.functional.linear (library routine), then the whole forward with
+    this fusion against Hugging Face's decoder layers."""
+    cfg = tiny_cfg(dgf_proj=0, fusion=1)
+    top, layers = synth.make_weights(cfg)
+    g = torch.Generator().manual_seed(6)
+    f = torch.randn(3, cfg.hidden, dtype=torch.float64, generator=g)
+    toks = torch.tensor([1, 7, 10])
+    e = top["embed"][toks].double()
+    want = torch.nn.functional.linear(torch.cat([f, e], -1), top["dgf_wg"].double(), top["dgf_bg"].double()).numpy()
+    for i in range(3):
+        np.testing.assert_allclose(_fl(cfg, top, layers, f[i].numpy(), int(toks[i])), want[i], rtol=1e-12)
+    L, R, cap = 5, 3, 12
+    k, v = synth.make_kv(cfg, cap, L)
+    feats, tokens = synth.make_inputs(cfg, R)
+    slots = [L + i for i in range(R)]
+    allowed = [list(range(L + i + 1)) for i in range(R)]
+    hh, kc, vc = _oracle_forward(cfg, top, layers, k, v, cap, slots, slots, allowed, feats, tokens)
+    ref = RefDraft(cfg, top, layers)
+    ref.preload(k, v, L)
+    np.testing.assert_allclose(hh, ref.rows(feats, tokens, slots).numpy(), rtol=2e-6, atol=2e-6)
+
+
+def test_fusion_linear_differs_from_dgf_on_the_same_weights():
+    """A dropped dispatch (fusion flag ignored) would make the two variants coincide."""
+    cfg0, cfg1 = tiny_cfg(dgf_proj=0, fusion=0), tiny_cfg(dgf_proj=0, fusion=1)
+    top, layers = synth.make_weights(cfg1)
+    f = np.random.default_rng(7).normal(size=cfg1.hidden)
+    assert np.abs(_fl(cfg1, top, layers, f, 2) - _dgf(cfg0, top, layers, f, 2)).max() > 1e-3
+
+
 # ---- O4 decoder block vs Hugging Face (P4) ---------------------------------
 
 def _oracle_forward(cfg, top, layers, k, v, cap, slots, pos, allowed, feats, tokens):
