@@ -15,6 +15,7 @@
 #pragma once
 #include <cuda_bf16.h>
 
+#include "epilogue.cuh"
 #include "ptx.cuh"
 #include "state.cuh"
 
@@ -27,6 +28,7 @@ struct AttnParams {
   const StepDyn* dyn;
   const float* qkv;        // [M][dq + 2*dkv] raw q, k, v of this level's rows (fp32)
   float* obuf;             // [M][dq]
+  SplitOut so;             // the same as split-bf16 planes for the O-projection GEMV (epilogue.cuh), or xs == NULL
   const RowTables* rows;
   const float2* rope;      // [table rows][dh/2] = (cos, sin) of the rotary angle
   int32_t rope_row0;       // table row of m = 0
@@ -328,7 +330,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
       }
       if (n_chunks == 1) {
         const int m = qv / grp, hq = hk * grp + qv % grp;
-        p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+        {
+          const float ov = oo / ll;
+          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
+          if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+        }
       } else {
         float* r = p.ws + ((static_cast<size_t>(hk) * n_chunks + c) * p.qv_cap + qv) * WSTR;
         r[dd] = oo;
@@ -363,7 +369,11 @@ __global__ void __launch_bounds__(kThreads, 2) k_tree_attention(const AttnParams
           oo += __ldcg(r + dd) * cw;
         }
         const int m = qv / grp, hq = hk * grp + qv % grp;
-        p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+        {
+          const float ov = oo / ll;
+          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
+          if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+        }
       }
       if (tid == 0) p.counters[hk] = 0;
     }

@@ -443,7 +443,11 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
         }
         if (n_groups == 1) {
           const int m = qv / grp, hq = hk * grp + qv % grp;
-          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+          {
+            const float ov = oo / ll;
+            p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
+            if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+          }
         } else {
           float* rr = p.ws + ((static_cast<size_t>(hk) * n_groups + group) * p.qv_cap + qv) * WSTR;
           rr[dd] = oo;
@@ -505,7 +509,11 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
             oo += rr[dd] * cw;
           }
           const int m = qv / grp, hq = hk * grp + qv % grp;
-          p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = oo / ll;
+          {
+            const float ov = oo / ll;
+            p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
+            if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+          }
         }
         am_consumer_sync();
       }

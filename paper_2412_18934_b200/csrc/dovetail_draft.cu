@@ -58,6 +58,10 @@ struct dovetail_draft {
   float2* rope = nullptr;
   double* inv_freq = nullptr;
   float *hbuf = nullptr, *hhat = nullptr, *qkv = nullptr, *obuf = nullptr, *act = nullptr;
+  // split-bf16 planes of the activations, the B operands of the tensor-core GEMV (epilogue.cuh): [3][rows][ld]
+  __nv_bfloat16 *xs_feat = nullptr, *xs_hhat = nullptr, *xs_x = nullptr, *xs_h12 = nullptr, *xs_o = nullptr, *xs_act = nullptr;
+  int ld_d = 0, ld_2d = 0, ld_dq = 0, ld_f = 0;  // row strides (elements, multiples of 8)
+  float* ssq = nullptr;  // [num_sms][kMaxRows] partial sums of squares of the residual stream
   float* attn_ws = nullptr;
   int32_t* attn_cnt = nullptr;
   float* cand_val = nullptr;
@@ -243,7 +247,7 @@ int div_up(int a, int b) { return (a + b - 1) / b; }
 // Geometry of the tensor-core GEMV (gemv_mma.cuh) for a [*, K] bf16 matrix, M draft rows and
 // at most max_cnt rows per CTA.
 struct MmaShape {
-  int NT, RBMAX, S, ncols, PC, RS, KC, KP, seg_stride, bs_stride, stage_bytes, n_stages, smem;
+  int NT, RBMAX, S, ncols, PC, RS, KC, seg_stride, stage_bytes, n_stages, smem;
   bool ok;
 };
 
@@ -259,36 +263,28 @@ MmaShape mma_shape(int K, int M, int max_cnt) {
   s.RBMAX = s.NT == 8 ? 2 : 4;
   s.ncols = M * s.S;
   s.PC = (s.ncols + 1) & ~1;
-  // Rows per stage, K-chunk and B-store budget: the first candidate that leaves a ring of >= 3 stages or
-  // >= 120 KB (else the deepest ring found). Wide levels need the smaller stages: their B store and partial
-  // buffers take most of the shared memory.
+  // Rows per stage and K-chunk: the first candidate that leaves a ring of >= 3 stages or >= 120 KB (else the
+  // deepest ring found). A stage holds RS weight rows and ncols activation columns of one K-chunk. Wide levels
+  // take the smaller stages: their B columns and partial buffers use most of the shared memory.
   const int rs_max = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
   MmaShape best{};
   for (int rs = rs_max; rs >= 16; rs -= 16) {
     if (kConsumerWarps * rs * s.PC * 4 > 32768 && rs > 16) continue;
-    for (int kc0 : {512, 256}) {
-      for (int bbudget : {65536, 49152, 32768}) {
-        MmaShape c = s;
-        c.RS = rs;
-        c.KC = (rs * 2 * kc0 <= 16384) ? 1024 : kc0;
-        c.KC = std::min(c.KC, (K + 63) / 64 * 64);
-        int kpmax = (bbudget / c.ncols / 2) / c.KC * c.KC;
-        if (kpmax < c.KC) kpmax = c.KC;
-        const int n_panels = div_up(K, kpmax);
-        c.KP = div_up(div_up(K, n_panels), c.KC) * c.KC;
-        c.seg_stride = c.KC * 2 + 16;
-        c.bs_stride = c.KP * 2 + 16;
-        c.stage_bytes = c.RS * c.seg_stride;
-        int fixed = 128 + 16 + (4 + 8 + 4 * kConsumerWarps) * kMmaMaxM + c.ncols * c.bs_stride + 16 +
-                    kConsumerWarps * c.RS * c.PC * 4 + max_cnt * M * 4;
-        fixed = (fixed + 15) / 16 * 16;
-        c.n_stages = std::min(8, (kSmemMax - fixed - 64) / c.stage_bytes);
-        c.smem = c.n_stages * c.stage_bytes + fixed;
-        c.ok = c.n_stages >= 2;
-        if (!c.ok) continue;
-        if (c.n_stages >= 3 || c.n_stages * c.stage_bytes >= 120 * 1024) return c;  // two 66 KB stages stream as well as four 33 KB ones
-        if (!best.ok || c.n_stages * c.stage_bytes > best.n_stages * best.stage_bytes) best = c;
-      }
+    for (int kc0 : {512, 256, 128}) {
+      MmaShape c = s;
+      c.RS = rs;
+      c.KC = ((rs + s.ncols) * 2 * kc0 <= 16384) ? 1024 : kc0;
+      c.KC = std::min(c.KC, (K + 63) / 64 * 64);
+      c.seg_stride = c.KC * 2 + 16;
+      c.stage_bytes = (c.RS + c.ncols) * c.seg_stride;
+      int fixed = 3 * 64 + 16 + 4 * kMmaMaxM + kConsumerWarps * c.RS * c.PC * 4 + max_cnt * M * 4;
+      fixed = (fixed + 15) / 16 * 16;
+      c.n_stages = std::min(8, (kSmemMax - fixed - 64) / c.stage_bytes);
+      c.smem = c.n_stages * c.stage_bytes + fixed;
+      c.ok = c.n_stages >= 2;
+      if (!c.ok) continue;
+      if (c.n_stages >= 3 || c.n_stages * c.stage_bytes >= 120 * 1024) return c;  // two 66 KB stages stream as well as four 33 KB ones
+      if (!best.ok || c.n_stages * c.stage_bytes > best.n_stages * best.stage_bytes) best = c;
     }
   }
   s = best;
@@ -323,9 +319,8 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
   }
   p.dyn = h->dyn;
   if (h->es == 2) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
-    // Levels wider than 16 rows run in chunks of <= 16 rows (the weights are streamed once per chunk):
-    // beyond 32 B columns the split activations no longer fit next to a useful ring.
-    const int Mtot = p.M, chunk = Mtot > 16 ? 16 : Mtot;
+    // Levels wider than 32 rows run in chunks of <= 32 rows (64 B columns; the weights are streamed once per chunk).
+    const int Mtot = p.M, chunk = Mtot > kMmaMaxM ? kMmaMaxM : Mtot;
     if (mma_shape(p.K, chunk, max_cnt).ok) {
       for (int m0 = 0; m0 < Mtot; m0 += chunk) {
         const int mc = std::min(chunk, Mtot - m0);
@@ -337,10 +332,8 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
         p.stage_bytes = ms.stage_bytes;
         p.row_bytes = p.K * 2;
         p.kc = ms.KC;
-        p.kp = ms.KP;
-        p.split = ms.S;
         p.seg_stride = ms.seg_stride;
-        p.bs_stride = ms.bs_stride;
+        for (int g = 0; g < n_groups; ++g) p.g[g].S = p.g[g].xkind == X_EMBED ? 1 : ms.S;
         if (m0 > 0) h->cur_bytes = 0;  // the algorithmic bytes are counted once
         p.trace = trace_slot(h);
         cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
@@ -372,6 +365,23 @@ GemvGroup rows_group(const float* xsrc, int64_t xld, const int32_t* xidx, int fr
   g.x_from_dyn = from_dyn;
   g.gain = gain;
   return g;
+}
+
+// split-bf16 planes of an activation buffer with `rows` rows of stride ld (epilogue.cuh), first row row0
+SplitOut planes(__nv_bfloat16* xs, int64_t rows, int64_t ld, int64_t row0 = 0) {
+  SplitOut o{};
+  if (xs) {
+    o.xs = xs + row0 * ld;
+    o.plane = rows * ld;
+    o.ld = ld;
+  }
+  return o;
+}
+
+void with_planes(GemvGroup& g, const SplitOut& o) {
+  g.xs = o.xs;
+  g.xs_plane = o.plane;
+  g.xs_ld = o.ld;
 }
 
 int validate_tree(dovetail_draft* h, const dovetail_tree_spec_t* t, int n_new, std::vector<LevelPlan>& plan,
@@ -418,6 +428,8 @@ cudaError_t dmalloc(T** p, size_t n) {
 void free_all(dovetail_draft* h) {
   cudaFree(h->dyn); cudaFree(h->ts); cudaFree(h->rt); cudaFree(h->rope); cudaFree(h->inv_freq);
   cudaFree(h->hbuf); cudaFree(h->hhat); cudaFree(h->qkv); cudaFree(h->obuf); cudaFree(h->act);
+  cudaFree(h->xs_feat); cudaFree(h->xs_hhat); cudaFree(h->xs_x); cudaFree(h->xs_h12); cudaFree(h->xs_o); cudaFree(h->xs_act);
+  cudaFree(h->ssq);
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
@@ -436,8 +448,13 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
   cudaError_t e = cudaSuccess;
   const size_t xoff = static_cast<size_t>(lp.row0) * d, xbytes = static_cast<size_t>(M) * d * sizeof(float);
   if (k.tap_hhat) e = cudaMemcpyAsync(k.tap_hhat + xoff, h->hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
-  if (k.force_hhat && e == cudaSuccess)
+  if (k.force_hhat && e == cudaSuccess) {
     e = cudaMemcpyAsync(h->hhat + xoff, k.force_hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
+    if (h->xs_hhat && e == cudaSuccess) {  // the children read the forced rows as split-bf16 planes
+      k_resplit_rows<<<M, 256, 0, st>>>(h->hhat + xoff, d, planes(h->xs_hhat, h->max_step_rows, h->ld_d, lp.row0));
+      e = cudaGetLastError();
+    }
+  }
   const size_t pitch = static_cast<size_t>(kv->capacity) * dh * h->es, width = static_cast<size_t>(M) * dh * h->es;
   const size_t off = static_cast<size_t>(l == 0 ? L : Lp + lp.t0) * dh * h->es;
   const size_t height = static_cast<size_t>(c.n_layers) * c.n_kv_heads;
@@ -494,8 +511,10 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   // k_step_begin is launched WITHOUT programmatic serialization: it starts only once everything
   // enqueued before the step has completed, which is what lets later kernels read the committed
   // prefix (cache rows < L) before their griddepcontrol.wait.
-  e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(64), 0, st, dv, h->dyn, h->ts, h->rt,
-               h->rope, static_cast<const double*>(h->inv_freq), half, V, trace_slot(h));
+  const int64_t R = c.max_rows, SR = h->max_step_rows;
+  const int nct_d = std::min(nsm, d);  // CTAs of the GEMVs that produce the residual stream (and its sums of squares)
+  e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(512), 0, st, dv, h->dyn, h->ts, h->rt,
+               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h->xs_feat, R, h->ld_d), trace_slot(h));
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
 
   for (int l = 0; l < tree->depth; ++l) {
@@ -510,6 +529,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
     if (c.dgf_proj) {
       GemvParams p{};
       p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
+      with_planes(p.g[0], l == 0 ? planes(h->xs_feat, R, h->ld_d) : planes(h->xs_hhat, SR, h->ld_d));
       p.g[0].w[0] = h->w.dgf_w1;
       p.g[0].rows[0] = d;
       p.g[0].n_mat = 1;
@@ -527,6 +547,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       p.epi = EPI_STORE;
       p.out = h->hbuf;
       p.out_ld = 2 * d;
+      p.so = planes(h->xs_h12, R, h->ld_2d);
       rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)), 1);
       if (rc) return rc;
     } else {
@@ -536,16 +557,17 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       if (bf16)
         e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
                    static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
-                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d, trace_slot(h));
+                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d, planes(h->xs_h12, R, h->ld_2d), trace_slot(h));
       else
         e = launch(h, k_fill_h<float>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
                    static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
-                   static_cast<const float*>(h->w.embed), h->hbuf, M, d, trace_slot(h));
+                   static_cast<const float*>(h->w.embed), h->hbuf, M, d, SplitOut{}, trace_slot(h));
       if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
     }
     {  // S1: gate, sigmoid, blend; or the single Linear of the EAGLE-2 fusion (:104)
       GemvParams p{};
       p.g[0] = rows_group(h->hbuf, 2 * d, nullptr, 0, nullptr);
+      with_planes(p.g[0], planes(h->xs_h12, R, h->ld_2d));
       p.g[0].w[0] = h->w.dgf_wg;
       p.g[0].rows[0] = d;
       p.g[0].n_mat = 1;
@@ -557,7 +579,11 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       p.hbuf = h->hbuf;
       p.bias = h->w.dgf_bg;
       p.d = d;
-      rc = run_gemv(h, st, p, 1, std::min(nsm, d), 2);
+      // x feeds the first block's QKV: planes of x * g_attn (raw x when the first input norm is skipped)
+      p.so = planes(h->xs_x, R, h->ld_d);
+      p.gain_out = c.first_layer_input_norm ? h->layers[0].g_attn : nullptr;
+      p.ssq_out = h->ssq;
+      rc = run_gemv(h, st, p, 1, nct_d, 2);
       if (rc) return rc;
     }
 
@@ -567,6 +593,9 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         GemvParams p{};
         const void* gain = (ly == 0 && !c.first_layer_input_norm) ? nullptr : W.g_attn;
         p.g[0] = rows_group(x, d, nullptr, 0, gain);
+        with_planes(p.g[0], planes(h->xs_x, R, h->ld_d));
+        p.ssq_in = gain ? h->ssq : nullptr;
+        p.ssq_nct = nct_d;
         p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq;
         p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv;
         p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv;
@@ -604,6 +633,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         h->cur_kind = 4;
         h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
         a.trace = trace_slot(h);
+        a.so = planes(h->xs_o, R, h->ld_dq);
         if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
           a.kc = kv->k;
           a.vc = kv->v;
@@ -638,18 +668,25 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       {  // S4: x += Wo o
         GemvParams p{};
         p.g[0] = rows_group(h->obuf, dq, nullptr, 0, nullptr);
+        with_planes(p.g[0], planes(h->xs_o, R, h->ld_dq));
         p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
         p.K = dq;
         p.M = M;
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 5);
+        p.so = planes(h->xs_x, R, h->ld_d);  // feeds gate / up through the post-attention norm
+        p.gain_out = W.g_ffn;
+        p.ssq_out = h->ssq;
+        rc = run_gemv(h, st, p, 1, nct_d, 5);
         if (rc) return rc;
       }
       {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
         GemvParams p{};
         p.g[0] = rows_group(x, d, nullptr, 0, W.g_ffn);
+        with_planes(p.g[0], planes(h->xs_x, R, h->ld_d));
+        p.ssq_in = h->ssq;
+        p.ssq_nct = nct_d;
         p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F;
         p.g[0].w[1] = W.wup; p.g[0].rows[1] = F;
         p.g[0].n_mat = 2;
@@ -660,19 +697,34 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         p.epi = EPI_SWIGLU;
         p.out = h->act;
         p.out_ld = F;
+        p.so = planes(h->xs_act, R, h->ld_f);
         rc = run_gemv(h, st, p, 1, std::min(nsm, F), 6);
         if (rc) return rc;
       }
       {  // S5b: x += Wdown act
         GemvParams p{};
         p.g[0] = rows_group(h->act, F, nullptr, 0, nullptr);
+        with_planes(p.g[0], planes(h->xs_act, R, h->ld_f));
         p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
         p.K = F;
         p.M = M;
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, d), 7);
+        if (ly + 1 < c.n_layers) {  // feeds the next block's QKV through its input norm
+          p.so = planes(h->xs_x, R, h->ld_d);
+          p.gain_out = h->layers[ly + 1].g_attn;
+          p.ssq_out = h->ssq;
+        } else {
+          // the block stack's output: feature of this row's children (raw) and input of the LM head
+          p.so_raw = planes(h->xs_hhat, SR, h->ld_d, lp.row0);
+          if (c.final_norm) {
+            p.so = planes(h->xs_x, R, h->ld_d);
+            p.gain_out = h->w.g_final;
+            p.ssq_out = h->ssq;
+          }
+        }
+        rc = run_gemv(h, st, p, 1, nct_d, 7);
         if (rc) return rc;
       }
     }
@@ -682,6 +734,12 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       GemvParams p{};
       const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
       p.g[0] = rows_group(xs, d, nullptr, 0, c.final_norm ? h->w.g_final : nullptr);
+      const int lm_row = l == 0 ? n_new - 1 : 0;  // first row of the level whose list is expanded
+      with_planes(p.g[0], c.final_norm ? planes(h->xs_x, R, h->ld_d, lm_row) : planes(h->xs_hhat, SR, h->ld_d, lp.row0 + lm_row));
+      if (c.final_norm) {
+        p.ssq_in = h->ssq + lm_row;
+        p.ssq_nct = nct_d;
+      }
       p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1;
       p.K = d;
       p.M = lp.rows_lm;
@@ -808,6 +866,17 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   A(dmalloc(&h->qkv, R * h->ldq));
   A(dmalloc(&h->obuf, R * dq));
   A(dmalloc(&h->act, R * c.ffn));
+  auto up8 = [](int k) { return (k + 7) / 8 * 8; };
+  h->ld_d = up8(c.hidden); h->ld_2d = up8(2 * c.hidden); h->ld_dq = up8(dq); h->ld_f = up8(c.ffn);
+  if (es == 2) {
+    A(dmalloc(&h->xs_feat, kSplitPlanes * R * h->ld_d));
+    A(dmalloc(&h->xs_hhat, static_cast<size_t>(kSplitPlanes) * h->max_step_rows * h->ld_d));
+    A(dmalloc(&h->xs_x, kSplitPlanes * R * h->ld_d));
+    A(dmalloc(&h->xs_h12, kSplitPlanes * R * h->ld_2d));
+    A(dmalloc(&h->xs_o, kSplitPlanes * R * h->ld_dq));
+    A(dmalloc(&h->xs_act, kSplitPlanes * R * h->ld_f));
+    A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
+  }
   A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));
   A(dmalloc(&h->cand_val, R * h->num_sms * kMaxBranch));

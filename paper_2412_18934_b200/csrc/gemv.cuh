@@ -20,6 +20,7 @@
 #pragma once
 #include <cuda_bf16.h>
 
+#include "epilogue.cuh"
 #include "ptx.cuh"
 #include "state.cuh"
 
@@ -44,6 +45,11 @@ struct GemvGroup {
   const int32_t* tokens; //          token of each m
   const void* gain;      // RMSNorm gain [K] (storage dtype) or NULL: no norm
   int32_t out_off;       // EPI_STORE: offset added to the output column
+  // k_gemv_mma: the B operand of this group as split-bf16 planes (epilogue.cuh), left by the producer of
+  // the activation. Row of draft row m: xidx ? xidx[m] : m. X_EMBED: the embedding table itself (one plane).
+  const __nv_bfloat16* xs;
+  int64_t xs_plane, xs_ld;
+  int32_t S;             // planes read per draft row: 3 (all 24 mantissa bits), 2 (16 bits), 1 (bf16 source)
 };
 
 struct GemvParams {
@@ -51,9 +57,9 @@ struct GemvParams {
   const StepDyn* dyn;
   int32_t K, M;
   int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
-  // k_gemv_mma only: K-chunk per stage, K-panel of the B store, split ways, strides (bytes)
-  int32_t kc, kp, split, seg_stride, bs_stride;
-  int32_t m0;            // k_gemv_mma: first draft row of this launch (levels wider than 16 rows run in row chunks)
+  // k_gemv_mma only: K-chunk per stage, stride of a row / column within a stage (bytes)
+  int32_t kc, seg_stride;
+  int32_t m0;            // k_gemv_mma: first draft row of this launch (levels wider than 32 rows run in row chunks)
   int32_t epi;
   float eps;
   float* out;            // STORE/SWIGLU: [M, out_ld]; DGF/RESID: residual stream rows x [M, out_ld]
@@ -67,6 +73,15 @@ struct GemvParams {
   int32_t* cand_id;
   float* stat;           // LMHEAD: [kMaxRows][grid][2] = (max, sum exp)
   float* tap;            // LMHEAD: optional logits tap rows [M, vocab]
+  // k_gemv_mma, RMSNorm of the input: partial sums of squares of the raw x, [ssq_nct][kMaxRows], left by the
+  // epilogue that produced x (the gain is already folded into the planes); NULL: no norm
+  const float* ssq_in;
+  int32_t ssq_nct;
+  // what the epilogue leaves for the next GEMV (epilogue.cuh); all optional
+  SplitOut so;           // planes of (result * gain_out)   [draft row][out_off + column]
+  const void* gain_out;  // RMSNorm gain of the consumer [N] (storage dtype) or NULL
+  SplitOut so_raw;       // planes of the raw result (the last block's x: next level's feature, LM-head input)
+  float* ssq_out;        // [gridDim.x][kMaxRows] sum of squares of the raw result over this CTA's columns
   unsigned long long* trace;  // dovetail_trace_*: {first CTA start, last CTA end} of this launch, or NULL
 };
 
@@ -138,11 +153,90 @@ __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& r
   }
 }
 
-__device__ __forceinline__ float sigmoidf_acc(float z) { return 1.0f / (1.0f + expf(-z)); }
-
-// strict order of LM-head candidates: logit descending, token id ascending (reading A7)
-__device__ __forceinline__ bool cand_before(float va, int ia, float vb, int ib) {
-  return va > vb || (va == vb && ia < ib);
+// ---- fused epilogue over the CTA's results --------------------------------------------------
+// res(v, m): result of the CTA's virtual row v for draft row mbase + m, m < Mt (already scaled by 1 / rms
+// when the input is normed). Runs on the kConsumerThreads consumer threads of either GEMV kernel.
+template <typename Res>
+__device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGroup& G, const RowRange& rr, Res res,
+                                              int Mt, int mbase, int c, int nct, bool bf16) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int cnt = rr.cnt;
+  if (p.epi == EPI_STORE || p.epi == EPI_DGF || p.epi == EPI_RESID) {
+    for (int idx = tid; idx < cnt * Mt; idx += kConsumerThreads) {
+      const int m = idx / cnt, v = idx - m * cnt;
+      const int64_t mm = mbase + m, n = rr.g0 + v;
+      float y = res(v, m);
+      float* dst = p.out + mm * p.out_ld + G.out_off + n;
+      if (p.epi == EPI_STORE) {  // optional bias: the concat + Linear fusion
+        if (p.bias) y += load_storage(p.bias, n, bf16);
+      } else if (p.epi == EPI_DGF) {
+        // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
+        const float g = sigmoidf_acc(y + load_storage(p.bias, n, bf16));
+        const float h1 = p.hbuf[mm * 2 * p.d + n], h2 = p.hbuf[mm * 2 * p.d + p.d + n];
+        y = g * h1 + (1.0f - g) * h2;
+      } else {
+        y += *dst;  // residual stream
+      }
+      *dst = y;
+      res(v, m) = y;
+      if (p.so.xs) store_split(p.so, mm, G.out_off + n, p.gain_out ? y * load_storage(p.gain_out, n, bf16) : y);
+      if (p.so_raw.xs) store_split(p.so_raw, mm, n, y);
+    }
+    if (p.ssq_out) {  // sum of squares of the raw result over this CTA's columns, fixed order
+      consumer_sync();
+      for (int m = warp; m < Mt; m += kConsumerWarps) {
+        float t = 0.f;
+        for (int v = lane; v < cnt; v += 32) t = fmaf(res(v, m), res(v, m), t);
+        t = warp_sum(t);
+        if (lane == 0) p.ssq_out[static_cast<int64_t>(c) * kMaxRows + mbase + m] = t;
+      }
+    }
+  } else if (p.epi == EPI_SWIGLU) {
+    // act = SiLU(Wgate n) * (Wup n); gate rows are virtual rows [0, cr), up rows [cr, 2cr)
+    for (int idx = tid; idx < rr.cr * Mt; idx += kConsumerThreads) {
+      const int m = idx / rr.cr, r = idx - m * rr.cr;
+      const int64_t mm = mbase + m;
+      const float gv = res(r, m), uv = res(rr.cr + r, m);
+      const float y = gv * sigmoidf_acc(gv) * uv;
+      p.out[mm * p.out_ld + rr.n0 + r] = y;
+      if (p.so.xs) store_split(p.so, mm, rr.n0 + r, y);
+    }
+  } else {  // EPI_LMHEAD: logits of rows [g0, g0 + cnt) of the vocabulary
+    if (p.tap) {
+      for (int idx = tid; idx < cnt * Mt; idx += kConsumerThreads) {
+        const int m = idx / cnt, v = idx - m * cnt;
+        p.tap[static_cast<int64_t>(mbase + m) * p.vocab + rr.g0 + v] = res(v, m);
+      }
+    }
+    for (int m = warp; m < Mt; m += kConsumerWarps) {
+      float mx = -INFINITY;
+      for (int v = lane; v < cnt; v += 32) mx = fmaxf(mx, res(v, m));
+      mx = warp_max(mx);
+      float se = 0.f;
+      for (int v = lane; v < cnt; v += 32) se += expf(res(v, m) - mx);
+      se = warp_sum(se);
+      const int64_t pc = static_cast<int64_t>(mbase + m) * nct + c;
+      if (lane == 0) { p.stat[pc * 2] = mx; p.stat[pc * 2 + 1] = se; }
+      // local top-b: b rounds of "best candidate strictly after the previous pick"
+      float lv = INFINITY; int li = -1;
+      for (int jb = 0; jb < p.b; ++jb) {
+        float bv = -INFINITY; int bi = 0x7fffffff;
+        for (int v = lane; v < cnt; v += 32) {
+          const float val = res(v, m);
+          const int id = static_cast<int>(rr.g0) + v;
+          if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+          const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+          if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+        }
+        if (lane == 0) { p.cand_val[pc * kMaxBranch + jb] = bv; p.cand_id[pc * kMaxBranch + jb] = bi; }
+        lv = bv; li = bi;
+      }
+    }
+  }
 }
 
 template <typename WT, int MT, int NI>
@@ -337,83 +431,8 @@ __global__ void __launch_bounds__(kThreads, 1) k_gemv(const GemvParams p) {
       for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rstd_s[idx % MT];
       consumer_sync();
     }
-    if (p.epi == EPI_STORE) {  // optional bias: the concat + Linear fusion
-      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
-        const int v2 = idx / MT, mm = m0 + idx % MT;
-        float bz = 0.f;
-        if (p.bias) {
-          if (sizeof(WT) == 2) bz = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[rr.g0 + v2]);
-          else bz = static_cast<const float*>(p.bias)[rr.g0 + v2];
-        }
-        if (mm < p.M) p.out[mm * p.out_ld + G.out_off + rr.g0 + v2] = res[idx] + bz;
-      }
-    } else if (p.epi == EPI_DGF) {
-      // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
-      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
-        const int mm = m0 + idx % MT;
-        const int64_t n = rr.g0 + idx / MT;
-        if (mm < p.M) {
-          float bz;
-          if (sizeof(WT) == 2) bz = __bfloat162float(static_cast<const __nv_bfloat16*>(p.bias)[n]);
-          else bz = static_cast<const float*>(p.bias)[n];
-          const float g = sigmoidf_acc(res[idx] + bz);
-          const float h1 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + n];
-          const float h2 = p.hbuf[static_cast<int64_t>(mm) * 2 * p.d + p.d + n];
-          p.out[mm * p.out_ld + n] = g * h1 + (1.0f - g) * h2;
-        }
-      }
-    } else if (p.epi == EPI_RESID) {
-      for (int idx = tid; idx < nres; idx += kConsumerThreads) {
-        const int mm = m0 + idx % MT;
-        const int64_t n = rr.g0 + idx / MT;
-        if (mm < p.M) p.out[mm * p.out_ld + n] += res[idx];
-      }
-    } else if (p.epi == EPI_SWIGLU) {
-      // act = SiLU(Wgate n) * (Wup n); gate rows are virtual rows [0, cr), up rows [cr, 2cr)
-      for (int idx = tid; idx < rr.cr * MT; idx += kConsumerThreads) {
-        const int r = idx / MT, m = idx % MT, mm = m0 + m;
-        if (mm < p.M) {
-          const float gv = res[r * MT + m], uv = res[(rr.cr + r) * MT + m];
-          p.out[mm * p.out_ld + rr.n0 + r] = gv * sigmoidf_acc(gv) * uv;
-        }
-      }
-    } else {  // EPI_LMHEAD: logits of rows [g0, g0 + cnt) of the vocabulary
-      if (p.tap) {
-        for (int idx = tid; idx < nres; idx += kConsumerThreads) {
-          const int mm = m0 + idx % MT;
-          if (mm < p.M) p.tap[static_cast<int64_t>(mm) * p.vocab + rr.g0 + idx / MT] = res[idx];
-        }
-      }
-      if (warp < MT && m0 + warp < p.M) {
-        const int m = warp, mm = m0 + warp;
-        float mx = -INFINITY;
-        for (int v2 = lane; v2 < rr.cnt; v2 += 32) mx = fmaxf(mx, res[v2 * MT + m]);
-        mx = warp_max(mx);
-        float se = 0.f;
-        for (int v2 = lane; v2 < rr.cnt; v2 += 32) se += expf(res[v2 * MT + m] - mx);
-        se = warp_sum(se);
-        const int64_t pc = static_cast<int64_t>(mm) * nct + c;
-        if (lane == 0) { p.stat[pc * 2] = mx; p.stat[pc * 2 + 1] = se; }
-        // local top-b: b rounds of "best candidate strictly after the previous pick"
-        float lv = INFINITY; int li = -1;
-        for (int jb = 0; jb < p.b; ++jb) {
-          float bv = -INFINITY; int bi = 0x7fffffff;
-          for (int v2 = lane; v2 < rr.cnt; v2 += 32) {
-            const float val = res[v2 * MT + m];
-            const int id = static_cast<int>(rr.g0) + v2;
-            if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
-          }
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) {
-            const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-            const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-            if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-          }
-          if (lane == 0) { p.cand_val[pc * kMaxBranch + jb] = bv; p.cand_id[pc * kMaxBranch + jb] = bi; }
-          lv = bv; li = bi;
-        }
-      }
-    }
+    gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[v * MT + m]; }, min(MT, p.M - m0), m0, c, nct,
+                  sizeof(WT) == 2);
     consumer_sync();  // res is reused by the next m-tile
   }
   trace_end(p.trace);

@@ -26,7 +26,7 @@ struct Pool {  // device arrays of capacity pool_cap
 // ---- S0 ---------------------------------------------------------------------
 // grid = n_new + depth - 1 CTAs (one rotary-table row each) x 64 threads.
 __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, RowTables* rt0,
-                             float2* rope, const double* inv_freq, int half, int vocab,
+                             float2* rope, const double* inv_freq, int half, int vocab, int d, SplitOut feat_so,
                              unsigned long long* trace) {
   pdl_launch_dependents();
   trace_begin(trace);
@@ -39,6 +39,8 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
     sincos(static_cast<double>(pos) * inv_freq[i], &s, &c);
     rope[static_cast<size_t>(r) * half + i] = make_float2(static_cast<float>(c), static_cast<float>(s));
   }
+  // the caller's fp32 features as split-bf16 planes, the B operand of the DGF projection (epilogue.cuh)
+  if (r < n_new && feat_so.xs != nullptr) split_row(feat_so, r, dynv.feats + static_cast<size_t>(r) * d, d);
   if (r == 0) {
     if (threadIdx.x == 0) {
       *dyn = dynv;  // ts->status is sticky until dovetail_draft_status / kv_commit reads it
@@ -66,10 +68,15 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
   trace_end(trace);
 }
 
+// Test hook (teacher forcing, dovetail_hooks.h): planes of M forced hidden-state rows. grid = M.
+__global__ void k_resplit_rows(const float* x, int d, SplitOut so) {
+  split_row(so, blockIdx.x, x + static_cast<size_t>(blockIdx.x) * d, d);
+}
+
 // dgf_proj == 0: h1 = f, h2 = e (W1 = W2 = identity). grid-stride over M * 2d.
 template <typename WT>
 __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, int64_t xld,
-                         const RowTables* rt, int use_idx, const WT* embed, float* hbuf, int M, int d,
+                         const RowTables* rt, int use_idx, const WT* embed, float* hbuf, int M, int d, SplitOut so,
                          unsigned long long* trace) {
   pdl_launch_dependents();
   trace_begin(trace);
@@ -86,6 +93,7 @@ __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, in
       else v = *reinterpret_cast<const float*>(&e);
     }
     hbuf[idx] = v;
+    if (so.xs) store_split(so, m, k, v);
   }
   __syncthreads();
   trace_end(trace);
