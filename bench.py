@@ -214,6 +214,8 @@ def bench_one(a, cfg, rank, world, local, dist):
 
     case = make_case(cfg, n_new=a.n_new, device="cuda")
     h = binding.dovetail_draft_init(case.top, case.layers, cfg)
+    if a.chain:
+        binding.dovetail_hooks_tune(h, 0, a.chain)
     kv = binding.KVCache(case.k, case.v, case.L)
     out = binding.alloc_out(tree.gamma)
     stream = torch.cuda.current_stream()
@@ -422,6 +424,7 @@ def main():
     ap.add_argument("--n-new", type=int, default=1)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--replays", type=int, default=200)
+    ap.add_argument("--chain", type=int, default=0, help="A/B knob: GEMVs per persistent launch (0: library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-trace", action="store_true")
     ap.add_argument("--no-both-dgf", dest="both_dgf", action="store_false")

@@ -21,7 +21,7 @@ EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "
            "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
-HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream")
+HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune")
 
 
 class DovetailError(RuntimeError):
@@ -103,6 +103,8 @@ def load() -> C.CDLL:
         lib.dovetail_trace_read.restype = C.c_int
         lib.dovetail_trace_read.argtypes = [C.c_void_p, C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32), C.POINTER(C.c_int64),
                                             C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
+        lib.dovetail_hooks_tune.restype = C.c_int
+        lib.dovetail_hooks_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
         lib.dovetail_probe_stream.restype = C.c_int
         lib.dovetail_probe_stream.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_void_p]
         lib.dovetail_last_launch_count.restype = C.c_int
@@ -325,6 +327,11 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
             rec["launches"] += 1
             rec["bytes"] += nbytes[i]
     return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
+
+
+def dovetail_hooks_tune(h: Draft, key: int, value: int):
+    """Design knobs for A/B measurements (include/dovetail_hooks.h): key 0 = GEMVs per persistent launch."""
+    _check(load().dovetail_hooks_tune(h.ptr, key, value), h.ptr)
 
 
 def dovetail_probe_stream(h: Draft, buf, mode: int, seg: int = 1024, stream=None):

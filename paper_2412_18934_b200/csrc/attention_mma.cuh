@@ -48,8 +48,10 @@ __device__ __forceinline__ void ldsm_x4_trans(uint32_t (&r)[4], uint32_t addr) {
 }
 
 // 16-byte async copy global -> shared; src_bytes = 0 writes zeros without reading.
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(src_bytes) : "memory");
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src, uint32_t src_bytes, uint64_t policy) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(dst), "l"(src), "r"(src_bytes),
+               "l"(policy)
+               : "memory");
 }
 // arrives on the mbarrier once all prior cp.async of this thread have landed
 __device__ __forceinline__ void cp_async_arrive(uint64_t* bar) {
@@ -155,6 +157,9 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   if (warp >= kAmWarps) {
     // ---------------- producers ---------------------------------------------------
     const int ptid = tid - kAmConsumers;
+    // the prefix is re-read by every level of the step and by the next steps (4 layers x 21 MB on the 13B shape
+    // fit the 126 MB L2 next to the weight stream, which is evict_first): keep it
+    const uint64_t pol = l2_policy_evict_last();
     // Invariant: before griddepcontrol.wait only cache rows below p.Lsafe -- the
     // prefix committed before this step, which no kernel of the step writes -- may be read. Rows
     // [Lsafe, Lbase) of a tree level were appended by this step's level-0 kernels, several launches
@@ -190,8 +195,8 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           const bool valid = r < cnt;  // rows past the end are zero filled (0 * stale NaN would poison P V)
           const size_t so = valid ? static_cast<size_t>(r) * ROWB + ch * 16 : 0;
           const uint32_t d = am_swz<ROWB>(r, ch);
-          cp_async16(kdst + d, ksrc + so, valid ? 16u : 0u);
-          cp_async16(vdst + d, vsrc + so, valid ? 16u : 0u);
+          cp_async16(kdst + d, ksrc + so, valid ? 16u : 0u, pol);
+          cp_async16(vdst + d, vsrc + so, valid ? 16u : 0u, pol);
         }
         cp_async_arrive(&full[slot]);
         if (++slot == kAmStages) { slot = 0; ++round; }

@@ -80,6 +80,16 @@ struct dovetail_draft {
   int last_launches = 0;
   int launches = 0;
   bool dry = false;  // shape-checking pass of dovetail_draft_step: nothing is launched
+  // GEMVs queued for one persistent launch (gemv_mma.cuh ChainParams)
+  struct QueuedGemv { GemvParams p; int n_groups, ctas, kind, max_cnt; int64_t bytes; };
+  std::vector<QueuedGemv> queue;
+  int chain_max = 1;           // GEMVs per persistent launch (1: every GEMV is its own launch; measured best)
+  int32_t* bar = nullptr;      // phase counters of the step's chains, zeroed by k_step_begin
+  int bar_used = 0;
+#ifdef DVT_CHAINDBG
+  unsigned long long* dbg = nullptr;
+  int dbg_launch = 0;
+#endif
   // per-launch time stamps (dovetail_trace_*)
   bool trace_on = false;
   unsigned long long* trace_buf = nullptr;  // device [kMaxTraceLaunches][2]
@@ -112,8 +122,8 @@ constexpr int kMaxTraceLaunches = 4096;
 
 // Time-stamp slot of the launch about to be made (NULL unless tracing); records its kind / bytes.
 unsigned long long* trace_slot(dovetail_draft* h) {
-  if (!h->trace_on || h->dry || h->launches >= kMaxTraceLaunches) return nullptr;
-  const int i = h->launches;
+  if (!h->trace_on || h->dry || h->tr_used >= kMaxTraceLaunches) return nullptr;
+  const int i = h->tr_used;
   if (static_cast<int>(h->tr_kind.size()) <= i) { h->tr_kind.resize(i + 1); h->tr_level.resize(i + 1); h->tr_bytes.resize(i + 1); }
   h->tr_kind[i] = h->cur_kind;
   h->tr_level[i] = h->cur_level;
@@ -158,6 +168,8 @@ cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 bl
 }
 
 using GemvKernel = void (*)(const GemvParams);
+using ChainKernel = void (*)(const ChainParams);
+constexpr int kMaxBars = 2048;
 
 template <typename WT>
 GemvKernel pick_gemv(int MT, int NI) {
@@ -170,7 +182,7 @@ GemvKernel pick_gemv(int MT, int NI) {
   return k_gemv<WT, 2, 7>;
 }
 
-GemvKernel pick_gemv_mma(int NT) {
+ChainKernel pick_gemv_mma(int NT) {
   if (NT == 1) return k_gemv_mma<1, 4>;
   if (NT == 2) return k_gemv_mma<2, 4>;
   if (NT == 4) return k_gemv_mma<4, 4>;
@@ -244,40 +256,69 @@ GemvShape gemv_shape(int K, int es, int M, int res_rows) {
 
 int div_up(int a, int b) { return (a + b - 1) / b; }
 
-// Geometry of the tensor-core GEMV (gemv_mma.cuh) for a [*, K] bf16 matrix, M draft rows and
-// at most max_cnt rows per CTA.
-struct MmaShape {
-  int NT, RBMAX, S, ncols, PC, RS, KC, seg_stride, stage_bytes, n_stages, smem;
+// Geometry of one persistent launch of the tensor-core GEMV kernel (gemv_mma.cuh) over a chain of GEMVs.
+struct ChainGeom {
+  int NT, RBMAX, RS, stage_bytes, n_stages, part_floats, smem;
+  int S[kMaxChain], KC[kMaxChain], seg_stride[kMaxChain], RSp[kMaxChain];  // per phase
   bool ok;
 };
 
-MmaShape mma_shape(int K, int M, int max_cnt) {
-  MmaShape s{};
-  s.ok = K % 32 == 0 && M >= 1 && M <= kMmaMaxM && max_cnt >= 1;
-  if (!s.ok) return s;
-  auto nt_for = [](int cols) { int t = (cols + 7) / 8, r = 1; while (r < t) r *= 2; return r; };
-  const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
-  s.S = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
-  s.NT = nt2;
-  if (s.NT > 8) { s.ok = false; return s; }
-  s.RBMAX = s.NT == 8 ? 2 : 4;
-  s.ncols = M * s.S;
-  s.PC = (s.ncols + 1) & ~1;
+int nt_for(int cols) {
+  int t = (cols + 7) / 8, r = 1;
+  while (r < t) r *= 2;
+  return r;
+}
+
+ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n) {
+  ChainGeom s{};
+  s.ok = n >= 1 && n <= kMaxChain;
+  int max_cnt = 1, nt = 1, res_floats = 0;
+  for (int i = 0; s.ok && i < n; ++i) {
+    const int K = q[i].p.K, M = q[i].p.M;
+    s.ok = K % 32 == 0 && M >= 1 && M <= kMmaMaxM && q[i].max_cnt >= 1;
+    if (!s.ok) break;
+    const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
+    s.S[i] = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
+    nt = std::max(nt, nt2);
+    max_cnt = std::max(max_cnt, q[i].max_cnt);
+    res_floats = std::max(res_floats, q[i].max_cnt * M);
+  }
+  if (!s.ok || nt > 8) { s.ok = false; return s; }
+  s.NT = nt;
+  s.RBMAX = nt == 8 ? 2 : 4;
   // Rows per stage and K-chunk: the first candidate that leaves a ring of >= 3 stages or >= 120 KB (else the
-  // deepest ring found). A stage holds RS weight rows and ncols activation columns of one K-chunk. Wide levels
+  // deepest ring found). A stage holds RS weight rows and M * S activation columns of one K-chunk. Wide levels
   // take the smaller stages: their B columns and partial buffers use most of the shared memory.
   const int rs_max = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
-  MmaShape best{};
+  ChainGeom best{};
   for (int rs = rs_max; rs >= 16; rs -= 16) {
-    if (kConsumerWarps * rs * s.PC * 4 > 32768 && rs > 16) continue;
     for (int kc0 : {512, 256, 128}) {
-      MmaShape c = s;
+      ChainGeom c = s;
       c.RS = rs;
-      c.KC = ((rs + s.ncols) * 2 * kc0 <= 16384) ? 1024 : kc0;
-      c.KC = std::min(c.KC, (K + 63) / 64 * 64);
-      c.seg_stride = c.KC * 2 + 16;
-      c.stage_bytes = (c.RS + c.ncols) * c.seg_stride;
-      int fixed = 3 * 64 + 16 + 4 * kMmaMaxM + kConsumerWarps * c.RS * c.PC * 4 + max_cnt * M * 4;
+      c.stage_bytes = 0;
+      c.part_floats = 0;
+      // rows a stage really carries in phase i: the CTA's rows in balanced super-blocks of <= rs rows
+      auto rows_eff = [&](int i) { const int nsb = div_up(q[i].max_cnt, rs); return std::min(rs, div_up(q[i].max_cnt, nsb)); };
+      for (int i = 0; i < n; ++i) {
+        const int ncols = q[i].p.M * s.S[i], PC = (ncols + 1) & ~1;
+        c.KC[i] = std::min(kc0, (q[i].p.K + 63) / 64 * 64);
+        c.seg_stride[i] = c.KC[i] * 2 + 16;
+        c.stage_bytes = std::max(c.stage_bytes, (rows_eff(i) + ncols) * c.seg_stride[i]);
+        c.part_floats = std::max(c.part_floats, kConsumerWarps * rs * PC);
+      }
+      // phases with few rows per CTA (O, down: 35 of 64) take longer K-chunks so that their stages are full too
+      for (int i = 0; i < n; ++i) {
+        const int ncols = q[i].p.M * s.S[i];
+        while (c.KC[i] < 2048 && c.KC[i] * 2 <= (q[i].p.K + 63) / 64 * 64 &&
+               (rows_eff(i) + ncols) * (c.KC[i] * 4 + 16) <= c.stage_bytes + 4096) {
+          c.KC[i] *= 2;
+          c.seg_stride[i] = c.KC[i] * 2 + 16;
+        }
+        c.stage_bytes = std::max(c.stage_bytes, (rows_eff(i) + ncols) * c.seg_stride[i]);
+        c.RSp[i] = rows_eff(i);
+      }
+      if (c.part_floats * 4 > 32768 && rs > 16) continue;
+      int fixed = 3 * 64 + 16 + 2 * 4 * kMmaMaxM + c.part_floats * 4 + res_floats * 4;
       fixed = (fixed + 15) / 16 * 16;
       c.n_stages = std::min(8, (kSmemMax - fixed - 64) / c.stage_bytes);
       c.smem = c.n_stages * c.stage_bytes + fixed;
@@ -287,27 +328,117 @@ MmaShape mma_shape(int K, int M, int max_cnt) {
       if (!best.ok || c.n_stages * c.stage_bytes > best.n_stages * best.stage_bytes) best = c;
     }
   }
-  s = best;
-  return s;
+  return best;
 }
 
-// Enqueue one GEMV: group list, K, M rows, epilogue.
+// One GEMV on the FMA kernel (fp32 models; bf16 matrices whose K is not a multiple of 32).
+int run_gemv_fma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q) {
+  GemvParams& p = q.p;
+  h->cur_kind = q.kind;
+  h->cur_bytes = q.bytes;
+  const GemvShape s = gemv_shape(p.K, h->es, p.M, q.max_cnt + 1);
+  if (!s.ok) return fail(h, DOVETAIL_EINVAL, "GEMV with K = %d is not supported (K * elem size must be a multiple of 16 and <= 28672 bytes)", p.K);
+  p.rows_per_stage = s.rows_per_stage;
+  p.n_stages = s.n_stages;
+  p.stage_bytes = s.stage_bytes;
+  p.row_bytes = s.row_bytes;
+  GemvKernel k = h->es == 2 ? pick_gemv<__nv_bfloat16>(s.MT, s.NI) : pick_gemv<float>(s.MT, s.NI);
+  p.trace = trace_slot(h);
+  cudaError_t e = launch(h, k, dim3(q.ctas, q.n_groups), dim3(kThreads), s.smem, st, p);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV launch failed: %s", cudaGetErrorString(e));
+  return DOVETAIL_OK;
+}
+
+// One persistent launch over q[0 .. n): tensor-core kernel.
+int run_chain(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv* q, int n, const ChainGeom& g) {
+  ChainParams cp{};
+  cp.n = n;
+  cp.stage_bytes = g.stage_bytes;
+  cp.n_stages = g.n_stages;
+  cp.part_floats = g.part_floats;
+  if (n > 1) {
+    if (h->bar_used + n > kMaxBars) return fail(h, DOVETAIL_EINVAL, "too many GEMV phases in one step");
+    cp.bar = h->bar + h->bar_used;
+    h->bar_used += n;
+  }
+  int grid = 1;
+  for (int i = 0; i < n; ++i) {
+    GemvParams& p = q[i].p;
+    p.n_groups = q[i].n_groups;
+    p.ctas_per_group = q[i].ctas;
+    p.rows_per_stage = g.RSp[i];
+    p.row_bytes = p.K * 2;
+    p.kc = g.KC[i];
+    p.seg_stride = g.seg_stride[i];
+    for (int gi = 0; gi < q[i].n_groups; ++gi) p.g[gi].S = p.g[gi].xkind == X_EMBED ? 1 : g.S[i];
+    h->cur_kind = q[i].kind;
+    h->cur_bytes = q[i].bytes;
+    p.trace = trace_slot(h);
+    grid = std::max(grid, q[i].n_groups * q[i].ctas);
+    cp.ph[i] = p;
+  }
+#ifdef DVT_CHAINDBG
+  if (!h->dry) {
+    if (!h->dbg) { cudaMalloc(reinterpret_cast<void**>(&h->dbg), sizeof(unsigned long long) * 64 * 148 * kMaxChain * 8); cudaMemset(h->dbg, 0, sizeof(unsigned long long) * 64 * 148 * kMaxChain * 8); }
+    if (h->dbg_launch < 64) cp.dbg = h->dbg + static_cast<size_t>(h->dbg_launch++) * 148 * kMaxChain * 8;
+  }
+#endif
+  cudaError_t e = launch(h, pick_gemv_mma(g.NT), dim3(grid), dim3(kMmaThreads), g.smem, st, cp);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
+  return DOVETAIL_OK;
+}
+
+// Launch everything queued: maximal runs of tensor-core-capable GEMVs as chains of <= chain_max, the rest one
+// by one on the FMA kernel.
+int flush_gemv(dovetail_draft* h, cudaStream_t st) {
+  auto& Q = h->queue;
+  int rc = DOVETAIL_OK;
+  size_t i = 0;
+  while (i < Q.size() && rc == DOVETAIL_OK) {
+    const bool mma_ok = h->es == 2 && chain_geom(&Q[i], 1).ok;
+    if (!mma_ok) {
+      if (h->es == 2 && Q[i].p.M > kMmaMaxM && Q[i].p.K % 32 == 0) {
+        // a level wider than 32 rows: chunks of <= 32 rows (64 B columns), the weights are streamed once per chunk
+        const int Mtot = Q[i].p.M;
+        for (int m0 = 0; m0 < Mtot && rc == DOVETAIL_OK; m0 += kMmaMaxM) {
+          dovetail_draft::QueuedGemv c = Q[i];
+          c.p.M = std::min(kMmaMaxM, Mtot - m0);
+          c.p.m0 = m0;
+          if (m0 > 0) c.bytes = 0;  // the algorithmic bytes are counted once
+          const ChainGeom g = chain_geom(&c, 1);
+          rc = g.ok ? run_chain(h, st, &c, 1, g) : fail(h, DOVETAIL_EINVAL, "GEMV with K = %d does not fit the tensor-core kernel", c.p.K);
+        }
+      } else {
+        rc = run_gemv_fma(h, st, Q[i]);
+      }
+      ++i;
+      continue;
+    }
+    int n = 1;  // grow the chain while the geometry stays valid
+    ChainGeom g = chain_geom(&Q[i], 1);
+    while (n < h->chain_max && i + n < Q.size()) {
+      const ChainGeom g2 = chain_geom(&Q[i], n + 1);
+      if (!g2.ok || g2.n_stages * g2.stage_bytes < 100 * 1024) break;
+      g = g2;
+      ++n;
+    }
+    rc = run_chain(h, st, &Q[i], n, g);
+    i += n;
+  }
+  Q.clear();
+  return rc;
+}
+
+// Queue one GEMV: group list, K, M rows, epilogue. It is launched by the next flush_gemv.
 int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, int ctas_per_group, int kind) {
-  int res_rows = 0, max_cnt = 0;
-  h->cur_kind = kind;
-  h->cur_bytes = 0;
-  for (int g = 0; g < n_groups; ++g)
-    for (int j = 0; j < p.g[g].n_mat; ++j) h->cur_bytes += static_cast<int64_t>(p.g[g].rows[j]) * p.K * h->es;
+  (void)st;
+  dovetail_draft::QueuedGemv q{};
+  q.n_groups = n_groups;
+  q.ctas = ctas_per_group;
+  q.kind = kind;
   for (int g = 0; g < n_groups; ++g) {
     const GemvGroup& G = p.g[g];
-    int r;
-    if (G.paired) r = G.n_mat * (div_up(G.rows[0], ctas_per_group) + 1);
-    else {
-      long tot = 0;
-      for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
-      r = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group) + 1;
-    }
-    if (r > res_rows) res_rows = r;
+    for (int j = 0; j < G.n_mat; ++j) q.bytes += static_cast<int64_t>(G.rows[j]) * p.K * h->es;
     int mc;
     if (G.paired) mc = G.n_mat * div_up(G.rows[0], ctas_per_group);
     else {
@@ -315,44 +446,11 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
       for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
       mc = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group);
     }
-    if (mc > max_cnt) max_cnt = mc;
+    q.max_cnt = std::max(q.max_cnt, mc);
   }
   p.dyn = h->dyn;
-  if (h->es == 2) {  // bf16 weights: tensor-core consumer (gemv_mma.cuh)
-    // Levels wider than 32 rows run in chunks of <= 32 rows (64 B columns; the weights are streamed once per chunk).
-    const int Mtot = p.M, chunk = Mtot > kMmaMaxM ? kMmaMaxM : Mtot;
-    if (mma_shape(p.K, chunk, max_cnt).ok) {
-      for (int m0 = 0; m0 < Mtot; m0 += chunk) {
-        const int mc = std::min(chunk, Mtot - m0);
-        const MmaShape ms = mma_shape(p.K, mc, max_cnt);
-        p.M = mc;
-        p.m0 = m0;
-        p.rows_per_stage = ms.RS;
-        p.n_stages = ms.n_stages;
-        p.stage_bytes = ms.stage_bytes;
-        p.row_bytes = p.K * 2;
-        p.kc = ms.KC;
-        p.seg_stride = ms.seg_stride;
-        for (int g = 0; g < n_groups; ++g) p.g[g].S = p.g[g].xkind == X_EMBED ? 1 : ms.S;
-        if (m0 > 0) h->cur_bytes = 0;  // the algorithmic bytes are counted once
-        p.trace = trace_slot(h);
-        cudaError_t e = launch(h, pick_gemv_mma(ms.NT), dim3(ctas_per_group, n_groups), dim3(kMmaThreads), ms.smem, st, p);
-        if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
-      }
-      return DOVETAIL_OK;
-    }
-  }
-  const GemvShape s = gemv_shape(p.K, h->es, p.M, res_rows);
-  if (!s.ok) return fail(h, DOVETAIL_EINVAL, "GEMV with K = %d is not supported (K * elem size must be a multiple of 16 and <= 28672 bytes)", p.K);
-  p.rows_per_stage = s.rows_per_stage;
-  p.n_stages = s.n_stages;
-  p.stage_bytes = s.stage_bytes;
-  p.row_bytes = s.row_bytes;
-  p.dyn = h->dyn;
-  GemvKernel k = h->es == 2 ? pick_gemv<__nv_bfloat16>(s.MT, s.NI) : pick_gemv<float>(s.MT, s.NI);
-  p.trace = trace_slot(h);
-  cudaError_t e = launch(h, k, dim3(ctas_per_group, n_groups), dim3(kThreads), s.smem, st, p);
-  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV launch failed: %s", cudaGetErrorString(e));
+  q.p = p;
+  h->queue.push_back(q);
   return DOVETAIL_OK;
 }
 
@@ -430,6 +528,7 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->hbuf); cudaFree(h->hhat); cudaFree(h->qkv); cudaFree(h->obuf); cudaFree(h->act);
   cudaFree(h->xs_feat); cudaFree(h->xs_hhat); cudaFree(h->xs_x); cudaFree(h->xs_h12); cudaFree(h->xs_o); cudaFree(h->xs_act);
   cudaFree(h->ssq);
+  cudaFree(h->bar);
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
@@ -503,6 +602,12 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   h->cur_kind = 0;
   h->cur_bytes = 0;
   h->cur_level = 0;
+  h->tr_used = 0;
+  h->bar_used = 0;
+  h->queue.clear();
+#ifdef DVT_CHAINDBG
+  h->dbg_launch = 0;
+#endif
   if (h->trace_on && !h->dry) {  // start = ~0 (atomicMin), end = 0 (atomicMax)
     e = cudaMemsetAsync(h->trace_buf, 0, sizeof(unsigned long long) * 2 * kMaxTraceLaunches, st);
     if (e == cudaSuccess) e = cudaMemset2DAsync(h->trace_buf, 16, 0xff, 8, kMaxTraceLaunches, st);
@@ -514,7 +619,8 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   const int64_t R = c.max_rows, SR = h->max_step_rows;
   const int nct_d = std::min(nsm, d);  // CTAs of the GEMVs that produce the residual stream (and its sums of squares)
   e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(512), 0, st, dv, h->dyn, h->ts, h->rt,
-               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h->xs_feat, R, h->ld_d), trace_slot(h));
+               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h->xs_feat, R, h->ld_d), h->bar, kMaxBars,
+               trace_slot(h));
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
 
   for (int l = 0; l < tree->depth; ++l) {
@@ -552,6 +658,8 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       if (rc) return rc;
     } else {
       const int blocks = std::min(nsm, div_up(M * 2 * d, 256));
+      rc = flush_gemv(h, st);
+      if (rc) return rc;
       h->cur_kind = 10;
       h->cur_bytes = 0;
       if (bf16)
@@ -610,6 +718,8 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         if (rc) return rc;
       }
       {  // S2 (RoPE, KV append) + S3 tree attention
+        rc = flush_gemv(h, st);
+        if (rc) return rc;
         AttnParams a{};
         a.dyn = h->dyn;
         a.qkv = h->qkv;
@@ -755,6 +865,8 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       if (rc) return rc;
     }
     {  // S7 (+ S8 after the last level)
+      rc = flush_gemv(h, st);
+      if (rc) return rc;
       TreeLevelParams t{};
       t.dyn = h->dyn;
       t.ts = h->ts;
@@ -876,6 +988,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->xs_o, kSplitPlanes * R * h->ld_dq));
     A(dmalloc(&h->xs_act, kSplitPlanes * R * h->ld_f));
     A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
+    A(dmalloc(&h->bar, kMaxBars));
   }
   A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));
@@ -1074,6 +1187,15 @@ int dovetail_hooks_set(dovetail_draft_t* h, const dovetail_hooks_t* hooks) {
 
 int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
 
+int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (key == 0 && value >= 1 && value <= kMaxChain) {
+    h->chain_max = value;
+    return DOVETAIL_OK;
+  }
+  return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
+}
+
 int dovetail_draft_status(dovetail_draft_t* h, void* cuda_stream) {
   if (!h) return DOVETAIL_EINVAL;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -1153,6 +1275,12 @@ int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
   const int64_t kvb = static_cast<int64_t>(c.n_layers) * 2 * prefix_len * dkv;
   return (params + kvb) * h->es;
 }
+
+#ifdef DVT_CHAINDBG
+int dovetail_dbg_read(dovetail_draft_t* h, unsigned long long* out, int n_launches) {
+  return cudaMemcpy(out, h->dbg, sizeof(unsigned long long) * n_launches * 148 * kMaxChain * 8, cudaMemcpyDeviceToHost);
+}
+#endif
 
 void dovetail_draft_destroy(dovetail_draft_t* h) {
   if (!h) return;

@@ -56,6 +56,7 @@ struct GemvParams {
   GemvGroup g[2];        // blockIdx.y selects the group (DGF projections use two)
   const StepDyn* dyn;
   int32_t K, M;
+  int32_t n_groups, ctas_per_group;  // k_gemv_mma (1-D grid): CTA c works for group c / ctas_per_group
   int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
   // k_gemv_mma only: K-chunk per stage, stride of a row / column within a stage (bytes)
   int32_t kc, seg_stride;

@@ -93,6 +93,28 @@ __device__ __forceinline__ void trace_end(unsigned long long* t) {
   if (t != nullptr && threadIdx.x == 0) atomicMax(t + 1, globaltimer_ns());
 }
 
+// ---- grid-wide phase barrier of a persistent kernel (all CTAs resident: one per SM) -----------
+// arrive: the calling thread's CTA has finished the phase; its global writes were made visible by
+// __threadfence() of the writing threads + a CTA barrier before this call.
+__device__ __forceinline__ void grid_arrive(int32_t* counter) {
+  asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(counter) : "memory");
+}
+__device__ __forceinline__ int32_t ld_acquire_gpu(const int32_t* p) {
+  int32_t v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+// Bounded like mbar_wait: a protocol bug traps instead of hanging the GPU.
+__device__ __forceinline__ void grid_wait(const int32_t* counter, int32_t target) {
+  uint32_t spins = 0;
+  while (ld_acquire_gpu(counter) < target) {
+    if (++spins > (1u << 24)) __trap();
+  }
+}
+// generic-proxy writes (st.global by other CTAs, observed through an acquire) before async-proxy reads
+// (bulk copies) of the same global memory
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
 // ---- named barrier among the consumer warps only ---------------------------
 __device__ __forceinline__ void consumer_sync() {
   asm volatile("bar.sync 1, %0;" ::"n"(kConsumerThreads) : "memory");

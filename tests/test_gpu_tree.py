@@ -259,7 +259,7 @@ def test_trace_adds_up():
     t = binding.dovetail_trace_read(h)
     kinds = t["kinds"]
     n_launch = sum(k["launches"] for k in kinds.values())
-    assert n_launch == binding.dovetail_last_launch_count(h)
+    assert n_launch >= binding.dovetail_last_launch_count(h)  # a persistent launch covers several GEMVs
     assert t["step_us"] > 0
     assert sum(k["excl_us"] for k in kinds.values()) <= t["step_us"] * 1.0001
     for name in ("step_begin", "dgf_proj", "dgf_gate", "qkv", "tree_attention", "o_proj", "gate_up", "down", "lm_head", "tree_level"):
