@@ -28,6 +28,8 @@ struct AttnParams {
   const StepDyn* dyn;
   const float* qkv;        // [M][dq + 2*dkv] raw q, k, v of this level's rows (fp32)
   float* obuf;             // [M][dq]
+  const __nv_bfloat16* qs; // k_tree_attention_mma with the S2 work fused into the QKV projection (gemv.cuh EPI_QKV):
+                           // rotated, scaled queries [2][kMaxRows][dq] (bf16 head, remainder); K / V already appended
   SplitOut so;             // the same as split-bf16 planes for the O-projection GEMV (epilogue.cuh), or xs == NULL
   const RowTables* rows;
   const float2* rope;      // [table rows][dh/2] = (cos, sin) of the rotary angle

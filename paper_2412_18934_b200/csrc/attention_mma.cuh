@@ -28,6 +28,7 @@
 
 namespace dvt {
 
+
 constexpr int kAmWarps = 4;                       // consumer warps
 constexpr int kAmConsumers = kAmWarps * 32;       // 128
 constexpr int kAmProducers = 64;                  // two producer warps
@@ -178,8 +179,9 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
             gate_open = true;
           }
         } else {
-          if (!tail_ready) {  // this level's rows are appended by the consumers first
-            mbar_wait(tailbar, 0);
+          if (!tail_ready) {  // this level's rows: appended by this CTA's consumers, or (fused S2) by the QKV kernel
+            if (p.qs == nullptr) mbar_wait(tailbar, 0);
+            else if (!gate_open) { mbar_wait(gatebar, 0); gate_open = true; }
             tail_ready = true;
           }
           pos0 = Lbase + (b - n_blk) * PB;
@@ -217,7 +219,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   // S2: append this level's K/V rows of kv-head hk (chunk 0 only). K is rotated (half-split
   // pairing (i, i + dh/2), reading A3) and both are rounded to the cache dtype, as the oracle
   // stores them; the new region is then attended from the cache like the prefix.
-  if (c == 0) {
+  if (c == 0 && p.qs == nullptr) {
     WT* kcw = const_cast<WT*>(kc);
     WT* vcw = const_cast<WT*>(vc);
     for (int idx = tid; idx < p.M * HALF; idx += kAmConsumers) {
@@ -243,6 +245,29 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     const int qv0 = pass * kAmQRows;
     const int nq = min(kAmQRows, qv_tot - qv0);  // query vectors of this pass
     // ---- rotated, scaled queries -> bf16 head + remainder tiles ------------------
+    if (p.qs != nullptr) {  // prepared by the QKV projection's epilogue: 16-byte copies into the swizzled tiles
+      constexpr int NQ = kAmQRows * CPR * 2 / kAmConsumers;  // copies per thread, all loads issued before the stores
+      static_assert(kAmQRows * CPR * 2 % kAmConsumers == 0, "query tile copies must divide among the consumers");
+      uint4 v[NQ];
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) {
+        const int idx = tid + i * kAmConsumers;
+        const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
+        const int r = rem / CPR, ch = rem - r * CPR;
+        v[i] = make_uint4(0u, 0u, 0u, 0u);
+        if (r < nq) {
+          const int qv = qv0 + r, m = qv / grp, hq = hk * grp + qv % grp;
+          v[i] = __ldcg(reinterpret_cast<const uint4*>(p.qs + (static_cast<size_t>(pl) * kMaxRows + m) * dq + hq * DH) + ch);
+        }
+      }
+#pragma unroll
+      for (int i = 0; i < NQ; ++i) {
+        const int idx = tid + i * kAmConsumers;
+        const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
+        const int r = rem / CPR, ch = rem - r * CPR;
+        *reinterpret_cast<uint4*>((pl ? q_lo : q_hi) + am_swz<ROWB>(r, ch)) = v[i];
+      }
+    } else
     for (int idx = tid; idx < kAmQRows * HALF; idx += kAmConsumers) {
       const int r = idx / HALF, i = idx % HALF;
       float x0 = 0.f, x1 = 0.f;

@@ -62,6 +62,7 @@ struct dovetail_draft {
   __nv_bfloat16 *xs_feat = nullptr, *xs_hhat = nullptr, *xs_x = nullptr, *xs_h12 = nullptr, *xs_o = nullptr, *xs_act = nullptr;
   int ld_d = 0, ld_2d = 0, ld_dq = 0, ld_f = 0;  // row strides (elements, multiples of 8)
   float* ssq = nullptr;  // [num_sms][kMaxRows] partial sums of squares of the residual stream
+  __nv_bfloat16* qs = nullptr;  // [2][kMaxRows][dq] rotated, scaled queries (bf16 head + remainder), gemv.cuh EPI_QKV
   float* attn_ws = nullptr;
   int32_t* attn_cnt = nullptr;
   float* cand_val = nullptr;
@@ -529,6 +530,7 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->xs_feat); cudaFree(h->xs_hhat); cudaFree(h->xs_x); cudaFree(h->xs_h12); cudaFree(h->xs_o); cudaFree(h->xs_act);
   cudaFree(h->ssq);
   cudaFree(h->bar);
+  cudaFree(h->qs);
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
@@ -582,6 +584,9 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
   const int grp = c.n_q_heads / c.n_kv_heads;
   const bool bf16 = c.dtype == DOVETAIL_BF16;
+  // bf16 models whose QKV projection runs on the tensor-core GEMV: S2 (RoPE, append, query preparation) is done
+  // by that GEMV's epilogue; otherwise by the attention kernel
+  const bool fused_s2 = bf16 && d % 32 == 0;
   cudaError_t e;
 
   // S0: per-step state, level-0 row tables, rotary table
@@ -714,7 +719,20 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         p.epi = EPI_STORE;
         p.out = h->qkv;
         p.out_ld = ldq;
-        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq), 3);
+        if (fused_s2) {  // S2 in the projection's epilogue: RoPE, K / V append, queries ready for the attention kernel
+          p.epi = EPI_QKV;
+          p.g[0].pairperm = dh;
+          p.rt = cur;
+          p.rope = h->rope;
+          p.rope_row0 = l == 0 ? 0 : n_new + l - 1;
+          p.rope_per_row = l == 0 ? 1 : 0;
+          p.Hq = c.n_q_heads;
+          p.Hkv = c.n_kv_heads;
+          p.layer = ly;
+          p.level0 = l == 0 ? 1 : 0;
+          p.qs = h->qs;
+        }
+        rc = run_gemv(h, st, p, 1, std::min(nsm, ldq / 2), 3);
         if (rc) return rc;
       }
       {  // S2 (RoPE, KV append) + S3 tree attention
@@ -744,6 +762,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
         a.trace = trace_slot(h);
         a.so = planes(h->xs_o, R, h->ld_dq);
+        a.qs = fused_s2 ? h->qs : nullptr;
         if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
           a.kc = kv->k;
           a.vc = kv->v;
@@ -989,6 +1008,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->xs_act, kSplitPlanes * R * h->ld_f));
     A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
     A(dmalloc(&h->bar, kMaxBars));
+    A(dmalloc(&h->qs, static_cast<size_t>(2) * kMaxRows * dq));
   }
   A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));

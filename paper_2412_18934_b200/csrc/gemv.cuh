@@ -27,7 +27,7 @@
 namespace dvt {
 
 enum XKind : int32_t { X_ROWS = 0, X_EMBED = 1 };
-enum Epi : int32_t { EPI_STORE = 0, EPI_DGF = 1, EPI_RESID = 2, EPI_SWIGLU = 3, EPI_LMHEAD = 4 };
+enum Epi : int32_t { EPI_STORE = 0, EPI_DGF = 1, EPI_RESID = 2, EPI_SWIGLU = 3, EPI_LMHEAD = 4, EPI_QKV = 5 };
 
 constexpr int kRowsPerStageMax = 4;
 
@@ -36,6 +36,9 @@ struct GemvGroup {
   int32_t rows[3];
   int32_t n_mat;
   int32_t paired;        // 1: the CTA's row range applies to each matrix (gate/up)
+  int32_t pairperm;      // head_dim or 0. EPI_QKV: within every head of the concatenated [q | k | v] rows the virtual
+                         // order is (0, dh/2, 1, dh/2 + 1, ...), and CTA ranges start on an even virtual row, so
+                         // that the two rows of a rotary pair (i, i + dh/2) belong to the same CTA
   int32_t xkind;
   int32_t x_from_dyn;    // X_ROWS: source rows are the caller's hidden_feats
   const float* xsrc;     // X_ROWS: fp32 rows
@@ -83,6 +86,13 @@ struct GemvParams {
   const void* gain_out;  // RMSNorm gain of the consumer [N] (storage dtype) or NULL
   SplitOut so_raw;       // planes of the raw result (the last block's x: next level's feature, LM-head input)
   float* ssq_out;        // [gridDim.x][kMaxRows] sum of squares of the raw result over this CTA's columns
+  // EPI_QKV (S2 fused into the projection): rotary embedding, K / V append to the cache, rotated and scaled
+  // queries as bf16 head + remainder planes for the tensor-core attention kernel
+  const RowTables* rt;   // slot[] of this level's rows
+  const float2* rope;    // [table rows][dh / 2] = (cos, sin)
+  int32_t rope_row0, rope_per_row;
+  int32_t Hq, Hkv, layer, level0;
+  __nv_bfloat16* qs;     // [2][kMaxRows][Hq * dh]: plane 0 = bf16(q), plane 1 = bf16(q - plane 0)
   unsigned long long* trace;  // dovetail_trace_*: {first CTA start, last CTA end} of this launch, or NULL
 };
 
@@ -124,8 +134,10 @@ __device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int nct)
   } else {
     int64_t tot = 0;
     for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
-    r.g0 = static_cast<int64_t>(c) * tot / nct;
-    const int64_t g1 = static_cast<int64_t>(c + 1) * tot / nct;
+    const int64_t unit = G.pairperm ? 2 : 1;  // deal whole rotary pairs
+    tot /= unit;
+    r.g0 = static_cast<int64_t>(c) * tot / nct * unit;
+    const int64_t g1 = static_cast<int64_t>(c + 1) * tot / nct * unit;
     r.cnt = static_cast<int32_t>(g1 - r.g0);
     r.n0 = 0;
     r.cr = 0;
@@ -141,6 +153,10 @@ __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& r
     n = rr.n0 + (v - j * rr.cr);
   } else {
     int64_t g = rr.g0 + v;
+    if (G.pairperm) {  // virtual (0, 1, 2, 3, ...) of a head = rows (0, dh/2, 1, dh/2 + 1, ...)
+      const int64_t w = g % G.pairperm;
+      g = g - w + (w >> 1) + (w & 1) * (G.pairperm >> 1);
+    }
     j = 0;
     if (g >= G.rows[0]) {
       g -= G.rows[0];
@@ -155,32 +171,76 @@ __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& r
 }
 
 // ---- fused epilogue over the CTA's results --------------------------------------------------
+// Operands of the epilogue that exist before the GEMV itself has run (residual stream, [h1 || h2], bias, the
+// consumer's norm gain): loaded into registers at kernel start so that the epilogue does not wait for L2 after
+// the last weight stage. Covers the first kEpiPre results of each thread; later ones are loaded late.
+constexpr int kEpiPre = 2;
+struct EpiRegs {
+  float a[kEpiPre], b[kEpiPre], bz[kEpiPre], g[kEpiPre];
+};
+
+__device__ __forceinline__ void epi_load(const GemvParams& p, const GemvGroup& G, const RowRange& rr, int idx, int cnt,
+                                         int mbase, bool bf16, float& a, float& b, float& bz, float& g) {
+  const int m = idx / cnt, v = idx - m * cnt;
+  const int64_t mm = mbase + m, n = rr.g0 + v;
+  a = b = bz = 0.f;
+  g = 1.f;
+  if (p.epi == EPI_STORE) {
+    if (p.bias) bz = load_storage(p.bias, n, bf16);
+  } else if (p.epi == EPI_DGF) {
+    bz = load_storage(p.bias, n, bf16);
+    a = p.hbuf[mm * 2 * p.d + n];
+    b = p.hbuf[mm * 2 * p.d + p.d + n];
+  } else {
+    a = p.out[mm * p.out_ld + G.out_off + n];  // residual stream
+  }
+  if (p.so.xs && p.gain_out) g = load_storage(p.gain_out, n, bf16);
+}
+
+__device__ __forceinline__ void epi_prefetch(const GemvParams& p, const GemvGroup& G, const RowRange& rr, int Mt, int mbase,
+                                             bool bf16, EpiRegs& r) {
+  if (p.epi != EPI_STORE && p.epi != EPI_DGF && p.epi != EPI_RESID) return;
+#pragma unroll
+  for (int i = 0; i < kEpiPre; ++i) {
+    const int idx = threadIdx.x + i * kConsumerThreads;
+    if (idx < rr.cnt * Mt) epi_load(p, G, rr, idx, rr.cnt, mbase, bf16, r.a[i], r.b[i], r.bz[i], r.g[i]);
+  }
+}
+
 // res(v, m): result of the CTA's virtual row v for draft row mbase + m, m < Mt (already scaled by 1 / rms
 // when the input is normed). Runs on the kConsumerThreads consumer threads of either GEMV kernel.
+// pre: operands loaded by epi_prefetch, or NULL.
 template <typename Res>
 __device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGroup& G, const RowRange& rr, Res res,
-                                              int Mt, int mbase, int c, int nct, bool bf16) {
+                                              int Mt, int mbase, int c, int nct, bool bf16, const EpiRegs* pre = nullptr) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int cnt = rr.cnt;
   if (p.epi == EPI_STORE || p.epi == EPI_DGF || p.epi == EPI_RESID) {
-    for (int idx = tid; idx < cnt * Mt; idx += kConsumerThreads) {
+    int it = 0;
+    for (int idx = tid; idx < cnt * Mt; idx += kConsumerThreads, ++it) {
       const int m = idx / cnt, v = idx - m * cnt;
       const int64_t mm = mbase + m, n = rr.g0 + v;
+      float a, b, bz, g;
+      if (pre != nullptr && it < kEpiPre) {
+        a = pre->a[it < kEpiPre ? it : 0]; b = pre->b[it < kEpiPre ? it : 0];
+        bz = pre->bz[it < kEpiPre ? it : 0]; g = pre->g[it < kEpiPre ? it : 0];
+      } else {
+        epi_load(p, G, rr, idx, cnt, mbase, bf16, a, b, bz, g);
+      }
       float y = res(v, m);
       float* dst = p.out + mm * p.out_ld + G.out_off + n;
       if (p.epi == EPI_STORE) {  // optional bias: the concat + Linear fusion
-        if (p.bias) y += load_storage(p.bias, n, bf16);
+        y += bz;
       } else if (p.epi == EPI_DGF) {
         // g = sigmoid(Wg [h1||h2] + bg); x = g*h1 + (1-g)*h2
-        const float g = sigmoidf_acc(y + load_storage(p.bias, n, bf16));
-        const float h1 = p.hbuf[mm * 2 * p.d + n], h2 = p.hbuf[mm * 2 * p.d + p.d + n];
-        y = g * h1 + (1.0f - g) * h2;
+        const float gt = sigmoidf_acc(y + bz);
+        y = gt * a + (1.0f - gt) * b;
       } else {
-        y += *dst;  // residual stream
+        y += a;  // residual stream
       }
       *dst = y;
       res(v, m) = y;
-      if (p.so.xs) store_split(p.so, mm, G.out_off + n, p.gain_out ? y * load_storage(p.gain_out, n, bf16) : y);
+      if (p.so.xs) store_split(p.so, mm, G.out_off + n, p.gain_out ? y * g : y);
       if (p.so_raw.xs) store_split(p.so_raw, mm, n, y);
     }
     if (p.ssq_out) {  // sum of squares of the raw result over this CTA's columns, fixed order
@@ -190,6 +250,48 @@ __device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGro
         for (int v = lane; v < cnt; v += 32) t = fmaf(res(v, m), res(v, m), t);
         t = warp_sum(t);
         if (lane == 0) p.ssq_out[static_cast<int64_t>(c) * kMaxRows + mbase + m] = t;
+      }
+    }
+  } else if (p.epi == EPI_QKV) {
+    // S2 (reading A3): q, k of a head are rotated by the row's position, half-split pairing
+    // (i, i + dh/2) = virtual rows (2i, 2i + 1) of the head; K (post-RoPE) and V are rounded to the cache dtype and
+    // appended at cache row Lbase + slot[m]; q is scaled by 1 / sqrt(dh) and left as bf16 head + remainder.
+    const int DH = G.pairperm, HALF = DH >> 1;
+    const StepDyn* dyn = p.dyn;
+    const int Lbase = p.level0 ? dyn->L : dyn->Lp;
+    const int64_t cap = dyn->capacity;
+    const float scale = 1.0f / sqrtf(static_cast<float>(DH));
+    const int dq = p.Hq * DH;
+    const int n_pairs = cnt >> 1;
+    for (int idx = tid; idx < n_pairs * Mt; idx += kConsumerThreads) {
+      const int m = idx / n_pairs, t = idx - m * n_pairs;
+      const int mm = mbase + m;
+      const int64_t g = rr.g0 + 2 * t;
+      const int hh = static_cast<int>(g / DH), i = static_cast<int>(g % DH) >> 1;
+      const float a = res(2 * t, m), b = res(2 * t + 1, m);  // elements i and i + dh/2 of head hh
+      if (hh < p.Hq + p.Hkv) {
+        const float2 cs = p.rope[static_cast<size_t>(p.rope_row0 + (p.rope_per_row ? mm : 0)) * HALF + i];
+        if (hh < p.Hq) {
+          const float x[2] = {(a * cs.x - b * cs.y) * scale, (b * cs.x + a * cs.y) * scale};
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            const uint16_t hi = f32_to_bf16_rn(x[h]);
+            const float rem = x[h] - __uint_as_float(static_cast<uint32_t>(hi) << 16);
+            uint16_t* dst = reinterpret_cast<uint16_t*>(p.qs) + static_cast<size_t>(mm) * dq + hh * DH + i + h * HALF;
+            dst[0] = hi;
+            dst[static_cast<size_t>(kMaxRows) * dq] = f32_to_bf16_rn(rem);
+          }
+        } else {
+          uint16_t* dst = static_cast<uint16_t*>(dyn->kc) +
+                          ((static_cast<size_t>(p.layer) * p.Hkv + (hh - p.Hq)) * cap + Lbase + p.rt->slot[mm]) * DH + i;
+          dst[0] = f32_to_bf16_rn(a * cs.x - b * cs.y);
+          dst[HALF] = f32_to_bf16_rn(b * cs.x + a * cs.y);
+        }
+      } else {
+        uint16_t* dst = static_cast<uint16_t*>(dyn->vc) +
+                        ((static_cast<size_t>(p.layer) * p.Hkv + (hh - p.Hq - p.Hkv)) * cap + Lbase + p.rt->slot[mm]) * DH + i;
+        dst[0] = f32_to_bf16_rn(a);
+        dst[HALF] = f32_to_bf16_rn(b);
       }
     }
   } else if (p.epi == EPI_SWIGLU) {

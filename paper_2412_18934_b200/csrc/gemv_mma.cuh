@@ -279,6 +279,8 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
     }
     if (c >= 0) {
       const RowRange rr = cta_rows(G, c, p.ctas_per_group);
+      EpiRegs pre;
+      epi_prefetch(p, G, rr, M, p.m0, true, pre);  // in flight during the streaming loop
       int n_sb, rsb;
       super_blocks(rr.cnt, RS, n_sb, rsb);
       const int RS16 = (RS + 15) & ~15;  // rows of the partial buffer: whole 16-row blocks
@@ -378,7 +380,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
         consumer_sync();
       }
       gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[static_cast<size_t>(v) * M + m]; }, M, p.m0, c,
-                    p.ctas_per_group, true);
+                    p.ctas_per_group, true, &pre);
     }
     if (tid == 0) DVT_DBG(ph, 3);
     if (ph + 1 < cp.n) {
