@@ -208,6 +208,55 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
 int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32_t* accepted_path,
                        int32_t n_acc, int32_t mode, int32_t* n_committed, void* cuda_stream);
 
+/* ---- after the draft step: verification bookkeeping and the acceptance rule ----
+ * "These candidates are then sent to the target model ... for parallel verification. The target model
+ * computes the logits of the candidate tokens in a single forward pass and applies a speculative sampling
+ * algorithm to determine the accepted tokens."
+ * Verifier rows: row 0 is the root (the last verified token, which the target has not forwarded yet), row
+ * i + 1 is candidate i of the step's output. gamma = capacity of the step's output arrays. */
+
+/* Device buffers of what the verifier's single forward needs. */
+typedef struct {
+  uint8_t* mask;         /* dev [(gamma+1) x (gamma+1)] row-major; mask[r][c] = 1 iff row c is r or an ancestor of r */
+  int32_t* position_ids; /* dev [gamma+1]; root_position + depth (root depth 0)                                    */
+  int32_t* paths;        /* dev [gamma x max_depth]; candidate indices root -> leaf of every leaf, padded with -1   */
+  int32_t* n_paths;      /* dev [1]                                                                                */
+} dovetail_verify_plan_t;
+
+/* Fills plan from the last step's output (token tree in pool order). Rows past n_out are zero / -1.
+ * Asynchronous on cuda_stream. Errors: EINVAL (null pointers, gamma < 1, max_depth < 1), ECUDA. */
+int dovetail_verify_plan(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma,
+                         int32_t root_position, int32_t max_depth, const dovetail_verify_plan_t* plan,
+                         void* cuda_stream);
+
+/* The target's answer, device memory. mode 0 needs tgt_argmax; mode 1 the other three. */
+typedef struct {
+  const int32_t* tgt_argmax; /* dev [gamma+1] the target's argmax token at every verifier row              */
+  const float* p_cand;       /* dev [gamma] target probability of candidate i's token at its parent's row  */
+  const float* uniforms;     /* dev [gamma+1] U[0,1): one per candidate, then one for the bonus token      */
+  const float* p_full;       /* dev [gamma+1][vocab] the target's distribution at every verifier row       */
+} dovetail_verify_in_t;
+
+typedef struct {
+  int32_t* accepted_path; /* dev [max_depth] candidate indices root -> last accepted node (input of kv_commit) */
+  int32_t* n_acc;         /* dev [1]                                                                          */
+  int32_t* bonus_token;   /* dev [1] the target's own next token after the accepted path; -1: no mass left   */
+} dovetail_verify_out_t;
+
+/* The acceptance rule. Walks down from the root; at each node its children are tried in candidate order.
+ *   mode 0, greedy (T = 0): a child is accepted iff its token is the target's argmax at the parent's row;
+ *           bonus token = the argmax at the last accepted row.
+ *   mode 1, speculative sampling (T = 1): the draft tree is a deterministic top-k expansion, so every child
+ *           is a point-mass proposal: it is accepted with probability p_cand / rem, rem = 1 - the target
+ *           probability of the siblings already rejected at that node (decision: uniforms[i] * rem < p_cand[i]
+ *           in fp32); the bonus token is drawn with uniforms[n_out] from p_full at the last accepted row with
+ *           the rejected children's tokens removed. The emitted tokens follow the target's distribution exactly.
+ * Asynchronous on cuda_stream; copy accepted_path / n_acc to the host for dovetail_kv_commit.
+ * Errors: EINVAL (null pointers for the chosen mode, bad mode, gamma < 1, max_depth < 1), ECUDA. */
+int dovetail_verify_accept(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma, int32_t mode,
+                           int32_t max_depth, const dovetail_verify_in_t* in, const dovetail_verify_out_t* res,
+                           void* cuda_stream);
+
 /* Tree bookkeeping alone, for bit-exact checks of the
  * integer path: replays expansion, scoring, frontier selection and the final
  * rerank from caller-supplied per-row top-k lists instead of LM-head results.

@@ -21,4 +21,6 @@ from .oracle import (  # noqa: F401
     step,
     topk,
     tree_replay,
+    verify_accept,
+    verify_plan,
 )

@@ -612,3 +612,111 @@ int dovetail_oracle_kv_commit(const orc_config_t* c, void* kc, void* vc, int32_t
   }
   return moved;
 }
+
+/* ---- verification-side bookkeeping and acceptance ---------------------------
+ * "These candidates are then sent to the target model ... for parallel verification. The target model
+ * computes the logits of the candidate tokens in a single forward pass and applies a speculative sampling
+ * algorithm to determine the accepted tokens. The accepted tokens are returned to the ... draft model."
+ *
+ * Verifier rows: row 0 is the root (the last verified token, whose successor distribution the target has
+ * not computed yet), row i + 1 is candidate i of the draft step's output (pool order: parents precede
+ * children, siblings in rank order). */
+
+/* O10: what the verifier's single forward needs. mask [(n+1) x (n+1)] row-major, mask[r][c] = 1 iff row c is
+ * row r itself or one of its ancestors (the root is everybody's ancestor); position_ids[r] = root_position +
+ * depth(r) (root depth 0); paths [n_paths x (max_depth)] = the candidate indices root -> leaf of every leaf
+ * (a candidate that is nobody's parent), leaves in candidate order, padded with -1. Returns n_paths. */
+int dovetail_oracle_verify_plan(const int32_t* parents, const int32_t* depths, int32_t n, int32_t root_position,
+                                int32_t max_depth, uint8_t* mask, int32_t* position_ids, int32_t* paths) {
+  int R = n + 1;
+  memset(mask, 0, (size_t)R * R);
+  position_ids[0] = root_position;
+  mask[0] = 1;
+  for (int i = 0; i < n; ++i) {
+    int r = i + 1;
+    position_ids[r] = root_position + depths[i];
+    mask[(size_t)r * R + 0] = 1;
+    for (int a = i; a >= 0; a = parents[a]) mask[(size_t)r * R + a + 1] = 1;
+  }
+  int n_paths = 0;
+  for (int i = 0; i < n; ++i) {
+    int is_parent = 0;
+    for (int j = 0; j < n; ++j) if (parents[j] == i) is_parent = 1;
+    if (is_parent) continue;
+    int32_t* row = paths + (size_t)n_paths * max_depth;
+    for (int k = 0; k < max_depth; ++k) row[k] = -1;
+    int len = 0;
+    for (int a = i; a >= 0; a = parents[a]) ++len;
+    int k = len - 1;
+    for (int a = i; a >= 0; a = parents[a]) row[k--] = a;
+    ++n_paths;
+  }
+  return n_paths;
+}
+
+/* O11: the acceptance rule. Walk down from the root; at the current node try its children in candidate order.
+ *   mode 0 (greedy, T = 0): child i is accepted iff token_ids[i] == tgt_argmax[row of the current node].
+ *   mode 1 (speculative sampling, T = 1; reading A18): the draft tree is a deterministic top-k expansion, so each
+ *          child is a point-mass proposal. Child i with target probability p_cand[i] (of its token under the
+ *          target's distribution at its parent) is accepted with probability p_cand[i] / rem, where rem = 1 - the
+ *          target probability of the siblings already rejected at this node, i.e. iff uniforms[i] * rem <
+ *          p_cand[i] (one fp32 multiply, one fp32 compare); on rejection rem -= p_cand[i] (fp32).
+ * The first accepted child becomes the current node; when no child is accepted the walk stops. accepted_path
+ * receives the candidate indices root -> last accepted node, *n_acc their count.
+ * The bonus token (the target's own next token after the last accepted node): mode 0: tgt_argmax of that row;
+ * mode 1: drawn from the target's distribution at that row, p_full[row][*], with the tokens of the children
+ * rejected there removed: weights w(x) = (uint64)(p(x) * 2^32) (exact), W = sum of the kept weights,
+ * r = (uint64)((double)uniforms[n] * (double)W), bonus = the smallest x (kept) whose running sum exceeds r
+ * (integer arithmetic: any summation order gives the same token); -1 if W == 0. */
+int dovetail_oracle_verify_accept(const int32_t* token_ids, const int32_t* parents, int32_t n, int32_t mode,
+                                  const int32_t* tgt_argmax, const float* p_cand, const float* uniforms,
+                                  const float* p_full, int32_t vocab, int32_t* accepted_path, int32_t* n_acc,
+                                  int32_t* bonus_token) {
+  int cur = -1, na = 0;
+  int32_t* rej = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+  int n_rej = 0;
+  for (;;) {
+    float rem = 1.0f;
+    int found = -1;
+    n_rej = 0;
+    for (int i = 0; i < n && found < 0; ++i) {
+      if (parents[i] != cur) continue;
+      if (mode == 0) {
+        if (token_ids[i] == tgt_argmax[cur + 1]) found = i;
+      } else {
+        float lhs = uniforms[i] * rem;
+        if (lhs < p_cand[i]) found = i;
+        else { rem = rem - p_cand[i]; rej[n_rej++] = token_ids[i]; }
+      }
+    }
+    if (found < 0) break;
+    accepted_path[na++] = found;
+    cur = found;
+  }
+  *n_acc = na;
+  if (mode == 0) {
+    *bonus_token = tgt_argmax[cur + 1];
+  } else {
+    const float* p = p_full + (size_t)(cur + 1) * vocab;
+    uint64_t W = 0;
+    for (int x = 0; x < vocab; ++x) {
+      int r = 0;
+      for (int k = 0; k < n_rej; ++k) if (rej[k] == x) r = 1;
+      if (!r) W += (uint64_t)(p[x] * 4294967296.0f);
+    }
+    int tok = -1;
+    if (W > 0) {
+      uint64_t r = (uint64_t)((double)uniforms[n] * (double)W), acc = 0;
+      for (int x = 0; x < vocab && tok < 0; ++x) {
+        int rj = 0;
+        for (int k = 0; k < n_rej; ++k) if (rej[k] == x) rj = 1;
+        if (rj) continue;
+        acc += (uint64_t)(p[x] * 4294967296.0f);
+        if (acc > r) tok = x;
+      }
+    }
+    *bonus_token = tok;
+  }
+  free(rej);
+  return 0;
+}

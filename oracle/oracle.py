@@ -55,6 +55,8 @@ def _load():
         _lib.dovetail_oracle_step.restype = C.c_int
         _lib.dovetail_oracle_tree_replay.restype = C.c_int
         _lib.dovetail_oracle_kv_commit.restype = C.c_int
+        _lib.dovetail_oracle_verify_plan.restype = C.c_int
+        _lib.dovetail_oracle_verify_accept.restype = C.c_int
     return _lib
 
 
@@ -312,3 +314,34 @@ def kv_commit(cfg: OracleConfig, kc: np.ndarray, vc: np.ndarray, capacity: int, 
     return int(_load().dovetail_oracle_kv_commit(C.byref(cc), _ptr(kc), _ptr(vc), C.c_int32(capacity),
                                                  C.c_int32(Lp), _ptr(p), C.c_int32(len(p)),
                                                  C.c_int32(mode)))
+
+
+def verify_plan(parents, depths, root_position: int, max_depth: int) -> dict:
+    """O10: verifier inputs (ancestor mask, position ids, root-to-leaf paths) from a step's output."""
+    parents = np.ascontiguousarray(parents, dtype=np.int32)
+    depths = np.ascontiguousarray(depths, dtype=np.int32)
+    n = len(parents)
+    mask = np.zeros((n + 1, n + 1), np.uint8)
+    pos = np.zeros(n + 1, np.int32)
+    paths = np.full((max(n, 1), max_depth), -1, np.int32)
+    k = _load().dovetail_oracle_verify_plan(_ptr(parents), _ptr(depths), C.c_int32(n), C.c_int32(root_position),
+                                             C.c_int32(max_depth), _ptr(mask), _ptr(pos), _ptr(paths))
+    return dict(mask=mask, position_ids=pos, paths=paths[:k], n_paths=int(k))
+
+
+def verify_accept(token_ids, parents, mode: int, tgt_argmax=None, p_cand=None, uniforms=None, p_full=None) -> dict:
+    """O11: greedy (mode 0) or speculative-sampling (mode 1) acceptance + bonus token."""
+    token_ids = np.ascontiguousarray(token_ids, dtype=np.int32)
+    parents = np.ascontiguousarray(parents, dtype=np.int32)
+    n = len(parents)
+    f32 = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float32)
+    tgt_argmax = None if tgt_argmax is None else np.ascontiguousarray(tgt_argmax, dtype=np.int32)
+    p_cand, uniforms, p_full = f32(p_cand), f32(uniforms), f32(p_full)
+    vocab = 0 if p_full is None else p_full.shape[1]
+    path = np.full(max(n, 1), -1, np.int32)
+    n_acc = np.zeros(1, np.int32)
+    bonus = np.zeros(1, np.int32)
+    _load().dovetail_oracle_verify_accept(_ptr(token_ids), _ptr(parents), C.c_int32(n), C.c_int32(mode), _ptr(tgt_argmax),
+                                           _ptr(p_cand), _ptr(uniforms), _ptr(p_full), C.c_int32(vocab), _ptr(path),
+                                           _ptr(n_acc), _ptr(bonus))
+    return dict(accepted_path=path[:int(n_acc[0])].copy(), n_acc=int(n_acc[0]), bonus_token=int(bonus[0]))

@@ -18,7 +18,7 @@ OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 # include/dovetail.h
 EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "dovetail_tree_replay",
-           "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
+           "dovetail_verify_plan", "dovetail_verify_accept", "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
 HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune")
@@ -63,6 +63,18 @@ class DraftOutT(C.Structure):
                 ("depths", C.c_void_p), ("n_out", C.c_void_p)]
 
 
+class VerifyPlanT(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("mask", "position_ids", "paths", "n_paths")]
+
+
+class VerifyInT(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("tgt_argmax", "p_cand", "uniforms", "p_full")]
+
+
+class VerifyOutT(C.Structure):
+    _fields_ = [(n, C.c_void_p) for n in ("accepted_path", "n_acc", "bonus_token")]
+
+
 HOOK_FIELDS = ("tap_logits", "tap_hhat", "tap_k", "tap_v", "tap_pool_token", "tap_pool_cum",
                "force_hhat", "force_k", "force_v", "force_pool_token", "force_pool_cum")
 
@@ -94,6 +106,12 @@ def load() -> C.CDLL:
         lib.dovetail_tree_replay.restype = C.c_int
         lib.dovetail_tree_replay.argtypes = [C.c_void_p, C.POINTER(TreeSpecT), C.c_void_p, C.c_void_p, C.c_int32,
                                              C.c_int32, C.POINTER(DraftOutT)] + [C.c_void_p] * 6
+        lib.dovetail_verify_plan.restype = C.c_int
+        lib.dovetail_verify_plan.argtypes = [C.c_void_p, C.POINTER(DraftOutT), C.c_int32, C.c_int32, C.c_int32,
+                                             C.POINTER(VerifyPlanT), C.c_void_p]
+        lib.dovetail_verify_accept.restype = C.c_int
+        lib.dovetail_verify_accept.argtypes = [C.c_void_p, C.POINTER(DraftOutT), C.c_int32, C.c_int32, C.c_int32,
+                                               C.POINTER(VerifyInT), C.POINTER(VerifyOutT), C.c_void_p]
         lib.dovetail_hooks_set.restype = C.c_int
         lib.dovetail_hooks_set.argtypes = [C.c_void_p, C.POINTER(HooksT)]
         lib.dovetail_draft_status.restype = C.c_int
@@ -253,6 +271,41 @@ def dovetail_kv_commit(h: Draft, kv: KVCache, accepted_path, mode: int = 0, stre
     rc = load().dovetail_kv_commit(h.ptr, C.byref(kv.c), path, len(accepted_path), mode, C.byref(n), _stream(stream))
     _check(rc, h.ptr)
     return n.value
+
+
+def dovetail_verify_plan(h: Draft, out: Dict, root_position: int, max_depth: int, stream=None) -> Dict:
+    """Verifier inputs from a step's output (include/dovetail.h): device tensors mask [(g+1), (g+1)] uint8,
+    position_ids [g+1], paths [g, max_depth], n_paths [1]. Asynchronous."""
+    import torch
+    g = out["token_ids"].numel()
+    dev = out["token_ids"].device
+    plan = dict(mask=torch.zeros((g + 1, g + 1), dtype=torch.uint8, device=dev),
+                position_ids=torch.zeros(g + 1, dtype=torch.int32, device=dev),
+                paths=torch.zeros((g, max_depth), dtype=torch.int32, device=dev),
+                n_paths=torch.zeros(1, dtype=torch.int32, device=dev))
+    o = _out_t(out)
+    t = VerifyPlanT(_dp(plan["mask"]), _dp(plan["position_ids"]), _dp(plan["paths"]), _dp(plan["n_paths"]))
+    _check(load().dovetail_verify_plan(h.ptr, C.byref(o), g, root_position, max_depth, C.byref(t), _stream(stream)), h.ptr)
+    return plan
+
+
+def dovetail_verify_accept(h: Draft, out: Dict, mode: int, max_depth: int, tgt_argmax=None, p_cand=None, uniforms=None,
+                           p_full=None, stream=None) -> Dict:
+    """Acceptance rule (include/dovetail.h): mode 0 greedy, 1 speculative sampling. Device results, asynchronous."""
+    import torch
+    g = out["token_ids"].numel()
+    dev = out["token_ids"].device
+    for name, t, dt in (("tgt_argmax", tgt_argmax, torch.int32), ("p_cand", p_cand, torch.float32),
+                        ("uniforms", uniforms, torch.float32), ("p_full", p_full, torch.float32)):
+        if t is not None and t.dtype != dt:
+            raise TypeError(f"{name} must be {dt}")
+    res = dict(accepted_path=torch.full((max_depth,), -1, dtype=torch.int32, device=dev),
+               n_acc=torch.zeros(1, dtype=torch.int32, device=dev), bonus_token=torch.zeros(1, dtype=torch.int32, device=dev))
+    o = _out_t(out)
+    i = VerifyInT(_dp(tgt_argmax), _dp(p_cand), _dp(uniforms), _dp(p_full))
+    r = VerifyOutT(_dp(res["accepted_path"]), _dp(res["n_acc"]), _dp(res["bonus_token"]))
+    _check(load().dovetail_verify_accept(h.ptr, C.byref(o), g, mode, max_depth, C.byref(i), C.byref(r), _stream(stream)), h.ptr)
+    return res
 
 
 def dovetail_tree_replay(h: Draft, tree: TreeSpec, cand_tokens, cand_logp, out: Optional[Dict] = None,

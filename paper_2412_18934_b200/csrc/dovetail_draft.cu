@@ -23,6 +23,7 @@
 #include "state.cuh"
 #include "stream_probe.cuh"
 #include "tree.cuh"
+#include "verify.cuh"
 
 using namespace dvt;
 
@@ -1113,6 +1114,61 @@ int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32
   kv->committed_len += h->ts_host->commit_n;
   if (n_committed) *n_committed = h->ts_host->commit_n;
   h->have_step = false;
+  return DOVETAIL_OK;
+}
+
+int dovetail_verify_plan(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma, int32_t root_position,
+                         int32_t max_depth, const dovetail_verify_plan_t* plan, void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (!out || !out->parents || !out->depths || !out->n_out || !plan || !plan->mask || !plan->position_ids || !plan->paths ||
+      !plan->n_paths)
+    return fail(h, DOVETAIL_EINVAL, "null argument (the step's output must include depths)");
+  if (gamma < 1 || gamma > h->pool_cap || max_depth < 1) return fail(h, DOVETAIL_EINVAL, "gamma / max_depth out of range");
+  VerifyPlanParams p{};
+  p.parents = out->parents;
+  p.depths = out->depths;
+  p.n_out = out->n_out;
+  p.gamma = gamma;
+  p.root_position = root_position;
+  p.max_depth = max_depth;
+  p.mask = plan->mask;
+  p.position_ids = plan->position_ids;
+  p.paths = plan->paths;
+  p.n_paths = plan->n_paths;
+  k_verify_plan<<<1, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(p);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "verify_plan launch failed: %s", cudaGetErrorString(e));
+  return DOVETAIL_OK;
+}
+
+int dovetail_verify_accept(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma, int32_t mode, int32_t max_depth,
+                           const dovetail_verify_in_t* in, const dovetail_verify_out_t* res, void* cuda_stream) {
+  if (!h) return DOVETAIL_EINVAL;
+  if (!out || !out->token_ids || !out->parents || !out->n_out || !in || !res || !res->accepted_path || !res->n_acc ||
+      !res->bonus_token)
+    return fail(h, DOVETAIL_EINVAL, "null argument");
+  if (mode != 0 && mode != 1) return fail(h, DOVETAIL_EINVAL, "mode must be 0 (greedy) or 1 (speculative sampling)");
+  if (mode == 0 && !in->tgt_argmax) return fail(h, DOVETAIL_EINVAL, "greedy acceptance needs tgt_argmax");
+  if (mode == 1 && (!in->p_cand || !in->uniforms || !in->p_full)) return fail(h, DOVETAIL_EINVAL, "sampling needs p_cand, uniforms, p_full");
+  if (gamma < 1 || gamma > h->pool_cap || max_depth < 1) return fail(h, DOVETAIL_EINVAL, "gamma / max_depth out of range");
+  VerifyAcceptParams p{};
+  p.token_ids = out->token_ids;
+  p.parents = out->parents;
+  p.n_out = out->n_out;
+  p.gamma = gamma;
+  p.mode = mode;
+  p.vocab = h->cfg.vocab;
+  p.tgt_argmax = in->tgt_argmax;
+  p.p_cand = in->p_cand;
+  p.uniforms = in->uniforms;
+  p.p_full = in->p_full;
+  p.accepted_path = res->accepted_path;
+  p.n_acc = res->n_acc;
+  p.bonus_token = res->bonus_token;
+  p.max_depth = max_depth;
+  k_verify_accept<<<1, kVerifyThreads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(p);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "verify_accept launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
 }
 
