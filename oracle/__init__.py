@@ -16,6 +16,7 @@ from .oracle import (  # noqa: F401
     lm_head,
     log_softmax,
     matvec,
+    matvec_q8,
     rmsnorm,
     rope,
     step,

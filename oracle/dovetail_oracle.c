@@ -33,10 +33,12 @@ typedef struct {
   double rope_theta, rms_eps;
   int32_t dtype, dgf_proj, first_layer_input_norm, final_norm;
   int32_t fusion; /* 0: Dynamic Gating Fusion (the paper's); 1: concat + one Linear (the EAGLE-2 baseline, "w/o both") */
+  int32_t wquant; /* 0: matrices stored in dtype; 1: int8 with one fp32 scale per output row */
 } orc_config_t;
 
 typedef struct {
   const void *g_attn, *wq, *wk, *wv, *wo, *g_ffn, *wgate, *wup, *wdown;
+  const float *sq, *sk, *sv, *so, *sgate, *sup, *sdown; /* wquant: per-row scales of the seven matrices */
 } orc_layer_t;
 
 typedef struct {
@@ -44,6 +46,7 @@ typedef struct {
   const orc_layer_t* layers;
   const void* g_final;
   const void* lm_head;
+  const float *dgf_s1, *dgf_s2, *dgf_sg, *lm_head_s; /* wquant: per-row scales */
 } orc_weights_t;
 
 /* ---- stored-value access ------------------------------------------------ */
@@ -86,6 +89,23 @@ static void st(void* p, size_t i, int dtype, double x) {
 
 /* ---- primitive steps (exported so the tests can pin each one) ----------- */
 
+/* int8 weight-quantised draft (App. C.2: "it is advisable to apply int8 quantization to the drafting
+ * model on the GPU"): a matrix is stored as int8 q[N,K] with one fp32 scale per output row; its value is the
+ * dequantised W[n,k] = scale[n] * q[n,k] (exact in double), and everything else is the same fp64 arithmetic.
+ * y[n] = sum_k (scale[n] * q[n,k]) x[k]. */
+void orc_matvec_q8(const int8_t* Q, const float* scale, int N, int K, const double* x, double* y) {
+#pragma omp parallel for schedule(static)
+  for (int n = 0; n < N; ++n) {
+    double s = 0.0, sc = (double)scale[n];
+    size_t base = (size_t)n * (size_t)K;
+    for (int k = 0; k < K; ++k) s += (sc * (double)Q[base + k]) * x[k];
+    y[n] = s;
+  }
+}
+
+/* A weight matrix of the model: stored in dtype, or (scale != NULL) int8 with per-row scales. */
+static void mat(const void* W, const float* scale, int dtype, int N, int K, const double* x, double* y);
+
 /* y[n] = sum_k W[n,k] x[k], W row-major [N,K]. */
 void orc_matvec(const void* W, int dtype, int N, int K, const double* x, double* y) {
 #pragma omp parallel for schedule(static)
@@ -95,6 +115,11 @@ void orc_matvec(const void* W, int dtype, int N, int K, const double* x, double*
     for (int k = 0; k < K; ++k) s += ld(W, base + k, dtype) * x[k];
     y[n] = s;
   }
+}
+
+static void mat(const void* W, const float* scale, int dtype, int N, int K, const double* x, double* y) {
+  if (scale) orc_matvec_q8((const int8_t*)W, scale, N, K, x, y);
+  else orc_matvec(W, dtype, N, K, x, y);
 }
 
 /* RMSNorm: y = x / sqrt(mean(x^2) + eps) * g   (LLaMA block, reading A3). */
@@ -132,12 +157,12 @@ void orc_dgf(const orc_config_t* c, const orc_weights_t* w, const double* f, int
   double* z = (double*)malloc(sizeof(double) * d);
   for (int i = 0; i < d; ++i) e[i] = ld(w->embed, (size_t)token * d + i, dt);
   if (c->dgf_proj) {
-    orc_matvec(w->dgf_w1, dt, d, d, f, h);
-    orc_matvec(w->dgf_w2, dt, d, d, e, h + d);
+    mat(w->dgf_w1, c->wquant ? w->dgf_s1 : NULL, dt, d, d, f, h);
+    mat(w->dgf_w2, c->wquant ? w->dgf_s2 : NULL, dt, d, d, e, h + d);
   } else {
     for (int i = 0; i < d; ++i) { h[i] = f[i]; h[d + i] = e[i]; }
   }
-  orc_matvec(w->dgf_wg, dt, d, 2 * d, h, z);
+  mat(w->dgf_wg, c->wquant ? w->dgf_sg : NULL, dt, d, 2 * d, h, z);
   for (int i = 0; i < d; ++i) {
     double g = sigmoid(z[i] + ld(w->dgf_bg, i, dt));
     x[i] = g * h[i] + (1.0 - g) * h[d + i];
@@ -153,7 +178,7 @@ void orc_fusion_linear(const orc_config_t* c, const orc_weights_t* w, const doub
   int d = c->hidden, dt = c->dtype;
   double* h = (double*)malloc(sizeof(double) * 2 * d);
   for (int i = 0; i < d; ++i) { h[i] = f[i]; h[d + i] = ld(w->embed, (size_t)token * d + i, dt); }
-  orc_matvec(w->dgf_wg, dt, d, 2 * d, h, x);
+  mat(w->dgf_wg, c->wquant ? w->dgf_sg : NULL, dt, d, 2 * d, h, x);
   for (int i = 0; i < d; ++i) x[i] += ld(w->dgf_bg, i, dt);
   free(h);
 }
@@ -259,9 +284,9 @@ static void forward_rows(const orc_config_t* c, const orc_weights_t* w, void* kc
       double* xr = x + (size_t)r * d;
       if (l == 0 && !c->first_layer_input_norm) memcpy(n, xr, sizeof(double) * d);
       else orc_rmsnorm(xr, L->g_attn, dt, d, c->rms_eps, n);
-      orc_matvec(L->wq, dt, dq, d, n, q + (size_t)r * dq);
-      orc_matvec(L->wk, dt, dkv, d, n, k);
-      orc_matvec(L->wv, dt, dkv, d, n, v);
+      mat(L->wq, c->wquant ? L->sq : NULL, dt, dq, d, n, q + (size_t)r * dq);
+      mat(L->wk, c->wquant ? L->sk : NULL, dt, dkv, d, n, k);
+      mat(L->wv, c->wquant ? L->sv : NULL, dt, dkv, d, n, v);
       for (int h = 0; h < Hq; ++h) orc_rope(q + (size_t)r * dq + h * dh, dh, rows[r].pos, c->rope_theta);
       for (int h = 0; h < Hkv; ++h) orc_rope(k + h * dh, dh, rows[r].pos, c->rope_theta);
       for (int h = 0; h < Hkv; ++h) {
@@ -276,13 +301,13 @@ static void forward_rows(const orc_config_t* c, const orc_weights_t* w, void* kc
       double* xr = x + (size_t)r * d;
       orc_attention_row(c, kc, vc, capacity, l, q + (size_t)r * dq, rows[r].allowed,
                         rows[r].n_allowed, o);
-      orc_matvec(L->wo, dt, d, dq, o, t);
+      mat(L->wo, c->wquant ? L->so : NULL, dt, d, dq, o, t);
       for (int i = 0; i < d; ++i) xr[i] += t[i];
       orc_rmsnorm(xr, L->g_ffn, dt, d, c->rms_eps, n);
-      orc_matvec(L->wgate, dt, F, d, n, ga);
-      orc_matvec(L->wup, dt, F, d, n, up);
+      mat(L->wgate, c->wquant ? L->sgate : NULL, dt, F, d, n, ga);
+      mat(L->wup, c->wquant ? L->sup : NULL, dt, F, d, n, up);
       for (int i = 0; i < F; ++i) ga[i] = silu(ga[i]) * up[i];
-      orc_matvec(L->wdown, dt, d, F, ga, t);
+      mat(L->wdown, c->wquant ? L->sdown : NULL, dt, d, F, ga, t);
       for (int i = 0; i < d; ++i) xr[i] += t[i];
     }
   }
@@ -296,10 +321,10 @@ void orc_lm_head(const orc_config_t* c, const orc_weights_t* w, const double* hh
   if (c->final_norm) {
     double* n = (double*)malloc(sizeof(double) * d);
     orc_rmsnorm(hhat, w->g_final, c->dtype, d, c->rms_eps, n);
-    orc_matvec(w->lm_head, c->dtype, c->vocab, d, n, logits);
+    mat(w->lm_head, c->wquant ? w->lm_head_s : NULL, c->dtype, c->vocab, d, n, logits);
     free(n);
   } else {
-    orc_matvec(w->lm_head, c->dtype, c->vocab, d, hhat, logits);
+    mat(w->lm_head, c->wquant ? w->lm_head_s : NULL, c->dtype, c->vocab, d, hhat, logits);
   }
 }
 

@@ -34,17 +34,22 @@ class _Cfg(C.Structure):
     _fields_ = [(n, C.c_int32) for n in
                 ("hidden", "n_q_heads", "n_kv_heads", "head_dim", "n_layers", "ffn", "vocab")] + \
                [("rope_theta", C.c_double), ("rms_eps", C.c_double)] + \
-               [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm", "fusion")]
+               [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm", "fusion", "wquant")]
+
+
+SCALE_KEYS = ("sq", "sk", "sv", "so", "sgate", "sup", "sdown")
+TOP_SCALE_KEYS = ("dgf_s1", "dgf_s2", "dgf_sg", "lm_head_s")
 
 
 class _Layer(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in
-                ("g_attn", "wq", "wk", "wv", "wo", "g_ffn", "wgate", "wup", "wdown")]
+                ("g_attn", "wq", "wk", "wv", "wo", "g_ffn", "wgate", "wup", "wdown") + SCALE_KEYS]
 
 
 class _Weights(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("embed", "dgf_w1", "dgf_w2", "dgf_wg", "dgf_bg")] + \
-               [("layers", C.POINTER(_Layer)), ("g_final", C.c_void_p), ("lm_head", C.c_void_p)]
+               [("layers", C.POINTER(_Layer)), ("g_final", C.c_void_p), ("lm_head", C.c_void_p)] + \
+               [(n, C.c_void_p) for n in TOP_SCALE_KEYS]
 
 
 def _load():
@@ -76,11 +81,12 @@ class OracleConfig:
     first_layer_input_norm: int = 1
     final_norm: int = 0
     fusion: int = 0  # 0 DGF; 1 concat + Linear, the EAGLE-2 baseline
+    wquant: int = 0  # 1: matrices are int8 with one fp32 scale per output row
 
     def c(self) -> _Cfg:
         return _Cfg(self.hidden, self.n_q_heads, self.n_kv_heads, self.head_dim, self.n_layers,
                     self.ffn, self.vocab, float(self.rope_theta), float(self.rms_eps), self.dtype,
-                    self.dgf_proj, self.first_layer_input_norm, self.final_norm, self.fusion)
+                    self.dgf_proj, self.first_layer_input_norm, self.final_norm, self.fusion, self.wquant)
 
 
 def _np(a):
@@ -117,12 +123,12 @@ class OracleWeights:
     _keep: list = field(default_factory=list)
 
     def c(self) -> _Weights:
-        top = {k: _np(self.top.get(k)) for k in TOP_KEYS}
-        lay = [{k: _np(l[k]) for k in LAYER_KEYS} for l in self.layers]
-        arr = (_Layer * len(lay))(*[_Layer(*[_ptr(l[k]) for k in LAYER_KEYS]) for l in lay])
+        top = {k: _np(self.top.get(k)) for k in TOP_KEYS + TOP_SCALE_KEYS}
+        lay = [{k: _np(l.get(k)) for k in LAYER_KEYS + SCALE_KEYS} for l in self.layers]
+        arr = (_Layer * len(lay))(*[_Layer(*[_ptr(l[k]) for k in LAYER_KEYS + SCALE_KEYS]) for l in lay])
         w = _Weights(_ptr(top["embed"]), _ptr(top["dgf_w1"]), _ptr(top["dgf_w2"]),
                      _ptr(top["dgf_wg"]), _ptr(top["dgf_bg"]), arr, _ptr(top["g_final"]),
-                     _ptr(top["lm_head"]))
+                     _ptr(top["lm_head"]), *[_ptr(top[k]) for k in TOP_SCALE_KEYS])
         self._keep = [top, lay, arr]
         return w
 
@@ -142,6 +148,17 @@ def matvec(W, dtype: int, x: np.ndarray) -> np.ndarray:
     assert x.shape == (K,)
     y = np.empty(N, dtype=np.float64)
     _load().orc_matvec(_ptr(W), C.c_int(dtype), C.c_int(N), C.c_int(K), _ptr(x), _ptr(y))
+    return y
+
+
+def matvec_q8(Q, scale, x: np.ndarray) -> np.ndarray:
+    """int8 matrix with one fp32 scale per output row: y = (scale[:, None] * Q) @ x in fp64."""
+    Q = np.ascontiguousarray(_np(Q), dtype=np.int8)
+    scale = np.ascontiguousarray(_np(scale), dtype=np.float32)
+    N, K = Q.shape
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty(N, dtype=np.float64)
+    _load().orc_matvec_q8(_ptr(Q), _ptr(scale), C.c_int(N), C.c_int(K), _ptr(x), _ptr(y))
     return y
 
 

@@ -49,6 +49,8 @@ class DraftConfig:
     first_layer_input_norm: int = 1
     final_norm: int = 0
     fusion: int = 0           # 0: DGF; 1: concat + one Linear 2d -> d, the EAGLE-2 baseline
+    wquant: int = 0           # 1: weight matrices are int8 with one fp32 scale per output row; the
+                              #    embedding, norm gains, gate bias and KV cache stay in dtype (bf16)
     prefix: int = 64          # committed KV length L of the workload
     feat_scale: float = 1.0   # features ~ N(0,1) * feat_scale
     tree: TreeSpec = field(default_factory=lambda: TreeSpec(1, (1,), (0,), 1))
@@ -81,6 +83,13 @@ class DraftConfig:
         byte once + the prefix K/V of every layer once."""
         p = self.weight_params()
         w = (p["dgf"] + p["layers"] + p["final_norm"] + p["lm_head"]) * self.esize
+        if self.wquant:  # matrices at 1 byte per element + 4 bytes of scale per output row; vectors in dtype
+            d, F = self.hidden, self.ffn
+            dq, dkv = self.n_q_heads * self.head_dim, self.n_kv_heads * self.head_dim
+            vec = d + 2 * d * self.n_layers + p["final_norm"]
+            mats = p["dgf"] + p["layers"] + p["final_norm"] + p["lm_head"] - vec
+            rows = (2 * d if (self.dgf_proj and self.fusion == 0) else 0) + d + self.n_layers * (dq + 2 * dkv + d + 2 * F + d) + self.vocab
+            w = mats + 4 * rows + vec * self.esize
         kv = self.n_layers * 2 * prefix_len * self.n_kv_heads * self.head_dim * self.esize
         return w + kv
 

@@ -50,7 +50,38 @@ def make_weights(cfg: DraftConfig, device="cpu", seed=None) -> Tuple[Dict[str, t
             g_ffn=torch.ones(d, device=device, dtype=dt),
             wgate=r(F, d), wup=r(F, d), wdown=r(d, F),
         ))
+    if cfg.wquant:
+        top, layers = quantize_weights(top, layers)
     return top, layers
+
+
+MATRIX_SCALES = {"wq": "sq", "wk": "sk", "wv": "sv", "wo": "so", "wgate": "sgate", "wup": "sup", "wdown": "sdown"}
+TOP_MATRIX_SCALES = {"dgf_w1": "dgf_s1", "dgf_w2": "dgf_s2", "dgf_wg": "dgf_sg", "lm_head": "lm_head_s"}
+
+
+def quantize_rows(w: torch.Tensor):
+    """Symmetric int8 with one scale per output row: scale = max|row| / 127 (rounded to a bf16-representable fp32 so
+    that scale * q is exact in fp32 too), q = round-to-nearest-even(w / scale) clipped to [-127, 127]. Input
+    preparation for the weight-quantised workload; not part of the method's arithmetic."""
+    wf = w.float()
+    scale = (wf.abs().amax(dim=1).clamp_min(1e-12) / 127.0).to(torch.bfloat16).float()
+    q = torch.clamp(torch.round(wf / scale[:, None]), -127, 127).to(torch.int8).contiguous()
+    return q, scale.contiguous()
+
+
+def quantize_weights(top: Dict, layers: List[Dict]):
+    """int8 version of a weight set: matrices -> (int8, scale); embedding, gains, bias untouched."""
+    top = dict(top)
+    for k, sk in TOP_MATRIX_SCALES.items():
+        if top.get(k) is not None:
+            top[k], top[sk] = quantize_rows(top[k])
+    out = []
+    for l in layers:
+        l = dict(l)
+        for k, sk in MATRIX_SCALES.items():
+            l[k], l[sk] = quantize_rows(l[k])
+        out.append(l)
+    return top, out
 
 
 def make_kv(cfg: DraftConfig, capacity: int, prefix: int, device="cpu", seed=None):

@@ -23,7 +23,7 @@ def tiny_cfg(**kw) -> DraftConfig:
 def ocfg(cfg: DraftConfig) -> oracle.OracleConfig:
     return oracle.OracleConfig(cfg.hidden, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.n_layers,
                                cfg.ffn, cfg.vocab, cfg.rope_theta, cfg.rms_eps, cfg.dtype, cfg.dgf_proj,
-                               cfg.first_layer_input_norm, cfg.final_norm, cfg.fusion)
+                               cfg.first_layer_input_norm, cfg.final_norm, cfg.fusion, cfg.wquant)
 
 
 def oweights(top, layers) -> oracle.OracleWeights:
