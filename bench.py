@@ -157,11 +157,13 @@ def _to_host(case):
 
 
 def all_configs():
-    from paper_2412_18934_b200.configs import CONFIGS, c4_sweep, depth_sweep
+    from paper_2412_18934_b200.configs import CONFIGS, c4_sweep, depth_sweep, int8_variants
     cfgs = {c.name: c for c in CONFIGS.values()}
     cfgs.update({k: v for k, v in CONFIGS.items()})
     cfgs.update({c.name: c for c in c4_sweep()})
     cfgs.update({c.name: c for c in depth_sweep()})
+    cfgs.update({c.name: c for c in int8_variants()})
+    cfgs.update({c.name.split("_")[0] + "_int8": c for c in int8_variants()})  # c2_int8, c3_int8, c5_int8
     return cfgs
 
 
@@ -369,7 +371,8 @@ def bench_one(a, cfg, rank, world, local, dist):
     e2e_val = world * tree.gamma * K / (ms_e2e * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "bf16 weights and KV cache, f32 activations and accumulation" if cfg.dtype == 1 else "f32",
+            "dtype": ("int8 weights (per-row scales), bf16 KV cache, f32 activations and accumulation" if cfg.wquant else
+                      "bf16 weights and KV cache, f32 activations and accumulation") if cfg.dtype == 1 else "f32",
             "data": "synthetic", "config": workload(cfg, a.n_new, world),
             "draft_step_us": step_ms * 1e3, "draft_step_us_replays": dist_us,
             "forward_us": step_ms * 1e3 / tree.depth, "forward_us_per_level": per_level,
@@ -460,7 +463,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfgs = all_configs()
     if a.config == "all":
-        names = ["c1", "c2", "c5"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
+        names = ["c1", "c2", "c5", "c2_int8", "c3_int8", "c5_int8"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
     else:
         names = [a.config]
     for i, name in enumerate(names):

@@ -83,6 +83,11 @@ typedef struct {
   int32_t max_tree_slots; /* largest sum over tree levels of forwarded rows (<= 128) */
   int32_t max_branch;   /* largest branch[] a step may use (<= 32)                   */
   int32_t fusion;       /* dovetail_fusion_t: how the feature and the embedding are fused */
+  int32_t weight_quant; /* 0: matrices stored in dtype. 1: every weight MATRIX (DGF, blocks, LM head) is int8, row-major
+                           [out, in], with one fp32 scale per output row: W[n,k] = scale[n] * q[n,k] ("it is advisable
+                           to apply int8 quantization to the drafting model on the GPU"). Needs dtype =
+                           BF16 (embedding, norm gains, gate bias, KV cache stay bf16) and every inner dimension a
+                           multiple of 32. */
 } dovetail_config_t;
 
 /* Device pointers to one decoder layer's weights. */
@@ -96,6 +101,14 @@ typedef struct {
   const void* wgate;  /* [F, d]                                 */
   const void* wup;    /* [F, d]                                 */
   const void* wdown;  /* [d, F]                                 */
+  /* weight_quant == 1: fp32 per-row scales of the seven matrices, [out] each; ignored otherwise */
+  const float* sq;
+  const float* sk;
+  const float* sv;
+  const float* so;
+  const float* sgate;
+  const float* sup;
+  const float* sdown;
 } dovetail_layer_weights_t;
 
 /* Device pointers to all weights. BORROWED: the caller keeps them alive and
@@ -110,6 +123,11 @@ typedef struct {
   const dovetail_layer_weights_t* layers; /* host array [n_layers]       */
   const void* g_final; /* [d] or NULL (required iff final_norm)          */
   const void* lm_head; /* [V, d]                                         */
+  /* weight_quant == 1: fp32 per-row scales of dgf_w1, dgf_w2, dgf_wg, lm_head; ignored otherwise */
+  const float* dgf_s1;
+  const float* dgf_s2;
+  const float* dgf_sg;
+  const float* lm_head_s;
 } dovetail_weights_t;
 
 /* Draft KV cache, caller-owned device memory.

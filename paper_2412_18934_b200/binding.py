@@ -34,19 +34,22 @@ class ConfigT(C.Structure):
     _fields_ = [(n, C.c_int32) for n in ("hidden", "n_q_heads", "n_kv_heads", "head_dim", "n_layers", "ffn", "vocab")] + \
                [("rope_theta", C.c_float), ("rms_eps", C.c_float)] + \
                [(n, C.c_int32) for n in ("dtype", "dgf_proj", "first_layer_input_norm", "final_norm",
-                                         "max_rows", "max_tree_slots", "max_branch", "fusion")]
+                                         "max_rows", "max_tree_slots", "max_branch", "fusion", "weight_quant")]
 
 
 LAYER_KEYS = ("g_attn", "wq", "wk", "wv", "wo", "g_ffn", "wgate", "wup", "wdown")
+LAYER_SCALE_KEYS = ("sq", "sk", "sv", "so", "sgate", "sup", "sdown")
+TOP_SCALE_KEYS = ("dgf_s1", "dgf_s2", "dgf_sg", "lm_head_s")
 
 
 class LayerWeightsT(C.Structure):
-    _fields_ = [(n, C.c_void_p) for n in LAYER_KEYS]
+    _fields_ = [(n, C.c_void_p) for n in LAYER_KEYS + LAYER_SCALE_KEYS]
 
 
 class WeightsT(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in ("embed", "dgf_w1", "dgf_w2", "dgf_wg", "dgf_bg")] + \
-               [("layers", C.POINTER(LayerWeightsT)), ("g_final", C.c_void_p), ("lm_head", C.c_void_p)]
+               [("layers", C.POINTER(LayerWeightsT)), ("g_final", C.c_void_p), ("lm_head", C.c_void_p)] + \
+               [(n, C.c_void_p) for n in TOP_SCALE_KEYS]
 
 
 class KVCacheT(C.Structure):
@@ -140,7 +143,7 @@ def load() -> C.CDLL:
 def config_t(cfg: DraftConfig, max_rows: int = 64, max_tree_slots: int = 128, max_branch: int = 32) -> ConfigT:
     return ConfigT(cfg.hidden, cfg.n_q_heads, cfg.n_kv_heads, cfg.head_dim, cfg.n_layers, cfg.ffn, cfg.vocab,
                    float(cfg.rope_theta), float(cfg.rms_eps), cfg.dtype, cfg.dgf_proj,
-                   cfg.first_layer_input_norm, cfg.final_norm, max_rows, max_tree_slots, max_branch, cfg.fusion)
+                   cfg.first_layer_input_norm, cfg.final_norm, max_rows, max_tree_slots, max_branch, cfg.fusion, cfg.wquant)
 
 
 def tree_spec_t(tree: TreeSpec) -> TreeSpecT:
@@ -216,9 +219,16 @@ def dovetail_draft_init(top: Dict, layers: List[Dict], cfg: DraftConfig, max_row
                         max_tree_slots: int = 128, max_branch: int = 32) -> Draft:
     """top / layers: device tensors as produced by synth.make_weights(cfg, device='cuda')."""
     lib = load()
-    arr = (LayerWeightsT * len(layers))(*[LayerWeightsT(*[_dp(l[k]) for k in LAYER_KEYS]) for l in layers])
+    import torch
+    if cfg.wquant:  # the ABI takes raw pointers: check what it will reinterpret
+        for d_, keys in [(top, ("dgf_wg", "lm_head"))] + [(l, ("wq", "wk", "wv", "wo", "wgate", "wup", "wdown")) for l in layers]:
+            for k in keys:
+                if d_[k].dtype != torch.int8:
+                    raise TypeError(f"weight_quant = 1: {k} must be int8, got {d_[k].dtype}")
+    arr = (LayerWeightsT * len(layers))(*[LayerWeightsT(*[_dp(l.get(k)) for k in LAYER_KEYS + LAYER_SCALE_KEYS]) for l in layers])
     w = WeightsT(_dp(top["embed"]), _dp(top.get("dgf_w1")), _dp(top.get("dgf_w2")), _dp(top["dgf_wg"]),
-                 _dp(top["dgf_bg"]), arr, _dp(top.get("g_final")), _dp(top["lm_head"]))
+                 _dp(top["dgf_bg"]), arr, _dp(top.get("g_final")), _dp(top["lm_head"]),
+                 *[_dp(top.get(k)) for k in TOP_SCALE_KEYS])
     c = config_t(cfg, max_rows, max_tree_slots, max_branch)
     out = C.c_void_p()
     rc = lib.dovetail_draft_init(C.byref(w), C.byref(c), C.byref(out))

@@ -145,6 +145,12 @@ def depth_sweep() -> List[DraftConfig]:
     return out
 
 
+def int8_variants() -> List[DraftConfig]:
+    """the 7B / 13B / Llama-3-8B shaped workloads with int8 weight matrices and per-row scales
+    ("it is advisable to apply int8 quantization to the drafting model on the GPU", PAPER.md:414)."""
+    return [replace(c, name=c.name + "_int8", wquant=1) for c in (_C2, _C3, _C5)]
+
+
 def paper_preset(server: bool = True) -> TreeSpec:
     """width 10 / depth 7 / 16 candidates (servers); 10 / 4 / 7 (PC)."""
     D, g = (7, 16) if server else (4, 7)

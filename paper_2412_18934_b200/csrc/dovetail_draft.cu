@@ -50,6 +50,8 @@ struct dovetail_draft {
   dovetail_weights_t w;
   std::vector<dovetail_layer_weights_t> layers;
   int num_sms = 0, es = 2;
+  int wq = 0;  // 1: int8 weight matrices with per-row scales (cfg.weight_quant)
+  __nv_bfloat16* xs_emb = nullptr;  // int8: embedding rows of the level, as a (permuted) plane [1][rows][ld_d]
   int dq = 0, dkv = 0, ldq = 0;
   int max_step_rows = 0, pool_cap = 0, attn_chunks_cap = 1, qv_cap = 1;
   // device scratch (owned)
@@ -184,11 +186,17 @@ GemvKernel pick_gemv(int MT, int NI) {
   return k_gemv<WT, 2, 7>;
 }
 
-ChainKernel pick_gemv_mma(int NT) {
-  if (NT == 1) return k_gemv_mma<1, 4>;
-  if (NT == 2) return k_gemv_mma<2, 4>;
-  if (NT == 4) return k_gemv_mma<4, 4>;
-  return k_gemv_mma<8, 2>;
+ChainKernel pick_gemv_mma(int NT, int wq) {
+  if (wq) {
+    if (NT == 1) return k_gemv_mma<1, 4, 1>;
+    if (NT == 2) return k_gemv_mma<2, 4, 1>;
+    if (NT == 4) return k_gemv_mma<4, 4, 1>;
+    return k_gemv_mma<8, 2, 1>;
+  }
+  if (NT == 1) return k_gemv_mma<1, 4, 0>;
+  if (NT == 2) return k_gemv_mma<2, 4, 0>;
+  if (NT == 4) return k_gemv_mma<4, 4, 0>;
+  return k_gemv_mma<8, 2, 0>;
 }
 
 using AttnKernel = void (*)(const AttnParams);
@@ -212,7 +220,8 @@ cudaError_t set_max_smem_all() {
     cudaError_t r = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
     if (r != cudaSuccess) e = r;
   };
-  for (int nt = 1; nt <= 8; nt *= 2) set(reinterpret_cast<const void*>(pick_gemv_mma(nt)));
+  for (int nt = 1; nt <= 8; nt *= 2)
+    for (int wq = 0; wq < 2; ++wq) set(reinterpret_cast<const void*>(pick_gemv_mma(nt, wq)));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<64>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<128>));
   const int mts[3] = {1, 2, 4};
@@ -260,8 +269,8 @@ int div_up(int a, int b) { return (a + b - 1) / b; }
 
 // Geometry of one persistent launch of the tensor-core GEMV kernel (gemv_mma.cuh) over a chain of GEMVs.
 struct ChainGeom {
-  int NT, RBMAX, RS, stage_bytes, n_stages, part_floats, smem;
-  int S[kMaxChain], KC[kMaxChain], seg_stride[kMaxChain], RSp[kMaxChain];  // per phase
+  int NT, RBMAX, RS, stage_bytes, n_stages, part_floats, res_floats, smem;
+  int S[kMaxChain], KC[kMaxChain], seg_stride[kMaxChain], aseg_stride[kMaxChain], RSp[kMaxChain];  // per phase
   bool ok;
 };
 
@@ -271,8 +280,10 @@ int nt_for(int cols) {
   return r;
 }
 
-ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n) {
+// wq: int8 weights (one byte per element in the A part of a stage)
+ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n, int wq) {
   ChainGeom s{};
+  const int aes = wq ? 1 : 2;
   s.ok = n >= 1 && n <= kMaxChain;
   int max_cnt = 1, nt = 1, res_floats = 0;
   for (int i = 0; s.ok && i < n; ++i) {
@@ -281,6 +292,7 @@ ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n) {
     if (!s.ok) break;
     const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
     s.S[i] = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
+    if (q[i].p.g[0].S_fixed) s.S[i] = std::max(s.S[i], q[i].p.g[0].S_fixed);
     nt = std::max(nt, nt2);
     max_cnt = std::max(max_cnt, q[i].max_cnt);
     res_floats = std::max(res_floats, q[i].max_cnt * M);
@@ -294,7 +306,7 @@ ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n) {
   const int rs_max = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
   ChainGeom best{};
   for (int rs = rs_max; rs >= 16; rs -= 16) {
-    for (int kc0 : {512, 256, 128}) {
+    for (int kc0 : {wq ? 1024 : 512, wq ? 512 : 256, wq ? 256 : 128}) {
       ChainGeom c = s;
       c.RS = rs;
       c.stage_bytes = 0;
@@ -305,22 +317,25 @@ ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n) {
         const int ncols = q[i].p.M * s.S[i], PC = (ncols + 1) & ~1;
         c.KC[i] = std::min(kc0, (q[i].p.K + 63) / 64 * 64);
         c.seg_stride[i] = c.KC[i] * 2 + 16;
-        c.stage_bytes = std::max(c.stage_bytes, (rows_eff(i) + ncols) * c.seg_stride[i]);
+        c.aseg_stride[i] = c.KC[i] * aes + 16;
+        c.stage_bytes = std::max(c.stage_bytes, rows_eff(i) * c.aseg_stride[i] + ncols * c.seg_stride[i]);
         c.part_floats = std::max(c.part_floats, kConsumerWarps * rs * PC);
       }
       // phases with few rows per CTA (O, down: 35 of 64) take longer K-chunks so that their stages are full too
       for (int i = 0; i < n; ++i) {
         const int ncols = q[i].p.M * s.S[i];
-        while (c.KC[i] < 2048 && c.KC[i] * 2 <= (q[i].p.K + 63) / 64 * 64 &&
-               (rows_eff(i) + ncols) * (c.KC[i] * 4 + 16) <= c.stage_bytes + 4096) {
+        while (c.KC[i] < 2048 * (wq ? 2 : 1) && c.KC[i] * 2 <= (q[i].p.K + 63) / 64 * 64 &&
+               rows_eff(i) * (c.KC[i] * 2 * aes + 16) + ncols * (c.KC[i] * 4 + 16) <= c.stage_bytes + 4096) {
           c.KC[i] *= 2;
           c.seg_stride[i] = c.KC[i] * 2 + 16;
+          c.aseg_stride[i] = c.KC[i] * aes + 16;
         }
-        c.stage_bytes = std::max(c.stage_bytes, (rows_eff(i) + ncols) * c.seg_stride[i]);
+        c.stage_bytes = std::max(c.stage_bytes, rows_eff(i) * c.aseg_stride[i] + ncols * c.seg_stride[i]);
         c.RSp[i] = rows_eff(i);
       }
       if (c.part_floats * 4 > 32768 && rs > 16) continue;
-      int fixed = 3 * 64 + 16 + 2 * 4 * kMmaMaxM + c.part_floats * 4 + res_floats * 4;
+      c.res_floats = res_floats;
+      int fixed = 3 * 64 + 16 + 2 * 4 * kMmaMaxM + c.part_floats * 4 + res_floats * 4 + (wq ? max_cnt * 4 : 0);
       fixed = (fixed + 15) / 16 * 16;
       c.n_stages = std::min(8, (kSmemMax - fixed - 64) / c.stage_bytes);
       c.smem = c.n_stages * c.stage_bytes + fixed;
@@ -358,6 +373,7 @@ int run_chain(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv* q,
   cp.stage_bytes = g.stage_bytes;
   cp.n_stages = g.n_stages;
   cp.part_floats = g.part_floats;
+  cp.res_floats = g.res_floats;
   if (n > 1) {
     if (h->bar_used + n > kMaxBars) return fail(h, DOVETAIL_EINVAL, "too many GEMV phases in one step");
     cp.bar = h->bar + h->bar_used;
@@ -369,10 +385,12 @@ int run_chain(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv* q,
     p.n_groups = q[i].n_groups;
     p.ctas_per_group = q[i].ctas;
     p.rows_per_stage = g.RSp[i];
-    p.row_bytes = p.K * 2;
+    p.row_bytes = p.K * (h->wq ? 1 : 2);
     p.kc = g.KC[i];
     p.seg_stride = g.seg_stride[i];
-    for (int gi = 0; gi < q[i].n_groups; ++gi) p.g[gi].S = p.g[gi].xkind == X_EMBED ? 1 : g.S[i];
+    p.aseg_stride = g.aseg_stride[i];
+    for (int gi = 0; gi < q[i].n_groups; ++gi)
+      p.g[gi].S = p.g[gi].xkind == X_EMBED ? 1 : (p.g[gi].S_fixed ? p.g[gi].S_fixed : g.S[i]);
     h->cur_kind = q[i].kind;
     h->cur_bytes = q[i].bytes;
     p.trace = trace_slot(h);
@@ -385,7 +403,7 @@ int run_chain(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv* q,
     if (h->dbg_launch < 64) cp.dbg = h->dbg + static_cast<size_t>(h->dbg_launch++) * 148 * kMaxChain * 8;
   }
 #endif
-  cudaError_t e = launch(h, pick_gemv_mma(g.NT), dim3(grid), dim3(kMmaThreads), g.smem, st, cp);
+  cudaError_t e = launch(h, pick_gemv_mma(g.NT, h->wq), dim3(grid), dim3(kMmaThreads), g.smem, st, cp);
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
 }
@@ -397,7 +415,7 @@ int flush_gemv(dovetail_draft* h, cudaStream_t st) {
   int rc = DOVETAIL_OK;
   size_t i = 0;
   while (i < Q.size() && rc == DOVETAIL_OK) {
-    const bool mma_ok = h->es == 2 && chain_geom(&Q[i], 1).ok;
+    const bool mma_ok = h->es == 2 && chain_geom(&Q[i], 1, h->wq).ok;
     if (!mma_ok) {
       if (h->es == 2 && Q[i].p.M > kMmaMaxM && Q[i].p.K % 32 == 0) {
         // a level wider than 32 rows: chunks of <= 32 rows (64 B columns), the weights are streamed once per chunk
@@ -407,9 +425,11 @@ int flush_gemv(dovetail_draft* h, cudaStream_t st) {
           c.p.M = std::min(kMmaMaxM, Mtot - m0);
           c.p.m0 = m0;
           if (m0 > 0) c.bytes = 0;  // the algorithmic bytes are counted once
-          const ChainGeom g = chain_geom(&c, 1);
+          const ChainGeom g = chain_geom(&c, 1, h->wq);
           rc = g.ok ? run_chain(h, st, &c, 1, g) : fail(h, DOVETAIL_EINVAL, "GEMV with K = %d does not fit the tensor-core kernel", c.p.K);
         }
+      } else if (h->wq) {
+        rc = fail(h, DOVETAIL_EINVAL, "int8 weights: GEMV with K = %d, M = %d does not fit the tensor-core kernel", Q[i].p.K, Q[i].p.M);
       } else {
         rc = run_gemv_fma(h, st, Q[i]);
       }
@@ -417,9 +437,9 @@ int flush_gemv(dovetail_draft* h, cudaStream_t st) {
       continue;
     }
     int n = 1;  // grow the chain while the geometry stays valid
-    ChainGeom g = chain_geom(&Q[i], 1);
+    ChainGeom g = chain_geom(&Q[i], 1, h->wq);
     while (n < h->chain_max && i + n < Q.size()) {
-      const ChainGeom g2 = chain_geom(&Q[i], n + 1);
+      const ChainGeom g2 = chain_geom(&Q[i], n + 1, h->wq);
       if (!g2.ok || g2.n_stages * g2.stage_bytes < 100 * 1024) break;
       g = g2;
       ++n;
@@ -440,13 +460,15 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
   q.kind = kind;
   for (int g = 0; g < n_groups; ++g) {
     const GemvGroup& G = p.g[g];
-    for (int j = 0; j < G.n_mat; ++j) q.bytes += static_cast<int64_t>(G.rows[j]) * p.K * h->es;
+    for (int j = 0; j < G.n_mat; ++j)
+      q.bytes += h->wq ? static_cast<int64_t>(G.rows[j]) * (p.K + 4) : static_cast<int64_t>(G.rows[j]) * p.K * h->es;
     int mc;
     if (G.paired) mc = G.n_mat * div_up(G.rows[0], ctas_per_group);
     else {
       long tot = 0;
       for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
-      mc = static_cast<int>((tot + ctas_per_group - 1) / ctas_per_group);
+      const long unit = G.pairperm ? 2 : 1;  // rotary pairs are dealt whole (gemv.cuh cta_rows)
+      mc = static_cast<int>(unit * ((tot / unit + ctas_per_group - 1) / ctas_per_group));
     }
     q.max_cnt = std::max(q.max_cnt, mc);
   }
@@ -468,12 +490,13 @@ GemvGroup rows_group(const float* xsrc, int64_t xld, const int32_t* xidx, int fr
 }
 
 // split-bf16 planes of an activation buffer with `rows` rows of stride ld (epilogue.cuh), first row row0
-SplitOut planes(__nv_bfloat16* xs, int64_t rows, int64_t ld, int64_t row0 = 0) {
+SplitOut planes(const dovetail_draft* h, __nv_bfloat16* xs, int64_t rows, int64_t ld, int64_t row0 = 0) {
   SplitOut o{};
   if (xs) {
     o.xs = xs + row0 * ld;
     o.plane = rows * ld;
     o.ld = ld;
+    o.perm = h->wq;  // int8 weights: the planes are stored in the consumer's k order (epilogue.cuh split_pos)
   }
   return o;
 }
@@ -532,6 +555,7 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->ssq);
   cudaFree(h->bar);
   cudaFree(h->qs);
+  cudaFree(h->xs_emb);
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
@@ -553,7 +577,7 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
   if (k.force_hhat && e == cudaSuccess) {
     e = cudaMemcpyAsync(h->hhat + xoff, k.force_hhat + xoff, xbytes, cudaMemcpyDeviceToDevice, st);
     if (h->xs_hhat && e == cudaSuccess) {  // the children read the forced rows as split-bf16 planes
-      k_resplit_rows<<<M, 256, 0, st>>>(h->hhat + xoff, d, planes(h->xs_hhat, h->max_step_rows, h->ld_d, lp.row0));
+      k_resplit_rows<<<M, 256, 0, st>>>(h->hhat + xoff, d, planes(h, h->xs_hhat, h->max_step_rows, h->ld_d, lp.row0));
       e = cudaGetLastError();
     }
   }
@@ -625,7 +649,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   const int64_t R = c.max_rows, SR = h->max_step_rows;
   const int nct_d = std::min(nsm, d);  // CTAs of the GEMVs that produce the residual stream (and its sums of squares)
   e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(512), 0, st, dv, h->dyn, h->ts, h->rt,
-               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h->xs_feat, R, h->ld_d), h->bar, kMaxBars,
+               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h, h->xs_feat, R, h->ld_d), h->bar, kMaxBars,
                trace_slot(h));
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
 
@@ -638,11 +662,21 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
     float* x = h->hhat + static_cast<size_t>(lp.row0) * d;  // residual stream rows of this level
 
     // S0 + S1: gather, DGF projections h1 = W1 f, h2 = W2 e
+    if (c.dgf_proj && h->wq) {  // int8 weights: the level's embedding rows as a plane in the consumer's k order
+      rc = flush_gemv(h, st);
+      if (rc) return rc;
+      h->cur_kind = 10;
+      h->cur_bytes = 0;
+      e = launch(h, k_embed_plane, dim3(M), dim3(640), 0, st, static_cast<const RowTables*>(cur),
+                 static_cast<const __nv_bfloat16*>(h->w.embed), d, planes(h, h->xs_emb, R, h->ld_d), trace_slot(h));
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+    }
     if (c.dgf_proj) {
       GemvParams p{};
       p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
-      with_planes(p.g[0], l == 0 ? planes(h->xs_feat, R, h->ld_d) : planes(h->xs_hhat, SR, h->ld_d));
+      with_planes(p.g[0], l == 0 ? planes(h, h->xs_feat, R, h->ld_d) : planes(h, h->xs_hhat, SR, h->ld_d));
       p.g[0].w[0] = h->w.dgf_w1;
+      p.g[0].ws[0] = h->w.dgf_s1;
       p.g[0].rows[0] = d;
       p.g[0].n_mat = 1;
       p.g[0].out_off = 0;
@@ -651,7 +685,13 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       p.g[1].embed = h->w.embed;
       p.g[1].tokens = cur->token;
       p.g[1].w[0] = h->w.dgf_w2;
+      p.g[1].ws[0] = h->w.dgf_s2;
       p.g[1].rows[0] = d;
+      if (h->wq) {  // int8 consumer: the embedding rows come as a plane in its k order (k_embed_plane below)
+        p.g[1].xkind = X_ROWS;
+        with_planes(p.g[1], planes(h, h->xs_emb, R, h->ld_d));
+        p.g[1].S_fixed = 2;  // bf16 value = two fp16 terms exactly
+      }
       p.g[1].n_mat = 1;
       p.g[1].out_off = d;
       p.K = d;
@@ -659,7 +699,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       p.epi = EPI_STORE;
       p.out = h->hbuf;
       p.out_ld = 2 * d;
-      p.so = planes(h->xs_h12, R, h->ld_2d);
+      p.so = planes(h, h->xs_h12, R, h->ld_2d);
       rc = run_gemv(h, st, p, 2, std::max(1, std::min(nsm / 2, d)), 1);
       if (rc) return rc;
     } else {
@@ -671,7 +711,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       if (bf16)
         e = launch(h, k_fill_h<__nv_bfloat16>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
                    static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
-                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d, planes(h->xs_h12, R, h->ld_2d), trace_slot(h));
+                   static_cast<const __nv_bfloat16*>(h->w.embed), h->hbuf, M, d, planes(h, h->xs_h12, R, h->ld_2d), trace_slot(h));
       else
         e = launch(h, k_fill_h<float>, dim3(blocks), dim3(256), 0, st, static_cast<const StepDyn*>(h->dyn), l == 0 ? 1 : 0,
                    static_cast<const float*>(h->hhat), static_cast<int64_t>(d), static_cast<const RowTables*>(cur), l == 0 ? 0 : 1,
@@ -681,8 +721,9 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
     {  // S1: gate, sigmoid, blend; or the single Linear of the EAGLE-2 fusion (:104)
       GemvParams p{};
       p.g[0] = rows_group(h->hbuf, 2 * d, nullptr, 0, nullptr);
-      with_planes(p.g[0], planes(h->xs_h12, R, h->ld_2d));
+      with_planes(p.g[0], planes(h, h->xs_h12, R, h->ld_2d));
       p.g[0].w[0] = h->w.dgf_wg;
+      p.g[0].ws[0] = h->w.dgf_sg;
       p.g[0].rows[0] = d;
       p.g[0].n_mat = 1;
       p.K = 2 * d;
@@ -694,7 +735,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       p.bias = h->w.dgf_bg;
       p.d = d;
       // x feeds the first block's QKV: planes of x * g_attn (raw x when the first input norm is skipped)
-      p.so = planes(h->xs_x, R, h->ld_d);
+      p.so = planes(h, h->xs_x, R, h->ld_d);
       p.gain_out = c.first_layer_input_norm ? h->layers[0].g_attn : nullptr;
       p.ssq_out = h->ssq;
       rc = run_gemv(h, st, p, 1, nct_d, 2);
@@ -707,12 +748,12 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         GemvParams p{};
         const void* gain = (ly == 0 && !c.first_layer_input_norm) ? nullptr : W.g_attn;
         p.g[0] = rows_group(x, d, nullptr, 0, gain);
-        with_planes(p.g[0], planes(h->xs_x, R, h->ld_d));
+        with_planes(p.g[0], planes(h, h->xs_x, R, h->ld_d));
         p.ssq_in = gain ? h->ssq : nullptr;
         p.ssq_nct = nct_d;
-        p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq;
-        p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv;
-        p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv;
+        p.g[0].w[0] = W.wq; p.g[0].rows[0] = dq; p.g[0].ws[0] = W.sq;
+        p.g[0].w[1] = W.wk; p.g[0].rows[1] = dkv; p.g[0].ws[1] = W.sk;
+        p.g[0].w[2] = W.wv; p.g[0].rows[2] = dkv; p.g[0].ws[2] = W.sv;
         p.g[0].n_mat = 3;
         p.K = d;
         p.M = M;
@@ -762,7 +803,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         h->cur_kind = 4;
         h->cur_bytes = static_cast<int64_t>(2) * Lbase * dkv * h->es;
         a.trace = trace_slot(h);
-        a.so = planes(h->xs_o, R, h->ld_dq);
+        a.so = planes(h, h->xs_o, R, h->ld_dq);
         a.qs = fused_s2 ? h->qs : nullptr;
         if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
           a.kc = kv->k;
@@ -798,14 +839,14 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       {  // S4: x += Wo o
         GemvParams p{};
         p.g[0] = rows_group(h->obuf, dq, nullptr, 0, nullptr);
-        with_planes(p.g[0], planes(h->xs_o, R, h->ld_dq));
-        p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        with_planes(p.g[0], planes(h, h->xs_o, R, h->ld_dq));
+        p.g[0].w[0] = W.wo; p.g[0].rows[0] = d; p.g[0].n_mat = 1; p.g[0].ws[0] = W.so;
         p.K = dq;
         p.M = M;
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
-        p.so = planes(h->xs_x, R, h->ld_d);  // feeds gate / up through the post-attention norm
+        p.so = planes(h, h->xs_x, R, h->ld_d);  // feeds gate / up through the post-attention norm
         p.gain_out = W.g_ffn;
         p.ssq_out = h->ssq;
         rc = run_gemv(h, st, p, 1, nct_d, 5);
@@ -814,11 +855,11 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       {  // S5a: act = SiLU(Wgate n) * (Wup n), n = RMSNorm(x)
         GemvParams p{};
         p.g[0] = rows_group(x, d, nullptr, 0, W.g_ffn);
-        with_planes(p.g[0], planes(h->xs_x, R, h->ld_d));
+        with_planes(p.g[0], planes(h, h->xs_x, R, h->ld_d));
         p.ssq_in = h->ssq;
         p.ssq_nct = nct_d;
-        p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F;
-        p.g[0].w[1] = W.wup; p.g[0].rows[1] = F;
+        p.g[0].w[0] = W.wgate; p.g[0].rows[0] = F; p.g[0].ws[0] = W.sgate;
+        p.g[0].w[1] = W.wup; p.g[0].rows[1] = F; p.g[0].ws[1] = W.sup;
         p.g[0].n_mat = 2;
         p.g[0].paired = 1;
         p.K = d;
@@ -827,29 +868,29 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         p.epi = EPI_SWIGLU;
         p.out = h->act;
         p.out_ld = F;
-        p.so = planes(h->xs_act, R, h->ld_f);
+        p.so = planes(h, h->xs_act, R, h->ld_f);
         rc = run_gemv(h, st, p, 1, std::min(nsm, F), 6);
         if (rc) return rc;
       }
       {  // S5b: x += Wdown act
         GemvParams p{};
         p.g[0] = rows_group(h->act, F, nullptr, 0, nullptr);
-        with_planes(p.g[0], planes(h->xs_act, R, h->ld_f));
-        p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1;
+        with_planes(p.g[0], planes(h, h->xs_act, R, h->ld_f));
+        p.g[0].w[0] = W.wdown; p.g[0].rows[0] = d; p.g[0].n_mat = 1; p.g[0].ws[0] = W.sdown;
         p.K = F;
         p.M = M;
         p.epi = EPI_RESID;
         p.out = x;
         p.out_ld = d;
         if (ly + 1 < c.n_layers) {  // feeds the next block's QKV through its input norm
-          p.so = planes(h->xs_x, R, h->ld_d);
+          p.so = planes(h, h->xs_x, R, h->ld_d);
           p.gain_out = h->layers[ly + 1].g_attn;
           p.ssq_out = h->ssq;
         } else {
           // the block stack's output: feature of this row's children (raw) and input of the LM head
-          p.so_raw = planes(h->xs_hhat, SR, h->ld_d, lp.row0);
+          p.so_raw = planes(h, h->xs_hhat, SR, h->ld_d, lp.row0);
           if (c.final_norm) {
-            p.so = planes(h->xs_x, R, h->ld_d);
+            p.so = planes(h, h->xs_x, R, h->ld_d);
             p.gain_out = h->w.g_final;
             p.ssq_out = h->ssq;
           }
@@ -865,12 +906,12 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
       p.g[0] = rows_group(xs, d, nullptr, 0, c.final_norm ? h->w.g_final : nullptr);
       const int lm_row = l == 0 ? n_new - 1 : 0;  // first row of the level whose list is expanded
-      with_planes(p.g[0], c.final_norm ? planes(h->xs_x, R, h->ld_d, lm_row) : planes(h->xs_hhat, SR, h->ld_d, lp.row0 + lm_row));
+      with_planes(p.g[0], c.final_norm ? planes(h, h->xs_x, R, h->ld_d, lm_row) : planes(h, h->xs_hhat, SR, h->ld_d, lp.row0 + lm_row));
       if (c.final_norm) {
         p.ssq_in = h->ssq + lm_row;
         p.ssq_nct = nct_d;
       }
-      p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1;
+      p.g[0].w[0] = h->w.lm_head; p.g[0].rows[0] = V; p.g[0].n_mat = 1; p.g[0].ws[0] = h->w.lm_head_s;
       p.K = d;
       p.M = lp.rows_lm;
       p.eps = c.rms_eps;
@@ -952,6 +993,18 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   for (int K : Ks)
     if (!gemv_shape(K, es, 1, 1).ok)
       return fail(nullptr, DOVETAIL_EINVAL, "dimension %d not supported: rows must be a multiple of 16 bytes and at most 28672 bytes", K);
+  if (c.weight_quant != 0 && c.weight_quant != 1) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant must be 0 or 1");
+  if (c.weight_quant) {
+    if (c.dtype != DOVETAIL_BF16) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1 needs dtype = BF16");
+    for (int K : Ks)
+      if (K % 32 != 0) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1: dimension %d is not a multiple of 32", K);
+    bool ok = w->dgf_sg && w->lm_head_s && (!c.dgf_proj || (w->dgf_s1 && w->dgf_s2));
+    for (int l = 0; ok && w->layers && l < c.n_layers; ++l) {
+      const dovetail_layer_weights_t& L = w->layers[l];
+      ok = L.sq && L.sk && L.sv && L.so && L.sgate && L.sup && L.sdown;
+    }
+    if (!ok) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1: missing scale pointer");
+  }
   if (!w->embed || !w->dgf_wg || !w->dgf_bg || !w->layers || !w->lm_head ||
       (c.dgf_proj && (!w->dgf_w1 || !w->dgf_w2)) || (c.final_norm && !w->g_final))
     return fail(nullptr, DOVETAIL_EINVAL, "missing weight pointer");
@@ -976,6 +1029,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   h->w.layers = h->layers.data();
   h->num_sms = prop.multiProcessorCount;
   h->es = es;
+  h->wq = c.weight_quant;
   h->dq = dq;
   h->dkv = dkv;
   h->ldq = dq + 2 * dkv;
@@ -1010,6 +1064,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
     A(dmalloc(&h->bar, kMaxBars));
     A(dmalloc(&h->qs, static_cast<size_t>(2) * kMaxRows * dq));
+    if (c.weight_quant) A(dmalloc(&h->xs_emb, kSplitPlanes * R * h->ld_d));
   }
   A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));
@@ -1349,6 +1404,11 @@ int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
   params += static_cast<int64_t>(c.n_layers) * (d * dq + 2 * d * dkv + dq * d + 3 * d * F + 2 * d);
   params += static_cast<int64_t>(c.vocab) * d + (c.final_norm ? d : 0);
   const int64_t kvb = static_cast<int64_t>(c.n_layers) * 2 * prefix_len * dkv;
+  if (h->wq) {  // matrices: one byte per element + one fp32 scale per output row; vectors and K/V in bf16
+    const int64_t vec = d + static_cast<int64_t>(c.n_layers) * 2 * d + (c.final_norm ? d : 0);
+    const int64_t rows = (c.dgf_proj ? 2 * d : 0) + d + static_cast<int64_t>(c.n_layers) * (dq + 2 * dkv + d + 2 * F + d) + c.vocab;
+    return (params - vec) + 4 * rows + (vec + kvb) * h->es;
+  }
   return (params + kvb) * h->es;
 }
 

@@ -11,6 +11,7 @@
 // of all CTAs in CTA order and scales its results by 1 / rms (pre-norm LLaMA block).
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include "ptx.cuh"
 #include "state.cuh"
@@ -23,14 +24,43 @@ struct SplitOut {
   __nv_bfloat16* xs;  // [kSplitPlanes][rows][ld] or NULL: nothing to leave
   int64_t plane;      // elements between planes
   int64_t ld;         // elements between rows (>= K of the consumer, multiple of 8)
+  int32_t perm;       // 1: int8 weights -- the terms are fp16 with rescaled remainders (store_split; the int8 consumer
+                      // multiplies in fp16) and, within every aligned block of 32 k, stored in the order the
+                      // consumer's fragments need (split_pos); 0: bf16 terms in natural order
 };
 
+// int8 weights (gemv_mma.cuh, WQ = 1): one ldmatrix gives a thread the weights k = 4t .. 4t + 3 and 16 + 4t .. 16 +
+// 4t + 3 of a 32-block (t = lane & 3), i.e. the pairs (4t, 4t+1), (16+4t, ..) for the first mma and (4t+2, 4t+3),
+// (18+4t, ..) for the second. The activation planes are stored so that a plain ldmatrix of B delivers exactly
+// those pairs: k = 16a + 4t + 2b + e  ->  position 8(a + 2b) + 2t + e.
+__device__ __forceinline__ int64_t split_pos(int64_t col, int perm) {
+  if (!perm) return col;
+  const int k = static_cast<int>(col & 31);
+  const int a = k >> 4, t = (k >> 2) & 3, b = (k >> 1) & 1, e = k & 1;
+  return (col & ~static_cast<int64_t>(31)) + 8 * (a + 2 * b) + 2 * t + e;
+}
+
 __device__ __forceinline__ void store_split(const SplitOut& o, int64_t row, int64_t col, float x) {
+  if (o.perm) {
+    // fp16 terms with rescaled remainders: x = h0 + 2^-11 h1 + 2^-22 h2, h1 = fp16((x - h0) 2^11), h2 likewise, so
+    // that the remainders sit in fp16's normal range whatever the magnitude of x (a plain x - h0 of a small x is
+    // subnormal: measured 9x the error on features of magnitude 1e-2). The consumer applies the powers of two when
+    // it adds the terms' dot products. Needs |x| < 65504.
+    const __half h0 = __float2half_rn(x);
+    const float r1 = (x - __half2float(h0)) * 2048.0f;
+    const __half h1 = __float2half_rn(r1);
+    const __half h2 = __float2half_rn((r1 - __half2float(h1)) * 2048.0f);
+    __half* dst = reinterpret_cast<__half*>(o.xs) + row * o.ld + split_pos(col, 1);
+    dst[0] = h0;
+    dst[o.plane] = h1;
+    dst[2 * o.plane] = h2;
+    return;
+  }
   const uint16_t h0 = f32_to_bf16_rn(x);
   const float r1 = x - __uint_as_float(static_cast<uint32_t>(h0) << 16);
   const uint16_t h1 = f32_to_bf16_rn(r1);
   const float r2 = r1 - __uint_as_float(static_cast<uint32_t>(h1) << 16);
-  uint16_t* dst = reinterpret_cast<uint16_t*>(o.xs) + row * o.ld + col;
+  uint16_t* dst = reinterpret_cast<uint16_t*>(o.xs) + row * o.ld + split_pos(col, o.perm);
   dst[0] = h0;
   dst[o.plane] = h1;
   dst[2 * o.plane] = f32_to_bf16_rn(r2);

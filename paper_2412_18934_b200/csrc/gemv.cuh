@@ -33,6 +33,7 @@ constexpr int kRowsPerStageMax = 4;
 
 struct GemvGroup {
   const void* w[3];      // up to three matrices sharing K and X
+  const float* ws[3];    // int8 matrices (k_gemv_mma, WQ = 1): fp32 scale of every output row of w[j]
   int32_t rows[3];
   int32_t n_mat;
   int32_t paired;        // 1: the CTA's row range applies to each matrix (gate/up)
@@ -53,6 +54,7 @@ struct GemvGroup {
   const __nv_bfloat16* xs;
   int64_t xs_plane, xs_ld;
   int32_t S;             // planes read per draft row: 3 (all 24 mantissa bits), 2 (16 bits), 1 (bf16 source)
+  int32_t S_fixed;       // != 0: S is this (1: the planes hold bf16 values, e.g. embedding rows), else chosen by M
 };
 
 struct GemvParams {
@@ -63,6 +65,7 @@ struct GemvParams {
   int32_t rows_per_stage, n_stages, stage_bytes, row_bytes;
   // k_gemv_mma only: K-chunk per stage, stride of a row / column within a stage (bytes)
   int32_t kc, seg_stride;
+  int32_t aseg_stride;   // stride of a weight row within a stage (int8 weights: half of the bf16 stride)
   int32_t m0;            // k_gemv_mma: first draft row of this launch (levels wider than 32 rows run in row chunks)
   int32_t epi;
   float eps;

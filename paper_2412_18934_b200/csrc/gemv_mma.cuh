@@ -92,6 +92,7 @@ struct ChainParams {
   int32_t n;
   int32_t stage_bytes, n_stages;  // ring geometry, common to the phases
   int32_t part_floats;            // floats of the partial buffer (largest phase)
+  int32_t res_floats;             // floats of the result buffer (largest phase)
   int32_t* bar;                   // [n] phase counters, zeroed at the start of the step
   unsigned long long* dbg;        // DVT_CHAINDBG builds only
 };
@@ -110,9 +111,34 @@ __device__ __forceinline__ int chain_cta(const GemvParams& p, int c, int& g) {
   return c - g * p.ctas_per_group;
 }
 
-// NT: 8-column tiles of B (columns = M * S <= 8 * NT); RBMAX: 16-row blocks per stage.
-template <int NT, int RBMAX>
+// four int8 (one 32-bit word, k ascending from the low byte) -> two fp16x2 words, exact: byte ^ 0x80 under the
+// exponent byte 0x64 is the half 1024 + (q + 128); subtracting 1152 leaves q. Five instructions per four weights
+// (the fp32 / bf16 route needs eleven, which made the int8 consumer instruction-bound: measured).
+__device__ __forceinline__ void cvt_i8x4_f16x2(uint32_t r, uint32_t& lo, uint32_t& hi) {
+  const uint32_t x = r ^ 0x80808080u;
+  const uint32_t bias = 0x64806480u;  // (1152.0h, 1152.0h)
+  uint32_t l = __byte_perm(x, 0x64646464u, 0x4140), h = __byte_perm(x, 0x64646464u, 0x4342);
+  asm("sub.f16x2 %0, %0, %1;" : "+r"(l) : "r"(bias));
+  asm("sub.f16x2 %0, %0, %1;" : "+r"(h) : "r"(bias));
+  lo = l;
+  hi = h;
+}
+
+__device__ __forceinline__ void mma_f16_16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+      "{%0, %1, %2, %3};"
+      : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// NT: 8-column tiles of B (columns = M * S <= 8 * NT); RBMAX: 16-row blocks per stage; WQ: 1 = int8 weights with
+// one fp32 scale per output row: half the bytes per weight, converted to fp16 in registers (exact),
+// multiplied with fp16 activation terms (products exact in fp32), the scale applied to the row's result; the
+// activation planes are stored in the matching k order (epilogue.cuh split_pos).
+template <int NT, int RBMAX, int WQ>
 __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_constant__ ChainParams cp) {
+  constexpr int AES = WQ ? 1 : 2;  // bytes per weight
   extern __shared__ __align__(128) uint8_t smem[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int c_grid = blockIdx.x, n_grid = gridDim.x;
@@ -126,6 +152,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
   float* rstd_s = reinterpret_cast<float*>(zero16 + 4);       // [2][32], alternating by phase
   float* part = rstd_s + 2 * kMmaMaxM;                        // [warps][RS][PC]
   float* res = part + cp.part_floats;                         // [cnt][M]
+  float* wsc = res + cp.res_floats;                           // [cnt] row scales (int8 weights)
 
   trace_begin(cp.ph[0].trace);
   if (tid == 0) {
@@ -227,11 +254,11 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
         for (int k0 = 0; k0 < K; k0 += KC) {
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
           if (pw == 0 && lane == 0 && sb == 0 && k0 == 0) DVT_DBG(ph, 7);
-          const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * 2u;
+          const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * AES;
           if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(my_rows) * segb);
           __syncwarp();
           uint8_t* dst = ring + static_cast<size_t>(slot) * cp.stage_bytes + a_off;
-          if (mine) bulk_g2s(dst + static_cast<size_t>(r) * p.seg_stride, src + static_cast<size_t>(k0) * 2, segb, &full_a[slot], pol);
+          if (mine) bulk_g2s(dst + static_cast<size_t>(r) * p.aseg_stride, src + static_cast<size_t>(k0) * AES, segb, &full_a[slot], pol);
           if (++slot == NS) { slot = 0; ++round; }
         }
       }
@@ -281,6 +308,13 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
       const RowRange rr = cta_rows(G, c, p.ctas_per_group);
       EpiRegs pre;
       epi_prefetch(p, G, rr, M, p.m0, true, pre);  // in flight during the streaming loop
+      if (WQ) {  // scale of each of the CTA's rows; read after the barriers of the first meet
+        for (int v = tid; v < rr.cnt; v += kConsumerThreads) {
+          int j, n;
+          locate_row(G, rr, v, j, n);
+          wsc[v] = __ldg(G.ws[j] + n);
+        }
+      }
       int n_sb, rsb;
       super_blocks(rr.cnt, RS, n_sb, rsb);
       const int RS16 = (RS + 15) & ~15;  // rows of the partial buffer: whole 16-row blocks
@@ -298,7 +332,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
         const int rbs = (nr + 15) >> 4;
         uint32_t a_row[RBMAX];  // rows past the super-block's last one were never copied: read the last row instead
 #pragma unroll
-        for (int rb = 0; rb < RBMAX; ++rb) a_row[rb] = static_cast<uint32_t>(min(rb * 16 + a_lrow, nr - 1)) * p.seg_stride;
+        for (int rb = 0; rb < RBMAX; ++rb) a_row[rb] = static_cast<uint32_t>(min(rb * 16 + a_lrow, nr - 1)) * p.aseg_stride;
         float acc[RBMAX][NT][4];
 #pragma unroll
         for (int rb = 0; rb < RBMAX; ++rb)
@@ -321,13 +355,25 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
             for (int rb = 0; rb < RBMAX; ++rb) {
               if (rb < rbs) {
                 uint32_t a0[4], a1[4];
-                const uint32_t aaddr = sbase + a_lane + a_row[rb] + u * 64;
-                ldsm_x4(a0, aaddr);
-                ldsm_x4(a1, aaddr + 32);
+                if (WQ) {  // 16 rows x 32 int8: one ldmatrix, then the exact conversion; pairs as split_pos orders B
+                  uint32_t q[4];
+                  ldsm_x4(q, sbase + a_lane + a_row[rb] + u * 32);
+#pragma unroll
+                  for (int e = 0; e < 4; ++e) cvt_i8x4_f16x2(q[e], a0[e], a1[e]);
+                } else {
+                  const uint32_t aaddr = sbase + a_lane + a_row[rb] + u * 64;
+                  ldsm_x4(a0, aaddr);
+                  ldsm_x4(a1, aaddr + 32);
+                }
 #pragma unroll
                 for (int t = 0; t < NT; ++t) {
-                  mma_bf16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
-                  mma_bf16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
+                  if (WQ) {
+                    mma_f16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
+                    mma_f16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
+                  } else {
+                    mma_bf16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
+                    mma_bf16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
+                  }
                 }
               }
             }
@@ -362,11 +408,16 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
           for (int w = 0; w < kConsumerWarps; ++w) {
             const float* q = part + (static_cast<size_t>(w) * RS16 + r) * PC + m * S;
             float tw = q[0];
-            if (S >= 2) tw += q[1];
-            if (S == 3) tw += q[2];
+            if (WQ) {  // fp16 terms carry 2^-11 and 2^-22 (epilogue.cuh store_split)
+              if (S >= 2) tw += q[1] * 4.8828125e-4f;
+              if (S == 3) tw += q[2] * 2.384185791015625e-7f;
+            } else {
+              if (S >= 2) tw += q[1];
+              if (S == 3) tw += q[2];
+            }
             t += tw;
           }
-          res[static_cast<size_t>(v0 + r) * M + m] = t;
+          res[static_cast<size_t>(v0 + r) * M + m] = WQ ? t * wsc[v0 + r] : t;
         }
         consumer_sync();  // part is reused by the next super-block
       }

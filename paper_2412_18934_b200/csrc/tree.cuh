@@ -75,6 +75,32 @@ __global__ void k_resplit_rows(const float* x, int d, SplitOut so) {
   split_row(so, blockIdx.x, x + static_cast<size_t>(blockIdx.x) * d, d);
 }
 
+// int8 weights: the embedding row of each of the level's tokens as activation planes in the int8 consumer's
+// format (fp16 terms, its k order). grid = M rows.
+__global__ void k_embed_plane(const RowTables* rt, const __nv_bfloat16* embed, int d, SplitOut so, unsigned long long* trace) {
+  pdl_launch_dependents();
+  trace_begin(trace);
+  pdl_wait();
+  const int m = blockIdx.x;
+  const __nv_bfloat16* src = embed + static_cast<size_t>(rt->token[m]) * d;
+  constexpr int B = 8;  // loads of a round are issued before any store
+  for (int k0 = threadIdx.x; k0 < d; k0 += blockDim.x * B) {
+    float v[B];
+#pragma unroll
+    for (int i = 0; i < B; ++i) {
+      const int k = k0 + i * blockDim.x;
+      v[i] = k < d ? __bfloat162float(src[k]) : 0.f;
+    }
+#pragma unroll
+    for (int i = 0; i < B; ++i) {
+      const int k = k0 + i * blockDim.x;
+      if (k < d) store_split(so, m, k, v[i]);
+    }
+  }
+  __syncthreads();
+  trace_end(trace);
+}
+
 // dgf_proj == 0: h1 = f, h2 = e (W1 = W2 = identity). grid-stride over M * 2d.
 template <typename WT>
 __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, int64_t xld,

@@ -44,9 +44,9 @@ def test_no_environment_variables_in_the_library():
 
 def test_struct_layouts_match_header():
     # sizes implied by include/dovetail.h (LP64): 7 int32 + 2 float + 8 int32; 9 pointers; ...
-    assert C.sizeof(binding.ConfigT) == 17 * 4
-    assert C.sizeof(binding.LayerWeightsT) == 9 * 8
-    assert C.sizeof(binding.WeightsT) == 8 * 8
+    assert C.sizeof(binding.ConfigT) == 18 * 4
+    assert C.sizeof(binding.LayerWeightsT) == 16 * 8
+    assert C.sizeof(binding.WeightsT) == 12 * 8
     assert C.sizeof(binding.KVCacheT) == 24
     assert C.sizeof(binding.TreeSpecT) == 4 * (1 + 16 + 16 + 1)
     assert C.sizeof(binding.DraftOutT) == 5 * 8
@@ -71,8 +71,8 @@ def test_no_device_means_error_not_fallback(lib):
     cfg = CONFIGS["c1"]
     c = binding.config_t(cfg)
     dummy = C.c_void_p(16)  # never dereferenced: the device check comes first
-    layers = (binding.LayerWeightsT * cfg.n_layers)(*[binding.LayerWeightsT(*[16] * 9) for _ in range(cfg.n_layers)])
-    w = binding.WeightsT(16, 16, 16, 16, 16, layers, None, 16)
+    layers = (binding.LayerWeightsT * cfg.n_layers)(*[binding.LayerWeightsT(*[16] * 16) for _ in range(cfg.n_layers)])
+    w = binding.WeightsT(16, 16, 16, 16, 16, layers, None, 16, None, None, None, None)
     out = C.c_void_p()
     rc = lib.dovetail_draft_init(C.byref(w), C.byref(c), C.byref(out))
     assert rc == binding.ECUDA and not out.value

@@ -25,7 +25,10 @@ def small_cfg(**kw) -> DraftConfig:
 
 def _boost(case, lm=40.0, emb=20.0):
     """Spread the toy distributions so that the top-k decisions are far from ties."""
-    case.top["lm_head"] = (case.top["lm_head"].float() * lm).to(case.top["lm_head"].dtype)
+    if case.top["lm_head"].dtype == torch.int8:  # int8 weights: the per-row scales carry the magnitude
+        case.top["lm_head_s"] = case.top["lm_head_s"] * lm
+    else:
+        case.top["lm_head"] = (case.top["lm_head"].float() * lm).to(case.top["lm_head"].dtype)
     case.top["embed"] = (case.top["embed"].float() * emb).to(case.top["embed"].dtype)
     return case
 
@@ -132,6 +135,47 @@ def test_depth_sweep_ends(name):
     case = make_case(cfg, n_new=1)
     s, gpu, ora = _run(case, tight=True)
     assert gpu["n_out"] == 16
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "fusion_linear", "n_new5", "wide", "very_wide", "max_branch",
+                                     "n_new33"])
+def test_step_parity_small_int8(variant):
+    """int8 weight matrices with per-row scales against the oracle on the dequantised
+    values; the same shapes as the bf16 cases (inner dimensions multiples of 32)."""
+    kw, n_new = dict(dtype=BF16, wquant=1, ffn=352), 1
+    if variant == "mha_dh128":
+        kw.update(hidden=256, n_q_heads=2, n_kv_heads=2, head_dim=128)
+    elif variant == "mqa":
+        kw.update(n_q_heads=4, n_kv_heads=1)
+    elif variant == "no_proj":
+        kw.update(dgf_proj=0)
+    elif variant == "fusion_linear":
+        kw.update(dgf_proj=0, fusion=1)
+    elif variant == "n_new5":
+        n_new = 5
+    elif variant == "wide":
+        kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    elif variant == "very_wide":
+        kw.update(tree=TreeSpec(2, (20, 2), (0, 20), 24))
+    elif variant == "max_branch":
+        kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    elif variant == "n_new33":
+        n_new = 33
+    case = _boost(make_case(small_cfg(**kw), n_new=n_new))
+    s, gpu, ora = _run(case)
+    assert s["same_tree"]
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("name", ["c2_llama2_7b_int8", "c3_llama2_13b_int8", "c5_llama3_8b_int8"])
+def test_full_size_configs_int8(name):
+    """The 7B / 13B / Llama-3-8B shaped workloads with int8 weights at full size."""
+    from paper_2412_18934_b200.configs import int8_variants
+    cfg = [c for c in int8_variants() if c.name == name][0]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case, tight=True)
+    assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
     assert s["free"]["same_tree"] or s["free"]["tie"] is not None
 
 
