@@ -216,8 +216,9 @@ def bench_one(a, cfg, rank, world, local, dist):
 
     case = make_case(cfg, n_new=a.n_new, device="cuda")
     h = binding.dovetail_draft_init(case.top, case.layers, cfg)
-    if a.chain:
-        binding.dovetail_hooks_tune(h, 0, a.chain)
+    for kv_ in a.tune:
+        k_, v_ = kv_.split("=")
+        binding.dovetail_hooks_tune(h, int(k_), int(v_))
     kv = binding.KVCache(case.k, case.v, case.L)
     out = binding.alloc_out(tree.gamma)
     stream = torch.cuda.current_stream()
@@ -427,7 +428,8 @@ def main():
     ap.add_argument("--n-new", type=int, default=1)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--replays", type=int, default=200)
-    ap.add_argument("--chain", type=int, default=0, help="A/B knob: GEMVs per persistent launch (0: library default)")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="A/B knob of include/dovetail_hooks.h dovetail_hooks_tune (repeatable)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-trace", action="store_true")
     ap.add_argument("--no-both-dgf", dest="both_dgf", action="store_false")

@@ -73,10 +73,9 @@ int dovetail_trace_enable(dovetail_draft_t* h, int32_t enable);
 int dovetail_trace_read(dovetail_draft_t* h, int32_t cap, int32_t* kind, int32_t* level, int64_t* bytes,
                         uint64_t* t0_ns, uint64_t* t1_ns, int32_t* n);
 
-/* Design knobs for A/B measurements (bench.py --chain). They change how the step is launched, never what it
- * computes.
- *   key 0: GEMVs per persistent launch, 1 ... 4. 1 (default) = every GEMV is its own kernel launch.
- * Errors: EINVAL. */
+/* Design knobs for A/B measurements (bench.py --tune KEY=VALUE). They change how the step is launched, never
+ * what it computes. Keys are listed here as they are added; an unknown key or a value out of range returns
+ * EINVAL. */
 int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
 
 /* Read-only HBM streaming ceilings, run by bench.py next to the step: reads `bytes`

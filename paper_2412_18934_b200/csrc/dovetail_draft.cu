@@ -84,12 +84,9 @@ struct dovetail_draft {
   int last_launches = 0;
   int launches = 0;
   bool dry = false;  // shape-checking pass of dovetail_draft_step: nothing is launched
-  // GEMVs queued for one persistent launch (gemv_mma.cuh ChainParams)
+  // GEMVs queued by run_gemv, launched by flush_gemv
   struct QueuedGemv { GemvParams p; int n_groups, ctas, kind, max_cnt; int64_t bytes; };
   std::vector<QueuedGemv> queue;
-  int chain_max = 1;           // GEMVs per persistent launch (1: every GEMV is its own launch; measured best)
-  int32_t* bar = nullptr;      // phase counters of the step's chains, zeroed by k_step_begin
-  int bar_used = 0;
 #ifdef DVT_CHAINDBG
   unsigned long long* dbg = nullptr;
   int dbg_launch = 0;
@@ -172,8 +169,7 @@ cudaError_t launch(dovetail_draft* h, void (*kern)(KArgs...), dim3 grid, dim3 bl
 }
 
 using GemvKernel = void (*)(const GemvParams);
-using ChainKernel = void (*)(const ChainParams);
-constexpr int kMaxBars = 2048;
+using MmaKernel = void (*)(const MmaParams);
 
 template <typename WT>
 GemvKernel pick_gemv(int MT, int NI) {
@@ -186,7 +182,7 @@ GemvKernel pick_gemv(int MT, int NI) {
   return k_gemv<WT, 2, 7>;
 }
 
-ChainKernel pick_gemv_mma(int NT, int wq) {
+MmaKernel pick_gemv_mma(int NT, int wq) {
   if (wq) {
     if (NT == 1) return k_gemv_mma<1, 4, 1>;
     if (NT == 2) return k_gemv_mma<2, 4, 1>;
@@ -267,10 +263,10 @@ GemvShape gemv_shape(int K, int es, int M, int res_rows) {
 
 int div_up(int a, int b) { return (a + b - 1) / b; }
 
-// Geometry of one persistent launch of the tensor-core GEMV kernel (gemv_mma.cuh) over a chain of GEMVs.
-struct ChainGeom {
+// Geometry of one launch of the tensor-core GEMV kernel (gemv_mma.cuh).
+struct MmaGeom {
   int NT, RBMAX, RS, stage_bytes, n_stages, part_floats, res_floats, smem;
-  int S[kMaxChain], KC[kMaxChain], seg_stride[kMaxChain], aseg_stride[kMaxChain], RSp[kMaxChain];  // per phase
+  int S, KC, seg_stride, aseg_stride, RSp;
   bool ok;
 };
 
@@ -281,58 +277,42 @@ int nt_for(int cols) {
 }
 
 // wq: int8 weights (one byte per element in the A part of a stage)
-ChainGeom chain_geom(const dovetail_draft::QueuedGemv* q, int n, int wq) {
-  ChainGeom s{};
+MmaGeom mma_geom(const dovetail_draft::QueuedGemv& q, int wq) {
+  MmaGeom s{};
   const int aes = wq ? 1 : 2;
-  s.ok = n >= 1 && n <= kMaxChain;
-  int max_cnt = 1, nt = 1, res_floats = 0;
-  for (int i = 0; s.ok && i < n; ++i) {
-    const int K = q[i].p.K, M = q[i].p.M;
-    s.ok = K % 32 == 0 && M >= 1 && M <= kMmaMaxM && q[i].max_cnt >= 1;
-    if (!s.ok) break;
-    const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
-    s.S[i] = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
-    if (q[i].p.g[0].S_fixed) s.S[i] = std::max(s.S[i], q[i].p.g[0].S_fixed);
-    nt = std::max(nt, nt2);
-    max_cnt = std::max(max_cnt, q[i].max_cnt);
-    res_floats = std::max(res_floats, q[i].max_cnt * M);
-  }
-  if (!s.ok || nt > 8) { s.ok = false; return s; }
+  const int K = q.p.K, M = q.p.M;
+  s.ok = K % 32 == 0 && M >= 1 && M <= kMmaMaxM && q.max_cnt >= 1;
+  if (!s.ok) return s;
+  const int nt2 = nt_for(2 * M), nt3 = nt_for(3 * M);
+  s.S = nt3 == nt2 ? 3 : 2;  // the exact 3-way split when it costs no extra column tile
+  if (q.p.g[0].S_fixed) s.S = std::max(s.S, q.p.g[0].S_fixed);
+  const int nt = nt2, max_cnt = q.max_cnt, res_floats = q.max_cnt * M;
+  if (nt > 8) { s.ok = false; return s; }
   s.NT = nt;
   s.RBMAX = nt == 8 ? 2 : 4;
   // Rows per stage and K-chunk: the first candidate that leaves a ring of >= 3 stages or >= 120 KB (else the
   // deepest ring found). A stage holds RS weight rows and M * S activation columns of one K-chunk. Wide levels
   // take the smaller stages: their B columns and partial buffers use most of the shared memory.
   const int rs_max = std::min(16 * s.RBMAX, (max_cnt + 15) / 16 * 16);
-  ChainGeom best{};
+  const int ncols = M * s.S, PC = (ncols + 1) & ~1;
+  MmaGeom best{};
   for (int rs = rs_max; rs >= 16; rs -= 16) {
+    // rows a stage really carries: the CTA's rows in balanced super-blocks of <= rs rows
+    const int nsb = div_up(max_cnt, rs), rows_eff = std::min(rs, div_up(max_cnt, nsb));
     for (int kc0 : {wq ? 1024 : 512, wq ? 512 : 256, wq ? 256 : 128}) {
-      ChainGeom c = s;
+      MmaGeom c = s;
       c.RS = rs;
-      c.stage_bytes = 0;
-      c.part_floats = 0;
-      // rows a stage really carries in phase i: the CTA's rows in balanced super-blocks of <= rs rows
-      auto rows_eff = [&](int i) { const int nsb = div_up(q[i].max_cnt, rs); return std::min(rs, div_up(q[i].max_cnt, nsb)); };
-      for (int i = 0; i < n; ++i) {
-        const int ncols = q[i].p.M * s.S[i], PC = (ncols + 1) & ~1;
-        c.KC[i] = std::min(kc0, (q[i].p.K + 63) / 64 * 64);
-        c.seg_stride[i] = c.KC[i] * 2 + 16;
-        c.aseg_stride[i] = c.KC[i] * aes + 16;
-        c.stage_bytes = std::max(c.stage_bytes, rows_eff(i) * c.aseg_stride[i] + ncols * c.seg_stride[i]);
-        c.part_floats = std::max(c.part_floats, kConsumerWarps * rs * PC);
-      }
-      // phases with few rows per CTA (O, down: 35 of 64) take longer K-chunks so that their stages are full too
-      for (int i = 0; i < n; ++i) {
-        const int ncols = q[i].p.M * s.S[i];
-        while (c.KC[i] < 2048 * (wq ? 2 : 1) && c.KC[i] * 2 <= (q[i].p.K + 63) / 64 * 64 &&
-               rows_eff(i) * (c.KC[i] * 2 * aes + 16) + ncols * (c.KC[i] * 4 + 16) <= c.stage_bytes + 4096) {
-          c.KC[i] *= 2;
-          c.seg_stride[i] = c.KC[i] * 2 + 16;
-          c.aseg_stride[i] = c.KC[i] * aes + 16;
-        }
-        c.stage_bytes = std::max(c.stage_bytes, rows_eff(i) * c.aseg_stride[i] + ncols * c.seg_stride[i]);
-        c.RSp[i] = rows_eff(i);
-      }
+      c.KC = std::min(kc0, (K + 63) / 64 * 64);
+      c.part_floats = kConsumerWarps * rs * PC;
+      // matrices with few rows per CTA (O, down: 35 of 64) take longer K-chunks so that their stages are full too
+      const int full_stage = rs * (c.KC * aes + 16) + ncols * (c.KC * 2 + 16);
+      while (c.KC < 2048 * (wq ? 2 : 1) && c.KC * 2 <= (K + 63) / 64 * 64 &&
+             rows_eff * (c.KC * 2 * aes + 16) + ncols * (c.KC * 4 + 16) <= full_stage + 4096)
+        c.KC *= 2;
+      c.seg_stride = c.KC * 2 + 16;
+      c.aseg_stride = c.KC * aes + 16;
+      c.stage_bytes = rows_eff * c.aseg_stride + ncols * c.seg_stride;
+      c.RSp = rows_eff;
       if (c.part_floats * 4 > 32768 && rs > 16) continue;
       c.res_floats = res_floats;
       int fixed = 3 * 64 + 16 + 2 * 4 * kMmaMaxM + c.part_floats * 4 + res_floats * 4 + (wq ? max_cnt * 4 : 0);
@@ -366,86 +346,64 @@ int run_gemv_fma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv&
   return DOVETAIL_OK;
 }
 
-// One persistent launch over q[0 .. n): tensor-core kernel.
-int run_chain(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv* q, int n, const ChainGeom& g) {
-  ChainParams cp{};
-  cp.n = n;
+// One launch of the tensor-core kernel.
+int run_mma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, const MmaGeom& g) {
+  MmaParams cp{};
   cp.stage_bytes = g.stage_bytes;
   cp.n_stages = g.n_stages;
   cp.part_floats = g.part_floats;
   cp.res_floats = g.res_floats;
-  if (n > 1) {
-    if (h->bar_used + n > kMaxBars) return fail(h, DOVETAIL_EINVAL, "too many GEMV phases in one step");
-    cp.bar = h->bar + h->bar_used;
-    h->bar_used += n;
-  }
-  int grid = 1;
-  for (int i = 0; i < n; ++i) {
-    GemvParams& p = q[i].p;
-    p.n_groups = q[i].n_groups;
-    p.ctas_per_group = q[i].ctas;
-    p.rows_per_stage = g.RSp[i];
-    p.row_bytes = p.K * (h->wq ? 1 : 2);
-    p.kc = g.KC[i];
-    p.seg_stride = g.seg_stride[i];
-    p.aseg_stride = g.aseg_stride[i];
-    for (int gi = 0; gi < q[i].n_groups; ++gi)
-      p.g[gi].S = p.g[gi].xkind == X_EMBED ? 1 : (p.g[gi].S_fixed ? p.g[gi].S_fixed : g.S[i]);
-    h->cur_kind = q[i].kind;
-    h->cur_bytes = q[i].bytes;
-    p.trace = trace_slot(h);
-    grid = std::max(grid, q[i].n_groups * q[i].ctas);
-    cp.ph[i] = p;
-  }
+  GemvParams& p = q.p;
+  p.n_groups = q.n_groups;
+  p.ctas_per_group = q.ctas;
+  p.rows_per_stage = g.RSp;
+  p.row_bytes = p.K * (h->wq ? 1 : 2);
+  p.kc = g.KC;
+  p.seg_stride = g.seg_stride;
+  p.aseg_stride = g.aseg_stride;
+  for (int gi = 0; gi < q.n_groups; ++gi)
+    p.g[gi].S = p.g[gi].xkind == X_EMBED ? 1 : (p.g[gi].S_fixed ? p.g[gi].S_fixed : g.S);
+  h->cur_kind = q.kind;
+  h->cur_bytes = q.bytes;
+  p.trace = trace_slot(h);
+  cp.p = p;
 #ifdef DVT_CHAINDBG
   if (!h->dry) {
-    if (!h->dbg) { cudaMalloc(reinterpret_cast<void**>(&h->dbg), sizeof(unsigned long long) * 64 * 148 * kMaxChain * 8); cudaMemset(h->dbg, 0, sizeof(unsigned long long) * 64 * 148 * kMaxChain * 8); }
-    if (h->dbg_launch < 64) cp.dbg = h->dbg + static_cast<size_t>(h->dbg_launch++) * 148 * kMaxChain * 8;
+    if (!h->dbg) { cudaMalloc(reinterpret_cast<void**>(&h->dbg), sizeof(unsigned long long) * 64 * 148 * 16); cudaMemset(h->dbg, 0, sizeof(unsigned long long) * 64 * 148 * 16); }
+    if (h->dbg_launch < 64) cp.dbg = h->dbg + static_cast<size_t>(h->dbg_launch++) * 148 * 16;
   }
 #endif
-  cudaError_t e = launch(h, pick_gemv_mma(g.NT, h->wq), dim3(grid), dim3(kMmaThreads), g.smem, st, cp);
+  cudaError_t e = launch(h, pick_gemv_mma(g.NT, h->wq), dim3(q.n_groups * q.ctas), dim3(kMmaThreads), g.smem, st, cp);
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (mma) launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
 }
 
-// Launch everything queued: maximal runs of tensor-core-capable GEMVs as chains of <= chain_max, the rest one
-// by one on the FMA kernel.
+// Launch everything queued: tensor-core-capable GEMVs on k_gemv_mma, the rest on the FMA kernel. (Running several
+// GEMVs in one persistent launch with a grid barrier between them was built and measured slower than separate
+// launches with programmatic dependent launch: DESIGN.md, negative results.)
 int flush_gemv(dovetail_draft* h, cudaStream_t st) {
   auto& Q = h->queue;
   int rc = DOVETAIL_OK;
-  size_t i = 0;
-  while (i < Q.size() && rc == DOVETAIL_OK) {
-    const bool mma_ok = h->es == 2 && chain_geom(&Q[i], 1, h->wq).ok;
-    if (!mma_ok) {
-      if (h->es == 2 && Q[i].p.M > kMmaMaxM && Q[i].p.K % 32 == 0) {
-        // a level wider than 32 rows: chunks of <= 32 rows (64 B columns), the weights are streamed once per chunk
-        const int Mtot = Q[i].p.M;
-        for (int m0 = 0; m0 < Mtot && rc == DOVETAIL_OK; m0 += kMmaMaxM) {
-          dovetail_draft::QueuedGemv c = Q[i];
-          c.p.M = std::min(kMmaMaxM, Mtot - m0);
-          c.p.m0 = m0;
-          if (m0 > 0) c.bytes = 0;  // the algorithmic bytes are counted once
-          const ChainGeom g = chain_geom(&c, 1, h->wq);
-          rc = g.ok ? run_chain(h, st, &c, 1, g) : fail(h, DOVETAIL_EINVAL, "GEMV with K = %d does not fit the tensor-core kernel", c.p.K);
-        }
-      } else if (h->wq) {
-        rc = fail(h, DOVETAIL_EINVAL, "int8 weights: GEMV with K = %d, M = %d does not fit the tensor-core kernel", Q[i].p.K, Q[i].p.M);
-      } else {
-        rc = run_gemv_fma(h, st, Q[i]);
+  for (size_t i = 0; i < Q.size() && rc == DOVETAIL_OK; ++i) {
+    const MmaGeom g = h->es == 2 ? mma_geom(Q[i], h->wq) : MmaGeom{};
+    if (g.ok) {
+      rc = run_mma(h, st, Q[i], g);
+    } else if (h->es == 2 && Q[i].p.M > kMmaMaxM && Q[i].p.K % 32 == 0) {
+      // a level wider than 32 rows: chunks of <= 32 rows (64 B columns), the weights are streamed once per chunk
+      const int Mtot = Q[i].p.M;
+      for (int m0 = 0; m0 < Mtot && rc == DOVETAIL_OK; m0 += kMmaMaxM) {
+        dovetail_draft::QueuedGemv c = Q[i];
+        c.p.M = std::min(kMmaMaxM, Mtot - m0);
+        c.p.m0 = m0;
+        if (m0 > 0) c.bytes = 0;  // the algorithmic bytes are counted once
+        const MmaGeom gc = mma_geom(c, h->wq);
+        rc = gc.ok ? run_mma(h, st, c, gc) : fail(h, DOVETAIL_EINVAL, "GEMV with K = %d does not fit the tensor-core kernel", c.p.K);
       }
-      ++i;
-      continue;
+    } else if (h->wq) {
+      rc = fail(h, DOVETAIL_EINVAL, "int8 weights: GEMV with K = %d, M = %d does not fit the tensor-core kernel", Q[i].p.K, Q[i].p.M);
+    } else {
+      rc = run_gemv_fma(h, st, Q[i]);
     }
-    int n = 1;  // grow the chain while the geometry stays valid
-    ChainGeom g = chain_geom(&Q[i], 1, h->wq);
-    while (n < h->chain_max && i + n < Q.size()) {
-      const ChainGeom g2 = chain_geom(&Q[i], n + 1, h->wq);
-      if (!g2.ok || g2.n_stages * g2.stage_bytes < 100 * 1024) break;
-      g = g2;
-      ++n;
-    }
-    rc = run_chain(h, st, &Q[i], n, g);
-    i += n;
   }
   Q.clear();
   return rc;
@@ -553,7 +511,6 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->hbuf); cudaFree(h->hhat); cudaFree(h->qkv); cudaFree(h->obuf); cudaFree(h->act);
   cudaFree(h->xs_feat); cudaFree(h->xs_hhat); cudaFree(h->xs_x); cudaFree(h->xs_h12); cudaFree(h->xs_o); cudaFree(h->xs_act);
   cudaFree(h->ssq);
-  cudaFree(h->bar);
   cudaFree(h->qs);
   cudaFree(h->xs_emb);
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
@@ -633,7 +590,6 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   h->cur_bytes = 0;
   h->cur_level = 0;
   h->tr_used = 0;
-  h->bar_used = 0;
   h->queue.clear();
 #ifdef DVT_CHAINDBG
   h->dbg_launch = 0;
@@ -649,8 +605,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   const int64_t R = c.max_rows, SR = h->max_step_rows;
   const int nct_d = std::min(nsm, d);  // CTAs of the GEMVs that produce the residual stream (and its sums of squares)
   e = launch_c(h, 1, false, k_step_begin, dim3(n_new + tree->depth - 1), dim3(512), 0, st, dv, h->dyn, h->ts, h->rt,
-               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h, h->xs_feat, R, h->ld_d), h->bar, kMaxBars,
-               trace_slot(h));
+               h->rope, static_cast<const double*>(h->inv_freq), half, V, d, planes(h, h->xs_feat, R, h->ld_d), trace_slot(h));
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
 
   for (int l = 0; l < tree->depth; ++l) {
@@ -1062,7 +1017,6 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->xs_o, kSplitPlanes * R * h->ld_dq));
     A(dmalloc(&h->xs_act, kSplitPlanes * R * h->ld_f));
     A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
-    A(dmalloc(&h->bar, kMaxBars));
     A(dmalloc(&h->qs, static_cast<size_t>(2) * kMaxRows * dq));
     if (c.weight_quant) A(dmalloc(&h->xs_emb, kSplitPlanes * R * h->ld_d));
   }
@@ -1320,10 +1274,6 @@ int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_l
 
 int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
   if (!h) return DOVETAIL_EINVAL;
-  if (key == 0 && value >= 1 && value <= kMaxChain) {
-    h->chain_max = value;
-    return DOVETAIL_OK;
-  }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
 
@@ -1414,7 +1364,7 @@ int64_t dovetail_forward_bytes(const dovetail_draft_t* h, int32_t prefix_len) {
 
 #ifdef DVT_CHAINDBG
 int dovetail_dbg_read(dovetail_draft_t* h, unsigned long long* out, int n_launches) {
-  return cudaMemcpy(out, h->dbg, sizeof(unsigned long long) * n_launches * 148 * kMaxChain * 8, cudaMemcpyDeviceToHost);
+  return cudaMemcpy(out, h->dbg, sizeof(unsigned long long) * n_launches * 148 * 16, cudaMemcpyDeviceToHost);
 }
 #endif
 

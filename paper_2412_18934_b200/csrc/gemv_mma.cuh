@@ -74,26 +74,17 @@ __device__ __forceinline__ uint32_t pack_bf16x2_rn(float lo, float hi) {
   return *reinterpret_cast<const uint32_t*>(&h);
 }
 
-// A chain of up to kMaxChain GEMVs executed by ONE persistent launch (one CTA per SM, all resident): the
-// weight producers roll from one matrix straight into the next -- weights never depend on activations, so the
-// HBM stream does not stop at a GEMV boundary -- while the activation producer and the consumers of phase i + 1
-// wait until every CTA has finished phase i (grid_arrive / grid_wait on a counter in global memory: the
-// activations of phase i + 1 are the results of phase i from all CTAs). A single GEMV is a chain of one.
-constexpr int kMaxChain = 4;
-
-#ifdef DVT_CHAINDBG  // working builds only: per-CTA time stamps of the phases of a chain
-#define DVT_DBG(ph, i) do { if (cp.dbg) cp.dbg[(static_cast<size_t>(blockIdx.x) * kMaxChain + (ph)) * 8 + (i)] = globaltimer_ns(); } while (0)
+#ifdef DVT_CHAINDBG  // working builds only: per-CTA time stamps inside one launch
+#define DVT_DBG(i) do { if (cp.dbg) cp.dbg[static_cast<size_t>(blockIdx.x) * 16 + (i)] = globaltimer_ns(); } while (0)
 #else
-#define DVT_DBG(ph, i) do { } while (0)
+#define DVT_DBG(i) do { } while (0)
 #endif
 
-struct ChainParams {
-  GemvParams ph[kMaxChain];
-  int32_t n;
-  int32_t stage_bytes, n_stages;  // ring geometry, common to the phases
-  int32_t part_floats;            // floats of the partial buffer (largest phase)
-  int32_t res_floats;             // floats of the result buffer (largest phase)
-  int32_t* bar;                   // [n] phase counters, zeroed at the start of the step
+struct MmaParams {
+  GemvParams p;
+  int32_t stage_bytes, n_stages;  // ring geometry
+  int32_t part_floats;            // floats of the partial buffer
+  int32_t res_floats;             // floats of the result buffer
   unsigned long long* dbg;        // DVT_CHAINDBG builds only
 };
 
@@ -104,11 +95,28 @@ __device__ __forceinline__ void super_blocks(int cnt, int RS, int& n_sb, int& rs
   rsb = n_sb > 0 ? (cnt + n_sb - 1) / n_sb : 0;
 }
 
-// which group of the phase this CTA works for, and its index within the group's CTAs (or -1: idle)
-__device__ __forceinline__ int chain_cta(const GemvParams& p, int c, int& g) {
-  g = c / p.ctas_per_group;
-  if (g >= p.n_groups) { g = 0; return -1; }
-  return c - g * p.ctas_per_group;
+// Which rows this CTA works on: group g, index c within the group's CTAs (or c < 0: idle). The integer divisions
+// behind it (64-bit ones in cta_rows) are a dependent chain of about a microsecond, so every role computes it
+// BEFORE griddepcontrol.wait (it depends on the launch arguments only) and pins the results there: measured,
+// the consumers otherwise spend it after the wait, with the ring full and the HBM stream stopped.
+struct CtaGeom {
+  int c, g, n_sb, rsb;
+  RowRange rr;
+};
+__device__ __forceinline__ CtaGeom cta_geom(const GemvParams& p, int c_grid) {
+  CtaGeom q;
+  q.g = c_grid / p.ctas_per_group;
+  q.c = c_grid - q.g * p.ctas_per_group;
+  if (q.g >= p.n_groups) { q.g = 0; q.c = -1; }
+  q.n_sb = q.rsb = 0;
+  q.rr.cnt = q.rr.n0 = q.rr.cr = 0;
+  q.rr.g0 = 0;
+  if (q.c >= 0) {
+    q.rr = cta_rows(p.g[q.g], q.c, p.ctas_per_group);
+    super_blocks(q.rr.cnt, p.rows_per_stage, q.n_sb, q.rsb);
+  }
+  asm volatile("" : "+r"(q.c), "+r"(q.g), "+r"(q.n_sb), "+r"(q.rsb), "+r"(q.rr.cnt), "+r"(q.rr.n0), "+r"(q.rr.cr), "+l"(q.rr.g0));
+  return q;
 }
 
 // four int8 (one 32-bit word, k ascending from the low byte) -> two fp16x2 words, exact: byte ^ 0x80 under the
@@ -137,24 +145,25 @@ __device__ __forceinline__ void mma_f16_16816(float (&c)[4], const uint32_t (&a)
 // multiplied with fp16 activation terms (products exact in fp32), the scale applied to the row's result; the
 // activation planes are stored in the matching k order (epilogue.cuh split_pos).
 template <int NT, int RBMAX, int WQ>
-__global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_constant__ ChainParams cp) {
+__global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_constant__ MmaParams cp) {
   constexpr int AES = WQ ? 1 : 2;  // bytes per weight
   extern __shared__ __align__(128) uint8_t smem[];
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int c_grid = blockIdx.x, n_grid = gridDim.x;
   const int NS = cp.n_stages;
+  const GemvParams& p = cp.p;
 
   uint8_t* ring = smem;
   uint64_t* full_a = reinterpret_cast<uint64_t*>(smem + static_cast<size_t>(NS) * cp.stage_bytes);
   uint64_t* full_b = full_a + 8;
   uint64_t* empty = full_b + 8;
   uint32_t* zero16 = reinterpret_cast<uint32_t*>(empty + 8);  // B columns past ncols read these zeros
-  float* rstd_s = reinterpret_cast<float*>(zero16 + 4);       // [2][32], alternating by phase
+  float* rstd_s = reinterpret_cast<float*>(zero16 + 4);       // [32]
   float* part = rstd_s + 2 * kMmaMaxM;                        // [warps][RS][PC]
   float* res = part + cp.part_floats;                         // [cnt][M]
   float* wsc = res + cp.res_floats;                           // [cnt] row scales (int8 weights)
 
-  trace_begin(cp.ph[0].trace);
+  trace_begin(p.trace);
+  if (tid == 0) DVT_DBG(0);
   if (tid == 0) {
     for (int s = 0; s < NS; ++s) {
       mbar_init(&full_a[s], kMmaProducerWarps);
@@ -167,57 +176,58 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
   __syncthreads();
   pdl_launch_dependents();
 
+  const CtaGeom q = cta_geom(p, blockIdx.x);
+  const int c = q.c;
+  const GemvGroup& G = p.g[q.g];
+  const RowRange rr = q.rr;
+  const int n_sb = q.n_sb, rsb = q.rsb;
+  const int K = p.K, KC = p.kc, M = p.M, S = G.S, ncols = M * S;
+
   if (warp >= kConsumerWarps + kMmaProducerWarps) {
     // ---------------- activation producer: one B column per lane (two when ncols > 32) -----------
-    pdl_wait();  // the planes of the first phase were written by the previous kernels
     const uint64_t pol = l2_policy_evict_last();
+    // everything that does not need the previous kernel's results is computed before the wait
+    int64_t off[2];  // element offset of the column's plane row (X_ROWS without a row index: complete)
+    int cm[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int col = lane + 32 * h;
+      cm[h] = col / S;
+      const int s = col - cm[h] * S;
+      off[h] = s * G.xs_plane + (G.xidx ? 0 : (p.m0 + cm[h]) * G.xs_ld);
+    }
+    asm volatile("" : "+l"(off[0]), "+l"(off[1]), "+r"(cm[0]), "+r"(cm[1]));
+    pdl_wait();  // the planes were written by the previous kernels
+    if (lane == 0) DVT_DBG(5);
+    if (c < 0) return;
+    const uint8_t* src[2] = {nullptr, nullptr};
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      if (lane + 32 * h < ncols) {
+        if (G.xkind == X_ROWS) {
+          const int64_t ro = G.xidx ? static_cast<int64_t>(G.xidx[p.m0 + cm[h]]) * G.xs_ld : 0;
+          src[h] = reinterpret_cast<const uint8_t*>(G.xs + off[h] + ro);
+        } else {  // embedding rows are bf16 already: one plane
+          src[h] = reinterpret_cast<const uint8_t*>(static_cast<const __nv_bfloat16*>(G.embed) +
+                                                    static_cast<size_t>(G.tokens[p.m0 + cm[h]]) * K);
+        }
+      }
+    }
     int slot = 0, round = 0;
-    for (int ph = 0; ph < cp.n; ++ph) {
-      const GemvParams& p = cp.ph[ph];
-      int g;
-      const int c = chain_cta(p, c_grid, g);
-      const GemvGroup& G = p.g[g];
-      const int K = p.K, KC = p.kc, M = p.M, S = G.S, RS = p.rows_per_stage, ncols = M * S;
-      if (ph > 0) {  // the planes (and sums of squares) of this phase come from every CTA of the previous one
-        if (lane == 0) grid_wait(cp.bar + ph - 1, n_grid);
+    for (int sb = 0; sb < n_sb; ++sb) {
+      for (int k0 = 0; k0 < K; k0 += KC) {
+        if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+        const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * 2u;
+        if (lane == 0) mbar_arrive_expect_tx(&full_b[slot], static_cast<uint32_t>(ncols) * segb);
         __syncwarp();
-        fence_proxy_async();
-        if (lane == 0) DVT_DBG(ph, 5);
-      }
-      if (lane == 0) DVT_DBG(ph, 6);
-      if (c < 0) continue;
-      const RowRange rr = cta_rows(G, c, p.ctas_per_group);
-      int n_sb, rsb;
-      super_blocks(rr.cnt, RS, n_sb, rsb);
-      const uint8_t* src[2] = {nullptr, nullptr};
+        uint8_t* dst = ring + static_cast<size_t>(slot) * cp.stage_bytes;  // B columns first, then the A rows
 #pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        const int col = lane + 32 * h;
-        if (col < ncols) {
-          const int m = col / S, s = col - m * S;
-          if (G.xkind == X_ROWS) {
-            const int64_t ri = G.xidx ? G.xidx[p.m0 + m] : p.m0 + m;
-            src[h] = reinterpret_cast<const uint8_t*>(G.xs + s * G.xs_plane + ri * G.xs_ld);
-          } else {  // embedding rows are bf16 already: one plane
-            src[h] = reinterpret_cast<const uint8_t*>(static_cast<const __nv_bfloat16*>(G.embed) +
-                                                      static_cast<size_t>(G.tokens[p.m0 + m]) * K);
-          }
-        }
-      }
-      for (int sb = 0; sb < n_sb; ++sb) {
-        for (int k0 = 0; k0 < K; k0 += KC) {
-          if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
-          const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * 2u;
-          if (lane == 0) mbar_arrive_expect_tx(&full_b[slot], static_cast<uint32_t>(ncols) * segb);
-          __syncwarp();
-          uint8_t* dst = ring + static_cast<size_t>(slot) * cp.stage_bytes;  // B columns first, then the A rows
-#pragma unroll
-          for (int h = 0; h < 2; ++h)
-            if (src[h])
-              bulk_g2s(dst + static_cast<size_t>(lane + 32 * h) * p.seg_stride, src[h] + static_cast<size_t>(k0) * 2, segb,
-                       &full_b[slot], pol);
-          if (++slot == NS) { slot = 0; ++round; }
-        }
+        for (int h = 0; h < 2; ++h)
+          if (src[h])
+            bulk_g2s(dst + static_cast<size_t>(lane + 32 * h) * p.seg_stride, src[h] + static_cast<size_t>(k0) * 2, segb,
+                     &full_b[slot], pol);
+        if (lane == 0 && sb == 0 && k0 == 0) DVT_DBG(6);
+        if (++slot == NS) { slot = 0; ++round; }
       }
     }
     return;
@@ -225,226 +235,202 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
 
   if (warp >= kConsumerWarps) {
     // ---------------- weight producers: warp pw copies rows [16 pw, 16 pw + 16) of every stage ---
-    // They never wait for a phase boundary: only for ring slots.
+    // They never wait for the previous kernel: weights do not depend on activations.
+    if (c < 0) return;
     const int pw = warp - kConsumerWarps;
     const uint64_t pol = l2_policy_evict_first();
+    const uint32_t a_off = static_cast<uint32_t>(ncols) * p.seg_stride;  // A rows follow the B columns
     int slot = 0, round = 0;
-    for (int ph = 0; ph < cp.n; ++ph) {
-      const GemvParams& p = cp.ph[ph];
-      int g;
-      const int c = chain_cta(p, c_grid, g);
-      if (c < 0) continue;
-      const GemvGroup& G = p.g[g];
-      const int K = p.K, KC = p.kc, RS = p.rows_per_stage;
-      const uint32_t a_off = static_cast<uint32_t>(p.M * G.S) * p.seg_stride;  // A rows follow the B columns
-      const RowRange rr = cta_rows(G, c, p.ctas_per_group);
-      int n_sb, rsb;
-      super_blocks(rr.cnt, RS, n_sb, rsb);
-      for (int sb = 0; sb < n_sb; ++sb) {
-        const int v0 = sb * rsb, nr = min(rsb, rr.cnt - v0);
-        const int r = pw * 16 + (lane & 15);  // this lane's row of the super-block (lanes 0..15)
-        const bool mine = lane < 16 && r < nr;
-        const int my_rows = max(0, min(16, nr - pw * 16));
-        const uint8_t* src = nullptr;
-        if (mine) {
-          int j, n;
-          locate_row(G, rr, v0 + r, j, n);
-          src = static_cast<const uint8_t*>(G.w[j]) + static_cast<size_t>(n) * p.row_bytes;
-        }
-        for (int k0 = 0; k0 < K; k0 += KC) {
-          if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
-          if (pw == 0 && lane == 0 && sb == 0 && k0 == 0) DVT_DBG(ph, 7);
-          const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * AES;
-          if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(my_rows) * segb);
-          __syncwarp();
-          uint8_t* dst = ring + static_cast<size_t>(slot) * cp.stage_bytes + a_off;
-          if (mine) bulk_g2s(dst + static_cast<size_t>(r) * p.aseg_stride, src + static_cast<size_t>(k0) * AES, segb, &full_a[slot], pol);
-          if (++slot == NS) { slot = 0; ++round; }
-        }
+    for (int sb = 0; sb < n_sb; ++sb) {
+      const int v0 = sb * rsb, nr = min(rsb, rr.cnt - v0);
+      const int r = pw * 16 + (lane & 15);  // this lane's row of the super-block (lanes 0..15)
+      const bool mine = lane < 16 && r < nr;
+      const int my_rows = max(0, min(16, nr - pw * 16));
+      const uint8_t* src = nullptr;
+      if (mine) {
+        int j, n;
+        locate_row(G, rr, v0 + r, j, n);
+        src = static_cast<const uint8_t*>(G.w[j]) + static_cast<size_t>(n) * p.row_bytes;
+      }
+      for (int k0 = 0; k0 < K; k0 += KC) {
+        if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+        if (pw == 0 && lane == 0 && sb == 0 && k0 == 0) DVT_DBG(7);
+        const uint32_t segb = static_cast<uint32_t>(min(KC, K - k0)) * AES;
+        if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(my_rows) * segb);
+        __syncwarp();
+        uint8_t* dst = ring + static_cast<size_t>(slot) * cp.stage_bytes + a_off;
+        if (mine) bulk_g2s(dst + static_cast<size_t>(r) * p.aseg_stride, src + static_cast<size_t>(k0) * AES, segb, &full_a[slot], pol);
+        if (++slot == NS) { slot = 0; ++round; }
       }
     }
     return;
   }
 
   // ---------------- consumers -------------------------------------------------
-  pdl_wait();  // residual stream, [h1 || h2]: written by the previous kernels
+  const int RS = p.rows_per_stage;
+  const int PC = (ncols + 1) & ~1;
+  const int RS16 = (RS + 15) & ~15;  // rows of the partial buffer: whole 16-row blocks
   const uint32_t ring_u = smem_u32(ring);
   const uint32_t zero_u = smem_u32(zero16);
-  int slot = 0, round = 0;
-  for (int ph = 0; ph < cp.n; ++ph) {
-    const GemvParams& p = cp.ph[ph];
-    int g;
-    const int c = chain_cta(p, c_grid, g);
-    const GemvGroup& G = p.g[g];
-    const int K = p.K, KC = p.kc, M = p.M, S = G.S, RS = p.rows_per_stage;
-    const int ncols = M * S, PC = (ncols + 1) & ~1;
-    if (ph > 0) trace_begin(p.trace);
-    if (tid == 0) DVT_DBG(ph, 0);
-    if (ph > 0) {
-      // Results of the previous phase from every CTA ([h1 || h2], residual stream, sums of squares) are read
-      // below: thread 0 acquires the phase counter, the barrier extends it to the CTA's consumers.
-      if (tid == 0) grid_wait(cp.bar + ph - 1, n_grid);
-      consumer_sync();
-    }
-    if (c >= 0 && p.ssq_in) {
-      // RMSNorm: 1 / rms of each draft row from the producers' partial sums of squares, fixed order (lane l adds
-      // CTAs l, l + 32, ...; then a butterfly). Overlaps the arrival of the phase's first activation chunk.
-      float* rs = rstd_s + (ph & 1) * kMmaMaxM;
-      for (int m = warp; m < M; m += kConsumerWarps) {
-        float v[8];
+  // per-lane ldmatrix address pieces (a stage: the B columns, then the A rows)
+  const int a_lrow = (lane & 7) + ((lane >> 3) & 1) * 8;  // this lane's row within a 16-row block
+  uint32_t a_lane = static_cast<uint32_t>(ncols) * p.seg_stride + (lane >> 4) * 16;
+  uint32_t b_lane[NT];  // offset within the B part of a stage, or ~0: the zero block
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-          const int cc = lane + 32 * j;
-          v[j] = cc < p.ssq_nct ? __ldcg(p.ssq_in + static_cast<int64_t>(cc) * kMaxRows + p.m0 + m) : 0.f;
-        }
-        float t = 0.f;
+  for (int t = 0; t < NT; ++t) {
+    const int col = t * 8 + (lane & 7);
+    b_lane[t] = col < ncols ? static_cast<uint32_t>(col) * p.seg_stride + (lane >> 3) * 16 : 0xffffffffu;
+    asm volatile("" : "+r"(b_lane[t]));
+  }
+  asm volatile("" : "+r"(a_lane));
+  pdl_wait();  // residual stream, [h1 || h2], sums of squares: written by the previous kernels
+  if (tid == 0) DVT_DBG(1);
+  if (c >= 0) {
+    // RMSNorm: the partial sums of squares of draft row `warp` are requested now and added after the streaming
+    // loop (their L2 round trip must not delay the first mma); rows >= 8 of a wide level are read there.
+    float ssq_v[8];
 #pragma unroll
-        for (int j = 0; j < 8; ++j) t += v[j];
-        t = warp_sum(t);
-        if (lane == 0) rs[m] = 1.0f / sqrtf(t / static_cast<float>(K) + p.eps);
+    for (int j = 0; j < 8; ++j) ssq_v[j] = 0.f;
+    if (p.ssq_in && warp < M) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) {
+        const int cc = lane + 32 * j;
+        if (cc < p.ssq_nct) ssq_v[j] = __ldcg(p.ssq_in + static_cast<int64_t>(cc) * kMaxRows + p.m0 + warp);
       }
     }
-    if (c >= 0) {
-      const RowRange rr = cta_rows(G, c, p.ctas_per_group);
-      EpiRegs pre;
-      epi_prefetch(p, G, rr, M, p.m0, true, pre);  // in flight during the streaming loop
-      if (WQ) {  // scale of each of the CTA's rows; read after the barriers of the first meet
-        for (int v = tid; v < rr.cnt; v += kConsumerThreads) {
-          int j, n;
-          locate_row(G, rr, v, j, n);
-          wsc[v] = __ldg(G.ws[j] + n);
-        }
+    EpiRegs pre;
+    epi_prefetch(p, G, rr, M, p.m0, true, pre);  // in flight during the streaming loop
+    if (WQ) {  // scale of each of the CTA's rows; read after the barriers of the first meet
+      for (int v = tid; v < rr.cnt; v += kConsumerThreads) {
+        int j, n;
+        locate_row(G, rr, v, j, n);
+        wsc[v] = __ldg(G.ws[j] + n);
       }
-      int n_sb, rsb;
-      super_blocks(rr.cnt, RS, n_sb, rsb);
-      const int RS16 = (RS + 15) & ~15;  // rows of the partial buffer: whole 16-row blocks
-      // per-lane ldmatrix address pieces (a stage: the B columns, then the A rows)
-      const int a_lrow = (lane & 7) + ((lane >> 3) & 1) * 8;  // this lane's row within a 16-row block
-      const uint32_t a_lane = static_cast<uint32_t>(ncols) * p.seg_stride + (lane >> 4) * 16;
-      uint32_t b_lane[NT];  // offset within the B part of a stage, or ~0: the zero block
+    }
+    int slot = 0, round = 0;
+    for (int sb = 0; sb < n_sb; ++sb) {
+      const int v0 = sb * rsb, nr = min(rsb, rr.cnt - v0);
+      const int rbs = (nr + 15) >> 4;
+      uint32_t a_row[RBMAX];  // rows past the super-block's last one were never copied: read the last row instead
 #pragma unroll
-      for (int t = 0; t < NT; ++t) {
-        const int col = t * 8 + (lane & 7);
-        b_lane[t] = col < ncols ? static_cast<uint32_t>(col) * p.seg_stride + (lane >> 3) * 16 : 0xffffffffu;
-      }
-      for (int sb = 0; sb < n_sb; ++sb) {
-        const int v0 = sb * rsb, nr = min(rsb, rr.cnt - v0);
-        const int rbs = (nr + 15) >> 4;
-        uint32_t a_row[RBMAX];  // rows past the super-block's last one were never copied: read the last row instead
+      for (int rb = 0; rb < RBMAX; ++rb) a_row[rb] = static_cast<uint32_t>(min(rb * 16 + a_lrow, nr - 1)) * p.aseg_stride;
+      float acc[RBMAX][NT][4];
 #pragma unroll
-        for (int rb = 0; rb < RBMAX; ++rb) a_row[rb] = static_cast<uint32_t>(min(rb * 16 + a_lrow, nr - 1)) * p.aseg_stride;
-        float acc[RBMAX][NT][4];
+      for (int rb = 0; rb < RBMAX; ++rb)
 #pragma unroll
-        for (int rb = 0; rb < RBMAX; ++rb)
+        for (int t = 0; t < NT; ++t)
 #pragma unroll
-          for (int t = 0; t < NT; ++t)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) acc[rb][t][e] = 0.f;
+          for (int e = 0; e < 4; ++e) acc[rb][t][e] = 0.f;
 
-        for (int k0 = 0; k0 < K; k0 += KC) {
-          const int n_units = min(KC, K - k0) >> 5;  // 32 k per unit
-          mbar_wait(&full_a[slot], round & 1);
-          mbar_wait(&full_b[slot], round & 1);
-          if (tid == 0 && sb == 0 && k0 == 0) DVT_DBG(ph, 1);
-          const uint32_t sbase = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
-          for (int u = warp; u < n_units; u += kConsumerWarps) {
-            uint32_t b[NT][4];
+      for (int k0 = 0; k0 < K; k0 += KC) {
+        const int n_units = min(KC, K - k0) >> 5;  // 32 k per unit
+        mbar_wait(&full_a[slot], round & 1);
+        mbar_wait(&full_b[slot], round & 1);
+        if (tid == 0 && sb == 0 && k0 == 0) DVT_DBG(2);
+        const uint32_t sbase = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
+        for (int u = warp; u < n_units; u += kConsumerWarps) {
+          uint32_t b[NT][4];
 #pragma unroll
-            for (int t = 0; t < NT; ++t) ldsm_x4(b[t], b_lane[t] == 0xffffffffu ? zero_u : sbase + b_lane[t] + u * 64);
-#pragma unroll
-            for (int rb = 0; rb < RBMAX; ++rb) {
-              if (rb < rbs) {
-                uint32_t a0[4], a1[4];
-                if (WQ) {  // 16 rows x 32 int8: one ldmatrix, then the exact conversion; pairs as split_pos orders B
-                  uint32_t q[4];
-                  ldsm_x4(q, sbase + a_lane + a_row[rb] + u * 32);
-#pragma unroll
-                  for (int e = 0; e < 4; ++e) cvt_i8x4_f16x2(q[e], a0[e], a1[e]);
-                } else {
-                  const uint32_t aaddr = sbase + a_lane + a_row[rb] + u * 64;
-                  ldsm_x4(a0, aaddr);
-                  ldsm_x4(a1, aaddr + 32);
-                }
-#pragma unroll
-                for (int t = 0; t < NT; ++t) {
-                  if (WQ) {
-                    mma_f16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
-                    mma_f16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
-                  } else {
-                    mma_bf16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
-                    mma_bf16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
-                  }
-                }
-              }
-            }
-          }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&empty[slot]);  // this warp's share of the stage is in registers
-          if (++slot == NS) { slot = 0; ++round; }
-        }
-
-        // ---- meet: partials -> shared memory, fixed-order sum over warps and split columns
-        {
-          const int gq = lane >> 2, tq = lane & 3;
-          float* pw = part + static_cast<size_t>(warp) * RS16 * PC;
+          for (int t = 0; t < NT; ++t) ldsm_x4(b[t], b_lane[t] == 0xffffffffu ? zero_u : sbase + b_lane[t] + u * 64);
 #pragma unroll
           for (int rb = 0; rb < RBMAX; ++rb) {
             if (rb < rbs) {
+              uint32_t a0[4], a1[4];
+              if (WQ) {  // 16 rows x 32 int8: one ldmatrix, then the exact conversion; pairs as split_pos orders B
+                uint32_t qw[4];
+                ldsm_x4(qw, sbase + a_lane + a_row[rb] + u * 32);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) cvt_i8x4_f16x2(qw[e], a0[e], a1[e]);
+              } else {
+                const uint32_t aaddr = sbase + a_lane + a_row[rb] + u * 64;
+                ldsm_x4(a0, aaddr);
+                ldsm_x4(a1, aaddr + 32);
+              }
 #pragma unroll
               for (int t = 0; t < NT; ++t) {
-                const int col = t * 8 + 2 * tq;
-                if (col < PC) {
-                  *reinterpret_cast<float2*>(pw + (rb * 16 + gq) * PC + col) = make_float2(acc[rb][t][0], acc[rb][t][1]);
-                  *reinterpret_cast<float2*>(pw + (rb * 16 + gq + 8) * PC + col) = make_float2(acc[rb][t][2], acc[rb][t][3]);
+                if (WQ) {
+                  mma_f16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
+                  mma_f16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
+                } else {
+                  mma_bf16_16816(acc[rb][t], a0, b[t][0], b[t][1]);
+                  mma_bf16_16816(acc[rb][t], a1, b[t][2], b[t][3]);
                 }
               }
             }
           }
         }
-        consumer_sync();
-        for (int idx = tid; idx < nr * M; idx += kConsumerThreads) {
-          const int r = idx / M, m = idx - r * M;
-          float t = 0.f;
-          for (int w = 0; w < kConsumerWarps; ++w) {
-            const float* q = part + (static_cast<size_t>(w) * RS16 + r) * PC + m * S;
-            float tw = q[0];
-            if (WQ) {  // fp16 terms carry 2^-11 and 2^-22 (epilogue.cuh store_split)
-              if (S >= 2) tw += q[1] * 4.8828125e-4f;
-              if (S == 3) tw += q[2] * 2.384185791015625e-7f;
-            } else {
-              if (S >= 2) tw += q[1];
-              if (S == 3) tw += q[2];
-            }
-            t += tw;
-          }
-          res[static_cast<size_t>(v0 + r) * M + m] = WQ ? t * wsc[v0 + r] : t;
-        }
-        consumer_sync();  // part is reused by the next super-block
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[slot]);  // this warp's share of the stage is in registers
+        if (++slot == NS) { slot = 0; ++round; }
       }
 
-      if (tid == 0) DVT_DBG(ph, 2);
-      // ---- fused epilogue over the CTA's results: res[v * M + m] ---------------------
-      const int nres = rr.cnt * M;
-      if (p.ssq_in) {  // rstd_s: written before the streaming loop; the barriers of the meet order it
-        const float* rs = rstd_s + (ph & 1) * kMmaMaxM;
-        for (int idx = tid; idx < nres; idx += kConsumerThreads) res[idx] *= rs[idx % M];
-        consumer_sync();
+      if (sb == 0 && p.ssq_in) {
+        // 1 / rms of each draft row from the producers' partial sums of squares, fixed order (lane l adds CTAs
+        // l, l + 32, ...; then a butterfly); visible to the epilogue through the barriers of the meet
+        for (int m = warp; m < M; m += kConsumerWarps) {
+          if (m != warp) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+              const int cc = lane + 32 * j;
+              ssq_v[j] = cc < p.ssq_nct ? __ldcg(p.ssq_in + static_cast<int64_t>(cc) * kMaxRows + p.m0 + m) : 0.f;
+            }
+          }
+          float t = 0.f;
+#pragma unroll
+          for (int j = 0; j < 8; ++j) t += ssq_v[j];
+          t = warp_sum(t);
+          if (lane == 0) rstd_s[m] = 1.0f / sqrtf(t / static_cast<float>(K) + p.eps);
+        }
       }
-      gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[static_cast<size_t>(v) * M + m]; }, M, p.m0, c,
-                    p.ctas_per_group, true, &pre);
-    }
-    if (tid == 0) DVT_DBG(ph, 3);
-    if (ph + 1 < cp.n) {
-      // This CTA's results of the phase are complete: count in. The writers order their generic-proxy stores
-      // before the other CTAs' bulk copies (async proxy); the CTA barrier makes them happen before thread 0's
-      // gpu-scope release, which is cumulative.
-      fence_proxy_async();
+
+      // ---- meet: partials -> shared memory, fixed-order sum over warps and split columns
+      {
+        const int gq = lane >> 2, tq = lane & 3;
+        float* pw = part + static_cast<size_t>(warp) * RS16 * PC;
+#pragma unroll
+        for (int rb = 0; rb < RBMAX; ++rb) {
+          if (rb < rbs) {
+#pragma unroll
+            for (int t = 0; t < NT; ++t) {
+              const int col = t * 8 + 2 * tq;
+              if (col < PC) {
+                *reinterpret_cast<float2*>(pw + (rb * 16 + gq) * PC + col) = make_float2(acc[rb][t][0], acc[rb][t][1]);
+                *reinterpret_cast<float2*>(pw + (rb * 16 + gq + 8) * PC + col) = make_float2(acc[rb][t][2], acc[rb][t][3]);
+              }
+            }
+          }
+        }
+      }
       consumer_sync();
-      if (tid == 0) grid_arrive(cp.bar + ph);
+      for (int idx = tid; idx < nr * M; idx += kConsumerThreads) {
+        const int r = idx / M, m = idx - r * M;
+        float t = 0.f;
+        for (int w = 0; w < kConsumerWarps; ++w) {
+          const float* qp = part + (static_cast<size_t>(w) * RS16 + r) * PC + m * S;
+          float tw = qp[0];
+          if (WQ) {  // fp16 terms carry 2^-11 and 2^-22 (epilogue.cuh store_split)
+            if (S >= 2) tw += qp[1] * 4.8828125e-4f;
+            if (S == 3) tw += qp[2] * 2.384185791015625e-7f;
+          } else {
+            if (S >= 2) tw += qp[1];
+            if (S == 3) tw += qp[2];
+          }
+          t += tw;
+        }
+        if (WQ) t *= wsc[v0 + r];
+        if (p.ssq_in) t *= rstd_s[m];  // written before this super-block's barrier
+        res[static_cast<size_t>(v0 + r) * M + m] = t;
+      }
+      consumer_sync();  // part is reused by the next super-block
     }
-    if (tid == 0) DVT_DBG(ph, 4);
-    trace_end(p.trace);
+
+    if (tid == 0) DVT_DBG(3);
+    // ---- fused epilogue over the CTA's results: res[v * M + m] ---------------------
+    gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[static_cast<size_t>(v) * M + m]; }, M, p.m0, c,
+                  p.ctas_per_group, true, &pre);
   }
+  if (tid == 0) DVT_DBG(4);
+  trace_end(p.trace);
 }
 
 }  // namespace dvt

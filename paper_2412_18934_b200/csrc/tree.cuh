@@ -27,7 +27,7 @@ struct Pool {  // device arrays of capacity pool_cap
 // grid = n_new + depth - 1 CTAs (one rotary-table row each) x 64 threads.
 __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, RowTables* rt0,
                              float2* rope, const double* inv_freq, int half, int vocab, int d, SplitOut feat_so,
-                             int32_t* bar, int n_bar, unsigned long long* trace) {
+                             unsigned long long* trace) {
   pdl_launch_dependents();
   trace_begin(trace);
   pdl_wait();
@@ -42,8 +42,6 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
   // the caller's fp32 features as split-bf16 planes, the B operand of the DGF projection (epilogue.cuh)
   if (r < n_new && feat_so.xs != nullptr) split_row(feat_so, r, dynv.feats + static_cast<size_t>(r) * d, d);
   if (r == 0) {
-    if (bar != nullptr)  // phase counters of the step's persistent GEMV chains (gemv_mma.cuh)
-      for (int i = threadIdx.x; i < n_bar; i += blockDim.x) bar[i] = 0;
     if (threadIdx.x == 0) {
       *dyn = dynv;  // ts->status is sticky until dovetail_draft_status / kv_commit reads it
       ts->pool_size = 0;
