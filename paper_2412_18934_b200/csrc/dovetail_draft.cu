@@ -420,14 +420,19 @@ int run_gemv(dovetail_draft* h, cudaStream_t st, GemvParams& p, int n_groups, in
     const GemvGroup& G = p.g[g];
     for (int j = 0; j < G.n_mat; ++j)
       q.bytes += h->wq ? static_cast<int64_t>(G.rows[j]) * (p.K + 4) : static_cast<int64_t>(G.rows[j]) * p.K * h->es;
-    int mc;
-    if (G.paired) mc = G.n_mat * div_up(G.rows[0], ctas_per_group);
+    // dealing of the group's rows (units: rows, rows of each paired matrix, or rotary pairs) to its CTAs
+    long units;
+    int per_unit;
+    if (G.paired) { units = G.rows[0]; per_unit = G.n_mat; }
     else {
       long tot = 0;
       for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
-      const long unit = G.pairperm ? 2 : 1;  // rotary pairs are dealt whole (gemv.cuh cta_rows)
-      mc = static_cast<int>(unit * ((tot / unit + ctas_per_group - 1) / ctas_per_group));
+      per_unit = G.pairperm ? 2 : 1;  // rotary pairs are dealt whole (gemv.cuh cta_rows)
+      units = tot / per_unit;
     }
+    p.g[g].deal_base = static_cast<int32_t>(units / ctas_per_group);
+    p.g[g].deal_rem = static_cast<int32_t>(units % ctas_per_group);
+    const int mc = per_unit * (p.g[g].deal_base + (p.g[g].deal_rem > 0 ? 1 : 0));
     q.max_cnt = std::max(q.max_cnt, mc);
   }
   p.dyn = h->dyn;

@@ -40,6 +40,10 @@ struct GemvGroup {
   int32_t pairperm;      // head_dim or 0. EPI_QKV: within every head of the concatenated [q | k | v] rows the virtual
                          // order is (0, dh/2, 1, dh/2 + 1, ...), and CTA ranges start on an even virtual row, so
                          // that the two rows of a rotary pair (i, i + dh/2) belong to the same CTA
+  int32_t deal_base, deal_rem;  // dealing of the rows to the group's CTAs, set by the host: CTA c takes deal_base units
+                         // (+ 1 for c < deal_rem) starting at unit c * deal_base + min(c, deal_rem); a unit is one row
+                         // (of each matrix when paired) or one rotary pair. No division on the device: cta_rows sits
+                         // on every role's start-up path.
   int32_t xkind;
   int32_t x_from_dyn;    // X_ROWS: source rows are the caller's hidden_feats
   const float* xsrc;     // X_ROWS: fp32 rows
@@ -126,22 +130,18 @@ struct RowRange {  // the CTA's share of the group's rows, as a list of "virtual
   int64_t g0;      // linearised: first global row
 };
 
-__device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int nct) {
+__device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int /*nct*/) {
   RowRange r;
+  const int32_t u0 = c * G.deal_base + min(c, G.deal_rem), un = G.deal_base + (c < G.deal_rem ? 1 : 0);
   if (G.paired) {
-    r.n0 = static_cast<int32_t>(static_cast<int64_t>(c) * G.rows[0] / nct);
-    const int32_t n1 = static_cast<int32_t>(static_cast<int64_t>(c + 1) * G.rows[0] / nct);
-    r.cr = n1 - r.n0;
-    r.cnt = r.cr * G.n_mat;
+    r.n0 = u0;
+    r.cr = un;
+    r.cnt = un * G.n_mat;
     r.g0 = 0;
   } else {
-    int64_t tot = 0;
-    for (int j = 0; j < G.n_mat; ++j) tot += G.rows[j];
-    const int64_t unit = G.pairperm ? 2 : 1;  // deal whole rotary pairs
-    tot /= unit;
-    r.g0 = static_cast<int64_t>(c) * tot / nct * unit;
-    const int64_t g1 = static_cast<int64_t>(c + 1) * tot / nct * unit;
-    r.cnt = static_cast<int32_t>(g1 - r.g0);
+    const int32_t unit = G.pairperm ? 2 : 1;  // whole rotary pairs
+    r.g0 = static_cast<int64_t>(u0) * unit;
+    r.cnt = un * unit;
     r.n0 = 0;
     r.cr = 0;
   }
@@ -152,12 +152,12 @@ __device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int nct)
 __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& rr, int v, int& j,
                                            int& n) {
   if (G.paired) {
-    j = v / rr.cr;
+    j = (v >= rr.cr ? 1 : 0) + (v >= 2 * rr.cr ? 1 : 0);  // n_mat <= 3
     n = rr.n0 + (v - j * rr.cr);
   } else {
-    int64_t g = rr.g0 + v;
-    if (G.pairperm) {  // virtual (0, 1, 2, 3, ...) of a head = rows (0, dh/2, 1, dh/2 + 1, ...)
-      const int64_t w = g % G.pairperm;
+    int32_t g = static_cast<int32_t>(rr.g0) + v;
+    if (G.pairperm) {  // virtual (0, 1, 2, 3, ...) of a head = rows (0, dh/2, 1, dh/2 + 1, ...); dh is a power of two
+      const int32_t w = g & (G.pairperm - 1);
       g = g - w + (w >> 1) + (w & 1) * (G.pairperm >> 1);
     }
     j = 0;
@@ -169,7 +169,7 @@ __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& r
         j = 2;
       }
     }
-    n = static_cast<int32_t>(g);
+    n = g;
   }
 }
 
@@ -270,7 +270,8 @@ __device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGro
       const int m = idx / n_pairs, t = idx - m * n_pairs;
       const int mm = mbase + m;
       const int64_t g = rr.g0 + 2 * t;
-      const int hh = static_cast<int>(g / DH), i = static_cast<int>(g % DH) >> 1;
+      const int dsh = DH == 128 ? 7 : 6;  // head_dim is 64 or 128
+      const int hh = static_cast<int>(g >> dsh), i = static_cast<int>(g & (DH - 1)) >> 1;
       const float a = res(2 * t, m), b = res(2 * t + 1, m);  // elements i and i + dh/2 of head hh
       if (hh < p.Hq + p.Hkv) {
         const float2 cs = p.rope[static_cast<size_t>(p.rope_row0 + (p.rope_per_row ? mm : 0)) * HALF + i];

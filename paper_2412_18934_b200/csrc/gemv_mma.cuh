@@ -95,17 +95,18 @@ __device__ __forceinline__ void super_blocks(int cnt, int RS, int& n_sb, int& rs
   rsb = n_sb > 0 ? (cnt + n_sb - 1) / n_sb : 0;
 }
 
-// Which rows this CTA works on: group g, index c within the group's CTAs (or c < 0: idle). The integer divisions
-// behind it (64-bit ones in cta_rows) are a dependent chain of about a microsecond, so every role computes it
-// BEFORE griddepcontrol.wait (it depends on the launch arguments only) and pins the results there: measured,
-// the consumers otherwise spend it after the wait, with the ring full and the HBM stream stopped.
+// Which rows this CTA works on: group g, index c within the group's CTAs (or c < 0: idle). Every role computes
+// it BEFORE griddepcontrol.wait (it depends on the launch arguments only) and pins the results there. Measured:
+// with 64-bit divisions in cta_rows this was a dependent chain of more than a microsecond that the consumers
+// spent after the wait (ring full, HBM stream stopped) and the weight producers before their first copy; the
+// host now supplies the quotients (GemvGroup::deal_base / deal_rem).
 struct CtaGeom {
   int c, g, n_sb, rsb;
   RowRange rr;
 };
 __device__ __forceinline__ CtaGeom cta_geom(const GemvParams& p, int c_grid) {
   CtaGeom q;
-  q.g = c_grid / p.ctas_per_group;
+  q.g = c_grid >= p.ctas_per_group ? 1 : 0;  // at most two groups
   q.c = c_grid - q.g * p.ctas_per_group;
   if (q.g >= p.n_groups) { q.g = 0; q.c = -1; }
   q.n_sb = q.rsb = 0;
@@ -164,15 +165,13 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
 
   trace_begin(p.trace);
   if (tid == 0) DVT_DBG(0);
-  if (tid == 0) {
-    for (int s = 0; s < NS; ++s) {
-      mbar_init(&full_a[s], kMmaProducerWarps);
-      mbar_init(&full_b[s], 1);
-      mbar_init(&empty[s], kConsumerWarps);
-    }
+  if (tid < NS) {
+    mbar_init(&full_a[tid], kMmaProducerWarps);
+    mbar_init(&full_b[tid], 1);
+    mbar_init(&empty[tid], kConsumerWarps);
     mbar_fence_init();
   }
-  if (tid < 4) zero16[tid] = 0u;
+  if (tid >= 32 && tid < 36) zero16[tid - 32] = 0u;
   __syncthreads();
   pdl_launch_dependents();
 
@@ -192,7 +191,7 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
       const int col = lane + 32 * h;
-      cm[h] = col / S;
+      cm[h] = S == 1 ? col : (S == 2 ? col >> 1 : (col * 43) >> 7);  // col / S for col < 64, S <= 3
       const int s = col - cm[h] * S;
       off[h] = s * G.xs_plane + (G.xidx ? 0 : (p.m0 + cm[h]) * G.xs_ld);
     }

@@ -71,19 +71,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
       : "memory");
 }
 
-// ---- kernel parameters: warm the constant cache -------------------------------------------------
-// Kernel parameters live in a constant bank and are fetched lazily, one cache line per first use; every miss is
-// a serial L2 round trip of the warp that takes it (measured on the GEMV: 1.5 - 2 us between griddepcontrol.wait
-// and the first useful instruction of a warp that had not touched its parameters yet). All threads of the CTA
-// read the parameter block once at kernel start, before the wait, so that the lines are resident afterwards.
-template <typename P>
-__device__ __forceinline__ void warm_params(const P& prm) {
-  const uint32_t* w = reinterpret_cast<const uint32_t*>(&prm);
-  uint32_t acc = 0;
-  for (int i = threadIdx.x; i < static_cast<int>(sizeof(P) / 4); i += blockDim.x) acc ^= w[i];
-  asm volatile("" ::"r"(acc));
-}
-
 // ---- programmatic dependent launch -----------------------------------------
 // wait: all memory of the preceding kernels in the stream is visible after it.
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
