@@ -77,6 +77,14 @@ int dovetail_trace_read(dovetail_draft_t* h, int32_t cap, int32_t* kind, int32_t
  * what it computes. Keys are listed here as they are added; an unknown key or a value out of range returns
  * EINVAL. */
 int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
+/* key 1: tree levels (and level-0 row batches) of at least `value` rows run on the tcgen05 GEMV
+ * (csrc/gemv_umma.cuh) instead of the mma.sync GEMV; 1 ... 64, 65 = never. Default 9. bf16 weights only. */
+#define DOVETAIL_TUNE_UMMA_MIN_M 1
+
+/* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.
+ *   key 1: launches of the tcgen05 GEMV (k_gemv_umma). Unknown key or NULL handle: -1. */
+#define DOVETAIL_STAT_UMMA_LAUNCHES 1
+int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key);
 
 /* Read-only HBM streaming ceilings, run by bench.py next to the step: reads `bytes`
  * bytes of `buf` (device, 16-byte aligned, larger than L2) exactly once on cuda_stream.

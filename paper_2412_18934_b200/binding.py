@@ -21,7 +21,7 @@ EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "
            "dovetail_verify_plan", "dovetail_verify_accept", "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
-HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune")
+HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune", "dovetail_hooks_stat")
 
 
 class DovetailError(RuntimeError):
@@ -126,6 +126,8 @@ def load() -> C.CDLL:
                                             C.POINTER(C.c_uint64), C.POINTER(C.c_uint64), C.POINTER(C.c_int32)]
         lib.dovetail_hooks_tune.restype = C.c_int
         lib.dovetail_hooks_tune.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+        lib.dovetail_hooks_stat.restype = C.c_int
+        lib.dovetail_hooks_stat.argtypes = [C.c_void_p, C.c_int32]
         lib.dovetail_probe_stream.restype = C.c_int
         lib.dovetail_probe_stream.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_int32, C.c_int32, C.c_void_p]
         lib.dovetail_last_launch_count.restype = C.c_int
@@ -392,8 +394,18 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
     return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
 
 
+TUNE_UMMA_MIN_M = 1
+STAT_UMMA_LAUNCHES = 1
+
+
+def dovetail_hooks_stat(h: Draft, key: int) -> int:
+    """Counters of the last step (include/dovetail_hooks.h): key 1 = launches of the tcgen05 GEMV."""
+    return load().dovetail_hooks_stat(h.ptr, key)
+
+
 def dovetail_hooks_tune(h: Draft, key: int, value: int):
-    """Design knobs for A/B measurements (include/dovetail_hooks.h): key 0 = GEMVs per persistent launch."""
+    """Design knobs for A/B measurements (include/dovetail_hooks.h): key 1 = rows from which a level runs on the
+    tcgen05 GEMV (65: never)."""
     _check(load().dovetail_hooks_tune(h.ptr, key, value), h.ptr)
 
 

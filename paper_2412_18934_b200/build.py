@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libdovetail_draft.so")
 SOURCES = ["dovetail_draft.cu"]
-HEADERS = ["ptx.cuh", "state.cuh", "gemv.cuh", "gemv_mma.cuh", "attention.cuh", "attention_mma.cuh", "tree.cuh", "stream_probe.cuh", "verify.cuh", "epilogue.cuh"]
+HEADERS = ["ptx.cuh", "state.cuh", "gemv.cuh", "gemv_mma.cuh", "attention.cuh", "attention_mma.cuh", "tree.cuh", "stream_probe.cuh", "verify.cuh", "epilogue.cuh", "umma.cuh", "gemv_umma.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

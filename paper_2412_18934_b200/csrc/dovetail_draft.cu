@@ -3,14 +3,17 @@
 // enqueues the kernels of one draft step on the caller's
 // stream; every step of the method runs in the kernels of gemv.cuh,
 // attention.cuh and tree.cuh. There is no CPU fallback.
+#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <new>
 #include <vector>
 
@@ -20,6 +23,7 @@
 #include "attention_mma.cuh"
 #include "gemv.cuh"
 #include "gemv_mma.cuh"
+#include "gemv_umma.cuh"
 #include "state.cuh"
 #include "stream_probe.cuh"
 #include "tree.cuh"
@@ -83,10 +87,21 @@ struct dovetail_draft {
   int last_n_new = 0, last_depth = 0, last_gamma = 0;
   int last_launches = 0;
   int launches = 0;
+  int umma_launches = 0, last_umma_launches = 0;
   bool dry = false;  // shape-checking pass of dovetail_draft_step: nothing is launched
   // GEMVs queued by run_gemv, launched by flush_gemv
   struct QueuedGemv { GemvParams p; int n_groups, ctas, kind, max_cnt; int64_t bytes; };
   std::vector<QueuedGemv> queue;
+  // tcgen05 GEMV (gemv_umma.cuh): tensor maps of the weight matrices and activation planes (four box depths
+  // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
+  int umma_min_m = 9;               // levels of at least this many rows take the tcgen05 kernel (65: never)
+  CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
+  std::map<const void*, int> wmap_of;  // weight matrix -> first map index
+  struct PlaneBuf { const __nv_bfloat16* base; int64_t elems, ld; int cap, map; };
+  std::vector<PlaneBuf> plane_bufs;
+  struct UmmaTable { UmmaCtaTab* tab = nullptr; uint16_t* vpos = nullptr; int vpos_ld = 0, g_max = 0, g_min = 0; bool ok = false; };
+  std::map<std::array<int, 8>, UmmaTable> umma_tabs;
+  __nv_bfloat16* xs_par = nullptr;  // [3][max_rows][ld_d] parent hidden states of a wide level, gathered
 #ifdef DVT_CHAINDBG
   unsigned long long* dbg = nullptr;
   int dbg_launch = 0;
@@ -218,6 +233,7 @@ cudaError_t set_max_smem_all() {
   };
   for (int nt = 1; nt <= 8; nt *= 2)
     for (int wq = 0; wq < 2; ++wq) set(reinterpret_cast<const void*>(pick_gemv_mma(nt, wq)));
+  set(reinterpret_cast<const void*>(k_gemv_umma));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<64>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<128>));
   const int mts[3] = {1, 2, 4};
@@ -328,6 +344,252 @@ MmaGeom mma_geom(const dovetail_draft::QueuedGemv& q, int wq) {
   return best;
 }
 
+
+// ---- tcgen05 GEMV (gemv_umma.cuh): tensor maps, row tables, launch geometry --------------------------------
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// The library links only the CUDA runtime; the driver's tensor-map encoder is fetched through it.
+EncodeTiledFn tensor_map_encoder() {
+  void* f = nullptr;
+  cudaDriverEntryPointQueryResult q;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+      q != cudaDriverEntryPointSuccess)
+    return nullptr;
+  return reinterpret_cast<EncodeTiledFn>(f);
+}
+
+// Four maps (boxes of 1, 2, 4, 8 slabs) of a bf16 matrix [rows][ld], ld a multiple of 64: dimensions (k within a
+// 64-element slab, row, slab) with strides (2 ld, 128) bytes, box (64, 8, nslab), 128-byte swizzle: one copy
+// lands as nslab swizzle atoms [slab][8 rows][128 B] (gemv_umma.cuh).
+bool encode_maps(EncodeTiledFn enc, const void* base, int64_t rows, int64_t ld, std::vector<CUtensorMap>& out) {
+  for (int i = 0; i < 4; ++i) {
+    CUtensorMap m;
+    memset(&m, 0, sizeof m);
+    const int nslab = 1 << i;
+    if ((ld / 64) % nslab == 0) {
+      const cuuint64_t dims[3] = {64, static_cast<cuuint64_t>(rows), static_cast<cuuint64_t>(ld / 64)};
+      const cuuint64_t strides[2] = {static_cast<cuuint64_t>(ld) * 2, 128};
+      const cuuint32_t box[3] = {64, 8, static_cast<cuuint32_t>(nslab)};
+      const cuuint32_t es[3] = {1, 1, 1};
+      if (enc(&m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    }
+    out.push_back(m);
+  }
+  return true;
+}
+
+// Called once by dovetail_draft_init (bf16 weights). On any failure the tcgen05 path stays off and every level
+// runs on k_gemv_mma.
+void umma_init(dovetail_draft* h) {
+  h->umma_min_m = kUmmaMaxM + 1;
+  EncodeTiledFn enc = tensor_map_encoder();
+  if (!enc) return;
+  const dovetail_config_t& c = h->cfg;
+  std::vector<CUtensorMap> maps;
+  bool ok = true;
+  auto add_w = [&](const void* w, int rows, int K) {
+    if (!w || K % 64 != 0 || h->wmap_of.count(w)) return;
+    h->wmap_of[w] = static_cast<int>(maps.size());
+    ok = ok && encode_maps(enc, w, rows, K, maps);
+  };
+  const int d = c.hidden;
+  add_w(h->w.dgf_w1, d, d);
+  add_w(h->w.dgf_w2, d, d);
+  add_w(h->w.dgf_wg, d, 2 * d);
+  add_w(h->w.lm_head, c.vocab, d);
+  for (const dovetail_layer_weights_t& L : h->layers) {
+    add_w(L.wq, h->dq, d); add_w(L.wk, h->dkv, d); add_w(L.wv, h->dkv, d); add_w(L.wo, d, h->dq);
+    add_w(L.wgate, c.ffn, d); add_w(L.wup, c.ffn, d); add_w(L.wdown, d, c.ffn);
+  }
+  auto add_x = [&](const __nv_bfloat16* xs, int cap, int ld) {
+    if (!xs || ld % 64 != 0) return;
+    dovetail_draft::PlaneBuf b{xs, static_cast<int64_t>(kSplitPlanes) * cap * ld, ld, cap, static_cast<int>(maps.size())};
+    ok = ok && encode_maps(enc, xs, static_cast<int64_t>(kSplitPlanes) * cap, ld, maps);
+    h->plane_bufs.push_back(b);
+  };
+  const int R = c.max_rows;
+  add_x(h->xs_feat, R, h->ld_d); add_x(h->xs_hhat, h->max_step_rows, h->ld_d); add_x(h->xs_x, R, h->ld_d);
+  add_x(h->xs_h12, R, h->ld_2d); add_x(h->xs_o, R, h->ld_dq); add_x(h->xs_act, R, h->ld_f);
+  add_x(h->xs_emb, R, h->ld_d); add_x(h->xs_par, R, h->ld_d);
+  if (!ok || maps.empty()) return;
+  if (cudaMalloc(reinterpret_cast<void**>(&h->maps_dev), maps.size() * sizeof(CUtensorMap)) != cudaSuccess) { cudaGetLastError(); return; }
+  if (cudaMemcpy(h->maps_dev, maps.data(), maps.size() * sizeof(CUtensorMap), cudaMemcpyHostToDevice) != cudaSuccess) { cudaGetLastError(); return; }
+  h->umma_min_m = 9;
+}
+
+// Row tables of one dealing (gemv_umma.cuh UmmaCtaTab): the CTA's virtual rows sorted into contiguous memory
+// segments, each cut into 8-row boxes; boxes dealt to balanced super-blocks of <= 16 boxes.
+const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& G, int ctas) {
+  const std::array<int, 8> key = {G.rows[0], G.n_mat > 1 ? G.rows[1] : 0, G.n_mat > 2 ? G.rows[2] : 0, G.n_mat, G.paired,
+                                  G.pairperm, ctas, G.deal_base};
+  auto it = h->umma_tabs.find(key);
+  if (it != h->umma_tabs.end()) return it->second;
+  dovetail_draft::UmmaTable t;
+  int max_cnt = 0;
+  for (int c = 0; c < ctas; ++c) max_cnt = std::max(max_cnt, static_cast<int>(cta_rows(G, c, ctas).cnt));
+  t.vpos_ld = (max_cnt + 7) / 8 * 8;
+  std::vector<UmmaCtaTab> tabs(ctas);
+  std::vector<uint16_t> vpos(static_cast<size_t>(ctas) * std::max(1, t.vpos_ld), 0);
+  bool ok = max_cnt > 0;
+  t.g_max = 0;
+  t.g_min = kUmmaMaxGroups;
+  for (int c = 0; c < ctas && ok; ++c) {
+    const RowRange rr = cta_rows(G, c, ctas);
+    UmmaCtaTab& T = tabs[c];
+    memset(&T, 0, sizeof T);
+    if (rr.cnt == 0) continue;
+    std::vector<std::array<int, 3>> rows(rr.cnt);
+    for (int v = 0; v < rr.cnt; ++v) {
+      int j, n;
+      locate_row(G, rr, v, j, n);
+      rows[v] = {j, n, v};
+    }
+    std::sort(rows.begin(), rows.end());
+    std::vector<int> gcode;
+    std::vector<std::pair<int, int>> pos(rr.cnt);
+    for (int i = 0; i < rr.cnt;) {
+      int e = i + 1;
+      while (e < rr.cnt && rows[e][0] == rows[i][0] && rows[e][1] == rows[e - 1][1] + 1) ++e;
+      for (int off = i; off < e; off += 8) {
+        const int g = static_cast<int>(gcode.size());
+        gcode.push_back((rows[off][0] << 28) | rows[off][1]);
+        for (int r = 0; r < 8 && off + r < e; ++r) pos[rows[off + r][2]] = {g, r};
+      }
+      i = e;
+    }
+    const int Gt = static_cast<int>(gcode.size());
+    const int n_sb = div_up(Gt, kUmmaMaxGroups), per = div_up(Gt, n_sb);
+    if (n_sb > kUmmaMaxSb) { ok = false; break; }
+    T.n_sb = n_sb;
+    for (int g = 0; g < Gt; ++g) {
+      T.grp[g / per][g % per] = gcode[g];
+      T.n_grp[g / per] = g % per + 1;
+    }
+    for (int sb = 0; sb < n_sb; ++sb) { t.g_max = std::max(t.g_max, T.n_grp[sb]); t.g_min = std::min(t.g_min, T.n_grp[sb]); }
+    for (int v = 0; v < rr.cnt; ++v)
+      vpos[static_cast<size_t>(c) * t.vpos_ld + v] = static_cast<uint16_t>((pos[v].first / per) * 128 + (pos[v].first % per) * 8 + pos[v].second);
+  }
+  if (ok) {
+    ok = cudaMalloc(reinterpret_cast<void**>(&t.tab), tabs.size() * sizeof(UmmaCtaTab)) == cudaSuccess &&
+         cudaMalloc(reinterpret_cast<void**>(&t.vpos), vpos.size() * sizeof(uint16_t)) == cudaSuccess &&
+         cudaMemcpy(t.tab, tabs.data(), tabs.size() * sizeof(UmmaCtaTab), cudaMemcpyHostToDevice) == cudaSuccess &&
+         cudaMemcpy(t.vpos, vpos.data(), vpos.size() * sizeof(uint16_t), cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) cudaGetLastError();
+  }
+  t.ok = ok;
+  return h->umma_tabs.emplace(key, t).first->second;
+}
+
+struct UmmaGeom {
+  bool ok;
+  int nslab, n_stages, stage_bytes, b_groups, umma_m, tmem_cols, acc_cols, cnt_pad, ring_bytes, smem;
+};
+
+// Ring of one launch: the deepest K-chunk (64 * nslab elements) that leaves >= 3 stages or >= 120 KB in flight.
+UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
+  UmmaGeom u{};
+  const int M8 = (M + 7) / 8 * 8;
+  u.acc_cols = (s_max * M8 + 15) / 16 * 16;
+  u.b_groups = u.acc_cols / 8;
+  u.umma_m = g_max <= 8 ? 64 : 128;
+  u.tmem_cols = 32;
+  while (u.tmem_cols < 2 * u.acc_cols) u.tmem_cols *= 2;
+  u.cnt_pad = (max_cnt + 3) / 4 * 4;
+  const int tail = 2544 + M * u.cnt_pad * 4;  // barriers, 1 / rms, row map, results (gemv_umma.cuh)
+  UmmaGeom best{};
+  for (int nslab = 8; nslab >= 1; nslab >>= 1) {
+    if (K % (64 * nslab) != 0) continue;
+    UmmaGeom g = u;
+    const int gb = nslab * 1024;
+    g.nslab = nslab;
+    g.stage_bytes = (g.b_groups + g_max) * gb;
+    const int pad = (g.umma_m / 8 - g_max) * gb;  // the tensor core reads whole tiles: past the last stage's rows
+    g.n_stages = std::min(8, (kSmemMax - 1024 - tail - pad) / g.stage_bytes);
+    if (g.n_stages < 2) continue;
+    g.ring_bytes = g.n_stages * g.stage_bytes + pad;
+    g.smem = 1024 + g.ring_bytes + tail;
+    g.ok = true;
+    if (g.n_stages >= 3 || g.n_stages * g.stage_bytes >= 120 * 1024) return g;
+    if (!best.ok || g.n_stages * g.stage_bytes > best.n_stages * best.stage_bytes) best = g;
+  }
+  return best;
+}
+
+// Launches q on k_gemv_umma (in row chunks when the result buffer of a whole level does not fit). *done = false:
+// the GEMV does not fit the tcgen05 kernel and nothing was launched.
+int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, bool* done) {
+  *done = false;
+  GemvParams& p = q.p;
+  if (p.K % 64 != 0 || !h->maps_dev) return DOVETAIL_OK;
+  UmmaParams up{};
+  int s_max = 1, g_max = 0;
+  for (int gi = 0; gi < q.n_groups; ++gi) {
+    GemvGroup& G = p.g[gi];
+    if (G.xkind != X_ROWS || G.xidx != nullptr || !G.xs) return DOVETAIL_OK;
+    G.S = G.S_fixed ? G.S_fixed : 2;
+    s_max = std::max(s_max, G.S);
+    const dovetail_draft::PlaneBuf* pb = nullptr;
+    for (const auto& b : h->plane_bufs)
+      if (G.xs >= b.base && G.xs < b.base + b.elems) pb = &b;
+    if (!pb || pb->ld != G.xs_ld || G.xs_plane != static_cast<int64_t>(pb->cap) * pb->ld || pb->ld != p.K) return DOVETAIL_OK;
+    up.x_cap[gi] = pb->cap;
+    up.x_row0[gi] = static_cast<int32_t>((G.xs - pb->base) / pb->ld);
+    up.xmap[gi] = h->maps_dev + pb->map;  // + box depth below
+    for (int j = 0; j < G.n_mat; ++j) {
+      auto it = h->wmap_of.find(G.w[j]);
+      if (it == h->wmap_of.end()) return DOVETAIL_OK;
+      up.wmap[gi][j] = h->maps_dev + it->second;
+    }
+    const dovetail_draft::UmmaTable& T = umma_table(h, G, q.ctas);
+    if (!T.ok) return DOVETAIL_OK;
+    up.tab[gi] = T.tab;
+    up.vpos[gi] = T.vpos;
+    if (gi > 0 && T.vpos_ld != up.vpos_ld) return DOVETAIL_OK;  // groups of one launch share the dealing shape
+    up.vpos_ld = T.vpos_ld;
+    g_max = std::max(g_max, T.g_max);
+  }
+  const int Mtot = p.M;
+  int Mc = Mtot;
+  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+  while (!g.ok && Mc > 8) {
+    Mc = (Mc / 2 + 7) / 8 * 8;
+    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+  }
+  if (!g.ok) return DOVETAIL_OK;
+  int lg = 0;
+  while ((1 << lg) < g.nslab) ++lg;
+  for (int gi = 0; gi < q.n_groups; ++gi) {
+    up.xmap[gi] += lg;
+    for (int j = 0; j < p.g[gi].n_mat; ++j) up.wmap[gi][j] += lg;
+  }
+  up.nslab = g.nslab; up.n_stages = g.n_stages; up.stage_bytes = g.stage_bytes; up.b_groups = g.b_groups;
+  up.umma_m = g.umma_m; up.tmem_cols = g.tmem_cols; up.acc_cols = g.acc_cols; up.cnt_pad = g.cnt_pad;
+  up.ring_bytes = g.ring_bytes;
+  p.n_groups = q.n_groups;
+  p.ctas_per_group = q.ctas;
+  p.row_bytes = p.K * 2;
+  h->cur_kind = q.kind;
+  *done = true;
+  for (int m0 = 0; m0 < Mtot; m0 += Mc) {
+    p.M = std::min(Mc, Mtot - m0);
+    p.m0 = m0;
+    h->cur_bytes = m0 == 0 ? q.bytes : 0;  // the algorithmic bytes are counted once
+    p.trace = trace_slot(h);
+    up.p = p;
+    if (!h->dry) ++h->umma_launches;
+    cudaError_t e = launch(h, k_gemv_umma, dim3(q.n_groups * q.ctas), dim3(kUmmaThreads), g.smem, st, up);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (tcgen05) launch failed: %s", cudaGetErrorString(e));
+  }
+  p.M = Mtot;
+  p.m0 = 0;
+  return DOVETAIL_OK;
+}
+
 // One GEMV on the FMA kernel (fp32 models; bf16 matrices whose K is not a multiple of 32).
 int run_gemv_fma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q) {
   GemvParams& p = q.p;
@@ -385,6 +647,11 @@ int flush_gemv(dovetail_draft* h, cudaStream_t st) {
   auto& Q = h->queue;
   int rc = DOVETAIL_OK;
   for (size_t i = 0; i < Q.size() && rc == DOVETAIL_OK; ++i) {
+    if (h->es == 2 && !h->wq && Q[i].p.M >= h->umma_min_m && Q[i].p.M <= kUmmaMaxM) {  // wide level: tcgen05 consumer
+      bool done = false;
+      rc = run_umma(h, st, Q[i], &done);
+      if (done || rc != DOVETAIL_OK) continue;
+    }
     const MmaGeom g = h->es == 2 ? mma_geom(Q[i], h->wq) : MmaGeom{};
     if (g.ok) {
       rc = run_mma(h, st, Q[i], g);
@@ -518,6 +785,9 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->ssq);
   cudaFree(h->qs);
   cudaFree(h->xs_emb);
+  cudaFree(h->xs_par);
+  cudaFree(h->maps_dev);
+  for (auto& kv : h->umma_tabs) { cudaFree(kv.second.tab); cudaFree(kv.second.vpos); }
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
   cudaFree(h->pool.token); cudaFree(h->pool.parent); cudaFree(h->pool.depth); cudaFree(h->pool.cum);
   cudaFree(h->pool.row); cudaFree(h->treemask); cudaFree(h->out_pool_idx);
@@ -567,6 +837,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   const int L = kv->committed_len, Lp = L + n_new;
   int rc = DOVETAIL_OK;
   h->launches = 0;
+  h->umma_launches = 0;
   const int d = c.hidden, F = c.ffn, V = c.vocab, dh = c.head_dim, half = dh / 2;
   const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
   const int grp = c.n_q_heads / c.n_kv_heads;
@@ -631,10 +902,25 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
                  static_cast<const __nv_bfloat16*>(h->w.embed), d, planes(h, h->xs_emb, R, h->ld_d), trace_slot(h));
       if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
     }
+    // wide level on the tcgen05 GEMV (gemv_umma.cuh): its tensor-map copies read contiguous rows, so the parents'
+    // hidden states and the tokens' embedding rows are gathered first
+    const bool wide = bf16 && !h->wq && h->maps_dev && M >= h->umma_min_m && M <= kUmmaMaxM && d % 64 == 0;
+    if (c.dgf_proj && wide) {
+      rc = flush_gemv(h, st);
+      if (rc) return rc;
+      h->cur_kind = 10;
+      h->cur_bytes = 0;
+      e = launch(h, k_gather_level, dim3(M, kSplitPlanes + 1), dim3(256), 0, st, static_cast<const RowTables*>(cur),
+                 static_cast<const __nv_bfloat16*>(l == 0 ? nullptr : h->xs_hhat), static_cast<int64_t>(SR) * h->ld_d, h->xs_par,
+                 static_cast<int64_t>(R) * h->ld_d, static_cast<const __nv_bfloat16*>(h->w.embed), h->xs_emb,
+                 static_cast<int64_t>(h->ld_d), d, trace_slot(h));
+      if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "launch failed: %s", cudaGetErrorString(e));
+    }
     if (c.dgf_proj) {
       GemvParams p{};
-      p.g[0] = rows_group(h->hhat, d, l == 0 ? nullptr : cur->src, l == 0, nullptr);
-      with_planes(p.g[0], l == 0 ? planes(h, h->xs_feat, R, h->ld_d) : planes(h, h->xs_hhat, SR, h->ld_d));
+      p.g[0] = rows_group(h->hhat, d, (l == 0 || wide) ? nullptr : cur->src, l == 0, nullptr);
+      with_planes(p.g[0], l == 0 ? planes(h, h->xs_feat, R, h->ld_d)
+                                 : (wide ? planes(h, h->xs_par, R, h->ld_d) : planes(h, h->xs_hhat, SR, h->ld_d)));
       p.g[0].w[0] = h->w.dgf_w1;
       p.g[0].ws[0] = h->w.dgf_s1;
       p.g[0].rows[0] = d;
@@ -651,6 +937,10 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         p.g[1].xkind = X_ROWS;
         with_planes(p.g[1], planes(h, h->xs_emb, R, h->ld_d));
         p.g[1].S_fixed = 2;  // bf16 value = two fp16 terms exactly
+      } else if (wide) {  // the gathered embedding rows: one exact bf16 plane
+        p.g[1].xkind = X_ROWS;
+        with_planes(p.g[1], planes(h, h->xs_emb, R, h->ld_d));
+        p.g[1].S_fixed = 1;
       }
       p.g[1].n_mat = 1;
       p.g[1].out_off = d;
@@ -1023,7 +1313,8 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->xs_act, kSplitPlanes * R * h->ld_f));
     A(dmalloc(&h->ssq, static_cast<size_t>(h->num_sms) * kMaxRows));
     A(dmalloc(&h->qs, static_cast<size_t>(2) * kMaxRows * dq));
-    if (c.weight_quant) A(dmalloc(&h->xs_emb, kSplitPlanes * R * h->ld_d));
+    A(dmalloc(&h->xs_emb, kSplitPlanes * R * h->ld_d));
+    if (!c.weight_quant) A(dmalloc(&h->xs_par, kSplitPlanes * R * h->ld_d));
   }
   A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));
@@ -1055,6 +1346,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     delete h;
     return code;
   }
+  if (es == 2 && !c.weight_quant) umma_init(h);
   *out = h;
   return DOVETAIL_OK;
 }
@@ -1094,6 +1386,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
   h->last_depth = tree->depth;
   h->last_gamma = tree->gamma;
   h->last_launches = h->launches;
+  h->last_umma_launches = h->umma_launches;
   return DOVETAIL_OK;
 }
 
@@ -1277,8 +1570,19 @@ int dovetail_hooks_set(dovetail_draft_t* h, const dovetail_hooks_t* hooks) {
 
 int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
 
+int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
+  if (!h) return -1;
+  if (key == DOVETAIL_STAT_UMMA_LAUNCHES) return h->last_umma_launches;
+  return -1;
+}
+
 int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
   if (!h) return DOVETAIL_EINVAL;
+  if (key == DOVETAIL_TUNE_UMMA_MIN_M && value >= 1 && value <= kUmmaMaxM + 1) {
+    if (!h->maps_dev && value <= kUmmaMaxM) return fail(h, DOVETAIL_EINVAL, "the tcgen05 path is not available for this model");
+    h->umma_min_m = value;
+    return DOVETAIL_OK;
+  }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
 

@@ -130,9 +130,9 @@ struct RowRange {  // the CTA's share of the group's rows, as a list of "virtual
   int64_t g0;      // linearised: first global row
 };
 
-__device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int /*nct*/) {
+__host__ __device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int /*nct*/) {
   RowRange r;
-  const int32_t u0 = c * G.deal_base + min(c, G.deal_rem), un = G.deal_base + (c < G.deal_rem ? 1 : 0);
+  const int32_t u0 = c * G.deal_base + (c < G.deal_rem ? c : G.deal_rem), un = G.deal_base + (c < G.deal_rem ? 1 : 0);
   if (G.paired) {
     r.n0 = u0;
     r.cr = un;
@@ -149,7 +149,7 @@ __device__ __forceinline__ RowRange cta_rows(const GemvGroup& G, int c, int /*nc
 }
 
 // virtual row v -> matrix j, row n within it
-__device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& rr, int v, int& j,
+__host__ __device__ __forceinline__ void locate_row(const GemvGroup& G, const RowRange& rr, int v, int& j,
                                            int& n) {
   if (G.paired) {
     j = (v >= rr.cr ? 1 : 0) + (v >= 2 * rr.cr ? 1 : 0);  // n_mat <= 3

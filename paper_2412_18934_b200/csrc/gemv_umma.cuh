@@ -1,0 +1,272 @@
+// gemv_umma.cuh -- tcgen05 consumer for the weight-streaming GEMV at wide tree levels and level-0 catch-up
+// rows (SURVEY.md 8a S1, S2, S4, S5, S6 at M = 9 ... 64 rows; 8(f4): PAPER.md:94 prompt rows).
+//
+//   Y[m, n] = sum_k X[m, k] * W[n, k]      m < M <= 64 draft rows, W bf16 row-major [N, K], K % 64 == 0
+//
+// Same work split, same activation planes, same fused epilogues as k_gemv_mma (gemv_mma.cuh); what changes is
+// who multiplies. With mma.sync a warp keeps 16 weight rows x 8 columns per instruction in registers and the
+// column tiles of a wide level multiply its instruction count and the re-reads of the activation operand
+// (measured: 0.73 of the copy peak at M = 8, 0.45 at 16, 0.17 at 32). Here the 5th-generation tensor core reads
+// both operands from shared memory and accumulates in tensor memory:
+//   * swap-AB as before: the CTA's weight rows are the M side of tcgen05.mma (UMMA M = 64 or 128 tile rows), the
+//     draft rows' split-bf16 planes are the N side (N = S * ceil8(M) columns, a multiple of 16), fp32
+//     accumulators in TMEM, one column per (plane, draft row); the S planes of a row are added in the epilogue;
+//   * both operands arrive by tensor-map bulk copies (cp.async.bulk.tensor, 128-byte swizzle): a box is 8 rows
+//     x 64 k x nslab slabs, described by a 3-D map (k within slab, row, slab) so that one copy lands as nslab
+//     swizzle atoms [slab][8 rows][128 B]. The CTA's rows stay row-exact: its virtual rows (gemv.cuh cta_rows /
+//     locate_row) are grouped by the host into contiguous memory segments, each covered by 8-row boxes that
+//     start at the segment's first row (a box may overhang into rows of a neighbour CTA: they are multiplied
+//     and never read back; HBM still sees every row once, the overhang is an L2 hit);
+//   * a stage of the ring = [activation groups][weight groups] of one K-chunk (64 * nslab elements); 8-row
+//     groups are nslab KB apart (the descriptor's stride byte offset), a step of 16 k is +32 bytes;
+//   * one thread issues the MMAs of a stage and commits them to the stage's "empty" barrier; after the last
+//     chunk of a super-block (<= UMMA M tile rows) it commits to "tmem_full". Accumulators are double
+//     buffered so that the next super-block's MMAs run under this one's drain;
+//   * the 8 consumer warps only drain TMEM (tcgen05.ld, sum of the planes, 1 / rms) into the result buffer
+//     and run the fused epilogue of gemv.cuh over it.
+#pragma once
+#include <cuda_bf16.h>
+
+#include "gemv.cuh"
+#include "gemv_mma.cuh"
+#include "ptx.cuh"
+#include "state.cuh"
+#include "umma.cuh"
+
+namespace dvt {
+
+constexpr int kUmmaMaxSb = 8;       // super-blocks per CTA (LM head of a 128k vocabulary: 867 rows)
+constexpr int kUmmaMaxGroups = 16;  // 8-row groups per super-block: UMMA M = 128
+constexpr int kUmmaMaxM = 64;
+// warps: 8 consumers (TMEM drain + epilogue), weight producer, activation producer, MMA issuer
+constexpr int kUmmaThreads = kConsumerThreads + 3 * 32;
+
+// Built by the host for every CTA of a dealing (dovetail_draft.cu umma_tables): the 8-row boxes of each
+// super-block. grp = (matrix j << 28) | first row of the box within w[j].
+struct UmmaCtaTab {
+  int32_t n_sb;
+  int32_t n_grp[kUmmaMaxSb];
+  int32_t grp[kUmmaMaxSb][kUmmaMaxGroups];
+};
+
+struct UmmaParams {
+  GemvParams p;
+  const CUtensorMap* wmap[2][3];  // weight matrices of each group: 3-D maps with nslab slabs per box
+  const CUtensorMap* xmap[2];     // activation planes of each group (plane s = rows [s * x_cap, (s + 1) * x_cap))
+  int32_t x_cap[2], x_row0[2];
+  const UmmaCtaTab* tab[2];
+  const uint16_t* vpos[2];        // [ctas][vpos_ld]: super-block * 128 + tile row of every virtual row
+  int32_t vpos_ld;
+  int32_t nslab, n_stages, stage_bytes;
+  int32_t b_groups;               // 8-row groups reserved for the activation part of a stage
+  int32_t umma_m;                 // 64 or 128
+  int32_t tmem_cols, acc_cols;    // allocation (2 accumulators) and columns of one accumulator
+  int32_t cnt_pad;                // row stride of the result buffer res[m][v]
+  int32_t ring_bytes;             // ring + the pad the tensor core may read past the last stage
+};
+
+__global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_constant__ UmmaParams cp) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~static_cast<uintptr_t>(1023));
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const GemvParams& p = cp.p;
+  const int NS = cp.n_stages, nslab = cp.nslab;
+  const uint32_t GB = static_cast<uint32_t>(nslab) * 1024u;  // bytes of one 8-row group of a stage
+
+  uint8_t* ring = smem;
+  uint64_t* full_a = reinterpret_cast<uint64_t*>(smem + cp.ring_bytes);
+  uint64_t* full_b = full_a + 8;
+  uint64_t* empty = full_b + 8;
+  uint64_t* tm_full = empty + 8;   // [2]
+  uint64_t* tm_empty = tm_full + 2;  // [2]
+  uint32_t* tslot = reinterpret_cast<uint32_t*>(tm_empty + 2);
+  float* rstd_s = reinterpret_cast<float*>(tslot + 4);                // [kUmmaMaxM]
+  int16_t* rmap = reinterpret_cast<int16_t*>(rstd_s + kUmmaMaxM);     // [kUmmaMaxSb][128]: virtual row of a tile row, or -1
+  float* res = reinterpret_cast<float*>(rmap + kUmmaMaxSb * 128);     // [M][cnt_pad]
+
+  trace_begin(p.trace);
+  if (tid < NS) {
+    mbar_init(&full_a[tid], 1);
+    mbar_init(&full_b[tid], 1);
+    mbar_init(&empty[tid], 1);
+  }
+  if (tid >= 32 && tid < 34) {
+    mbar_init(&tm_full[tid - 32], 1);
+    mbar_init(&tm_empty[tid - 32], kConsumerWarps);
+  }
+  if (tid < 64) mbar_fence_init();
+  if (warp == kConsumerWarps + 2) tmem_alloc(tslot, static_cast<uint32_t>(cp.tmem_cols));
+  for (int i = tid; i < kUmmaMaxSb * 128; i += kUmmaThreads) rmap[i] = -1;
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  pdl_launch_dependents();
+  const uint32_t tmem = *tslot;
+
+  const CtaGeom q = cta_geom(p, blockIdx.x);
+  const int c = q.c, gi = q.g;
+  const GemvGroup& G = p.g[gi];
+  const RowRange rr = q.rr;
+  const int M = p.M, S = G.S, M8 = (M + 7) & ~7;
+  const int nB = S * (M8 >> 3);             // activation groups really loaded
+  const int N = (S * M8 + 15) & ~15;        // UMMA N
+  const int n_chunks = p.K / (64 * nslab);
+  const UmmaCtaTab* tab = c >= 0 ? cp.tab[gi] + c : nullptr;
+
+  if (warp == kConsumerWarps) {
+    // ---------------- weight producer: one box per lane and stage; never waits for the previous kernel -------
+    if (c >= 0) {
+      const uint64_t pol = l2_policy_evict_first();
+      const int n_sb = tab->n_sb;
+      int slot = 0, round = 0;
+      for (int sb = 0; sb < n_sb; ++sb) {
+        const int ng = tab->n_grp[sb];
+        const int gr = lane < ng ? tab->grp[sb][lane] : 0;
+        const CUtensorMap* map = cp.wmap[gi][gr >> 28];
+        const int row = gr & 0x0fffffff;
+        for (int ch = 0; ch < n_chunks; ++ch) {
+          if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+          if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(ng) * GB);
+          __syncwarp();
+          if (lane < ng)
+            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + (static_cast<uint32_t>(cp.b_groups) + lane) * GB, map,
+                        0, row, ch * nslab, &full_a[slot], pol);
+          if (++slot == NS) { slot = 0; ++round; }
+        }
+      }
+    }
+  } else if (warp == kConsumerWarps + 1) {
+    // ---------------- activation producer: planes left by the previous kernels (L2) ---------------------------
+    pdl_wait();
+    if (c >= 0) {
+      const uint64_t pol = l2_policy_evict_last();
+      const int n_sb = tab->n_sb;
+      const CUtensorMap* map = cp.xmap[gi];
+      const int mg = M8 >> 3;
+      const int s = lane / mg, g8 = lane - s * mg;  // lane < nB <= 24: plane s, rows [8 g8, 8 g8 + 8) of the level
+      const int row = s * cp.x_cap[gi] + cp.x_row0[gi] + p.m0 + g8 * 8;
+      int slot = 0, round = 0;
+      for (int sb = 0; sb < n_sb; ++sb) {
+        for (int ch = 0; ch < n_chunks; ++ch) {
+          if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
+          if (lane == 0) mbar_arrive_expect_tx(&full_b[slot], static_cast<uint32_t>(nB) * GB);
+          __syncwarp();
+          if (lane < nB)
+            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + static_cast<uint32_t>(lane) * GB, map, 0, row,
+                        ch * nslab, &full_b[slot], pol);
+          if (++slot == NS) { slot = 0; ++round; }
+        }
+      }
+    }
+  } else if (warp == kConsumerWarps + 2) {
+    // ---------------- MMA issuer ---------------------------------------------------------------------------
+    if (c >= 0) {
+      const int n_sb = tab->n_sb;
+      const uint32_t idesc = umma_idesc_bf16(cp.umma_m, N);
+      const uint32_t ring_u = smem_u32(ring);
+      int slot = 0, round = 0;
+      for (int sb = 0; sb < n_sb; ++sb) {
+        const int buf = sb & 1;
+        if (sb >= 2) mbar_wait(&tm_empty[buf], ((sb >> 1) & 1) ^ 1);  // drained by the consumers
+        tc_fence_after();
+        const uint32_t d_addr = tmem + static_cast<uint32_t>(buf * cp.acc_cols);
+        for (int ch = 0; ch < n_chunks; ++ch) {
+          mbar_wait(&full_a[slot], round & 1);
+          mbar_wait(&full_b[slot], round & 1);
+          tc_fence_after();
+          if (lane == 0) {
+            const uint32_t b_base = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
+            const uint32_t a_base = b_base + static_cast<uint32_t>(cp.b_groups) * GB;
+            for (int sl = 0; sl < nslab; ++sl) {
+#pragma unroll
+              for (int k = 0; k < 4; ++k) {
+                const uint32_t off = static_cast<uint32_t>(sl) * 1024u + static_cast<uint32_t>(k) * 32u;
+                umma_bf16(d_addr, umma_desc_sw128(a_base + off, GB), umma_desc_sw128(b_base + off, GB), idesc,
+                          (ch | sl | k) != 0 ? 1u : 0u);
+              }
+            }
+            umma_commit(&empty[slot]);                       // the stage may be refilled once these MMAs have read it
+            if (ch == n_chunks - 1) umma_commit(&tm_full[buf]);  // the super-block's accumulators are complete
+          }
+          __syncwarp();
+          if (++slot == NS) { slot = 0; ++round; }
+        }
+      }
+    }
+  } else {
+    // ---------------- consumers: drain TMEM, fused epilogue --------------------------------------------------
+    // tile row of every virtual row (static table) -> inverse map; nothing here depends on the previous kernel
+    if (c >= 0) {
+      const uint16_t* vp = cp.vpos[gi] + static_cast<size_t>(c) * cp.vpos_ld;
+      for (int v = tid; v < rr.cnt; v += kConsumerThreads) rmap[vp[v]] = static_cast<int16_t>(v);
+    }
+    pdl_wait();  // residual stream, [h1 || h2], sums of squares: written by the previous kernels
+    if (c >= 0) {
+      EpiRegs pre;
+      epi_prefetch(p, G, rr, M, p.m0, true, pre);
+      if (p.ssq_in) {
+        // 1 / rms of each draft row from the producers' partial sums of squares, fixed order
+        for (int m = warp; m < M; m += kConsumerWarps) {
+          float t = 0.f;
+#pragma unroll
+          for (int j = 0; j < 8; ++j) {
+            const int cc = lane + 32 * j;
+            if (cc < p.ssq_nct) t += __ldcg(p.ssq_in + static_cast<int64_t>(cc) * kMaxRows + p.m0 + m);
+          }
+          t = warp_sum(t);
+          if (lane == 0) rstd_s[m] = 1.0f / sqrtf(t / static_cast<float>(p.K) + p.eps);
+        }
+      }
+      consumer_sync();  // rmap, rstd_s
+      const int n_sb = tab->n_sb;
+      const int qd = warp & 3, half = warp >> 2;  // TMEM lane quarter of this warp; which half of the column chunks
+      const bool row_ok = cp.umma_m == 128 || lane < 16;
+      const int trow = cp.umma_m == 128 ? qd * 32 + lane : qd * 16 + lane;  // tile row held by this thread's TMEM lane
+      const int cpad = cp.cnt_pad;
+      for (int sb = 0; sb < n_sb; ++sb) {
+        const int buf = sb & 1;
+        mbar_wait(&tm_full[buf], (sb >> 1) & 1);
+        tc_fence_after();
+        const int v = row_ok ? rmap[sb * 128 + trow] : -1;
+        const uint32_t t0 = tmem + (static_cast<uint32_t>(qd * 32) << 16) + static_cast<uint32_t>(buf * cp.acc_cols);
+        for (int c8 = half; c8 < (M8 >> 3); c8 += 2) {
+          uint32_t a0[8], a1[8] = {0, 0, 0, 0, 0, 0, 0, 0}, a2[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+          tmem_ld8(t0 + c8 * 8, a0);
+          if (S >= 2) tmem_ld8(t0 + M8 + c8 * 8, a1);
+          if (S == 3) tmem_ld8(t0 + 2 * M8 + c8 * 8, a2);
+          tmem_ld_wait();
+          tmem_ld_use(a0);
+          tmem_ld_use(a1);
+          tmem_ld_use(a2);
+          if (v >= 0) {
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              const int m = c8 * 8 + i;
+              if (m < M) {
+                float t = __uint_as_float(a0[i]);
+                if (S >= 2) t += __uint_as_float(a1[i]);
+                if (S == 3) t += __uint_as_float(a2[i]);
+                if (p.ssq_in) t *= rstd_s[m];
+                res[m * cpad + v] = t;
+              }
+            }
+          }
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tm_empty[buf]);
+      }
+      consumer_sync();  // res complete
+      gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[m * cpad + v]; }, M, p.m0, c, p.ctas_per_group, true, &pre);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == kConsumerWarps + 2) {
+    tc_fence_after();
+    tmem_dealloc(tmem, static_cast<uint32_t>(cp.tmem_cols));
+  }
+  trace_end(p.trace);
+}
+
+}  // namespace dvt

@@ -99,6 +99,34 @@ __global__ void k_embed_plane(const RowTables* rt, const __nv_bfloat16* embed, i
   trace_end(trace);
 }
 
+// Wide levels (gemv_umma.cuh): the tensor-map copies of the tcgen05 GEMV read contiguous rows, so the level's
+// gathered inputs are laid out first. grid = (M, kSplitPlanes + 1): y < kSplitPlanes copies plane y of the
+// parent's hidden state (step row rt->src[m]) to row m of `par` (skipped when src == NULL: level 0 reads the
+// caller's rows in place); y == kSplitPlanes copies the token's embedding row (bf16: one exact plane) to `emb`.
+__global__ void k_gather_level(const RowTables* rt, const __nv_bfloat16* src, int64_t src_plane, __nv_bfloat16* par,
+                               int64_t par_plane, const __nv_bfloat16* embed, __nv_bfloat16* emb, int64_t ld, int d,
+                               unsigned long long* trace) {
+  pdl_launch_dependents();
+  trace_begin(trace);
+  pdl_wait();
+  const int m = blockIdx.x, y = blockIdx.y;
+  const uint4* s4 = nullptr;
+  uint4* d4 = nullptr;
+  if (y < kSplitPlanes) {
+    if (src != nullptr) {
+      s4 = reinterpret_cast<const uint4*>(src + y * src_plane + static_cast<int64_t>(rt->src[m]) * ld);
+      d4 = reinterpret_cast<uint4*>(par + y * par_plane + static_cast<int64_t>(m) * ld);
+    }
+  } else {
+    s4 = reinterpret_cast<const uint4*>(embed + static_cast<size_t>(rt->token[m]) * d);
+    d4 = reinterpret_cast<uint4*>(emb + static_cast<int64_t>(m) * ld);
+  }
+  if (s4 != nullptr)
+    for (int i = threadIdx.x; i < d / 8; i += blockDim.x) d4[i] = s4[i];
+  __syncthreads();
+  trace_end(trace);
+}
+
 // dgf_proj == 0: h1 = f, h2 = e (W1 = W2 = identity). grid-stride over M * 2d.
 template <typename WT>
 __global__ void k_fill_h(const StepDyn* dyn, int from_dyn, const float* xsrc, int64_t xld,

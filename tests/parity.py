@@ -69,7 +69,7 @@ def _kv_torch(a: np.ndarray, like: torch.Tensor) -> torch.Tensor:
 
 
 def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: int = 128, max_branch: int = 32,
-            force: Optional[dict] = None):
+            force: Optional[dict] = None, umma_min_m: Optional[int] = None):
     """One step through the C ABI. Returns (handle, kv, dict of host arrays).
 
     force = an oracle result: teacher forcing -- every level is computed from the oracle's hidden states,
@@ -79,6 +79,8 @@ def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: i
     h = binding.dovetail_draft_init(case.top, case.layers, cfg, max_rows, max_tree_slots, max_branch)
     k, v = case.k.clone(), case.v.clone()
     kv = binding.KVCache(k, v, case.L)
+    if umma_min_m is not None:  # which levels run on the tcgen05 GEMV (include/dovetail_hooks.h)
+        binding.dovetail_hooks_tune(h, binding.TUNE_UMMA_MIN_M, umma_min_m)
     hooks = {}
     n_new = case.tokens.shape[0]
     rows = n_new + tree.tree_rows()
@@ -104,7 +106,8 @@ def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: i
                parents=out["parents"][:n].cpu().numpy(), depths=out["depths"][:n].cpu().numpy(), n_out=n,
                logits=g("tap_logits"), hhat=g("tap_hhat"), pool_token=g("tap_pool_token"), pool_cum=g("tap_pool_cum"),
                k=kv_np(hooks.get("tap_k", k)), v=kv_np(hooks.get("tap_v", v)), forced=force is not None,
-               committed_len=kv.committed_len, launches=binding.dovetail_last_launch_count(h))
+               committed_len=kv.committed_len, launches=binding.dovetail_last_launch_count(h),
+               umma_launches=binding.dovetail_hooks_stat(h, binding.STAT_UMMA_LAUNCHES))
     return h, kv, res
 
 

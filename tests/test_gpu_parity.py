@@ -177,3 +177,45 @@ def test_full_size_configs_int8(name):
     s, gpu, ora = _run(case, tight=True)
     assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
     assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+# ---- tcgen05 GEMV (csrc/gemv_umma.cuh): wide levels and level-0 row batches --------------------------------------
+def umma_cfg(**kw) -> DraftConfig:
+    """Every K a multiple of 64 (hidden 192, 2 x hidden 384, q width 256, ffn 320), so that all seven GEMV kinds of a
+    level take the tcgen05 kernel; rows per CTA are ragged (192 / 148, 320 / 148, 1000 / 148)."""
+    base = dict(name="umma_small", hidden=192, n_q_heads=4, n_kv_heads=2, head_dim=64, n_layers=2, ffn=320,
+                vocab=1000, dtype=BF16, prefix=70, feat_scale=1.0, rope_theta=1e4,
+                tree=TreeSpec(3, (3, 2, 2), (0, 4, 5), 9), seed=17)
+    base.update(kw)
+    return DraftConfig(**base)
+
+
+@pytest.mark.parametrize("variant", ["m1_forced", "m12", "m20", "m32_max_branch", "n_new33", "n_new64", "mha_dh128_gqa", "no_proj",
+                                     "final_norm", "big_vocab"])
+def test_step_parity_umma(variant):
+    kw, n_new, min_m = {}, 1, None
+    if variant == "m1_forced":  # every level, 1 ... 5 rows, through the tcgen05 kernel (N = 16 columns)
+        min_m = 1
+    elif variant == "m12":
+        kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    elif variant == "m20":
+        kw.update(tree=TreeSpec(2, (20, 2), (0, 20), 24))
+    elif variant == "m32_max_branch":
+        kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    elif variant == "n_new33":
+        n_new = 33
+    elif variant == "n_new64":  # the widest single pass: 64 rows x 2 planes = 128 accumulator columns
+        n_new = 64
+    elif variant == "mha_dh128_gqa":
+        kw.update(hidden=256, n_q_heads=4, n_kv_heads=2, head_dim=128, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    elif variant == "no_proj":
+        kw.update(dgf_proj=0, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    elif variant == "final_norm":
+        kw.update(first_layer_input_norm=0, final_norm=1, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    elif variant == "big_vocab":  # 20000 / 148 = 136 rows per CTA: two super-blocks of the LM head
+        kw.update(vocab=20000, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    case = _boost(make_case(umma_cfg(**kw), n_new=n_new))
+    s, gpu, ora = _run(case, umma_min_m=min_m)
+    assert gpu["umma_launches"] > 0, "the tcgen05 GEMV did not run"
+    assert s["same_tree"]
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
