@@ -95,6 +95,7 @@ struct dovetail_draft {
   // tcgen05 GEMV (gemv_umma.cuh): tensor maps of the weight matrices and activation planes (four box depths
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 9;               // levels of at least this many rows take the tcgen05 kernel (65: never)
+  int umma_dbg = 0;
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
   struct PlaneBuf { const __nv_bfloat16* base; int64_t elems, ld; int cap, map; };
@@ -487,18 +488,20 @@ const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& 
 
 struct UmmaGeom {
   bool ok;
-  int nslab, n_stages, stage_bytes, b_groups, umma_m, tmem_cols, acc_cols, cnt_pad, ring_bytes, smem;
+  int nslab, n_stages, stage_bytes, a_groups, b_groups, umma_m, tmem_cols, acc_cols, k_split, cnt_pad, ring_bytes, smem;
 };
 
 // Ring of one launch: the deepest K-chunk (64 * nslab elements) that leaves >= 3 stages or >= 120 KB in flight.
-UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
+UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt, int force128 = 0) {
   UmmaGeom u{};
   const int M8 = (M + 7) / 8 * 8;
   u.acc_cols = (s_max * M8 + 15) / 16 * 16;
   u.b_groups = u.acc_cols / 8;
-  u.umma_m = g_max <= 8 ? 64 : 128;
+  u.a_groups = g_max;
+  u.umma_m = (g_max <= 8 && !force128) ? 64 : 128;
+  u.k_split = std::max(1, std::min(std::min(8, 256 / u.acc_cols), K / 512));  // K / 512: every part sees >= 1 chunk of any depth
   u.tmem_cols = 32;
-  while (u.tmem_cols < 2 * u.acc_cols) u.tmem_cols *= 2;
+  while (u.tmem_cols < 2 * u.k_split * u.acc_cols) u.tmem_cols *= 2;
   u.cnt_pad = (max_cnt + 3) / 4 * 4;
   const int tail = 2544 + M * u.cnt_pad * 4;  // barriers, 1 / rms, row map, results (gemv_umma.cuh)
   UmmaGeom best{};
@@ -508,7 +511,9 @@ UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
     const int gb = nslab * 1024;
     g.nslab = nslab;
     g.stage_bytes = (g.b_groups + g_max) * gb;
-    const int pad = (g.umma_m / 8 - g_max) * gb;  // the tensor core reads whole tiles: past the last stage's rows
+    // the tensor core reads whole 64- / 128-row tiles: past the weight groups into the activation part, and past
+    // the last stage only by what that part does not cover
+    const int pad = std::max(0, g.umma_m / 8 - g_max - g.b_groups) * gb;
     g.n_stages = std::min(8, (kSmemMax - 1024 - tail - pad) / g.stage_bytes);
     if (g.n_stages < 2) continue;
     g.ring_bytes = g.n_stages * g.stage_bytes + pad;
@@ -555,10 +560,10 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
   }
   const int Mtot = p.M;
   int Mc = Mtot;
-  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt, h->umma_dbg & 8);
   while (!g.ok && Mc > 8) {
     Mc = (Mc / 2 + 7) / 8 * 8;
-    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt, h->umma_dbg & 8);
   }
   if (!g.ok) return DOVETAIL_OK;
   int lg = 0;
@@ -567,8 +572,8 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
     up.xmap[gi] += lg;
     for (int j = 0; j < p.g[gi].n_mat; ++j) up.wmap[gi][j] += lg;
   }
-  up.nslab = g.nslab; up.n_stages = g.n_stages; up.stage_bytes = g.stage_bytes; up.b_groups = g.b_groups;
-  up.umma_m = g.umma_m; up.tmem_cols = g.tmem_cols; up.acc_cols = g.acc_cols; up.cnt_pad = g.cnt_pad;
+  up.nslab = g.nslab; up.n_stages = g.n_stages; up.stage_bytes = g.stage_bytes; up.a_groups = g.a_groups;
+  up.umma_m = g.umma_m; up.tmem_cols = g.tmem_cols; up.acc_cols = g.acc_cols; up.k_split = g.k_split; up.cnt_pad = g.cnt_pad;
   up.ring_bytes = g.ring_bytes;
   p.n_groups = q.n_groups;
   p.ctas_per_group = q.ctas;
@@ -1150,7 +1155,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       }
     }
 
-    const int lm_ctas = std::min(nsm, V);
+    const int lm_ctas = std::min(std::min(nsm, V), 256);  // k_tree_level merges at most 256 per-CTA lists per row
     {  // S6: LM head + per-CTA top-b + softmax statistics. Level 0: the last row seeds the tree.
       GemvParams p{};
       const float* xs = l == 0 ? x + static_cast<size_t>(n_new - 1) * d : x;
@@ -1583,6 +1588,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
     h->umma_min_m = value;
     return DOVETAIL_OK;
   }
+  if (key == 99) { h->umma_dbg = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
 

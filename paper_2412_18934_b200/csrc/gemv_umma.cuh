@@ -17,7 +17,7 @@
 //     locate_row) are grouped by the host into contiguous memory segments, each covered by 8-row boxes that
 //     start at the segment's first row (a box may overhang into rows of a neighbour CTA: they are multiplied
 //     and never read back; HBM still sees every row once, the overhang is an L2 hit);
-//   * a stage of the ring = [activation groups][weight groups] of one K-chunk (64 * nslab elements); 8-row
+//   * a stage of the ring = [weight groups][activation groups] of one K-chunk (64 * nslab elements); 8-row
 //     groups are nslab KB apart (the descriptor's stride byte offset), a step of 16 k is +32 bytes;
 //   * one thread issues the MMAs of a stage and commits them to the stage's "empty" barrier; after the last
 //     chunk of a super-block (<= UMMA M tile rows) it commits to "tmem_full". Accumulators are double
@@ -58,9 +58,15 @@ struct UmmaParams {
   const uint16_t* vpos[2];        // [ctas][vpos_ld]: super-block * 128 + tile row of every virtual row
   int32_t vpos_ld;
   int32_t nslab, n_stages, stage_bytes;
-  int32_t b_groups;               // 8-row groups reserved for the activation part of a stage
+  int32_t a_groups;               // 8-row groups reserved for the weight part of a stage; the activation part follows it,
+                                  // so that what the tensor core reads past the CTA's last weight group (whole 64- /
+                                  // 128-row tiles) is the activation part of the same stage, not foreign memory
   int32_t umma_m;                 // 64 or 128
-  int32_t tmem_cols, acc_cols;    // allocation (2 accumulators) and columns of one accumulator
+  int32_t tmem_cols, acc_cols;    // allocation (2 buffers x k_split accumulators) and columns of one accumulator
+  int32_t k_split;                // accumulators per super-block: K-chunk ch adds into accumulator ch % k_split. The tensor
+                                  // core's fp32 accumulation rounds towards zero; chains of K / 16 steps into one
+                                  // accumulator cost 3x the error of the mma.sync kernel's 8 shorter chains (measured),
+                                  // so the chain is cut and the parts are added in fp32 by the epilogue
   int32_t cnt_pad;                // row stride of the result buffer res[m][v]
   int32_t ring_bytes;             // ring + the pad the tensor core may read past the last stage
 };
@@ -129,7 +135,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
           if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(ng) * GB);
           __syncwarp();
           if (lane < ng)
-            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + (static_cast<uint32_t>(cp.b_groups) + lane) * GB, map,
+            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + static_cast<uint32_t>(lane) * GB, map,
                         0, row, ch * nslab, &full_a[slot], pol);
           if (++slot == NS) { slot = 0; ++round; }
         }
@@ -152,7 +158,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
           if (lane == 0) mbar_arrive_expect_tx(&full_b[slot], static_cast<uint32_t>(nB) * GB);
           __syncwarp();
           if (lane < nB)
-            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + static_cast<uint32_t>(lane) * GB, map, 0, row,
+            tma_load_3d(ring + static_cast<size_t>(slot) * cp.stage_bytes + static_cast<uint32_t>(cp.a_groups + lane) * GB, map, 0, row,
                         ch * nslab, &full_b[slot], pol);
           if (++slot == NS) { slot = 0; ++round; }
         }
@@ -163,27 +169,33 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
     if (c >= 0) {
       const int n_sb = tab->n_sb;
       const uint32_t idesc = umma_idesc_bf16(cp.umma_m, N);
+      const uint32_t desc_hi = umma_desc_hi_sw128(GB);
       const uint32_t ring_u = smem_u32(ring);
       int slot = 0, round = 0;
       for (int sb = 0; sb < n_sb; ++sb) {
         const int buf = sb & 1;
         if (sb >= 2) mbar_wait(&tm_empty[buf], ((sb >> 1) & 1) ^ 1);  // drained by the consumers
         tc_fence_after();
-        const uint32_t d_addr = tmem + static_cast<uint32_t>(buf * cp.acc_cols);
+        const uint32_t d_buf = tmem + static_cast<uint32_t>(buf * cp.k_split * cp.acc_cols);
+        int ks = 0;
         for (int ch = 0; ch < n_chunks; ++ch) {
+          const uint32_t d_addr = d_buf + static_cast<uint32_t>(ks * cp.acc_cols);
+          if (++ks == cp.k_split) ks = 0;
           mbar_wait(&full_a[slot], round & 1);
           mbar_wait(&full_b[slot], round & 1);
           tc_fence_after();
-          if (lane == 0) {
-            const uint32_t b_base = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
-            const uint32_t a_base = b_base + static_cast<uint32_t>(cp.b_groups) * GB;
-            for (int sl = 0; sl < nslab; ++sl) {
-#pragma unroll
-              for (int k = 0; k < 4; ++k) {
-                const uint32_t off = static_cast<uint32_t>(sl) * 1024u + static_cast<uint32_t>(k) * 32u;
-                umma_bf16(d_addr, umma_desc_sw128(a_base + off, GB), umma_desc_sw128(b_base + off, GB), idesc,
-                          (ch | sl | k) != 0 ? 1u : 0u);
-              }
+          if (elect_one()) {
+            const uint32_t a_base = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
+            uint32_t a_lo = umma_desc_lo(a_base), b_lo = umma_desc_lo(a_base + static_cast<uint32_t>(cp.a_groups) * GB);
+            uint32_t accum = ch >= cp.k_split ? 1u : 0u;
+            for (int sl = 0; sl < nslab; ++sl) {  // one slab = 64 k = four MMAs
+              umma_bf16(d_addr, a_lo, b_lo, desc_hi, idesc, accum);
+              umma_bf16(d_addr, a_lo + 2, b_lo + 2, desc_hi, idesc, 1u);
+              umma_bf16(d_addr, a_lo + 4, b_lo + 4, desc_hi, idesc, 1u);
+              umma_bf16(d_addr, a_lo + 6, b_lo + 6, desc_hi, idesc, 1u);
+              a_lo += 64;
+              b_lo += 64;
+              accum = 1u;
             }
             umma_commit(&empty[slot]);                       // the stage may be refilled once these MMAs have read it
             if (ch == n_chunks - 1) umma_commit(&tm_full[buf]);  // the super-block's accumulators are complete
@@ -228,24 +240,39 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
         mbar_wait(&tm_full[buf], (sb >> 1) & 1);
         tc_fence_after();
         const int v = row_ok ? rmap[sb * 128 + trow] : -1;
-        const uint32_t t0 = tmem + (static_cast<uint32_t>(qd * 32) << 16) + static_cast<uint32_t>(buf * cp.acc_cols);
+        const uint32_t t0 = tmem + (static_cast<uint32_t>(qd * 32) << 16) + static_cast<uint32_t>(buf * cp.k_split * cp.acc_cols);
         for (int c8 = half; c8 < (M8 >> 3); c8 += 2) {
-          uint32_t a0[8], a1[8] = {0, 0, 0, 0, 0, 0, 0, 0}, a2[8] = {0, 0, 0, 0, 0, 0, 0, 0};
-          tmem_ld8(t0 + c8 * 8, a0);
-          if (S >= 2) tmem_ld8(t0 + M8 + c8 * 8, a1);
-          if (S == 3) tmem_ld8(t0 + 2 * M8 + c8 * 8, a2);
-          tmem_ld_wait();
-          tmem_ld_use(a0);
-          tmem_ld_use(a1);
-          tmem_ld_use(a2);
+          // sum over the K-split accumulators (fixed order), then over the planes of a row
+          float acc[3][8];
+#pragma unroll
+          for (int s = 0; s < 3; ++s)
+#pragma unroll
+            for (int i = 0; i < 8; ++i) acc[s][i] = 0.f;
+          for (int ks = 0; ks < cp.k_split; ++ks) {
+            uint32_t a0[8], a1[8] = {0, 0, 0, 0, 0, 0, 0, 0}, a2[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+            const uint32_t tk = t0 + static_cast<uint32_t>(ks * cp.acc_cols + c8 * 8);
+            tmem_ld8(tk, a0);
+            if (S >= 2) tmem_ld8(tk + M8, a1);
+            if (S == 3) tmem_ld8(tk + 2 * M8, a2);
+            tmem_ld_wait();
+            tmem_ld_use(a0);
+            tmem_ld_use(a1);
+            tmem_ld_use(a2);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+              acc[0][i] += __uint_as_float(a0[i]);
+              acc[1][i] += __uint_as_float(a1[i]);
+              acc[2][i] += __uint_as_float(a2[i]);
+            }
+          }
           if (v >= 0) {
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               const int m = c8 * 8 + i;
               if (m < M) {
-                float t = __uint_as_float(a0[i]);
-                if (S >= 2) t += __uint_as_float(a1[i]);
-                if (S == 3) t += __uint_as_float(a2[i]);
+                float t = acc[0][i];
+                if (S >= 2) t += acc[1][i];
+                if (S == 3) t += acc[2][i];
                 if (p.ssq_in) t *= rstd_s[m];
                 res[m * cpad + v] = t;
               }

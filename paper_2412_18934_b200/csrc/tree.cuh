@@ -284,24 +284,43 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
       }
       se = warp_sum(se);
       const float logz = mg + logf(se);
-      // global top-b of the row: b rounds of "best candidate strictly after the previous pick"
-      float lv = INFINITY;
-      int li = -1;
+      // global top-b of the row: a b-round merge of the per-CTA lists, each of which is sorted in the strict
+      // candidate order (gemv.cuh EPI_LMHEAD). Lane l owns the lists of CTAs l, l + 32, ... and keeps their current
+      // heads in registers; a round picks the best head of the warp and the owning lane advances that list.
+      constexpr int kLists = 8;  // lists per lane: nct <= 256
+      float hv[kLists];
+      int hi[kLists], hp[kLists];
+#pragma unroll
+      for (int k = 0; k < kLists; ++k) {
+        const int c = lane + 32 * k;
+        hp[k] = 0;
+        hv[k] = -INFINITY;
+        hi[k] = 0x7fffffff;
+        if (c < p.nct) { hv[k] = cv[c * cstride]; hi[k] = ci[c * cstride]; }
+      }
       for (int jb = 0; jb < p.b; ++jb) {
         float bv = -INFINITY;
         int bi = 0x7fffffff;
-        for (int c = lane; c < p.nct; c += 32) {
-          for (int j = 0; j < p.b; ++j) {
-            const float val = cv[c * cstride + j];
-            const int id = ci[c * cstride + j];
-            if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
-          }
-        }
+#pragma unroll
+        for (int k = 0; k < kLists; ++k)
+          if (cand_before(hv[k], hi[k], bv, bi)) { bv = hv[k]; bi = hi[k]; }
+        const int mine = bi;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
           const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
           const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
           if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+        }
+        if (mine == bi && bi != 0x7fffffff) {  // token ids are unique across the lists: exactly one lane advances
+#pragma unroll
+          for (int k = 0; k < kLists; ++k) {
+            if (hi[k] == bi) {
+              const int c = lane + 32 * k;
+              ++hp[k];
+              if (hp[k] < p.b) { hv[k] = cv[c * cstride + hp[k]]; hi[k] = ci[c * cstride + hp[k]]; }
+              else { hv[k] = -INFINITY; hi[k] = 0x7fffffff; }
+            }
+          }
         }
         if (lane == 0) {
           P.token[base + jb] = bi;
@@ -310,8 +329,6 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
           P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
           P.row[base + jb] = -1;
         }
-        lv = bv;
-        li = bi;
       }
     }
     if (G == 0) break;     // ungrouped: the loop above covered every row
