@@ -208,6 +208,20 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
                         int32_t n_new, dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree,
                         const dovetail_draft_out_t* out, void* cuda_stream);
 
+/* Prompt / catch-up rows (the target first processes the prompt and hands
+ * its hidden states and tokens to the draft model, which has to build its own K/V over them before the
+ * first tree; limitation :274). Runs the draft model over n_rows (feature, token) pairs exactly as
+ * dovetail_draft_step runs its level-0 rows -- positions committed_len + i, causal among themselves after
+ * the committed prefix -- appends their K/V rows and advances kv->committed_len by n_rows.
+ * No LM head and no tree: prefill(rows 0 .. n-2) followed by step(row n-1) equals step(rows 0 .. n-1)
+ * (oracle pin P8). n_rows >= 1 is not bounded by cfg.max_rows: the rows run in batches of cfg.max_rows, each
+ * batch one pass over the weights (bf16 models: the tcgen05 GEMV, csrc/gemv_umma.cuh).
+ *   hidden_feats : dev fp32 [n_rows, d];  tokens : dev int32 [n_rows]
+ * Asynchronous on cuda_stream. Errors: EINVAL, ECAPACITY (committed_len + n_rows > capacity), ECUDA; shapes are
+ * checked before the first launch. A later dovetail_kv_commit needs a dovetail_draft_step first. */
+int dovetail_draft_prefill(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens, int32_t n_rows,
+                           dovetail_kv_cache_t* kv, void* cuda_stream);
+
 /* After verification: tell the draft which candidates the
  * target accepted.
  *   accepted_path : HOST int32 [n_acc], indices into the last step's output,

@@ -78,7 +78,7 @@ int dovetail_trace_read(dovetail_draft_t* h, int32_t cap, int32_t* kind, int32_t
  * EINVAL. */
 int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
 /* key 1: tree levels (and level-0 row batches) of at least `value` rows run on the tcgen05 GEMV
- * (csrc/gemv_umma.cuh) instead of the mma.sync GEMV; 1 ... 64, 65 = never. Default 9. bf16 weights only. */
+ * (csrc/gemv_umma.cuh) instead of the mma.sync GEMV; 1 ... 64, 65 = never. Default 8. bf16 weights only. */
 #define DOVETAIL_TUNE_UMMA_MIN_M 1
 
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.

@@ -17,7 +17,7 @@ MAX_DEPTH, MAX_LAYERS = 16, 16
 OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 # include/dovetail.h
-EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_kv_commit", "dovetail_tree_replay",
+EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_draft_prefill", "dovetail_kv_commit", "dovetail_tree_replay",
            "dovetail_verify_plan", "dovetail_verify_accept", "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
@@ -103,6 +103,8 @@ def load() -> C.CDLL:
         lib.dovetail_draft_step.restype = C.c_int
         lib.dovetail_draft_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(KVCacheT),
                                             C.POINTER(TreeSpecT), C.POINTER(DraftOutT), C.c_void_p]
+        lib.dovetail_draft_prefill.restype = C.c_int
+        lib.dovetail_draft_prefill.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(KVCacheT), C.c_void_p]
         lib.dovetail_kv_commit.restype = C.c_int
         lib.dovetail_kv_commit.argtypes = [C.c_void_p, C.POINTER(KVCacheT), C.POINTER(C.c_int32), C.c_int32,
                                            C.c_int32, C.POINTER(C.c_int32), C.c_void_p]
@@ -275,6 +277,21 @@ def dovetail_draft_step(h: Draft, hidden_feats, tokens, kv: KVCache, tree: TreeS
                                     C.byref(t), C.byref(o), _stream(stream))
     _check(rc, h.ptr)
     return out
+
+
+def dovetail_draft_prefill(h: Draft, hidden_feats, tokens, kv: KVCache, stream=None) -> None:
+    """Prompt / catch-up rows (include/dovetail.h): appends the K/V of every (feature, token) row and advances
+    kv.committed_len; no LM head, no tree. Asynchronous."""
+    import torch
+    d, cdt = h.cfg.hidden, (torch.bfloat16 if h.cfg.dtype == BF16 else torch.float32)
+    if hidden_feats.dtype != torch.float32 or hidden_feats.dim() != 2 or hidden_feats.shape[1] != d or not hidden_feats.is_contiguous():
+        raise TypeError(f"hidden_feats must be contiguous float32 [n_rows, {d}], got {hidden_feats.dtype} {tuple(hidden_feats.shape)}")
+    if tokens.dtype != torch.int32 or tokens.dim() != 1 or tokens.shape[0] != hidden_feats.shape[0]:
+        raise TypeError(f"tokens must be int32 [n_rows = {hidden_feats.shape[0]}], got {tokens.dtype} {tuple(tokens.shape)}")
+    if kv.k.dtype != cdt or kv.k.shape[0] != h.cfg.n_layers or kv.k.shape[1] != h.cfg.n_kv_heads or kv.k.shape[3] != h.cfg.head_dim:
+        raise TypeError(f"KV cache must be {cdt} [n_layers, n_kv_heads, capacity, head_dim], got {kv.k.dtype} {tuple(kv.k.shape)}")
+    rc = load().dovetail_draft_prefill(h.ptr, _dp(hidden_feats), _dp(tokens), int(tokens.shape[0]), C.byref(kv.c), _stream(stream))
+    _check(rc, h.ptr)
 
 
 def dovetail_kv_commit(h: Draft, kv: KVCache, accepted_path, mode: int = 0, stream=None) -> int:
