@@ -266,6 +266,20 @@ def bench_one(a, cfg, rank, world, local, dist):
         step_e2e()
     ms_e2e = timed(step_e2e, K)
     clk = clocks.stop() if rank == 0 else None
+    how = {0: "direct launches", 1: "CUDA graph replay", 2: "CUDA graph capture"}[binding.dovetail_hooks_stat(h, binding.STAT_GRAPH)]
+    # the same steps with direct launches (programmatic dependent launch, no graph): SURVEY.md 3(2)
+    launch_modes = None
+    if world == 1:
+        binding.dovetail_hooks_tune(h, binding.TUNE_GRAPHS, 0)
+        for _ in range(W):
+            step_device()
+        ms_d = timed(step_device, K)
+        for _ in range(W):
+            step_e2e()
+        ms_e2e_d = timed(step_e2e, K)
+        binding.dovetail_hooks_tune(h, binding.TUNE_GRAPHS, 1)
+        launch_modes = {"timed_as": how, "graph_us_per_step": ms / K * 1e3, "direct_us_per_step": ms_d / K * 1e3,
+                        "graph_e2e_us_per_step": ms_e2e / K * 1e3, "direct_e2e_us_per_step": ms_e2e_d / K * 1e3}
     launches = binding.dovetail_last_launch_count(h) * K
     n_out = int(out["n_out"].item())
     assert n_out == min(tree.gamma, tree.pool_size()), "the step did not produce its candidates"
@@ -385,7 +399,35 @@ def bench_one(a, cfg, rank, world, local, dist):
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e / K,
                     "h2d_bytes_per_step": feats_h.numel() * 4 + tok_h.numel() * 4,
                     "d2h_bytes_per_step": sum(v.numel() * v.element_size() for v in out_h.values())},
-            "gpu_launches": launches, "clocks": clk, "roofline": roof}
+            "gpu_launches": launches, "launch": launch_modes, "clocks": clk, "roofline": roof}
+
+    # ---- prompt / catch-up rows (dovetail_draft_prefill), batches of 64 rows -----------------
+    if a.prefill_rows > 0 and world == 1 and cfg.dtype == 1 and not cfg.wquant:
+        Rp = a.prefill_rows
+        shp = list(case.k.shape)
+        shp[2] = case.L + Rp + 8
+        k2, v2 = torch.zeros(shp, dtype=case.k.dtype, device="cuda"), torch.zeros(shp, dtype=case.v.dtype, device="cuda")
+        k2[:, :, :case.L], v2[:, :, :case.L] = case.k[:, :, :case.L], case.v[:, :, :case.L]
+        kv2 = binding.KVCache(k2, v2, case.L)
+        g = torch.Generator(device="cuda").manual_seed(cfg.seed + 7)
+        pf = (torch.randn((Rp, cfg.hidden), generator=g, device="cuda") * cfg.feat_scale).to(torch.bfloat16).float()
+        pt = torch.randint(0, cfg.vocab, (Rp,), generator=g, device="cuda", dtype=torch.int32)
+
+        def pre():
+            kv2.committed_len = case.L
+            binding.dovetail_draft_prefill(h, pf, pt, kv2)
+        for _ in range(3):
+            pre()
+        reps = 5
+        ms_p = timed(pre, reps) / reps
+        passes = -(-Rp // 64)
+        wbytes = binding.dovetail_forward_bytes(h, 0) - cfg.vocab * cfg.hidden * 2  # one pass over the block weights, no LM head
+        line["prefill"] = {"rows": Rp, "batch_rows": 64, "ms": ms_p, "rows_per_s": Rp / (ms_p * 1e-3),
+                           "weight_passes": passes, "hbm_gbs_weights": passes * wbytes / (ms_p * 1e-3) / 1e9,
+                           "umma_launches": binding.dovetail_hooks_stat(h, binding.STAT_UMMA_LAUNCHES),
+                           "note": "each 64-row batch streams the block weights once through the tcgen05 GEMV (weight-streaming "
+                                   "bound at 64 rows per pass, not yet a tile-reuse GEMM)"}
+        del k2, v2
 
     # ---- reading A1 "report both": the same step with dgf_proj = 0 (W1 = W2 = I) ----------------------------
     if a.both_dgf and world == 1 and cfg.dgf_proj == 1 and cfg.fusion == 0:
@@ -430,6 +472,7 @@ def main():
     ap.add_argument("--replays", type=int, default=200)
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="A/B knob of include/dovetail_hooks.h dovetail_hooks_tune (repeatable)")
+    ap.add_argument("--prefill-rows", type=int, default=256, help="rows of the dovetail_draft_prefill leg (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-trace", action="store_true")
     ap.add_argument("--no-both-dgf", dest="both_dgf", action="store_false")
@@ -472,7 +515,7 @@ def main():
         last = i == len(names) - 1
         if not last:  # the sweep lines carry the step numbers only
             aa = argparse.Namespace(**vars(a))
-            aa.no_cpu_baseline, aa.both_dgf, aa.replays = True, False, 0
+            aa.no_cpu_baseline, aa.both_dgf, aa.replays, aa.prefill_rows = True, False, 0, 0
         else:
             aa = a
         line = bench_one(aa, cfgs[name], rank, world, local, dist)

@@ -80,10 +80,15 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
 /* key 1: tree levels (and level-0 row batches) of at least `value` rows run on the tcgen05 GEMV
  * (csrc/gemv_umma.cuh) instead of the mma.sync GEMV; 1 ... 64, 65 = never. Default 8. bf16 weights only. */
 #define DOVETAIL_TUNE_UMMA_MIN_M 1
+/* key 2: 1 (default) = dovetail_draft_step replays one CUDA graph per (tree_spec, n_new, attention geometry);
+ * 0 = direct launches. Steps with test hooks or tracing set always launch directly. */
+#define DOVETAIL_TUNE_GRAPHS 2
 
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.
  *   key 1: launches of the tcgen05 GEMV (k_gemv_umma). Unknown key or NULL handle: -1. */
 #define DOVETAIL_STAT_UMMA_LAUNCHES 1
+/*   key 2: how the last step was launched: 0 direct launches, 1 graph replay, 2 graph captured and launched. */
+#define DOVETAIL_STAT_GRAPH 2
 int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key);
 
 /* Read-only HBM streaming ceilings, run by bench.py next to the step: reads `bytes`

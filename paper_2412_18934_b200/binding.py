@@ -411,8 +411,8 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
     return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
 
 
-TUNE_UMMA_MIN_M = 1
-STAT_UMMA_LAUNCHES = 1
+TUNE_UMMA_MIN_M, TUNE_GRAPHS = 1, 2
+STAT_UMMA_LAUNCHES, STAT_GRAPH = 1, 2
 
 
 def dovetail_hooks_stat(h: Draft, key: int) -> int:

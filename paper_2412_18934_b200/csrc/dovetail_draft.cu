@@ -103,6 +103,28 @@ struct dovetail_draft {
   struct UmmaTable { UmmaCtaTab* tab = nullptr; uint16_t* vpos = nullptr; int vpos_ld = 0, g_max = 0, g_min = 0; bool ok = false; };
   std::map<std::array<int, 8>, UmmaTable> umma_tabs;
   __nv_bfloat16* xs_par = nullptr;  // [3][max_rows][ld_d] parent hidden states of a wide level, gathered
+  // One CUDA graph per (tree_spec, n_new, attention geometry): the step's launch sequence with its
+  // programmatic edges, replayed with the per-call values patched into the nodes that take them as arguments
+  // (k_step_begin: caller pointers and lengths; tensor-core attention: cache pointers and lengths).
+  struct StepGraph {
+    std::vector<int> key;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphNode_t begin_node = nullptr;
+    cudaKernelNodeParams begin_params{};
+    std::vector<void*> begin_args;
+    StepDyn begin_dv{};
+    std::vector<cudaGraphNode_t> attn_nodes;
+    std::vector<cudaKernelNodeParams> attn_node_params;
+    std::vector<AttnParams> attn_params;
+    int launches = 0, umma_launches = 0;
+    unsigned long long used = 0;
+  };
+  bool graphs_on = true;
+  std::vector<StepGraph> graphs;
+  unsigned long long graph_clock = 0;
+  cudaStream_t cap_stream = nullptr;
+  int last_graph = 0;  // 1: the last step was a graph replay, 2: captured and launched, 0: direct launches
 #ifdef DVT_CHAINDBG
   unsigned long long* dbg = nullptr;
   int dbg_launch = 0;
@@ -783,6 +805,13 @@ cudaError_t dmalloc(T** p, size_t n) {
   return cudaMalloc(reinterpret_cast<void**>(p), n * sizeof(T));
 }
 
+void destroy_graph(dovetail_draft::StepGraph& g) {
+  if (g.exec) cudaGraphExecDestroy(g.exec);
+  if (g.graph) cudaGraphDestroy(g.graph);
+  g.exec = nullptr;
+  g.graph = nullptr;
+}
+
 void free_all(dovetail_draft* h) {
   cudaFree(h->dyn); cudaFree(h->ts); cudaFree(h->rt); cudaFree(h->rope); cudaFree(h->inv_freq);
   cudaFree(h->hbuf); cudaFree(h->hhat); cudaFree(h->qkv); cudaFree(h->obuf); cudaFree(h->act);
@@ -791,6 +820,9 @@ void free_all(dovetail_draft* h) {
   cudaFree(h->qs);
   cudaFree(h->xs_emb);
   cudaFree(h->xs_par);
+  for (auto& g : h->graphs) destroy_graph(g);
+  h->graphs.clear();
+  if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
   cudaFree(h->maps_dev);
   for (auto& kv : h->umma_tabs) { cudaFree(kv.second.tab); cudaFree(kv.second.vpos); }
   cudaFree(h->attn_ws); cudaFree(h->attn_cnt); cudaFree(h->cand_val); cudaFree(h->cand_id); cudaFree(h->stat);
@@ -832,6 +864,21 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
   cp2(kv->v, k.force_v);
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "tap / forcing copy failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
+}
+
+// Chunks per kv-head of the tensor-core attention kernel (measured on C2 / C3 / C5): at least two 64-position
+// blocks per chunk (a CTA's fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one
+// cluster of 8 no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
+void attn_mma_geom(const dovetail_draft* h, int Lbase, int& n_chunks, int& cs) {
+  const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
+  n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2));
+  if (n_chunks <= 8) {
+    n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
+    cs = n_chunks;
+  } else {
+    n_chunks = std::max(8, std::min(n_chunks, 200 / h->cfg.n_kv_heads) / 8 * 8);
+    cs = 8;
+  }
 }
 
 // Enqueues (or, with h->dry, only shape-checks) the kernels of one draft step.
@@ -1067,18 +1114,8 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
           a.cap = kv->capacity;
           a.Lbase = Lbase;
           a.Lsafe = L;
-          const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
-          // Chunks per kv-head (measured on C2 / C3 / C5): at least two 64-position blocks per chunk (a CTA's
-          // fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one cluster of 8
-          // no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
-          int n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2)), cs;
-          if (n_chunks <= 8) {
-            n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
-            cs = n_chunks;
-          } else {
-            n_chunks = std::max(8, std::min(n_chunks, 200 / c.n_kv_heads) / 8 * 8);
-            cs = 8;
-          }
+          int n_chunks, cs;
+          attn_mma_geom(h, Lbase, n_chunks, cs);
           const size_t smem = am_smem_bytes(dh);
           e = launch_c(h, cs, true, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
                        dim3(kAmThreads), smem, st, a);
@@ -1227,6 +1264,113 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       if (rc) return rc;
     }
   }
+  return DOVETAIL_OK;
+}
+
+// The step as one graph launch. Key: everything the launch SEQUENCE depends on -- the tree, n_new and the grids /
+// cluster sizes of the attention kernels (functions of the prefix length in 64-position blocks). Per-call values
+// that are kernel arguments are patched into the instantiated graph: k_step_begin's StepDyn (caller pointers,
+// committed length, outputs) and the tensor-core attention kernels' cache pointers and lengths.
+int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, const int32_t* tokens, int n_new,
+                  dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree, const dovetail_draft_out_t* out,
+                  const std::vector<LevelPlan>& plan, int pool_total) {
+  const dovetail_config_t& c = h->cfg;
+  const int L = kv->committed_len, Lp = L + n_new;
+  const bool bf16 = c.dtype == DOVETAIL_BF16;
+  std::vector<int> key = {tree->depth, tree->gamma, n_new};
+  for (int l = 0; l < tree->depth; ++l) { key.push_back(tree->branch[l]); key.push_back(tree->beam[l]); }
+  int nc[2] = {0, 0}, cs[2] = {0, 0};
+  if (bf16) {
+    attn_mma_geom(h, L, nc[0], cs[0]);
+    attn_mma_geom(h, Lp, nc[1], cs[1]);
+  } else {
+    nc[0] = std::min(h->attn_chunks_cap, std::max(1, div_up(L, 2 * kAttnStagePos)));
+    nc[1] = std::min(h->attn_chunks_cap, std::max(1, div_up(Lp, 2 * kAttnStagePos)));
+  }
+  key.insert(key.end(), {nc[0], cs[0], nc[1], cs[1], h->umma_min_m});
+  dovetail_draft::StepGraph* g = nullptr;
+  for (auto& x : h->graphs)
+    if (x.key == key) g = &x;
+  cudaError_t e = cudaSuccess;
+  if (!g) {
+    // shape check without launching, then capture the real launch sequence on the handle's own stream
+    h->dry = true;
+    int rc = enqueue_step(h, st, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
+    h->dry = false;
+    if (rc != DOVETAIL_OK) return rc;
+    if (!h->cap_stream && cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking) != cudaSuccess)
+      return fail(h, DOVETAIL_ECUDA, "stream creation failed");
+    dovetail_draft::StepGraph ng;
+    ng.key = key;
+    e = cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal);
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "graph capture failed: %s", cudaGetErrorString(e));
+    rc = enqueue_step(h, h->cap_stream, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
+    e = cudaStreamEndCapture(h->cap_stream, &ng.graph);
+    if (rc != DOVETAIL_OK) { destroy_graph(ng); cudaGetLastError(); return rc; }
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&ng.exec, ng.graph, 0);
+    if (e != cudaSuccess) { destroy_graph(ng); cudaGetLastError(); return fail(h, DOVETAIL_ECUDA, "graph instantiation failed: %s", cudaGetErrorString(e)); }
+    size_t n_nodes = 0;
+    cudaGraphGetNodes(ng.graph, nullptr, &n_nodes);
+    std::vector<cudaGraphNode_t> nodes(n_nodes);
+    cudaGraphGetNodes(ng.graph, nodes.data(), &n_nodes);
+    for (cudaGraphNode_t nd : nodes) {
+      cudaGraphNodeType ty;
+      if (cudaGraphNodeGetType(nd, &ty) != cudaSuccess || ty != cudaGraphNodeTypeKernel) continue;
+      cudaKernelNodeParams kp{};
+      if (cudaGraphKernelNodeGetParams(nd, &kp) != cudaSuccess) continue;
+      if (kp.func == reinterpret_cast<void*>(k_step_begin)) {
+        ng.begin_node = nd;
+        ng.begin_params = kp;
+        ng.begin_args.assign(kp.kernelParams, kp.kernelParams + 11);  // k_step_begin takes 11 arguments
+        ng.begin_dv = *static_cast<const StepDyn*>(kp.kernelParams[0]);
+      } else if (kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128>)) {
+        ng.attn_nodes.push_back(nd);
+        ng.attn_node_params.push_back(kp);
+        ng.attn_params.push_back(*static_cast<const AttnParams*>(kp.kernelParams[0]));
+      }
+    }
+    cudaGetLastError();
+    if (!ng.begin_node) { destroy_graph(ng); return fail(h, DOVETAIL_ECUDA, "graph capture: step-begin node not found"); }
+    ng.launches = h->launches;
+    ng.umma_launches = h->umma_launches;
+    if (h->graphs.size() >= 8) {  // evict the least recently used
+      size_t lru = 0;
+      for (size_t i = 1; i < h->graphs.size(); ++i)
+        if (h->graphs[i].used < h->graphs[lru].used) lru = i;
+      destroy_graph(h->graphs[lru]);
+      h->graphs.erase(h->graphs.begin() + lru);
+    }
+    h->graphs.push_back(std::move(ng));
+    g = &h->graphs.back();
+    h->last_graph = 2;
+  } else {
+    // patch the per-call values
+    StepDyn& dv = g->begin_dv;
+    dv.feats = hidden_feats; dv.tokens = tokens; dv.kc = kv->k; dv.vc = kv->v; dv.capacity = kv->capacity;
+    dv.L = L; dv.n_new = n_new; dv.Lp = Lp;
+    dv.out_ids = out->token_ids; dv.out_scores = out->scores; dv.out_parents = out->parents;
+    dv.out_depths = out->depths; dv.out_n = out->n_out;
+    g->begin_args[0] = &dv;
+    g->begin_params.kernelParams = g->begin_args.data();
+    e = cudaGraphExecKernelNodeSetParams(g->exec, g->begin_node, &g->begin_params);
+    for (size_t i = 0; i < g->attn_nodes.size() && e == cudaSuccess; ++i) {
+      AttnParams& a = g->attn_params[i];
+      a.kc = kv->k; a.vc = kv->v; a.cap = kv->capacity;
+      a.Lbase = a.level0 ? L : Lp;
+      a.Lsafe = L;
+      void* args[1] = {&a};
+      cudaKernelNodeParams kp = g->attn_node_params[i];
+      kp.kernelParams = args;
+      e = cudaGraphExecKernelNodeSetParams(g->exec, g->attn_nodes[i], &kp);
+    }
+    if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "graph update failed: %s", cudaGetErrorString(e));
+    h->launches = g->launches;
+    h->umma_launches = g->umma_launches;
+    h->last_graph = 1;
+  }
+  g->used = ++h->graph_clock;
+  e = cudaGraphLaunch(g->exec, st);
+  if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "graph launch failed: %s", cudaGetErrorString(e));
   return DOVETAIL_OK;
 }
 
@@ -1381,13 +1525,19 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
     return fail(h, DOVETAIL_ECAPACITY, "KV cache too small: %d committed + %d new + %d tree rows > capacity %d", L, n_new, tree_rows, kv->capacity);
 
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  // Pass 1 checks every shape of the plan without launching (on error nothing was enqueued);
-  // pass 2 enqueues.
-  for (int pass = 0; pass < 2; ++pass) {
-    h->dry = pass == 0;
-    rc = enqueue_step(h, st, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
-    h->dry = false;
+  h->last_graph = 0;
+  if (h->graphs_on && !h->hooks_on && !h->trace_on) {
+    rc = step_by_graph(h, st, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
     if (rc != DOVETAIL_OK) return rc;
+  } else {
+    // Pass 1 checks every shape of the plan without launching (on error nothing was enqueued);
+    // pass 2 enqueues.
+    for (int pass = 0; pass < 2; ++pass) {
+      h->dry = pass == 0;
+      rc = enqueue_step(h, st, hidden_feats, tokens, n_new, kv, tree, out, plan, pool_total);
+      h->dry = false;
+      if (rc != DOVETAIL_OK) return rc;
+    }
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "CUDA error: %s", cudaGetErrorString(e));
@@ -1628,6 +1778,7 @@ int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_l
 int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
   if (!h) return -1;
   if (key == DOVETAIL_STAT_UMMA_LAUNCHES) return h->last_umma_launches;
+  if (key == DOVETAIL_STAT_GRAPH) return h->last_graph;
   return -1;
 }
 
@@ -1638,6 +1789,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
     h->umma_min_m = value;
     return DOVETAIL_OK;
   }
+  if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
   if (key == 99) { h->umma_dbg = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
