@@ -83,6 +83,9 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
 /* key 2: 1 (default) = dovetail_draft_step replays one CUDA graph per (tree_spec, n_new, attention geometry);
  * 0 = direct launches. Steps with test hooks or tracing set always launch directly. */
 #define DOVETAIL_TUNE_GRAPHS 2
+/* key 3: attention launches with more than `value` query vectors (rows of the level x q-heads per kv-head) use the
+ * 64-vectors-per-pass kernel (csrc/attention_mma.cuh, QT = 4). Default 32; 4096 = never, 0 = always. */
+#define DOVETAIL_TUNE_ATTN_WIDE_MIN 3
 
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.
  *   key 1: launches of the tcgen05 GEMV (k_gemv_umma). Unknown key or NULL handle: -1. */

@@ -88,13 +88,19 @@ __device__ __forceinline__ uint32_t am_swz(int r, int ch) {
   return static_cast<uint32_t>(r) * ROWB + static_cast<uint32_t>((ch ^ (r & 7)) << 4);
 }
 
-constexpr size_t am_smem_bytes(int DH) {
+constexpr size_t am_smem_bytes(int DH, int QT = 1) {
   // q hi + lo tiles, ring of (K, V) blocks (the merge scratch aliases it), barriers
-  return static_cast<size_t>(2 * kAmQRows * DH * 2) + static_cast<size_t>(kAmStages) * 2 * kAmBlockPos * DH * 2 + 128;
+  return static_cast<size_t>(2 * QT * kAmQRows * DH * 2) + static_cast<size_t>(kAmStages) * 2 * kAmBlockPos * DH * 2 + 128;
 }
 
-template <int DH>
-__global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const AttnParams p) {
+// QT = 1: one tile of 16 query vectors per pass over the CTA's positions, the four consumer warps split the 64
+// positions of a block (tree levels of a few rows: latency matters, every warp works on every block).
+// QT = 4 ("wide": levels of many rows, level-0 batches of dovetail_draft_prefill): 64 query vectors per pass,
+// consumer warp w owns query tile w and walks all 64 positions of every block with its own online-softmax state,
+// the flash-attention arrangement -- the cache is streamed once per 64 query vectors instead of once per 16, and
+// no merge over the warps is needed.
+template <int DH, int QT>
+__global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_mma(const AttnParams p) {
   using WT = __nv_bfloat16;
   constexpr int ROWB = DH * 2;            // bytes of one K (or V) row
   constexpr int CPR = ROWB / 16;          // 16-byte chunks per row
@@ -103,11 +109,12 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   constexpr int PB = kAmBlockPos;
   constexpr int BLK_BYTES = 2 * PB * ROWB;
   constexpr int HALF = DH / 2;
-  constexpr int WSTR = DH + 2;            // partial record: o[DH], m, l
+  constexpr int WSTR = DH + 4;            // partial record: o[DH], m, l (rows 16-byte aligned: the merges read float4)
   extern __shared__ __align__(128) uint8_t smem[];
-  uint8_t* q_hi = smem;                   // [16][ROWB] swizzled bf16 heads of the rotated, scaled queries
-  uint8_t* q_lo = q_hi + kAmQRows * ROWB; // remainders
-  uint8_t* ring = q_lo + kAmQRows * ROWB;
+  constexpr int QROWS = QT * kAmQRows;    // query vectors per pass
+  uint8_t* q_hi = smem;                   // [QROWS][ROWB] swizzled bf16 heads of the rotated, scaled queries
+  uint8_t* q_lo = q_hi + QROWS * ROWB;    // remainders
+  uint8_t* ring = q_lo + QROWS * ROWB;
   uint64_t* full = reinterpret_cast<uint64_t*>(ring + kAmStages * BLK_BYTES);
   uint64_t* empty = full + 4;
   uint64_t* tailbar = empty + 4;
@@ -121,9 +128,10 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
   const int c = blockIdx.x, hk = blockIdx.y, n_chunks = gridDim.x;
   const int grp = p.Hq / p.Hkv;
   const int qv_tot = p.M * grp;
-  const int n_pass = (qv_tot + kAmQRows - 1) / kAmQRows;
-  const int QR = min(kAmQRows, qv_tot);  // rows of the warp-merge scratch
-  float* crec = wsm + static_cast<size_t>(kAmWarps) * QR * WSTR;  // [QR][WSTR] this CTA's record, read by the cluster leader
+  const int n_pass = (qv_tot + QROWS - 1) / QROWS;
+  const int QR = min(QROWS, qv_tot);  // rows of the warp-merge scratch
+  // [QR][WSTR] this CTA's record, read by the cluster ranks (wide: written by the warps directly, no warp merge)
+  float* crec = QT == 1 ? wsm + static_cast<size_t>(kAmWarps) * QR * WSTR : wsm;
   // chunks [group * CS, (group + 1) * CS) of a kv-head form a cluster (CS = 1 without the launch attribute)
   const int CS = static_cast<int>(cluster_nctarank()), crank = static_cast<int>(cluster_ctarank());
   const int n_groups = n_chunks / CS, group = c / CS;
@@ -242,33 +250,36 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
 
   int slot = 0, round = 0;
   for (int pass = 0; pass < n_pass; ++pass) {
-    const int qv0 = pass * kAmQRows;
-    const int nq = min(kAmQRows, qv_tot - qv0);  // query vectors of this pass
+    const int qv0 = pass * QROWS;
+    const int nq = min(QROWS, qv_tot - qv0);  // query vectors of this pass
     // ---- rotated, scaled queries -> bf16 head + remainder tiles ------------------
     if (p.qs != nullptr) {  // prepared by the QKV projection's epilogue: 16-byte copies into the swizzled tiles
-      constexpr int NQ = kAmQRows * CPR * 2 / kAmConsumers;  // copies per thread, all loads issued before the stores
+      constexpr int NQ = kAmQRows * CPR * 2 / kAmConsumers;  // copies per thread and round, all loads issued before the stores
       static_assert(kAmQRows * CPR * 2 % kAmConsumers == 0, "query tile copies must divide among the consumers");
-      uint4 v[NQ];
+#pragma unroll 1
+      for (int rd = 0; rd < QT; ++rd) {  // one round per 16-row tile
+        uint4 v[NQ];
 #pragma unroll
-      for (int i = 0; i < NQ; ++i) {
-        const int idx = tid + i * kAmConsumers;
-        const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
-        const int r = rem / CPR, ch = rem - r * CPR;
-        v[i] = make_uint4(0u, 0u, 0u, 0u);
-        if (r < nq) {
-          const int qv = qv0 + r, m = qv / grp, hq = hk * grp + qv % grp;
-          v[i] = __ldcg(reinterpret_cast<const uint4*>(p.qs + (static_cast<size_t>(pl) * kMaxRows + m) * dq + hq * DH) + ch);
+        for (int i = 0; i < NQ; ++i) {
+          const int idx = tid + i * kAmConsumers;
+          const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
+          const int r = rd * kAmQRows + rem / CPR, ch = rem % CPR;
+          v[i] = make_uint4(0u, 0u, 0u, 0u);
+          if (r < nq) {
+            const int qv = qv0 + r, m = qv / grp, hq = hk * grp + qv % grp;
+            v[i] = __ldcg(reinterpret_cast<const uint4*>(p.qs + (static_cast<size_t>(pl) * kMaxRows + m) * dq + hq * DH) + ch);
+          }
+        }
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) {
+          const int idx = tid + i * kAmConsumers;
+          const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
+          const int r = rd * kAmQRows + rem / CPR, ch = rem % CPR;
+          *reinterpret_cast<uint4*>((pl ? q_lo : q_hi) + am_swz<ROWB>(r, ch)) = v[i];
         }
       }
-#pragma unroll
-      for (int i = 0; i < NQ; ++i) {
-        const int idx = tid + i * kAmConsumers;
-        const int pl = idx / (kAmQRows * CPR), rem = idx - pl * (kAmQRows * CPR);
-        const int r = rem / CPR, ch = rem - r * CPR;
-        *reinterpret_cast<uint4*>((pl ? q_lo : q_hi) + am_swz<ROWB>(r, ch)) = v[i];
-      }
     } else
-    for (int idx = tid; idx < kAmQRows * HALF; idx += kAmConsumers) {
+    for (int idx = tid; idx < QROWS * HALF; idx += kAmConsumers) {
       const int r = idx / HALF, i = idx % HALF;
       float x0 = 0.f, x1 = 0.f;
       if (r < nq) {
@@ -296,7 +307,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     int mrow[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const int r = g + 8 * h;
+      const int r = (QT == 1 ? 0 : warp * kAmQRows) + g + 8 * h;  // wide: this warp's own query tile
       mrow[h] = r < nq ? (qv0 + r) / grp : -1;
     }
     float mrun[2] = {-INFINITY, -INFINITY}, lrun[2] = {0.f, 0.f};
@@ -315,41 +326,127 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
       const bool tail = b >= n_blk;
       const int cnt = tail ? min(PB, p.new_cnt - (b - n_blk) * PB) : min(PB, p_end - (p_begin + b * PB));
       mbar_wait(&full[slot], round & 1);
+      if constexpr (QT == 1) {
       const int t0 = warp * 16;  // this warp's tile of the block
-      if (t0 < cnt) {
+        if (t0 < cnt) {
+          const uint32_t kb = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vb = kb + PB * ROWB;
+          // four independent accumulation chains (head / remainder x two position tiles): a dependent
+          // HMMA chain of 16 per tile was the longest latency of the block
+          float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+          float sl[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+  #pragma unroll
+          for (int ks = 0; ks < KS; ++ks) {
+            uint32_t ah[4], al[4], kf[4];
+            ldsm_x4(ah, smem_u32(q_hi) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
+            ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
+            ldsm_x4(kf, kb + am_swz<ROWB>(t0 + k_row, ks * 2 + k_ch));
+            mma_bf16_16816(s[0], ah, kf[0], kf[1]);
+            mma_bf16_16816(sl[0], al, kf[0], kf[1]);
+            mma_bf16_16816(s[1], ah, kf[2], kf[3]);
+            mma_bf16_16816(sl[1], al, kf[2], kf[3]);
+          }
+  #pragma unroll
+          for (int nt = 0; nt < 2; ++nt)
+  #pragma unroll
+            for (int e = 0; e < 4; ++e) s[nt][e] += sl[nt][e];
+          // masks: positions past the block's end, padded query rows, and (new region) the
+          // ancestor mask of the row
+          // (a full prefix block needs none: padded query rows are zero vectors, their scores are 0 and
+          // their results are never read)
+          float mx[2] = {-INFINITY, -INFINITY};
+          const bool need_mask = tail || cnt < PB;  // uniform over the CTA
+  #pragma unroll
+          for (int nt = 0; nt < 2; ++nt)
+  #pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const int h = e >> 1;
+              if (need_mask) {
+                const int pos = t0 + nt * 8 + 2 * tq + (e & 1);
+                bool ok = pos < cnt && mrow[h] >= 0;
+                if (ok && tail) {
+                  const int j = (b - n_blk) * PB + pos;
+                  ok = (rows->mask[mrow[h]][j >> 5] >> (j & 31)) & 1u;
+                }
+                s[nt][e] = ok ? s[nt][e] : -INFINITY;
+              }
+              mx[h] = fmaxf(mx[h], s[nt][e]);
+            }
+          float corr[2];
+  #pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 1));
+            mx[h] = fmaxf(mx[h], __shfl_xor_sync(0xffffffffu, mx[h], 2));
+            const float mn = fmaxf(mrun[h], mx[h]);
+            corr[h] = (mrun[h] == -INFINITY) ? 0.f : __expf(mrun[h] - mn);
+            mrun[h] = mn;
+            lrun[h] *= corr[h];
+          }
+          uint32_t ph[4], pl[4];  // P as the A fragment of P V: head and remainder
+  #pragma unroll
+          for (int nt = 0; nt < 2; ++nt)
+  #pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              // ex2.approx of the difference to the running maximum (<= 0): relative error ~1e-6
+              const float p0 = (s[nt][2 * h] == -INFINITY) ? 0.f : __expf(s[nt][2 * h] - mrun[h]);
+              const float p1 = (s[nt][2 * h + 1] == -INFINITY) ? 0.f : __expf(s[nt][2 * h + 1] - mrun[h]);
+              lrun[h] += p0 + p1;
+              const uint32_t hi = pack_bf16x2_rn(p0, p1);
+              const float2 hf = bf16x2_to_f32x2(hi);
+              ph[nt * 2 + h] = hi;
+              pl[nt * 2 + h] = pack_bf16x2_rn(p0 - hf.x, p1 - hf.y);
+            }
+          if (__any_sync(0xffffffffu, corr[0] != 1.f || corr[1] != 1.f)) {  // the maximum rarely moves after the first tiles
+  #pragma unroll
+            for (int t = 0; t < DN; ++t) {
+              o[t][0] *= corr[0];
+              o[t][1] *= corr[0];
+              o[t][2] *= corr[1];
+              o[t][3] *= corr[1];
+            }
+          }
+  #pragma unroll
+          for (int t = 0; t < DN; t += 2) {
+            uint32_t vf[4];
+            ldsm_x4_trans(vf, vb + am_swz<ROWB>(t0 + v_row, t + v_ch));
+            mma_bf16_16816(o[t], ph, vf[0], vf[1]);
+            mma_bf16_16816(o[t], pl, vf[0], vf[1]);
+            mma_bf16_16816(o[t + 1], ph, vf[2], vf[3]);
+            mma_bf16_16816(o[t + 1], pl, vf[2], vf[3]);
+          }
+        }
+      } else if (warp * kAmQRows < nq) {
+        // ---- wide: this warp's 16 query vectors against all 64 positions of the block --------------------
         const uint32_t kb = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vb = kb + PB * ROWB;
-        // four independent accumulation chains (head / remainder x two position tiles): a dependent
-        // HMMA chain of 16 per tile was the longest latency of the block
-        float s[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
-        float sl[2][4] = {{0.f, 0.f, 0.f, 0.f}, {0.f, 0.f, 0.f, 0.f}};
+        const int q_row = warp * kAmQRows + a_row;
+        float s[8][4];  // eight independent chains already: head and remainder products share an accumulator
+#pragma unroll
+        for (int nt = 0; nt < 8; ++nt)
+#pragma unroll
+          for (int e = 0; e < 4; ++e) s[nt][e] = 0.f;
 #pragma unroll
         for (int ks = 0; ks < KS; ++ks) {
-          uint32_t ah[4], al[4], kf[4];
-          ldsm_x4(ah, smem_u32(q_hi) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
-          ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(a_row, ks * 2 + a_ch));
-          ldsm_x4(kf, kb + am_swz<ROWB>(t0 + k_row, ks * 2 + k_ch));
-          mma_bf16_16816(s[0], ah, kf[0], kf[1]);
-          mma_bf16_16816(sl[0], al, kf[0], kf[1]);
-          mma_bf16_16816(s[1], ah, kf[2], kf[3]);
-          mma_bf16_16816(sl[1], al, kf[2], kf[3]);
+          uint32_t ah[4], al[4];
+          ldsm_x4(ah, smem_u32(q_hi) + am_swz<ROWB>(q_row, ks * 2 + a_ch));
+          ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(q_row, ks * 2 + a_ch));
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            uint32_t kf[4];
+            ldsm_x4(kf, kb + am_swz<ROWB>(j * 16 + k_row, ks * 2 + k_ch));
+            mma_bf16_16816(s[2 * j], ah, kf[0], kf[1]);
+            mma_bf16_16816(s[2 * j + 1], ah, kf[2], kf[3]);
+            mma_bf16_16816(s[2 * j], al, kf[0], kf[1]);
+            mma_bf16_16816(s[2 * j + 1], al, kf[2], kf[3]);
+          }
         }
-#pragma unroll
-        for (int nt = 0; nt < 2; ++nt)
-#pragma unroll
-          for (int e = 0; e < 4; ++e) s[nt][e] += sl[nt][e];
-        // masks: positions past the block's end, padded query rows, and (new region) the
-        // ancestor mask of the row
-        // (a full prefix block needs none: padded query rows are zero vectors, their scores are 0 and
-        // their results are never read)
         float mx[2] = {-INFINITY, -INFINITY};
         const bool need_mask = tail || cnt < PB;  // uniform over the CTA
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt)
+        for (int nt = 0; nt < 8; ++nt)
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const int h = e >> 1;
             if (need_mask) {
-              const int pos = t0 + nt * 8 + 2 * tq + (e & 1);
+              const int pos = nt * 8 + 2 * tq + (e & 1);
               bool ok = pos < cnt && mrow[h] >= 0;
               if (ok && tail) {
                 const int j = (b - n_blk) * PB + pos;
@@ -369,21 +466,7 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           mrun[h] = mn;
           lrun[h] *= corr[h];
         }
-        uint32_t ph[4], pl[4];  // P as the A fragment of P V: head and remainder
-#pragma unroll
-        for (int nt = 0; nt < 2; ++nt)
-#pragma unroll
-          for (int h = 0; h < 2; ++h) {
-            // ex2.approx of the difference to the running maximum (<= 0): relative error ~1e-6
-            const float p0 = (s[nt][2 * h] == -INFINITY) ? 0.f : __expf(s[nt][2 * h] - mrun[h]);
-            const float p1 = (s[nt][2 * h + 1] == -INFINITY) ? 0.f : __expf(s[nt][2 * h + 1] - mrun[h]);
-            lrun[h] += p0 + p1;
-            const uint32_t hi = pack_bf16x2_rn(p0, p1);
-            const float2 hf = bf16x2_to_f32x2(hi);
-            ph[nt * 2 + h] = hi;
-            pl[nt * 2 + h] = pack_bf16x2_rn(p0 - hf.x, p1 - hf.y);
-          }
-        if (__any_sync(0xffffffffu, corr[0] != 1.f || corr[1] != 1.f)) {  // the maximum rarely moves after the first tiles
+        if (__any_sync(0xffffffffu, corr[0] != 1.f || corr[1] != 1.f)) {
 #pragma unroll
           for (int t = 0; t < DN; ++t) {
             o[t][0] *= corr[0];
@@ -393,13 +476,30 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
           }
         }
 #pragma unroll
-        for (int t = 0; t < DN; t += 2) {
-          uint32_t vf[4];
-          ldsm_x4_trans(vf, vb + am_swz<ROWB>(t0 + v_row, t + v_ch));
-          mma_bf16_16816(o[t], ph, vf[0], vf[1]);
-          mma_bf16_16816(o[t], pl, vf[0], vf[1]);
-          mma_bf16_16816(o[t + 1], ph, vf[2], vf[3]);
-          mma_bf16_16816(o[t + 1], pl, vf[2], vf[3]);
+        for (int j = 0; j < 4; ++j) {  // 16 positions per step of P V
+          uint32_t ph[4], pl[4];
+#pragma unroll
+          for (int n2 = 0; n2 < 2; ++n2)
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+              const int nt = 2 * j + n2;
+              const float p0 = (s[nt][2 * h] == -INFINITY || mrun[h] == -INFINITY) ? 0.f : __expf(s[nt][2 * h] - mrun[h]);
+              const float p1 = (s[nt][2 * h + 1] == -INFINITY || mrun[h] == -INFINITY) ? 0.f : __expf(s[nt][2 * h + 1] - mrun[h]);
+              lrun[h] += p0 + p1;
+              const uint32_t hi = pack_bf16x2_rn(p0, p1);
+              const float2 hf = bf16x2_to_f32x2(hi);
+              ph[n2 * 2 + h] = hi;
+              pl[n2 * 2 + h] = pack_bf16x2_rn(p0 - hf.x, p1 - hf.y);
+            }
+#pragma unroll
+          for (int t = 0; t < DN; t += 2) {
+            uint32_t vf[4];
+            ldsm_x4_trans(vf, vb + am_swz<ROWB>(j * 16 + v_row, t + v_ch));
+            mma_bf16_16816(o[t], ph, vf[0], vf[1]);
+            mma_bf16_16816(o[t], pl, vf[0], vf[1]);
+            mma_bf16_16816(o[t + 1], ph, vf[2], vf[3]);
+            mma_bf16_16816(o[t + 1], pl, vf[2], vf[3]);
+          }
         }
       }
       __syncwarp();
@@ -408,79 +508,110 @@ __global__ void __launch_bounds__(kAmThreads, 2) k_tree_attention_mma(const Attn
     }
     am_consumer_sync();  // every warp is done with the ring: the merge scratch aliases it
 
+    if constexpr (QT == 1) {
     // ---- merge the four warps (fixed order), then hand the chunk's partial on ------
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-      lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 1);
-      lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 2);
-      const int r = g + 8 * h;
-      if (r < nq) {
-        float* w = wsm + (static_cast<size_t>(warp) * QR + r) * WSTR;
-#pragma unroll
-        for (int t = 0; t < DN; ++t)
-          *reinterpret_cast<float2*>(w + t * 8 + 2 * tq) = make_float2(o[t][2 * h], o[t][2 * h + 1]);
-        if (tq == 0) { w[DH] = mrun[h]; w[DH + 1] = lrun[h]; }
+  #pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 1);
+        lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 2);
+        const int r = g + 8 * h;
+        if (r < nq) {
+          float* w = wsm + (static_cast<size_t>(warp) * QR + r) * WSTR;
+  #pragma unroll
+          for (int t = 0; t < DN; ++t)
+            *reinterpret_cast<float2*>(w + t * 8 + 2 * tq) = make_float2(o[t][2 * h], o[t][2 * h + 1]);
+          if (tq == 0) { w[DH] = mrun[h]; w[DH + 1] = lrun[h]; }
+        }
       }
-    }
-    am_consumer_sync();
-    for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
-      const int r = idx / DH, dd = idx % DH;
-      const int qv = qv0 + r;
-      float mm = -INFINITY;
-      for (int w = 0; w < kAmWarps; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
-      float ll = 0.f, oo = 0.f;
-      for (int w = 0; w < kAmWarps; ++w) {
-        const float* rr = wsm + (w * QR + r) * WSTR;
-        const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
-        ll += rr[DH + 1] * cw;
-        oo += rr[dd] * cw;
+      am_consumer_sync();
+      for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
+        const int r = idx / DH, dd = idx % DH;
+        const int qv = qv0 + r;
+        float mm = -INFINITY;
+        for (int w = 0; w < kAmWarps; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
+        float ll = 0.f, oo = 0.f;
+        for (int w = 0; w < kAmWarps; ++w) {
+          const float* rr = wsm + (w * QR + r) * WSTR;
+          const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
+          ll += rr[DH + 1] * cw;
+          oo += rr[dd] * cw;
+        }
+        float* rr = crec + static_cast<size_t>(r) * WSTR;
+        rr[dd] = oo;
+        if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
       }
-      float* rr = crec + static_cast<size_t>(r) * WSTR;
-      rr[dd] = oo;
-      if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
+    } else {
+      // wide: every warp owns its query vectors; its state is this CTA's record of them
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 1);
+        lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 2);
+        const int r = warp * kAmQRows + g + 8 * h;
+        if (r < nq) {
+          float* w = crec + static_cast<size_t>(r) * WSTR;
+#pragma unroll
+          for (int t = 0; t < DN; ++t)
+            *reinterpret_cast<float2*>(w + t * 8 + 2 * tq) = make_float2(o[t][2 * h], o[t][2 * h + 1]);
+          if (tq == 0) { w[DH] = mrun[h]; w[DH + 1] = lrun[h]; }
+        }
+      }
     }
     // ---- merge the chunks of the cluster in rank order through distributed shared memory ----
     cluster_sync_all();  // every CTA's record is complete and visible cluster-wide
-    {  // every rank merges its slice of the head dimension (the work of the merge is spread over the cluster)
+    {  // every rank merges its slice of the head dimension (the work of the merge is spread over the cluster),
+       // four consecutive d per thread and step: one 16-byte distributed-shared-memory load per rank
       const uint32_t crec_u = smem_u32(crec);
-      const int slice = (DH + CS - 1) / CS;
-      for (int idx = tid; idx < nq * slice; idx += kAmConsumers) {
-        const int r = idx / slice, dd = crank * slice + idx % slice;
-        if (dd >= DH) continue;
+      const int slice4 = (DH / 4 + CS - 1) / CS;  // float4 groups per rank
+      for (int idx = tid; idx < nq * slice4; idx += kAmConsumers) {
+        const int r = idx / slice4, d4 = crank * slice4 + idx % slice4;
+        if (d4 >= DH / 4) continue;
+        const int dd = d4 * 4;
         const int qv = qv0 + r;
         const uint32_t ra = crec_u + static_cast<uint32_t>(r * WSTR) * 4;
-        float mk[8], lk[8], ok[8];
+        float mk[8], lk[8];
+        float4 ok[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           mk[k] = -INFINITY;
           lk[k] = 0.f;
-          ok[k] = 0.f;
+          ok[k] = make_float4(0.f, 0.f, 0.f, 0.f);
           if (k < CS) {
-            mk[k] = ld_dsmem_f32(ra + DH * 4, k);
-            lk[k] = ld_dsmem_f32(ra + (DH + 1) * 4, k);
-            ok[k] = ld_dsmem_f32(ra + dd * 4, k);
+            uint32_t rk;
+            asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(rk) : "r"(ra), "r"(static_cast<uint32_t>(k)));
+            asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(mk[k]), "=f"(lk[k]) : "r"(rk + DH * 4) : "memory");
+            asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];"
+                         : "=f"(ok[k].x), "=f"(ok[k].y), "=f"(ok[k].z), "=f"(ok[k].w)
+                         : "r"(rk + dd * 4)
+                         : "memory");
           }
         }
         float mm = -INFINITY;
 #pragma unroll
         for (int k = 0; k < 8; ++k) mm = fmaxf(mm, mk[k]);
-        float ll = 0.f, oo = 0.f;
+        float ll = 0.f;
+        float4 oo = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           const float cw = (mk[k] == -INFINITY) ? 0.f : expf(mk[k] - mm);
           ll += lk[k] * cw;
-          oo += ok[k] * cw;
+          oo.x += ok[k].x * cw;
+          oo.y += ok[k].y * cw;
+          oo.z += ok[k].z * cw;
+          oo.w += ok[k].w * cw;
         }
         if (n_groups == 1) {
           const int m = qv / grp, hq = hk * grp + qv % grp;
-          {
-            const float ov = oo / ll;
-            p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
-            if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+          const float4 ov = make_float4(oo.x / ll, oo.y / ll, oo.z / ll, oo.w / ll);
+          *reinterpret_cast<float4*>(p.obuf + static_cast<size_t>(m) * dq + hq * DH + dd) = ov;
+          if (p.so.xs) {
+            store_split(p.so, m, hq * DH + dd, ov.x);
+            store_split(p.so, m, hq * DH + dd + 1, ov.y);
+            store_split(p.so, m, hq * DH + dd + 2, ov.z);
+            store_split(p.so, m, hq * DH + dd + 3, ov.w);
           }
         } else {
           float* rr = p.ws + ((static_cast<size_t>(hk) * n_groups + group) * p.qv_cap + qv) * WSTR;
-          rr[dd] = oo;
+          *reinterpret_cast<float4*>(rr + dd) = oo;
           if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
         }
       }

@@ -96,6 +96,7 @@ struct dovetail_draft {
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
   int umma_dbg = 0;
+  int attn_wide_min = 32;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
   struct PlaneBuf { const __nv_bfloat16* base; int64_t elems, ld; int cap, map; };
@@ -257,8 +258,10 @@ cudaError_t set_max_smem_all() {
   for (int nt = 1; nt <= 8; nt *= 2)
     for (int wq = 0; wq < 2; ++wq) set(reinterpret_cast<const void*>(pick_gemv_mma(nt, wq)));
   set(reinterpret_cast<const void*>(k_gemv_umma));
-  set(reinterpret_cast<const void*>(k_tree_attention_mma<64>));
-  set(reinterpret_cast<const void*>(k_tree_attention_mma<128>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 1>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 1>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 4>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 4>));
   const int mts[3] = {1, 2, 4};
   for (int mt : mts) {
     set(reinterpret_cast<const void*>(pick_gemv<__nv_bfloat16>(mt, 3)));
@@ -869,9 +872,10 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
 // Chunks per kv-head of the tensor-core attention kernel (measured on C2 / C3 / C5): at least two 64-position
 // blocks per chunk (a CTA's fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one
 // cluster of 8 no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
-void attn_mma_geom(const dovetail_draft* h, int Lbase, int& n_chunks, int& cs) {
+// wide: the 64-query-vector kernel (one CTA per SM).
+void attn_mma_geom(const dovetail_draft* h, int Lbase, bool wide, int& n_chunks, int& cs) {
   const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
-  n_chunks = std::max(1, std::min(h->attn_chunks_cap, n_blocks / 2));
+  n_chunks = std::max(1, std::min(wide ? std::max(1, h->attn_chunks_cap / 2) : h->attn_chunks_cap, n_blocks / 2));
   if (n_chunks <= 8) {
     n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
     cs = n_chunks;
@@ -1114,11 +1118,14 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
           a.cap = kv->capacity;
           a.Lbase = Lbase;
           a.Lsafe = L;
+          // more than 32 query vectors: 64 per pass over the cache, one query tile per warp (attention_mma.cuh)
+          const bool wide_q = qv_tot > h->attn_wide_min;
           int n_chunks, cs;
-          attn_mma_geom(h, Lbase, n_chunks, cs);
-          const size_t smem = am_smem_bytes(dh);
-          e = launch_c(h, cs, true, dh == 128 ? k_tree_attention_mma<128> : k_tree_attention_mma<64>, dim3(n_chunks, c.n_kv_heads),
-                       dim3(kAmThreads), smem, st, a);
+          attn_mma_geom(h, Lbase, wide_q, n_chunks, cs);
+          const size_t smem = am_smem_bytes(dh, wide_q ? 4 : 1);
+          auto kern = wide_q ? (dh == 128 ? k_tree_attention_mma<128, 4> : k_tree_attention_mma<64, 4>)
+                             : (dh == 128 ? k_tree_attention_mma<128, 1> : k_tree_attention_mma<64, 1>);
+          e = launch_c(h, cs, true, kern, dim3(n_chunks, c.n_kv_heads), dim3(kAmThreads), smem, st, a);
         } else {
           int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
           const int QT = qv_tot == 1 ? 1 : (qv_tot == 2 ? 2 : 4);
@@ -1281,8 +1288,12 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
   for (int l = 0; l < tree->depth; ++l) { key.push_back(tree->branch[l]); key.push_back(tree->beam[l]); }
   int nc[2] = {0, 0}, cs[2] = {0, 0};
   if (bf16) {
-    attn_mma_geom(h, L, nc[0], cs[0]);
-    attn_mma_geom(h, Lp, nc[1], cs[1]);
+    attn_mma_geom(h, L, false, nc[0], cs[0]);
+    attn_mma_geom(h, Lp, false, nc[1], cs[1]);
+    int wn[2], wc[2];  // the wide kernel's geometry (which levels take it follows from the tree and n_new)
+    attn_mma_geom(h, L, true, wn[0], wc[0]);
+    attn_mma_geom(h, Lp, true, wn[1], wc[1]);
+    key.insert(key.end(), {wn[0], wc[0], wn[1], wc[1], h->attn_wide_min});
   } else {
     nc[0] = std::min(h->attn_chunks_cap, std::max(1, div_up(L, 2 * kAttnStagePos)));
     nc[1] = std::min(h->attn_chunks_cap, std::max(1, div_up(Lp, 2 * kAttnStagePos)));
@@ -1323,7 +1334,8 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
         ng.begin_params = kp;
         ng.begin_args.assign(kp.kernelParams, kp.kernelParams + 11);  // k_step_begin takes 11 arguments
         ng.begin_dv = *static_cast<const StepDyn*>(kp.kernelParams[0]);
-      } else if (kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128>)) {
+      } else if (kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64, 1>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128, 1>) ||
+                 kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64, 4>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128, 4>)) {
         ng.attn_nodes.push_back(nd);
         ng.attn_node_params.push_back(kp);
         ng.attn_params.push_back(*static_cast<const AttnParams*>(kp.kernelParams[0]));
@@ -1471,7 +1483,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     A(dmalloc(&h->xs_emb, kSplitPlanes * R * h->ld_d));
     if (!c.weight_quant) A(dmalloc(&h->xs_par, kSplitPlanes * R * h->ld_d));
   }
-  A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 2)));
+  A(dmalloc(&h->attn_ws, static_cast<size_t>(c.n_kv_heads) * h->attn_chunks_cap * h->qv_cap * (c.head_dim + 4)));
   A(dmalloc(&h->attn_cnt, c.n_kv_heads));
   A(dmalloc(&h->cand_val, R * h->num_sms * kMaxBranch));
   A(dmalloc(&h->cand_id, R * h->num_sms * kMaxBranch));
@@ -1790,6 +1802,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
     return DOVETAIL_OK;
   }
   if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
+  if (key == DOVETAIL_TUNE_ATTN_WIDE_MIN && value >= 0 && value <= 4096) { h->attn_wide_min = value; return DOVETAIL_OK; }
   if (key == 99) { h->umma_dbg = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
