@@ -227,19 +227,21 @@ def bench_one(a, cfg, rank, world, local, dist):
         kv.committed_len = case.L  # untimed bookkeeping: discard the tree rows (kv_commit mode 0 semantics)
         binding.dovetail_draft_step(hh, case.feats, case.tokens, kv, tree, out)
 
-    # host-side buffers of the end-to-end path
-    feats_h = case.feats.cpu().pin_memory()
-    tok_h = case.tokens.cpu().pin_memory()
-    feats_d, tok_d = torch.empty_like(case.feats), torch.empty_like(case.tokens)
-    out_h = {k: torch.empty_like(v, device="cpu").pin_memory() for k, v in out.items()}
+    # host-side buffers of the end-to-end path: inputs in one pinned buffer (features, then the token ids as raw
+    # words), outputs in one pinned buffer (binding.alloc_out packs the step's outputs into one allocation)
+    n_f = case.feats.numel()
+    in_h = torch.empty(n_f + case.tokens.numel(), dtype=torch.float32).pin_memory()
+    in_h[:n_f] = case.feats.cpu().reshape(-1)
+    in_h[n_f:].view(torch.int32)[:] = case.tokens.cpu()
+    in_d = torch.empty_like(in_h, device="cuda")
+    feats_d, tok_d = in_d[:n_f].view(case.feats.shape), in_d[n_f:].view(torch.int32)
+    out_h = torch.empty_like(out["_packed"], device="cpu").pin_memory()
 
     def step_e2e():
         kv.committed_len = case.L
-        feats_d.copy_(feats_h, non_blocking=True)
-        tok_d.copy_(tok_h, non_blocking=True)
+        in_d.copy_(in_h, non_blocking=True)
         binding.dovetail_draft_step(h, feats_d, tok_d, kv, tree, out)
-        for k2 in out_h:
-            out_h[k2].copy_(out[k2], non_blocking=True)
+        out_h.copy_(out["_packed"], non_blocking=True)
         stream.synchronize()  # the caller consumes the candidates before the next round
 
     def timed(fn, steps):
@@ -397,8 +399,7 @@ def bench_one(a, cfg, rank, world, local, dist):
             "step_frac_of_8tbs_nominal": step_bytes / (step_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
             "algorithmic_bytes_per_step": step_bytes,
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": ms_e2e / K,
-                    "h2d_bytes_per_step": feats_h.numel() * 4 + tok_h.numel() * 4,
-                    "d2h_bytes_per_step": sum(v.numel() * v.element_size() for v in out_h.values())},
+                    "h2d_bytes_per_step": in_h.numel() * 4, "d2h_bytes_per_step": out_h.numel() * 4},
             "gpu_launches": launches, "launch": launch_modes, "clocks": clk, "roofline": roof}
 
     # ---- prompt / catch-up rows (dovetail_draft_prefill), batches of 64 rows -----------------

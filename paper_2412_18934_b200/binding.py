@@ -241,12 +241,12 @@ def dovetail_draft_init(top: Dict, layers: List[Dict], cfg: DraftConfig, max_row
 
 
 def alloc_out(gamma: int, device="cuda"):
+    """Output buffers of a step as views of ONE device allocation (out["_packed"], int32 words: ids | scores |
+    parents | depths | n_out), so that a caller can bring the whole result to the host with a single copy."""
     import torch
-    return dict(token_ids=torch.zeros(gamma, dtype=torch.int32, device=device),
-                scores=torch.zeros(gamma, dtype=torch.float32, device=device),
-                parents=torch.zeros(gamma, dtype=torch.int32, device=device),
-                depths=torch.zeros(gamma, dtype=torch.int32, device=device),
-                n_out=torch.zeros(1, dtype=torch.int32, device=device))
+    buf = torch.zeros(4 * gamma + 4, dtype=torch.int32, device=device)
+    return dict(token_ids=buf[0:gamma], scores=buf[gamma:2 * gamma].view(torch.float32), parents=buf[2 * gamma:3 * gamma],
+                depths=buf[3 * gamma:4 * gamma], n_out=buf[4 * gamma:4 * gamma + 1], _packed=buf)
 
 
 def _out_t(out: Dict) -> DraftOutT:
