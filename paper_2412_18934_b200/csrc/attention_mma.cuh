@@ -199,6 +199,7 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
         const uint32_t kdst = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vdst = kdst + PB * ROWB;
         const uint8_t* ksrc = reinterpret_cast<const uint8_t*>(kc + static_cast<size_t>(pos0) * DH);
         const uint8_t* vsrc = reinterpret_cast<const uint8_t*>(vc + static_cast<size_t>(pos0) * DH);
+        if (!((p.dbg & 1) && round > 0))
 #pragma unroll 4
         for (int i = ptid; i < PB * CPR; i += kAmProducers) {
           const int r = i / CPR, ch = i % CPR;
@@ -524,20 +525,26 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
         }
       }
       am_consumer_sync();
-      for (int idx = tid; idx < nq * DH; idx += kAmConsumers) {
-        const int r = idx / DH, dd = idx % DH;
-        const int qv = qv0 + r;
+      for (int idx = tid; idx < nq * (DH / 4); idx += kAmConsumers) {  // four d per thread: one set of weights per float4
+        const int r = idx / (DH / 4), dd = (idx % (DH / 4)) * 4;
         float mm = -INFINITY;
+#pragma unroll
         for (int w = 0; w < kAmWarps; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
-        float ll = 0.f, oo = 0.f;
+        float ll = 0.f;
+        float4 oo = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
         for (int w = 0; w < kAmWarps; ++w) {
           const float* rr = wsm + (w * QR + r) * WSTR;
           const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
+          const float4 ov = *reinterpret_cast<const float4*>(rr + dd);
           ll += rr[DH + 1] * cw;
-          oo += rr[dd] * cw;
+          oo.x += ov.x * cw;
+          oo.y += ov.y * cw;
+          oo.z += ov.z * cw;
+          oo.w += ov.w * cw;
         }
         float* rr = crec + static_cast<size_t>(r) * WSTR;
-        rr[dd] = oo;
+        *reinterpret_cast<float4*>(rr + dd) = oo;
         if (dd == 0) { rr[DH] = mm; rr[DH + 1] = ll; }
       }
     } else {

@@ -96,6 +96,7 @@ struct dovetail_draft {
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
   int umma_dbg = 0;
+  int attn_max_clusters[2][9] = {};  // [wide][cluster size]: clusters of the attention kernel resident at once
   int attn_wide_min = 16;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
@@ -873,15 +874,30 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
 // blocks per chunk (a CTA's fixed cost is ~6 us), at most two CTAs per SM, and when a head needs more than one
 // cluster of 8 no more than ~200 CTAs in all (larger grids of 8-clusters are placed in waves).
 // wide: the 64-query-vector kernel (one CTA per SM).
+// All clusters of a launch must be resident at once: a cluster is placed on one GPC, and the second wave of a grid
+// that does not fit costs a whole kernel time (measured on the 13B shape, 40 heads, prefix 2048: 7 chunks per head
+// 24.2 us, 6 chunks 14.0 us). attn_max_clusters[wide][cs] = cudaOccupancyMaxActiveClusters of the kernel at cluster
+// size cs (dovetail_draft_init); 0 = unknown.
 void attn_mma_geom(const dovetail_draft* h, int Lbase, bool wide, int& n_chunks, int& cs) {
   const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
+  const int Hkv = h->cfg.n_kv_heads;
+  const int* maxc = h->attn_max_clusters[wide ? 1 : 0];
   n_chunks = std::max(1, std::min(wide ? std::max(1, h->attn_chunks_cap / 2) : h->attn_chunks_cap, n_blocks / 2));
   if (n_chunks <= 8) {
+    while (n_chunks > 1 && maxc[n_chunks] > 0 && Hkv > maxc[n_chunks]) --n_chunks;
     n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
     cs = n_chunks;
   } else {
-    n_chunks = std::max(8, std::min(n_chunks, 200 / h->cfg.n_kv_heads) / 8 * 8);
-    cs = 8;
+    int groups = std::max(1, std::min(n_chunks, 200 / Hkv) / 8);
+    if (maxc[8] > 0) groups = std::max(1, std::min(groups, maxc[8] / Hkv));
+    if (maxc[8] > 0 && Hkv > maxc[8]) {  // not even one 8-cluster per head fits: smaller clusters, one per head
+      n_chunks = 7;
+      while (n_chunks > 1 && maxc[n_chunks] > 0 && Hkv > maxc[n_chunks]) --n_chunks;
+      cs = n_chunks;
+    } else {
+      n_chunks = 8 * groups;
+      cs = 8;
+    }
   }
 }
 
@@ -1112,6 +1128,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         a.trace = trace_slot(h);
         a.so = planes(h, h->xs_o, R, h->ld_dq);
         a.qs = fused_s2 ? h->qs : nullptr;
+        a.dbg = h->umma_dbg >> 4;
         if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
           a.kc = kv->k;
           a.vc = kv->v;
@@ -1514,6 +1531,27 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
     return code;
   }
   if (es == 2 && !c.weight_quant) umma_init(h);
+  if (es == 2) {  // how many clusters of each size the tensor-core attention kernel can have resident (attn_mma_geom)
+    for (int wide = 0; wide < 2; ++wide)
+      for (int cs = 1; cs <= 8; ++cs) {
+        cudaLaunchConfig_t lc{};
+        lc.gridDim = dim3(cs, c.n_kv_heads);
+        lc.blockDim = dim3(kAmThreads);
+        lc.dynamicSmemBytes = am_smem_bytes(c.head_dim, wide ? 4 : 1);
+        cudaLaunchAttribute at{};
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = cs;
+        at.val.clusterDim.y = 1;
+        at.val.clusterDim.z = 1;
+        lc.attrs = &at;
+        lc.numAttrs = 1;
+        const void* fn = wide ? (c.head_dim == 128 ? reinterpret_cast<const void*>(k_tree_attention_mma<128, 4>) : reinterpret_cast<const void*>(k_tree_attention_mma<64, 4>))
+                              : (c.head_dim == 128 ? reinterpret_cast<const void*>(k_tree_attention_mma<128, 1>) : reinterpret_cast<const void*>(k_tree_attention_mma<64, 1>));
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, fn, &lc) == cudaSuccess) h->attn_max_clusters[wide][cs] = n;
+        else cudaGetLastError();
+      }
+  }
   *out = h;
   return DOVETAIL_OK;
 }
@@ -1791,6 +1829,7 @@ int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
   if (!h) return -1;
   if (key == DOVETAIL_STAT_UMMA_LAUNCHES) return h->last_umma_launches;
   if (key == DOVETAIL_STAT_GRAPH) return h->last_graph;
+  if (key >= 100 && key < 118) return h->attn_max_clusters[(key - 100) / 9][(key - 100) % 9];
   return -1;
 }
 
@@ -1803,6 +1842,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
   }
   if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
   if (key == DOVETAIL_TUNE_ATTN_WIDE_MIN && value >= 0 && value <= 4096) { h->attn_wide_min = value; return DOVETAIL_OK; }
+  if (key == 98 && value >= 1) { h->attn_chunks_cap = value; return DOVETAIL_OK; }
   if (key == 99) { h->umma_dbg = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
