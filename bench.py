@@ -164,6 +164,11 @@ def all_configs():
     cfgs.update({c.name: c for c in depth_sweep()})
     cfgs.update({c.name: c for c in int8_variants()})
     cfgs.update({c.name.split("_")[0] + "_int8": c for c in int8_variants()})  # c2_int8, c3_int8, c5_int8
+    # the tree the paper itself runs (width 10, depth 7, 16 candidates) on the 7B / 13B shapes
+    import dataclasses
+    from paper_2412_18934_b200.configs import paper_preset
+    for base in ("c2", "c3"):
+        cfgs[base + "_paper_tree"] = dataclasses.replace(CONFIGS[base], name=CONFIGS[base].name + "_paper_tree", tree=paper_preset(True))
     return cfgs
 
 
@@ -509,7 +514,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfgs = all_configs()
     if a.config == "all":
-        names = ["c1", "c2", "c5", "c2_int8", "c3_int8", "c5_int8"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
+        names = ["c1", "c2", "c5", "c2_int8", "c3_int8", "c5_int8", "c2_paper_tree", "c3_paper_tree"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
     else:
         names = [a.config]
     for i, name in enumerate(names):

@@ -198,14 +198,12 @@ __device__ __forceinline__ bool node_before(const float* cum, int a, int b) {
   return ca > cb || (ca == cb && a < b);
 }
 
-constexpr int kTreeThreads = 256;
+constexpr int kTreeThreads = 512;  // one warp per expanded row for levels of <= 16 rows (a row's merge is a serial chain)
 constexpr int kPoolSmem = 4352;  // >= kMaxBranch + kMaxTreeSlots * kMaxBranch + slack
 
 __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelParams p) {
-  // phase A stages candidate lists (3 x kCandSmem words); phases B / C reuse the space for the pool scores
-  constexpr int kCandSmem = 3072;
-  static_assert(3 * kCandSmem >= 2 * kPoolSmem, "shared staging too small for the pool");
-  __shared__ float s_raw[3 * kCandSmem];
+  // phases B / C: pool scores and keep flags
+  __shared__ float s_raw[2 * kPoolSmem];
   __shared__ int32_t s_cnt[kTreeThreads + 1];
   float* s_cum = s_raw;
   int32_t* s_new = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);
@@ -216,123 +214,92 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   const Pool& P = p.pool;
 
   // ---- phase A: children of each expanded row --------------------------------
-  // The per-CTA top-b lists and softmax statistics of a group of rows are first brought into
-  // shared memory with independent loads (one L2 round trip); each row is then merged by one warp.
-  float* s_cv = s_raw;
-  int32_t* s_ci = reinterpret_cast<int32_t*>(s_raw + kCandSmem);
-  float* s_st = s_raw + 2 * kCandSmem;
-  const int per_row = p.rp_tokens ? 0 : p.nct * p.b;
-  int G = per_row > 0 ? min(kCandSmem / per_row, (kCandSmem / 2) / max(p.nct, 1)) : 0;  // rows per group
-  G = min(G, p.M);
-  for (int g0 = 0; g0 < p.M; g0 += max(G, 1)) {
-    const int gr = G > 0 ? min(G, p.M - g0) : 0;
-    if (gr > 0) {
-      const int n_c = gr * per_row;
-      for (int base = 0; base < n_c; base += kTreeThreads * 4) {
-        float v[4];
-        int id[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int idx = base + i * kTreeThreads + tid;
-          v[i] = 0.f;
-          id[i] = 0;
-          if (idx < n_c) {
-            const int mc = idx / p.b, j = idx - mc * p.b;  // mc = (row in group) * nct + cta
-            const size_t o = (static_cast<size_t>(g0) * p.nct + mc) * kMaxBranch + j;
-            v[i] = p.cand_val[o];
-            id[i] = p.cand_id[o];
-          }
-        }
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          const int idx = base + i * kTreeThreads + tid;
-          if (idx < n_c) { s_cv[idx] = v[i]; s_ci[idx] = id[i]; }
-        }
+  // One warp per row. The row's global top-b is a b-round merge of the per-CTA lists, each of which is sorted in the
+  // strict candidate order (gemv.cuh EPI_LMHEAD). Lane l owns the lists of CTAs l, l + 32, ... and keeps a window
+  // of two entries per list in registers: a round picks the best head of the warp, the owning lane shifts that
+  // list's window and requests the entry after it -- needed only if the same list wins twice more, so its L2
+  // round trip is off the critical path. (Staging whole lists through shared memory, two rows at a time, cost
+  // 53 us per level at 10 rows x 10 children; this takes the lists where they are.)
+  for (int m = warp; m < p.M; m += kTreeThreads / 32) {
+    const int parent = p.cur->pool[m];
+    const float pcum = parent < 0 ? 0.f : P.cum[parent];
+    const int base = p.pool_begin + m * p.b;
+    if (p.rp_tokens) {
+      if (lane < p.b) {
+        const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
+        P.token[base + lane] = p.rp_tokens[o];
+        P.parent[base + lane] = parent;
+        P.depth[base + lane] = p.level + 1;
+        P.cum[base + lane] = pcum + p.rp_logp[o];
+        P.row[base + lane] = -1;
       }
-      for (int idx = tid; idx < gr * p.nct * 2; idx += kTreeThreads) s_st[idx] = p.stat[static_cast<size_t>(g0) * p.nct * 2 + idx];
-      __syncthreads();
+      continue;
     }
-    const int m_end = G > 0 ? g0 + gr : p.M;
-    for (int m = g0 + warp; m < m_end; m += kTreeThreads / 32) {
-      const int parent = p.cur->pool[m];
-      const float pcum = parent < 0 ? 0.f : P.cum[parent];
-      const int base = p.pool_begin + m * p.b;
-      if (p.rp_tokens) {
-        if (lane < p.b) {
-          const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
-          P.token[base + lane] = p.rp_tokens[o];
-          P.parent[base + lane] = parent;
-          P.depth[base + lane] = p.level + 1;
-          P.cum[base + lane] = pcum + p.rp_logp[o];
-          P.row[base + lane] = -1;
-        }
-        continue;
-      }
-      // candidates and statistics of this row: shared memory (grouped) or global (lists too long)
-      const float* st = gr > 0 ? s_st + (m - g0) * p.nct * 2 : p.stat + static_cast<size_t>(m) * p.nct * 2;
-      const float* cv = gr > 0 ? s_cv + (m - g0) * per_row : p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
-      const int32_t* ci = gr > 0 ? s_ci + (m - g0) * per_row : p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
-      const int cstride = gr > 0 ? p.b : kMaxBranch;
-      // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order
-      float mg = -INFINITY;
-      for (int c = lane; c < p.nct; c += 32) mg = fmaxf(mg, st[c * 2]);
-      mg = warp_max(mg);
-      float se = 0.f;
-      for (int c = lane; c < p.nct; c += 32) {
-        const float mc = st[c * 2];
-        se += (mc == -INFINITY) ? 0.f : st[c * 2 + 1] * expf(mc - mg);
-      }
-      se = warp_sum(se);
-      const float logz = mg + logf(se);
-      // global top-b of the row: a b-round merge of the per-CTA lists, each of which is sorted in the strict
-      // candidate order (gemv.cuh EPI_LMHEAD). Lane l owns the lists of CTAs l, l + 32, ... and keeps their current
-      // heads in registers; a round picks the best head of the warp and the owning lane advances that list.
-      constexpr int kLists = 8;  // lists per lane: nct <= 256
-      float hv[kLists];
-      int hi[kLists], hp[kLists];
+    const float* st = p.stat + static_cast<size_t>(m) * p.nct * 2;
+    const float* cv = p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
+    const int32_t* ci = p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
+    constexpr int kLists = 8;  // lists per lane: nct <= 256 (host)
+    float hv[kLists], nv[kLists], smx[kLists], sse[kLists];
+    int hi[kLists], ni[kLists], hp[kLists];
 #pragma unroll
-      for (int k = 0; k < kLists; ++k) {
-        const int c = lane + 32 * k;
-        hp[k] = 0;
-        hv[k] = -INFINITY;
-        hi[k] = 0x7fffffff;
-        if (c < p.nct) { hv[k] = cv[c * cstride]; hi[k] = ci[c * cstride]; }
-      }
-      for (int jb = 0; jb < p.b; ++jb) {
-        float bv = -INFINITY;
-        int bi = 0x7fffffff;
-#pragma unroll
-        for (int k = 0; k < kLists; ++k)
-          if (cand_before(hv[k], hi[k], bv, bi)) { bv = hv[k]; bi = hi[k]; }
-        const int mine = bi;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-          if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-        }
-        if (mine == bi && bi != 0x7fffffff) {  // token ids are unique across the lists: exactly one lane advances
-#pragma unroll
-          for (int k = 0; k < kLists; ++k) {
-            if (hi[k] == bi) {
-              const int c = lane + 32 * k;
-              ++hp[k];
-              if (hp[k] < p.b) { hv[k] = cv[c * cstride + hp[k]]; hi[k] = ci[c * cstride + hp[k]]; }
-              else { hv[k] = -INFINITY; hi[k] = 0x7fffffff; }
-            }
-          }
-        }
-        if (lane == 0) {
-          P.token[base + jb] = bi;
-          P.parent[base + jb] = parent;
-          P.depth[base + jb] = p.level + 1;
-          P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
-          P.row[base + jb] = -1;
-        }
+    for (int k = 0; k < kLists; ++k) {  // every load of the row is issued before the first use
+      const int c = lane + 32 * k;
+      hp[k] = 0;
+      hv[k] = nv[k] = smx[k] = -INFINITY;
+      hi[k] = ni[k] = 0x7fffffff;
+      sse[k] = 0.f;
+      if (c < p.nct) {
+        hv[k] = __ldcg(cv + c * kMaxBranch);
+        hi[k] = __ldcg(ci + c * kMaxBranch);
+        if (p.b > 1) { nv[k] = __ldcg(cv + c * kMaxBranch + 1); ni[k] = __ldcg(ci + c * kMaxBranch + 1); }
+        smx[k] = __ldcg(st + c * 2);
+        sse[k] = __ldcg(st + c * 2 + 1);
       }
     }
-    if (G == 0) break;     // ungrouped: the loop above covered every row
-    __syncthreads();       // the group's staging is reused
+    // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order (lane-major, then butterfly)
+    float mg = -INFINITY;
+#pragma unroll
+    for (int k = 0; k < kLists; ++k) mg = fmaxf(mg, smx[k]);
+    mg = warp_max(mg);
+    float se = 0.f;
+#pragma unroll
+    for (int k = 0; k < kLists; ++k) se += (smx[k] == -INFINITY) ? 0.f : sse[k] * expf(smx[k] - mg);
+    se = warp_sum(se);
+    const float logz = mg + logf(se);
+    for (int jb = 0; jb < p.b; ++jb) {
+      float bv = -INFINITY;
+      int bi = 0x7fffffff;
+#pragma unroll
+      for (int k = 0; k < kLists; ++k)
+        if (cand_before(hv[k], hi[k], bv, bi)) { bv = hv[k]; bi = hi[k]; }
+      const int mine = bi;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
+        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+        if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
+      }
+      if (mine == bi && bi != 0x7fffffff) {  // token ids are unique across the lists: exactly one lane advances
+#pragma unroll
+        for (int k = 0; k < kLists; ++k) {
+          if (hi[k] == bi) {
+            const int c = lane + 32 * k;
+            ++hp[k];
+            hv[k] = nv[k];
+            hi[k] = ni[k];
+            if (hp[k] + 1 < p.b) { nv[k] = __ldcg(cv + c * kMaxBranch + hp[k] + 1); ni[k] = __ldcg(ci + c * kMaxBranch + hp[k] + 1); }
+            else { nv[k] = -INFINITY; ni[k] = 0x7fffffff; }
+          }
+        }
+      }
+      if (lane == 0) {
+        P.token[base + jb] = bi;
+        P.parent[base + jb] = parent;
+        P.depth[base + jb] = p.level + 1;
+        P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
+        P.row[base + jb] = -1;
+      }
+    }
   }
   __syncthreads();
 
@@ -393,9 +360,22 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   for (int i = lo; i < hi; ++i) cnt += s_new[i];
   s_cnt[tid + 1] = cnt;
   __syncthreads();
-  if (tid == 0) {
-    s_cnt[0] = 0;
-    for (int i = 1; i <= kTreeThreads; ++i) s_cnt[i] += s_cnt[i - 1];
+  if (warp == 0) {  // inclusive prefix over the per-thread counts: kTreeThreads / 32 entries per lane, then a warp scan
+    constexpr int E = kTreeThreads / 32;
+    int loc = 0;
+    for (int j = 0; j < E; ++j) loc += s_cnt[1 + lane * E + j];
+    int inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int v = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += v;
+    }
+    int run2 = inc - loc;
+    for (int j = 0; j < E; ++j) {
+      run2 += s_cnt[1 + lane * E + j];
+      s_cnt[1 + lane * E + j] = run2;
+    }
+    if (lane == 0) s_cnt[0] = 0;
   }
   __syncthreads();
   int run = s_cnt[tid];
