@@ -49,7 +49,6 @@ struct AttnParams {
   int32_t cap, Lbase;
   int32_t Lsafe;           // committed_len at step entry: rows below it are never written by the step
   unsigned long long* trace;  // dovetail_trace_*: {first CTA start, last CTA end} of this launch, or NULL
-  int32_t dbg;
 };
 
 struct SoftState {  // running (max, sum) of one query vector

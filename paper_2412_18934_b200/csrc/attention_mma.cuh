@@ -199,7 +199,6 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
         const uint32_t kdst = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vdst = kdst + PB * ROWB;
         const uint8_t* ksrc = reinterpret_cast<const uint8_t*>(kc + static_cast<size_t>(pos0) * DH);
         const uint8_t* vsrc = reinterpret_cast<const uint8_t*>(vc + static_cast<size_t>(pos0) * DH);
-        if (!((p.dbg & 1) && round > 0))
 #pragma unroll 4
         for (int i = ptid; i < PB * CPR; i += kAmProducers) {
           const int r = i / CPR, ch = i % CPR;

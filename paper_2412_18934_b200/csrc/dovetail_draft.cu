@@ -95,7 +95,6 @@ struct dovetail_draft {
   // tcgen05 GEMV (gemv_umma.cuh): tensor maps of the weight matrices and activation planes (four box depths
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
-  int umma_dbg = 0;
   int attn_max_clusters[2][9] = {};  // [wide][cluster size]: clusters of the attention kernel resident at once
   int attn_wide_min = 16;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
@@ -518,13 +517,13 @@ struct UmmaGeom {
 };
 
 // Ring of one launch: the deepest K-chunk (64 * nslab elements) that leaves >= 3 stages or >= 120 KB in flight.
-UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt, int force128 = 0) {
+UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
   UmmaGeom u{};
   const int M8 = (M + 7) / 8 * 8;
   u.acc_cols = (s_max * M8 + 15) / 16 * 16;
   u.b_groups = u.acc_cols / 8;
   u.a_groups = g_max;
-  u.umma_m = (g_max <= 8 && !force128) ? 64 : 128;
+  u.umma_m = g_max <= 8 ? 64 : 128;
   u.k_split = std::max(1, std::min(std::min(8, 256 / u.acc_cols), K / 512));  // K / 512: every part sees >= 1 chunk of any depth
   u.tmem_cols = 32;
   while (u.tmem_cols < 2 * u.k_split * u.acc_cols) u.tmem_cols *= 2;
@@ -586,10 +585,10 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
   }
   const int Mtot = p.M;
   int Mc = Mtot;
-  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt, h->umma_dbg & 8);
+  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
   while (!g.ok && Mc > 8) {
     Mc = (Mc / 2 + 7) / 8 * 8;
-    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt, h->umma_dbg & 8);
+    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
   }
   if (!g.ok) return DOVETAIL_OK;
   int lg = 0;
@@ -1128,7 +1127,6 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
         a.trace = trace_slot(h);
         a.so = planes(h, h->xs_o, R, h->ld_dq);
         a.qs = fused_s2 ? h->qs : nullptr;
-        a.dbg = h->umma_dbg >> 4;
         if (bf16) {  // tensor-core kernel, chunks of a kv-head merged in a cluster (attention_mma.cuh)
           a.kc = kv->k;
           a.vc = kv->v;
@@ -1829,7 +1827,6 @@ int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
   if (!h) return -1;
   if (key == DOVETAIL_STAT_UMMA_LAUNCHES) return h->last_umma_launches;
   if (key == DOVETAIL_STAT_GRAPH) return h->last_graph;
-  if (key >= 100 && key < 118) return h->attn_max_clusters[(key - 100) / 9][(key - 100) % 9];
   return -1;
 }
 
@@ -1842,8 +1839,6 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
   }
   if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
   if (key == DOVETAIL_TUNE_ATTN_WIDE_MIN && value >= 0 && value <= 4096) { h->attn_wide_min = value; return DOVETAIL_OK; }
-  if (key == 98 && value >= 1) { h->attn_chunks_cap = value; return DOVETAIL_OK; }
-  if (key == 99) { h->umma_dbg = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
 
