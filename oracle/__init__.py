@@ -10,12 +10,14 @@ from .oracle import (  # noqa: F401
     OracleWeights,
     build,
     dgf,
+    e4m3_to_double,
     forward,
     fusion_linear,
     kv_commit,
     lm_head,
     log_softmax,
     matvec,
+    matvec_f8,
     matvec_q8,
     rmsnorm,
     rope,

@@ -33,7 +33,7 @@ typedef struct {
   double rope_theta, rms_eps;
   int32_t dtype, dgf_proj, first_layer_input_norm, final_norm;
   int32_t fusion; /* 0: Dynamic Gating Fusion (the paper's); 1: concat + one Linear (the EAGLE-2 baseline, "w/o both") */
-  int32_t wquant; /* 0: matrices stored in dtype; 1: int8 with one fp32 scale per output row */
+  int32_t wquant; /* 0: matrices stored in dtype; 1: int8, 2: fp8 e4m3, each with one fp32 scale per output row */
 } orc_config_t;
 
 typedef struct {
@@ -103,8 +103,31 @@ void orc_matvec_q8(const int8_t* Q, const float* scale, int N, int K, const doub
   }
 }
 
-/* A weight matrix of the model: stored in dtype, or (scale != NULL) int8 with per-row scales. */
-static void mat(const void* W, const float* scale, int dtype, int N, int K, const double* x, double* y);
+/* The 8-bit float variant of the same scheme (reading A17b; SURVEY.md 8 f1 "int8 / fp8"): a matrix is stored as
+ * fp8 e4m3 bytes with one fp32 scale per output row, W[n,k] = scale[n] * e4m3(q[n,k]).
+ * e4m3 (the "fn" flavour: no infinities): 1 sign, 4 exponent (bias 7), 3 mantissa bits; exponent 0 is subnormal
+ * (m / 8 * 2^-6); exponent 15 with mantissa 7 is NaN; the largest finite value is 1.75 * 2^8 = 448. */
+double orc_e4m3_to_double(uint8_t b) {
+  int s = b >> 7, e = (b >> 3) & 15, m = b & 7;
+  double v;
+  if (e == 15 && m == 7) return NAN;
+  if (e == 0) v = ldexp((double)m / 8.0, -6);
+  else v = ldexp(1.0 + (double)m / 8.0, e - 7);
+  return s ? -v : v;
+}
+
+void orc_matvec_f8(const uint8_t* Q, const float* scale, int N, int K, const double* x, double* y) {
+#pragma omp parallel for schedule(static)
+  for (int n = 0; n < N; ++n) {
+    double s = 0.0, sc = (double)scale[n];
+    size_t base = (size_t)n * (size_t)K;
+    for (int k = 0; k < K; ++k) s += (sc * orc_e4m3_to_double(Q[base + k])) * x[k];
+    y[n] = s;
+  }
+}
+
+/* A weight matrix of the model: stored in dtype, or (scale != NULL) 8-bit (wquant 1: int8, 2: e4m3) with per-row scales. */
+static void mat(const void* W, const float* scale, int wquant, int dtype, int N, int K, const double* x, double* y);
 
 /* y[n] = sum_k W[n,k] x[k], W row-major [N,K]. */
 void orc_matvec(const void* W, int dtype, int N, int K, const double* x, double* y) {
@@ -117,8 +140,9 @@ void orc_matvec(const void* W, int dtype, int N, int K, const double* x, double*
   }
 }
 
-static void mat(const void* W, const float* scale, int dtype, int N, int K, const double* x, double* y) {
-  if (scale) orc_matvec_q8((const int8_t*)W, scale, N, K, x, y);
+static void mat(const void* W, const float* scale, int wquant, int dtype, int N, int K, const double* x, double* y) {
+  if (wquant == 1) orc_matvec_q8((const int8_t*)W, scale, N, K, x, y);
+  else if (wquant == 2) orc_matvec_f8((const uint8_t*)W, scale, N, K, x, y);
   else orc_matvec(W, dtype, N, K, x, y);
 }
 
@@ -157,12 +181,12 @@ void orc_dgf(const orc_config_t* c, const orc_weights_t* w, const double* f, int
   double* z = (double*)malloc(sizeof(double) * d);
   for (int i = 0; i < d; ++i) e[i] = ld(w->embed, (size_t)token * d + i, dt);
   if (c->dgf_proj) {
-    mat(w->dgf_w1, c->wquant ? w->dgf_s1 : NULL, dt, d, d, f, h);
-    mat(w->dgf_w2, c->wquant ? w->dgf_s2 : NULL, dt, d, d, e, h + d);
+    mat(w->dgf_w1, w->dgf_s1, c->wquant, dt, d, d, f, h);
+    mat(w->dgf_w2, w->dgf_s2, c->wquant, dt, d, d, e, h + d);
   } else {
     for (int i = 0; i < d; ++i) { h[i] = f[i]; h[d + i] = e[i]; }
   }
-  mat(w->dgf_wg, c->wquant ? w->dgf_sg : NULL, dt, d, 2 * d, h, z);
+  mat(w->dgf_wg, w->dgf_sg, c->wquant, dt, d, 2 * d, h, z);
   for (int i = 0; i < d; ++i) {
     double g = sigmoid(z[i] + ld(w->dgf_bg, i, dt));
     x[i] = g * h[i] + (1.0 - g) * h[d + i];
@@ -178,7 +202,7 @@ void orc_fusion_linear(const orc_config_t* c, const orc_weights_t* w, const doub
   int d = c->hidden, dt = c->dtype;
   double* h = (double*)malloc(sizeof(double) * 2 * d);
   for (int i = 0; i < d; ++i) { h[i] = f[i]; h[d + i] = ld(w->embed, (size_t)token * d + i, dt); }
-  mat(w->dgf_wg, c->wquant ? w->dgf_sg : NULL, dt, d, 2 * d, h, x);
+  mat(w->dgf_wg, w->dgf_sg, c->wquant, dt, d, 2 * d, h, x);
   for (int i = 0; i < d; ++i) x[i] += ld(w->dgf_bg, i, dt);
   free(h);
 }
@@ -284,9 +308,9 @@ static void forward_rows(const orc_config_t* c, const orc_weights_t* w, void* kc
       double* xr = x + (size_t)r * d;
       if (l == 0 && !c->first_layer_input_norm) memcpy(n, xr, sizeof(double) * d);
       else orc_rmsnorm(xr, L->g_attn, dt, d, c->rms_eps, n);
-      mat(L->wq, c->wquant ? L->sq : NULL, dt, dq, d, n, q + (size_t)r * dq);
-      mat(L->wk, c->wquant ? L->sk : NULL, dt, dkv, d, n, k);
-      mat(L->wv, c->wquant ? L->sv : NULL, dt, dkv, d, n, v);
+      mat(L->wq, L->sq, c->wquant, dt, dq, d, n, q + (size_t)r * dq);
+      mat(L->wk, L->sk, c->wquant, dt, dkv, d, n, k);
+      mat(L->wv, L->sv, c->wquant, dt, dkv, d, n, v);
       for (int h = 0; h < Hq; ++h) orc_rope(q + (size_t)r * dq + h * dh, dh, rows[r].pos, c->rope_theta);
       for (int h = 0; h < Hkv; ++h) orc_rope(k + h * dh, dh, rows[r].pos, c->rope_theta);
       for (int h = 0; h < Hkv; ++h) {
@@ -301,13 +325,13 @@ static void forward_rows(const orc_config_t* c, const orc_weights_t* w, void* kc
       double* xr = x + (size_t)r * d;
       orc_attention_row(c, kc, vc, capacity, l, q + (size_t)r * dq, rows[r].allowed,
                         rows[r].n_allowed, o);
-      mat(L->wo, c->wquant ? L->so : NULL, dt, d, dq, o, t);
+      mat(L->wo, L->so, c->wquant, dt, d, dq, o, t);
       for (int i = 0; i < d; ++i) xr[i] += t[i];
       orc_rmsnorm(xr, L->g_ffn, dt, d, c->rms_eps, n);
-      mat(L->wgate, c->wquant ? L->sgate : NULL, dt, F, d, n, ga);
-      mat(L->wup, c->wquant ? L->sup : NULL, dt, F, d, n, up);
+      mat(L->wgate, L->sgate, c->wquant, dt, F, d, n, ga);
+      mat(L->wup, L->sup, c->wquant, dt, F, d, n, up);
       for (int i = 0; i < F; ++i) ga[i] = silu(ga[i]) * up[i];
-      mat(L->wdown, c->wquant ? L->sdown : NULL, dt, d, F, ga, t);
+      mat(L->wdown, L->sdown, c->wquant, dt, d, F, ga, t);
       for (int i = 0; i < d; ++i) xr[i] += t[i];
     }
   }
@@ -321,10 +345,10 @@ void orc_lm_head(const orc_config_t* c, const orc_weights_t* w, const double* hh
   if (c->final_norm) {
     double* n = (double*)malloc(sizeof(double) * d);
     orc_rmsnorm(hhat, w->g_final, c->dtype, d, c->rms_eps, n);
-    mat(w->lm_head, c->wquant ? w->lm_head_s : NULL, c->dtype, c->vocab, d, n, logits);
+    mat(w->lm_head, w->lm_head_s, c->wquant, c->dtype, c->vocab, d, n, logits);
     free(n);
   } else {
-    mat(w->lm_head, c->wquant ? w->lm_head_s : NULL, c->dtype, c->vocab, d, hhat, logits);
+    mat(w->lm_head, w->lm_head_s, c->wquant, c->dtype, c->vocab, d, hhat, logits);
   }
 }
 

@@ -81,7 +81,7 @@ class OracleConfig:
     first_layer_input_norm: int = 1
     final_norm: int = 0
     fusion: int = 0  # 0 DGF; 1 concat + Linear, the EAGLE-2 baseline
-    wquant: int = 0  # 1: matrices are int8 with one fp32 scale per output row
+    wquant: int = 0  # 1: matrices are int8, 2: fp8 e4m3 bytes, with one fp32 scale per output row
 
     def c(self) -> _Cfg:
         return _Cfg(self.hidden, self.n_q_heads, self.n_kv_heads, self.head_dim, self.n_layers,
@@ -100,6 +100,8 @@ def _np(a):
     assert t.device.type == "cpu", "oracle inputs live in host memory"
     if t.dtype == torch.bfloat16:
         return t.view(torch.int16).numpy().view(np.uint16)
+    if t.dtype == getattr(torch, "float8_e4m3fn", None):  # fp8 weights travel as their bytes
+        return t.view(torch.uint8).numpy()
     return t.numpy()
 
 
@@ -159,6 +161,25 @@ def matvec_q8(Q, scale, x: np.ndarray) -> np.ndarray:
     x = np.ascontiguousarray(x, dtype=np.float64)
     y = np.empty(N, dtype=np.float64)
     _load().orc_matvec_q8(_ptr(Q), _ptr(scale), C.c_int(N), C.c_int(K), _ptr(x), _ptr(y))
+    return y
+
+
+def e4m3_to_double(b) -> np.ndarray:
+    """Value of every fp8 e4m3 byte of an array (reading A17b)."""
+    b = np.ascontiguousarray(b, dtype=np.uint8)
+    f = _load().orc_e4m3_to_double
+    f.restype, f.argtypes = C.c_double, [C.c_uint8]
+    return np.array([f(int(v)) for v in b.reshape(-1)], dtype=np.float64).reshape(b.shape)
+
+
+def matvec_f8(Q, scale, x: np.ndarray) -> np.ndarray:
+    """fp8 e4m3 matrix (bytes) with one fp32 scale per output row: y = (scale[:, None] * e4m3(Q)) @ x in fp64."""
+    Q = np.ascontiguousarray(_np(Q), dtype=np.uint8)
+    scale = np.ascontiguousarray(_np(scale), dtype=np.float32)
+    N, K = Q.shape
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    y = np.empty(N, dtype=np.float64)
+    _load().orc_matvec_f8(_ptr(Q), _ptr(scale), C.c_int(N), C.c_int(K), _ptr(x), _ptr(y))
     return y
 
 

@@ -151,6 +151,11 @@ def int8_variants() -> List[DraftConfig]:
     return [replace(c, name=c.name + "_int8", wquant=1) for c in (_C2, _C3, _C5)]
 
 
+def fp8_variants() -> List[DraftConfig]:
+    """The same workloads with fp8 e4m3 weight matrices and per-row scales (SURVEY.md 8(f1) "int8 / fp8")."""
+    return [replace(c, name=c.name + "_fp8", wquant=2) for c in (_C2, _C3, _C5)]
+
+
 def paper_preset(server: bool = True) -> TreeSpec:
     """width 10 / depth 7 / 16 candidates (servers); 10 / 4 / 7 (PC)."""
     D, g = (7, 16) if server else (4, 7)

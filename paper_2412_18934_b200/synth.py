@@ -51,7 +51,7 @@ def make_weights(cfg: DraftConfig, device="cpu", seed=None) -> Tuple[Dict[str, t
             wgate=r(F, d), wup=r(F, d), wdown=r(d, F),
         ))
     if cfg.wquant:
-        top, layers = quantize_weights(top, layers)
+        top, layers = quantize_weights(top, layers, fp8=cfg.wquant == 2)
     return top, layers
 
 
@@ -69,17 +69,27 @@ def quantize_rows(w: torch.Tensor):
     return q, scale.contiguous()
 
 
-def quantize_weights(top: Dict, layers: List[Dict]):
-    """int8 version of a weight set: matrices -> (int8, scale); embedding, gains, bias untouched."""
+def quantize_rows_f8(w: torch.Tensor):
+    """fp8 e4m3 with one scale per output row: scale = max|row| / 448 (bf16-representable), q = e4m3(w / scale),
+    round to nearest even, clamped to +-448 (the format has no infinity). Input preparation, as quantize_rows."""
+    wf = w.float()
+    scale = (wf.abs().amax(dim=1).clamp_min(1e-12) / 448.0).to(torch.bfloat16).float()
+    q = torch.clamp(wf / scale[:, None], -448.0, 448.0).to(torch.float8_e4m3fn).contiguous()
+    return q, scale.contiguous()
+
+
+def quantize_weights(top: Dict, layers: List[Dict], fp8: bool = False):
+    """8-bit version of a weight set: matrices -> (int8 or fp8 e4m3, scale); embedding, gains, bias untouched."""
+    qr = quantize_rows_f8 if fp8 else quantize_rows
     top = dict(top)
     for k, sk in TOP_MATRIX_SCALES.items():
         if top.get(k) is not None:
-            top[k], top[sk] = quantize_rows(top[k])
+            top[k], top[sk] = qr(top[k])
     out = []
     for l in layers:
         l = dict(l)
         for k, sk in MATRIX_SCALES.items():
-            l[k], l[sk] = quantize_rows(l[k])
+            l[k], l[sk] = qr(l[k])
         out.append(l)
     return top, out
 
