@@ -157,13 +157,15 @@ def _to_host(case):
 
 
 def all_configs():
-    from paper_2412_18934_b200.configs import CONFIGS, c4_sweep, depth_sweep, int8_variants
+    from paper_2412_18934_b200.configs import CONFIGS, c4_sweep, depth_sweep, fp8_variants, int8_variants
     cfgs = {c.name: c for c in CONFIGS.values()}
     cfgs.update({k: v for k, v in CONFIGS.items()})
     cfgs.update({c.name: c for c in c4_sweep()})
     cfgs.update({c.name: c for c in depth_sweep()})
     cfgs.update({c.name: c for c in int8_variants()})
     cfgs.update({c.name.split("_")[0] + "_int8": c for c in int8_variants()})  # c2_int8, c3_int8, c5_int8
+    cfgs.update({c.name: c for c in fp8_variants()})
+    cfgs.update({c.name.split("_")[0] + "_fp8": c for c in fp8_variants()})
     # the tree the paper itself runs (width 10, depth 7, 16 candidates) on the 7B / 13B shapes
     import dataclasses
     from paper_2412_18934_b200.configs import paper_preset
@@ -393,7 +395,7 @@ def bench_one(a, cfg, rank, world, local, dist):
     e2e_val = world * tree.gamma * K / (ms_e2e * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": ("int8 weights (per-row scales), bf16 KV cache, f32 activations and accumulation" if cfg.wquant else
+            "dtype": (("int8" if cfg.wquant == 1 else "fp8 e4m3") + " weights (per-row scales), bf16 KV cache, f32 activations and accumulation" if cfg.wquant else
                       "bf16 weights and KV cache, f32 activations and accumulation") if cfg.dtype == 1 else "f32",
             "data": "synthetic", "config": workload(cfg, a.n_new, world),
             "draft_step_us": step_ms * 1e3, "draft_step_us_replays": dist_us,
@@ -514,7 +516,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     cfgs = all_configs()
     if a.config == "all":
-        names = ["c1", "c2", "c5", "c2_int8", "c3_int8", "c5_int8", "c2_paper_tree", "c3_paper_tree"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
+        names = ["c1", "c2", "c5", "c2_int8", "c3_int8", "c5_int8", "c2_fp8", "c3_fp8", "c5_fp8", "c2_paper_tree", "c3_paper_tree"] + [n for n in cfgs if n.startswith("c4_") or n.startswith("depth_")] + ["c3"]
     else:
         names = [a.config]
     for i, name in enumerate(names):

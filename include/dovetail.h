@@ -87,7 +87,9 @@ typedef struct {
                            [out, in], with one fp32 scale per output row: W[n,k] = scale[n] * q[n,k] ("it is advisable
                            to apply int8 quantization to the drafting model on the GPU"). Needs dtype =
                            BF16 (embedding, norm gains, gate bias, KV cache stay bf16) and every inner dimension a
-                           multiple of 32. */
+                           multiple of 32. 2: the same with fp8 e4m3 bytes (the "fn" flavour: no infinities, largest
+                           value 448; NaN bytes must not occur) instead of int8: W[n,k] = scale[n] * e4m3(q[n,k])
+                           (SURVEY.md 8 f1). */
 } dovetail_config_t;
 
 /* Device pointers to one decoder layer's weights. */
@@ -101,7 +103,7 @@ typedef struct {
   const void* wgate;  /* [F, d]                                 */
   const void* wup;    /* [F, d]                                 */
   const void* wdown;  /* [d, F]                                 */
-  /* weight_quant == 1: fp32 per-row scales of the seven matrices, [out] each; ignored otherwise */
+  /* weight_quant != 0: fp32 per-row scales of the seven matrices, [out] each; ignored otherwise */
   const float* sq;
   const float* sk;
   const float* sv;
@@ -123,7 +125,7 @@ typedef struct {
   const dovetail_layer_weights_t* layers; /* host array [n_layers]       */
   const void* g_final; /* [d] or NULL (required iff final_norm)          */
   const void* lm_head; /* [V, d]                                         */
-  /* weight_quant == 1: fp32 per-row scales of dgf_w1, dgf_w2, dgf_wg, lm_head; ignored otherwise */
+  /* weight_quant != 0: fp32 per-row scales of dgf_w1, dgf_w2, dgf_wg, lm_head; ignored otherwise */
   const float* dgf_s1;
   const float* dgf_s2;
   const float* dgf_sg;

@@ -227,8 +227,9 @@ def dovetail_draft_init(top: Dict, layers: List[Dict], cfg: DraftConfig, max_row
     if cfg.wquant:  # the ABI takes raw pointers: check what it will reinterpret
         for d_, keys in [(top, ("dgf_wg", "lm_head"))] + [(l, ("wq", "wk", "wv", "wo", "wgate", "wup", "wdown")) for l in layers]:
             for k in keys:
-                if d_[k].dtype != torch.int8:
-                    raise TypeError(f"weight_quant = 1: {k} must be int8, got {d_[k].dtype}")
+                want = torch.int8 if cfg.wquant == 1 else torch.float8_e4m3fn
+                if d_[k].dtype != want:
+                    raise TypeError(f"weight_quant = {cfg.wquant}: {k} must be {want}, got {d_[k].dtype}")
     arr = (LayerWeightsT * len(layers))(*[LayerWeightsT(*[_dp(l.get(k)) for k in LAYER_KEYS + LAYER_SCALE_KEYS]) for l in layers])
     w = WeightsT(_dp(top["embed"]), _dp(top.get("dgf_w1")), _dp(top.get("dgf_w2")), _dp(top["dgf_wg"]),
                  _dp(top["dgf_bg"]), arr, _dp(top.get("g_final")), _dp(top["lm_head"]),

@@ -54,7 +54,7 @@ struct dovetail_draft {
   dovetail_weights_t w;
   std::vector<dovetail_layer_weights_t> layers;
   int num_sms = 0, es = 2;
-  int wq = 0;  // 1: int8 weight matrices with per-row scales (cfg.weight_quant)
+  int wq = 0;  // 1: int8, 2: fp8 e4m3 weight matrices with per-row scales (cfg.weight_quant)
   __nv_bfloat16* xs_emb = nullptr;  // int8: embedding rows of the level, as a (permuted) plane [1][rows][ld_d]
   int dq = 0, dkv = 0, ldq = 0;
   int max_step_rows = 0, pool_cap = 0, attn_chunks_cap = 1, qv_cap = 1;
@@ -222,6 +222,12 @@ GemvKernel pick_gemv(int MT, int NI) {
 }
 
 MmaKernel pick_gemv_mma(int NT, int wq) {
+  if (wq == 2) {
+    if (NT == 1) return k_gemv_mma<1, 4, 2>;
+    if (NT == 2) return k_gemv_mma<2, 4, 2>;
+    if (NT == 4) return k_gemv_mma<4, 4, 2>;
+    return k_gemv_mma<8, 2, 2>;
+  }
   if (wq) {
     if (NT == 1) return k_gemv_mma<1, 4, 1>;
     if (NT == 2) return k_gemv_mma<2, 4, 1>;
@@ -256,7 +262,7 @@ cudaError_t set_max_smem_all() {
     if (r != cudaSuccess) e = r;
   };
   for (int nt = 1; nt <= 8; nt *= 2)
-    for (int wq = 0; wq < 2; ++wq) set(reinterpret_cast<const void*>(pick_gemv_mma(nt, wq)));
+    for (int wq = 0; wq < 3; ++wq) set(reinterpret_cast<const void*>(pick_gemv_mma(nt, wq)));
   set(reinterpret_cast<const void*>(k_gemv_umma));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 1>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 1>));
@@ -1425,17 +1431,17 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   for (int K : Ks)
     if (!gemv_shape(K, es, 1, 1).ok)
       return fail(nullptr, DOVETAIL_EINVAL, "dimension %d not supported: rows must be a multiple of 16 bytes and at most 28672 bytes", K);
-  if (c.weight_quant != 0 && c.weight_quant != 1) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant must be 0 or 1");
+  if (c.weight_quant < 0 || c.weight_quant > 2) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant must be 0, 1 (int8) or 2 (fp8 e4m3)");
   if (c.weight_quant) {
-    if (c.dtype != DOVETAIL_BF16) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1 needs dtype = BF16");
+    if (c.dtype != DOVETAIL_BF16) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant != 0 needs dtype = BF16");
     for (int K : Ks)
-      if (K % 32 != 0) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1: dimension %d is not a multiple of 32", K);
+      if (K % 32 != 0) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant != 0: dimension %d is not a multiple of 32", K);
     bool ok = w->dgf_sg && w->lm_head_s && (!c.dgf_proj || (w->dgf_s1 && w->dgf_s2));
     for (int l = 0; ok && w->layers && l < c.n_layers; ++l) {
       const dovetail_layer_weights_t& L = w->layers[l];
       ok = L.sq && L.sk && L.sv && L.so && L.sgate && L.sup && L.sdown;
     }
-    if (!ok) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant = 1: missing scale pointer");
+    if (!ok) return fail(nullptr, DOVETAIL_EINVAL, "weight_quant != 0: missing scale pointer");
   }
   if (!w->embed || !w->dgf_wg || !w->dgf_bg || !w->layers || !w->lm_head ||
       (c.dgf_proj && (!w->dgf_w1 || !w->dgf_w2)) || (c.final_norm && !w->g_final))

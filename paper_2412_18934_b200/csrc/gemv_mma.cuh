@@ -133,6 +133,14 @@ __device__ __forceinline__ void cvt_i8x4_f16x2(uint32_t r, uint32_t& lo, uint32_
   hi = h;
 }
 
+// four fp8 e4m3 bytes (k ascending from the low byte) -> two fp16x2 words, exact (every e4m3 value is an fp16 value):
+// one cvt per pair of weights.
+__device__ __forceinline__ void cvt_e4m3x4_f16x2(uint32_t r, uint32_t& lo, uint32_t& hi) {
+  asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.rn.f16x2.e4m3x2 %0, l;\n\tcvt.rn.f16x2.e4m3x2 %1, h;\n\t}"
+      : "=r"(lo), "=r"(hi)
+      : "r"(r));
+}
+
 __device__ __forceinline__ void mma_f16_16816(float (&c)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
   asm volatile(
       "mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
@@ -141,7 +149,8 @@ __device__ __forceinline__ void mma_f16_16816(float (&c)[4], const uint32_t (&a)
       : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
-// NT: 8-column tiles of B (columns = M * S <= 8 * NT); RBMAX: 16-row blocks per stage; WQ: 1 = int8 weights with
+// NT: 8-column tiles of B (columns = M * S <= 8 * NT); RBMAX: 16-row blocks per stage; WQ: 2 = fp8 e4m3 weights (as
+// 1, with a hardware conversion per pair of weights); 1 = int8 weights with
 // one fp32 scale per output row: half the bytes per weight, converted to fp16 in registers (exact),
 // multiplied with fp16 activation terms (products exact in fp32), the scale applied to the row's result; the
 // activation planes are stored in the matching k order (epilogue.cuh split_pos).
@@ -339,7 +348,10 @@ __global__ void __launch_bounds__(kMmaThreads, 1) k_gemv_mma(const __grid_consta
                 uint32_t qw[4];
                 ldsm_x4(qw, sbase + a_lane + a_row[rb] + u * 32);
 #pragma unroll
-                for (int e = 0; e < 4; ++e) cvt_i8x4_f16x2(qw[e], a0[e], a1[e]);
+                for (int e = 0; e < 4; ++e) {
+                  if (WQ == 2) cvt_e4m3x4_f16x2(qw[e], a0[e], a1[e]);
+                  else cvt_i8x4_f16x2(qw[e], a0[e], a1[e]);
+                }
               } else {
                 const uint32_t aaddr = sbase + a_lane + a_row[rb] + u * 64;
                 ldsm_x4(a0, aaddr);

@@ -49,6 +49,10 @@ FORCED_HHAT_REL = {BF16: 5e-5, 0: 5e-6}
 # before rounding: a K/V entry is W . norm(x) with |entry| <~ 6.5 on these models, and the fp32 forward of one
 # level errs by <= 1.5e-5 relative (the hidden-state bound above is 5e-5 of the largest element): 6.5 x 1.5e-5 = 1e-4.
 KV_PRE = {BF16: 1e-4}
+# fp8 e4m3 weight matrices (reading A17b): the fp32 forward of the same shapes errs by 2.1x as much against fp64 as with
+# bf16 or int8 weights (hidden state 1.26e-5 against 0.60e-5 relative on the 13B shape, measured when the format was
+# added; still 4x under the hidden-state bound above), so the fixed pre-rounding bound is 2 x 1e-4 for those models.
+KV_PRE_FP8 = 2e-4
 
 # Free-running step, levels whose rows cannot meet the stated tolerance because the synthetic model amplifies
 # any perturbation from level to level: the GPU's error at level l may be at most
@@ -347,8 +351,9 @@ def compare(case: Case, gpu: dict, ora: dict, log=print, tight: bool = False) ->
             diff = np.abs(gf - of)
             summary[f"{name}_stored_differ_frac"] = float((ulp != 0).mean())
             summary[f"{name}_stored_max_abs_diff"] = float(diff.max())
-            bad = diff > one_ulp + KV_PRE[cfg.dtype]
-            assert not bad.any(), (f"{name} cache rows differ beyond one bf16 ulp + {KV_PRE[cfg.dtype]}: "
+            pre = KV_PRE_FP8 if getattr(cfg, "wquant", 0) == 2 else KV_PRE[cfg.dtype]
+            bad = diff > one_ulp + pre
+            assert not bad.any(), (f"{name} cache rows differ beyond one bf16 ulp + {pre:.2e}: "
                                    f"{int(bad.sum())} values, worst {diff.max():.3e}")
             assert (ulp != 0).mean() < 0.02, f"{name}: {(ulp != 0).mean():.3%} of stored values differ"
         else:

@@ -25,7 +25,7 @@ def small_cfg(**kw) -> DraftConfig:
 
 def _boost(case, lm=40.0, emb=20.0):
     """Spread the toy distributions so that the top-k decisions are far from ties."""
-    if case.top["lm_head"].dtype == torch.int8:  # int8 weights: the per-row scales carry the magnitude
+    if case.top["lm_head"].dtype in (torch.int8, torch.float8_e4m3fn):  # 8-bit weights: the per-row scales carry the magnitude
         case.top["lm_head_s"] = case.top["lm_head_s"] * lm
     else:
         case.top["lm_head"] = (case.top["lm_head"].float() * lm).to(case.top["lm_head"].dtype)
@@ -173,6 +173,40 @@ def test_full_size_configs_int8(name):
     """The 7B / 13B / Llama-3-8B shaped workloads with int8 weights at full size."""
     from paper_2412_18934_b200.configs import int8_variants
     cfg = [c for c in int8_variants() if c.name == name][0]
+    case = make_case(cfg, n_new=1)
+    s, gpu, ora = _run(case, tight=True)
+    assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("variant", ["base", "mha_dh128", "no_proj", "fusion_linear", "n_new5", "wide", "max_branch"])
+def test_step_parity_small_fp8(variant):
+    """SURVEY.md 8(f1), the fp8 e4m3 variant of the weight stream (reading A17b) against the oracle on the dequantised
+    values."""
+    kw, n_new = dict(dtype=BF16, wquant=2, ffn=352), 1
+    if variant == "mha_dh128":
+        kw.update(hidden=256, n_q_heads=2, n_kv_heads=2, head_dim=128)
+    elif variant == "no_proj":
+        kw.update(dgf_proj=0)
+    elif variant == "fusion_linear":
+        kw.update(dgf_proj=0, fusion=1)
+    elif variant == "n_new5":
+        n_new = 5
+    elif variant == "wide":
+        kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    elif variant == "max_branch":
+        kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    case = _boost(make_case(small_cfg(**kw), n_new=n_new))
+    assert case.layers[0]["wq"].dtype == torch.float8_e4m3fn
+    s, gpu, ora = _run(case)
+    assert s["same_tree"]
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("name", ["c2_llama2_7b_fp8", "c3_llama2_13b_fp8"])
+def test_full_size_configs_fp8(name):
+    from paper_2412_18934_b200.configs import fp8_variants
+    cfg = [c for c in fp8_variants() if c.name == name][0]
     case = make_case(cfg, n_new=1)
     s, gpu, ora = _run(case, tight=True)
     assert gpu["n_out"] == min(cfg.tree.gamma, cfg.tree.pool_size())
