@@ -17,6 +17,14 @@
  *     top-gamma candidate set
  *   - the KV bookkeeping after the target has verified the candidates
  *                                                      (last sentence)
+ *   - next to the step: prompt / catch-up rows (dovetail_draft_prefill),
+ *     the verifier's inputs and the acceptance rule (dovetail_verify_*)
+ *
+ * How a step is launched: the kernels of one step are captured once per (tree_spec,
+ * n_new, attention geometry) into a CUDA graph and replayed on the caller's stream
+ * with the per-call pointers and lengths patched in; nothing synchronises with the
+ * host. Levels of 1-7 rows stream the weights through k_gemv_mma (mma.sync), levels
+ * of 8-64 rows and prefill batches through k_gemv_umma (tcgen05, tensor memory).
  *
  * Conventions
  *   - All functions are extern "C", return 0 on success and a negative
