@@ -6,6 +6,7 @@
 #include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>  // header-only; a no-op unless a profiler injects itself
 
 #include <algorithm>
 #include <array>
@@ -38,6 +39,12 @@ constexpr int kSmemMax = 227 * 1024;
 constexpr int kAttnStages = 4;
 
 char g_init_error[512] = "no error";
+
+// NVTX range over one entry point (traces of the step / prefill / commit in a timeline profiler).
+struct NvtxRange {
+  explicit NvtxRange(const char* name) { nvtxRangePushA(name); }
+  ~NvtxRange() { nvtxRangePop(); }
+};
 
 struct LevelPlan {
   int rows;        // rows forwarded at this level (level 0: n_new)
@@ -1563,6 +1570,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
 int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens, int32_t n_new,
                         dovetail_kv_cache_t* kv, const dovetail_tree_spec_t* tree,
                         const dovetail_draft_out_t* out, void* cuda_stream) {
+  NvtxRange nvtx_range("dovetail_draft_step");
   if (!h) return DOVETAIL_EINVAL;
   if (!hidden_feats || !tokens || !kv || !tree || !out || !kv->k || !kv->v || !out->token_ids ||
       !out->scores || !out->parents || !out->n_out)
@@ -1607,6 +1615,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
 
 int dovetail_draft_prefill(dovetail_draft_t* h, const float* hidden_feats, const int32_t* tokens, int32_t n_rows,
                            dovetail_kv_cache_t* kv, void* cuda_stream) {
+  NvtxRange nvtx_range("dovetail_draft_prefill");
   if (!h) return DOVETAIL_EINVAL;
   if (!hidden_feats || !tokens || !kv || !kv->k || !kv->v) return fail(h, DOVETAIL_EINVAL, "null argument");
   if (n_rows < 1) return fail(h, DOVETAIL_EINVAL, "n_rows = %d: at least one row", n_rows);
@@ -1651,6 +1660,7 @@ int dovetail_draft_prefill(dovetail_draft_t* h, const float* hidden_feats, const
 
 int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32_t* accepted_path, int32_t n_acc,
                        int32_t mode, int32_t* n_committed, void* cuda_stream) {
+  NvtxRange nvtx_range("dovetail_kv_commit");
   if (!h) return DOVETAIL_EINVAL;
   if (n_committed) *n_committed = 0;
   if (!kv || !kv->k || !kv->v || (n_acc > 0 && !accepted_path)) return fail(h, DOVETAIL_EINVAL, "null argument");
@@ -1685,6 +1695,7 @@ int dovetail_kv_commit(dovetail_draft_t* h, dovetail_kv_cache_t* kv, const int32
 
 int dovetail_verify_plan(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma, int32_t root_position,
                          int32_t max_depth, const dovetail_verify_plan_t* plan, void* cuda_stream) {
+  NvtxRange nvtx_range("dovetail_verify_plan");
   if (!h) return DOVETAIL_EINVAL;
   if (!out || !out->parents || !out->depths || !out->n_out || !plan || !plan->mask || !plan->position_ids || !plan->paths ||
       !plan->n_paths)
@@ -1709,6 +1720,7 @@ int dovetail_verify_plan(dovetail_draft_t* h, const dovetail_draft_out_t* out, i
 
 int dovetail_verify_accept(dovetail_draft_t* h, const dovetail_draft_out_t* out, int32_t gamma, int32_t mode, int32_t max_depth,
                            const dovetail_verify_in_t* in, const dovetail_verify_out_t* res, void* cuda_stream) {
+  NvtxRange nvtx_range("dovetail_verify_accept");
   if (!h) return DOVETAIL_EINVAL;
   if (!out || !out->token_ids || !out->parents || !out->n_out || !in || !res || !res->accepted_path || !res->n_acc ||
       !res->bonus_token)
