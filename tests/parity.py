@@ -207,15 +207,24 @@ def oracle_sensitivity(case: Case, ora: dict):
     op = run_oracle(pert)
     rows, pools = level_layout(case)
     n_new = case.tokens.shape[0]
-    out, ok = [], True
+    out, ok = SensList(), True
     for l, rr in enumerate(rows):
         pb, m, b = pools[l]
         lm = [n_new - 1] if l == 0 else rr
         out.append((float(np.abs(op["row_logits"][lm] - ora["row_logits"][lm]).max()),
                     float(np.abs(op["row_hhat"][rr] - ora["row_hhat"][rr]).max())) if ok else None)
-        ok = ok and np.array_equal(op["pool_token"][pb:pb + m * b], ora["pool_token"][pb:pb + m * b]) and \
+        same = np.array_equal(op["pool_token"][pb:pb + m * b], ora["pool_token"][pb:pb + m * b]) and \
             np.array_equal(np.argsort(-op["pool_cum"][pb:pb + m * b], kind="stable"), np.argsort(-ora["pool_cum"][pb:pb + m * b], kind="stable"))
+        if ok and not same:
+            out.first_changed = l  # the ORACLE's own decisions at this level flip under the perturbation
+        ok = ok and same
     return out
+
+
+class SensList(list):
+    """oracle_sensitivity's per-level list + first_changed: the first level at which the oracle's own candidates
+    (tokens or their order) change under the SENS_ETA input perturbation, or None."""
+    first_changed = None
 
 
 def error_table(case: Case, gpu: dict, ora: dict) -> list:
