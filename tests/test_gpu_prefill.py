@@ -76,9 +76,13 @@ def _check(case, gpu, ora):
             np.testing.assert_allclose(gs, os_, **tol)
 
 
-@pytest.mark.parametrize("dtype,n,max_rows", [(BF16, 150, 64), (BF16, 65, 64), (BF16, 2, 64), (BF16, 100, 24), (F32, 70, 64)])
+@pytest.mark.parametrize("dtype,n,max_rows", [(BF16, 150, 64), (BF16, 65, 64), (BF16, 2, 64), (BF16, 100, 24), (F32, 70, 64),
+                                              ("int8", 70, 64), ("fp8", 40, 16)])
 def test_prefill_then_step_equals_one_batched_step(dtype, n, max_rows):
-    cfg = umma_cfg(prefix=37) if dtype == BF16 else small_cfg(dtype=F32, prefix=37)
+    if dtype in ("int8", "fp8"):  # 8-bit weight streams: batches run on k_gemv_mma in row chunks
+        cfg, dtype = small_cfg(dtype=BF16, wquant=1 if dtype == "int8" else 2, ffn=352, prefix=37), None
+    else:
+        cfg = umma_cfg(prefix=37) if dtype == BF16 else small_cfg(dtype=F32, prefix=37)
     case = _boost(make_case(cfg, n_new=n))
     ora = run_oracle(case)
     gpu = _prefill_then_step(case, max_rows=max_rows)
