@@ -1277,6 +1277,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
       const bool last = l + 1 == tree->depth;
       t.M_next = last ? 0 : plan[l + 1].rows;
       t.next_row0 = last ? 0 : plan[l + 1].row0;
+      t.cur_row0 = lp.row0;
       t.next_t0 = last ? 0 : plan[l + 1].t0;
       t.n_new = n_new;
       t.cur = cur;
@@ -1793,6 +1794,7 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, 
     const bool last = l + 1 == tree->depth;
     t.M_next = last ? 0 : plan[l + 1].rows;
     t.next_row0 = last ? 0 : plan[l + 1].row0;
+    t.cur_row0 = lp.row0;
     t.next_t0 = last ? 0 : plan[l + 1].t0;
     t.n_new = 1;
     t.cur = h->rt + (l & 1);

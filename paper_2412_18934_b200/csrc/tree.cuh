@@ -173,6 +173,7 @@ struct TreeLevelParams {
   int32_t pool_begin;      // pool index of this level's first child
   int32_t M_next;          // rows of the next level (0: this is the last level)
   int32_t next_row0;       // step row of the next level's first row
+  int32_t cur_row0;        // step row of this level's first expanded row (level 0: unused, the root row is n_new - 1)
   int32_t next_t0;         // tree-row index (= new-region slot) of the next level's first row
   int32_t n_new;           // step rows before the first tree row; root row = n_new - 1
   const RowTables* cur;
@@ -205,6 +206,7 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   // phases B / C: pool scores and keep flags
   __shared__ float s_raw[2 * kPoolSmem];
   __shared__ int32_t s_cnt[kTreeThreads + 1];
+  __shared__ int32_t s_tok[kMaxRows * kMaxBranch];  // this level's children: tokens (scores in s_cum), row-major [row][rank]
   float* s_cum = s_raw;
   int32_t* s_new = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);
   pdl_launch_dependents();
@@ -232,6 +234,8 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
         P.depth[base + lane] = p.level + 1;
         P.cum[base + lane] = pcum + p.rp_logp[o];
         P.row[base + lane] = -1;
+        s_tok[m * p.b + lane] = p.rp_tokens[o];
+        s_cum[m * p.b + lane] = pcum + p.rp_logp[o];
       }
       continue;
     }
@@ -298,6 +302,8 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
         P.depth[base + jb] = p.level + 1;
         P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
         P.row[base + jb] = -1;
+        s_tok[m * p.b + jb] = bi;  // phase B works from shared memory: no round trip through the pool
+        s_cum[m * p.b + jb] = pcum + (bv - logz);
       }
     }
   }
@@ -308,29 +314,35 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
     for (int i = tid; i < n; i += kTreeThreads) {
       const int node = p.pool_begin + i;
       if (p.tap_token) { p.tap_token[node] = P.token[node]; p.tap_cum[node] = P.cum[node]; }
-      if (p.force_token) { P.token[node] = p.force_token[node]; P.cum[node] = p.force_cum[node]; }
+      if (p.force_token) {
+        P.token[node] = p.force_token[node];
+        P.cum[node] = p.force_cum[node];
+        s_tok[i] = p.force_token[node];
+        s_cum[i] = p.force_cum[node];
+      }
     }
     __syncthreads();
   }
 
   // ---- phase B: frontier of the next level = top-M_next children by score -----
   if (p.M_next > 0) {
-    for (int i = tid; i < n; i += kTreeThreads) s_cum[i] = P.cum[p.pool_begin + i];
-    __syncthreads();
+    // Everything a selected child needs is its parent's row of THIS level (m = i / b): the node forwarded there
+    // (cur->pool[m]), that row's step row (cur_row0 + m) and its ancestor mask (cur->mask[m]) -- no dependent
+    // loads through the pool arrays.
     for (int i = tid; i < n; i += kTreeThreads) {
       int rank = 0;
       for (int j = 0; j < n; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
       if (rank < p.M_next) {
-        const int node = p.pool_begin + i, r = rank;
-        const int parent = P.parent[node];
+        const int node = p.pool_begin + i, r = rank, m = i / p.b;
+        const bool root = p.level == 0;
         const int t = p.next_t0 + r;  // tree-row index = new-region slot
-        p.next->token[r] = P.token[node];
-        p.next->src[r] = parent < 0 ? p.n_new - 1 : P.row[parent];
+        p.next->token[r] = s_tok[i];
+        p.next->src[r] = root ? p.n_new - 1 : p.cur_row0 + m;
         p.next->slot[r] = t;
         p.next->pool[r] = node;
         P.row[node] = p.next_row0 + r;
         for (int w = 0; w < kMaskWords; ++w) {
-          uint32_t mk = parent < 0 ? 0u : p.treemask[(P.row[parent] - p.n_new) * kMaskWords + w];
+          uint32_t mk = root ? 0u : p.cur->mask[m][w];
           if ((t >> 5) == w) mk |= 1u << (t & 31);
           p.treemask[t * kMaskWords + w] = mk;
           p.next->mask[r][w] = mk;
