@@ -84,7 +84,8 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
  * 0 = direct launches. Steps with test hooks or tracing set always launch directly. */
 #define DOVETAIL_TUNE_GRAPHS 2
 /* key 3: attention launches with more than `value` query vectors (rows of the level x q-heads per kv-head) use the
- * 64-vectors-per-pass kernel (csrc/attention_mma.cuh, QT = 4). Default 16 (measured: 55 vs 80 us at 32 vectors over 2048 positions, 32 vs 29.5 us at 16); 4096 = never, 0 = always. */
+ * 64-vectors-per-pass kernel (csrc/attention_mma.cuh, QT = 4). Default 32 (measured on the 13B shape: at 32 vectors two
+ * passes of the 16-vector kernel take 36 us against 43 us, at 48 vectors 38 against 30 us); 4096 = never, 0 = always. */
 #define DOVETAIL_TUNE_ATTN_WIDE_MIN 3
 
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.

@@ -103,7 +103,7 @@ struct dovetail_draft {
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
   int attn_max_clusters[2][9] = {};  // [wide][cluster size]: clusters of the attention kernel resident at once
-  int attn_wide_min = 16;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
+  int attn_wide_min = 32;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
   struct PlaneBuf { const __nv_bfloat16* base; int64_t elems, ld; int cap, map; };

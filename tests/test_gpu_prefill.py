@@ -104,6 +104,13 @@ def test_prefill_no_prefix_and_errors():
     assert e.value.code == binding.ECAPACITY and kv.committed_len == case.capacity - 10
     with pytest.raises(TypeError):
         binding.dovetail_draft_prefill(h, case.feats.double(), case.tokens, kv)
+    # a prefill leaves no tree behind: kv_commit needs a step first (include/dovetail.h)
+    kv2 = binding.KVCache(case.k.clone(), case.v.clone(), 0)
+    binding.dovetail_draft_prefill(h, case.feats[:5].contiguous(), case.tokens[:5].contiguous(), kv2)
+    assert kv2.committed_len == 5
+    with pytest.raises(binding.DovetailError) as e:
+        binding.dovetail_kv_commit(h, kv2, [0], mode=0)
+    assert e.value.code == binding.EINVAL
     binding.dovetail_draft_destroy(h)
 
 
