@@ -87,6 +87,9 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
  * 64-vectors-per-pass kernel (csrc/attention_mma.cuh, QT = 4). Default 32 (measured on the 13B shape: at 32 vectors two
  * passes of the 16-vector kernel take 36 us against 43 us, at 48 vectors 38 against 30 us); 4096 = never, 0 = always. */
 #define DOVETAIL_TUNE_ATTN_WIDE_MIN 3
+/* key 4: 1 (default) = attention launches with 17 ... 32 query vectors use the 32-vectors-per-pass kernel (QT = 2: one
+ * pass over the cache instead of two); 0 = two passes of the 16-vector kernel. */
+#define DOVETAIL_TUNE_ATTN_QT2 4
 
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.
  *   key 1: launches of the tcgen05 GEMV (k_gemv_umma). Unknown key or NULL handle: -1. */

@@ -412,7 +412,7 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
     return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
 
 
-TUNE_UMMA_MIN_M, TUNE_GRAPHS, TUNE_ATTN_WIDE_MIN = 1, 2, 3
+TUNE_UMMA_MIN_M, TUNE_GRAPHS, TUNE_ATTN_WIDE_MIN, TUNE_ATTN_QT2 = 1, 2, 3, 4
 STAT_UMMA_LAUNCHES, STAT_GRAPH = 1, 2
 
 

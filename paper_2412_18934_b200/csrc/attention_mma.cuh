@@ -95,12 +95,14 @@ constexpr size_t am_smem_bytes(int DH, int QT = 1) {
 
 // QT = 1: one tile of 16 query vectors per pass over the CTA's positions, the four consumer warps split the 64
 // positions of a block (tree levels of a few rows: latency matters, every warp works on every block).
+// QT = 2 (17 ... 32 query vectors): 32 per pass, warp w owns query tile w & 1 and the position half w >> 1 of every
+// block; the two halves of a tile are merged like the four warps of QT = 1. One pass over the cache instead of two.
 // QT = 4 ("wide": levels of many rows, level-0 batches of dovetail_draft_prefill): 64 query vectors per pass,
 // consumer warp w owns query tile w and walks all 64 positions of every block with its own online-softmax state,
 // the flash-attention arrangement -- the cache is streamed once per 64 query vectors instead of once per 16, and
 // no merge over the warps is needed.
 template <int DH, int QT>
-__global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_mma(const AttnParams p) {
+__global__ void __launch_bounds__(kAmThreads, QT <= 2 ? 2 : 1) k_tree_attention_mma(const AttnParams p) {
   using WT = __nv_bfloat16;
   constexpr int ROWB = DH * 2;            // bytes of one K (or V) row
   constexpr int CPR = ROWB / 16;          // 16-byte chunks per row
@@ -131,7 +133,8 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
   const int n_pass = (qv_tot + QROWS - 1) / QROWS;
   const int QR = min(QROWS, qv_tot);  // rows of the warp-merge scratch
   // [QR][WSTR] this CTA's record, read by the cluster ranks (wide: written by the warps directly, no warp merge)
-  float* crec = QT == 1 ? wsm + static_cast<size_t>(kAmWarps) * QR * WSTR : wsm;
+  constexpr int NPART = QT == 1 ? kAmWarps : (QT == 2 ? 2 : 1);  // partial states per query vector inside the CTA
+  float* crec = QT == 4 ? wsm : wsm + static_cast<size_t>(NPART) * QR * WSTR;
   // chunks [group * CS, (group + 1) * CS) of a kv-head form a cluster (CS = 1 without the launch attribute)
   const int CS = static_cast<int>(cluster_nctarank()), crank = static_cast<int>(cluster_ctarank());
   const int n_groups = n_chunks / CS, group = c / CS;
@@ -307,7 +310,7 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
     int mrow[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
-      const int r = (QT == 1 ? 0 : warp * kAmQRows) + g + 8 * h;  // wide: this warp's own query tile
+      const int r = (QT == 1 ? 0 : (QT == 2 ? (warp & 1) : warp) * kAmQRows) + g + 8 * h;  // QT > 1: this warp's own query tile
       mrow[h] = r < nq ? (qv0 + r) / grp : -1;
     }
     float mrun[2] = {-INFINITY, -INFINITY}, lrun[2] = {0.f, 0.f};
@@ -414,13 +417,16 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
             mma_bf16_16816(o[t + 1], pl, vf[2], vf[3]);
           }
         }
-      } else if (warp * kAmQRows < nq) {
-        // ---- wide: this warp's 16 query vectors against all 64 positions of the block --------------------
+      } else if ((QT == 2 ? (warp & 1) : warp) * kAmQRows < nq) {
+        // ---- QT = 4: this warp's 16 query vectors against all 64 positions of the block; QT = 2: against its half
+        constexpr int NJ = QT == 2 ? 2 : 4;                  // 16-position tiles of the block this warp walks
+        const int J0 = QT == 2 ? (warp >> 1) * 2 : 0;
+        const int qtile = QT == 2 ? (warp & 1) : warp;
         const uint32_t kb = smem_u32(ring) + static_cast<uint32_t>(slot) * BLK_BYTES, vb = kb + PB * ROWB;
-        const int q_row = warp * kAmQRows + a_row;
-        float s[8][4];  // eight independent chains already: head and remainder products share an accumulator
+        const int q_row = qtile * kAmQRows + a_row;
+        float s[2 * NJ][4];  // independent chains: head and remainder products share an accumulator
 #pragma unroll
-        for (int nt = 0; nt < 8; ++nt)
+        for (int nt = 0; nt < 2 * NJ; ++nt)
 #pragma unroll
           for (int e = 0; e < 4; ++e) s[nt][e] = 0.f;
 #pragma unroll
@@ -429,9 +435,9 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
           ldsm_x4(ah, smem_u32(q_hi) + am_swz<ROWB>(q_row, ks * 2 + a_ch));
           ldsm_x4(al, smem_u32(q_lo) + am_swz<ROWB>(q_row, ks * 2 + a_ch));
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
+          for (int j = 0; j < NJ; ++j) {
             uint32_t kf[4];
-            ldsm_x4(kf, kb + am_swz<ROWB>(j * 16 + k_row, ks * 2 + k_ch));
+            ldsm_x4(kf, kb + am_swz<ROWB>((J0 + j) * 16 + k_row, ks * 2 + k_ch));
             mma_bf16_16816(s[2 * j], ah, kf[0], kf[1]);
             mma_bf16_16816(s[2 * j + 1], ah, kf[2], kf[3]);
             mma_bf16_16816(s[2 * j], al, kf[0], kf[1]);
@@ -441,12 +447,12 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
         float mx[2] = {-INFINITY, -INFINITY};
         const bool need_mask = tail || cnt < PB;  // uniform over the CTA
 #pragma unroll
-        for (int nt = 0; nt < 8; ++nt)
+        for (int nt = 0; nt < 2 * NJ; ++nt)
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
             const int h = e >> 1;
             if (need_mask) {
-              const int pos = nt * 8 + 2 * tq + (e & 1);
+              const int pos = J0 * 16 + nt * 8 + 2 * tq + (e & 1);
               bool ok = pos < cnt && mrow[h] >= 0;
               if (ok && tail) {
                 const int j = (b - n_blk) * PB + pos;
@@ -476,7 +482,7 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
           }
         }
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {  // 16 positions per step of P V
+        for (int j = 0; j < NJ; ++j) {  // 16 positions per step of P V
           uint32_t ph[4], pl[4];
 #pragma unroll
           for (int n2 = 0; n2 < 2; ++n2)
@@ -494,7 +500,7 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
 #pragma unroll
           for (int t = 0; t < DN; t += 2) {
             uint32_t vf[4];
-            ldsm_x4_trans(vf, vb + am_swz<ROWB>(j * 16 + v_row, t + v_ch));
+            ldsm_x4_trans(vf, vb + am_swz<ROWB>((J0 + j) * 16 + v_row, t + v_ch));
             mma_bf16_16816(o[t], ph, vf[0], vf[1]);
             mma_bf16_16816(o[t], pl, vf[0], vf[1]);
             mma_bf16_16816(o[t + 1], ph, vf[2], vf[3]);
@@ -508,15 +514,16 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
     }
     am_consumer_sync();  // every warp is done with the ring: the merge scratch aliases it
 
-    if constexpr (QT == 1) {
-    // ---- merge the four warps (fixed order), then hand the chunk's partial on ------
+    if constexpr (QT != 4) {
+    // ---- merge the partial states of a query vector (QT = 1: four warps, QT = 2: two position halves; fixed order)
+      const int part = QT == 1 ? warp : (warp >> 1), rbase = QT == 1 ? 0 : (warp & 1) * kAmQRows;
   #pragma unroll
       for (int h = 0; h < 2; ++h) {
         lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 1);
         lrun[h] += __shfl_xor_sync(0xffffffffu, lrun[h], 2);
-        const int r = g + 8 * h;
+        const int r = rbase + g + 8 * h;
         if (r < nq) {
-          float* w = wsm + (static_cast<size_t>(warp) * QR + r) * WSTR;
+          float* w = wsm + (static_cast<size_t>(part) * QR + r) * WSTR;
   #pragma unroll
           for (int t = 0; t < DN; ++t)
             *reinterpret_cast<float2*>(w + t * 8 + 2 * tq) = make_float2(o[t][2 * h], o[t][2 * h + 1]);
@@ -528,11 +535,11 @@ __global__ void __launch_bounds__(kAmThreads, QT == 1 ? 2 : 1) k_tree_attention_
         const int r = idx / (DH / 4), dd = (idx % (DH / 4)) * 4;
         float mm = -INFINITY;
 #pragma unroll
-        for (int w = 0; w < kAmWarps; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
+        for (int w = 0; w < NPART; ++w) mm = fmaxf(mm, wsm[(w * QR + r) * WSTR + DH]);
         float ll = 0.f;
         float4 oo = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-        for (int w = 0; w < kAmWarps; ++w) {
+        for (int w = 0; w < NPART; ++w) {
           const float* rr = wsm + (w * QR + r) * WSTR;
           const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
           const float4 ov = *reinterpret_cast<const float4*>(rr + dd);

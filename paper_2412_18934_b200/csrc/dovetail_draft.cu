@@ -102,7 +102,8 @@ struct dovetail_draft {
   // tcgen05 GEMV (gemv_umma.cuh): tensor maps of the weight matrices and activation planes (four box depths
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
-  int attn_max_clusters[2][9] = {};  // [wide][cluster size]: clusters of the attention kernel resident at once
+  int attn_max_clusters[3][9] = {};  // [mode][cluster size]: clusters of the attention kernel resident at once
+  int attn_qt2 = 1;                 // 17 ... 32 query vectors take the 32-per-pass attention kernel
   int attn_wide_min = 32;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
@@ -273,6 +274,8 @@ cudaError_t set_max_smem_all() {
   set(reinterpret_cast<const void*>(k_gemv_umma));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 1>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 1>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 2>));
+  set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 2>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<64, 4>));
   set(reinterpret_cast<const void*>(k_tree_attention_mma<128, 4>));
   const int mts[3] = {1, 2, 4};
@@ -890,11 +893,18 @@ int level_hooks(dovetail_draft* h, cudaStream_t st, const dovetail_kv_cache_t* k
 // that does not fit costs a whole kernel time (measured on the 13B shape, 40 heads, prefix 2048: 7 chunks per head
 // 24.2 us, 6 chunks 14.0 us). attn_max_clusters[wide][cs] = cudaOccupancyMaxActiveClusters of the kernel at cluster
 // size cs (dovetail_draft_init); 0 = unknown.
-void attn_mma_geom(const dovetail_draft* h, int Lbase, bool wide, int& n_chunks, int& cs) {
+AttnKernel attn_mma_kernel(int dh, int qt) {
+  if (qt == 4) return dh == 128 ? k_tree_attention_mma<128, 4> : k_tree_attention_mma<64, 4>;
+  if (qt == 2) return dh == 128 ? k_tree_attention_mma<128, 2> : k_tree_attention_mma<64, 2>;
+  return dh == 128 ? k_tree_attention_mma<128, 1> : k_tree_attention_mma<64, 1>;
+}
+
+// mode: 0 = QT 1 (16 query vectors per pass), 1 = QT 4 (64, one CTA per SM), 2 = QT 2 (32).
+void attn_mma_geom(const dovetail_draft* h, int Lbase, int mode, int& n_chunks, int& cs) {
   const int n_blocks = std::max(1, div_up(Lbase, kAmBlockPos));
   const int Hkv = h->cfg.n_kv_heads;
-  const int* maxc = h->attn_max_clusters[wide ? 1 : 0];
-  n_chunks = std::max(1, std::min(wide ? std::max(1, h->attn_chunks_cap / 2) : h->attn_chunks_cap, n_blocks / 2));
+  const int* maxc = h->attn_max_clusters[mode];
+  n_chunks = std::max(1, std::min(mode == 1 ? std::max(1, h->attn_chunks_cap / 2) : h->attn_chunks_cap, n_blocks / 2));
   if (n_chunks <= 8) {
     while (n_chunks > 1 && maxc[n_chunks] > 0 && Hkv > maxc[n_chunks]) --n_chunks;
     n_chunks = div_up(n_blocks, div_up(n_blocks, n_chunks));  // fewest chunks with the same blocks per chunk
@@ -1147,12 +1157,13 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
           a.Lbase = Lbase;
           a.Lsafe = L;
           // more than 32 query vectors: 64 per pass over the cache, one query tile per warp (attention_mma.cuh)
-          const bool wide_q = qv_tot > h->attn_wide_min;
+          // 17 ... 32 query vectors: 32 per pass (QT = 2); more: 64 per pass, one query tile per warp (QT = 4)
+          const int mode = qv_tot > h->attn_wide_min ? 1 : (qv_tot > kAmQRows && h->attn_qt2 ? 2 : 0);
           int n_chunks, cs;
-          attn_mma_geom(h, Lbase, wide_q, n_chunks, cs);
-          const size_t smem = am_smem_bytes(dh, wide_q ? 4 : 1);
-          auto kern = wide_q ? (dh == 128 ? k_tree_attention_mma<128, 4> : k_tree_attention_mma<64, 4>)
-                             : (dh == 128 ? k_tree_attention_mma<128, 1> : k_tree_attention_mma<64, 1>);
+          attn_mma_geom(h, Lbase, mode, n_chunks, cs);
+          const int qt = mode == 1 ? 4 : (mode == 2 ? 2 : 1);
+          const size_t smem = am_smem_bytes(dh, qt);
+          auto kern = attn_mma_kernel(dh, qt);
           e = launch_c(h, cs, true, kern, dim3(n_chunks, c.n_kv_heads), dim3(kAmThreads), smem, st, a);
         } else {
           int n_chunks = std::min(h->attn_chunks_cap, std::max(1, div_up(Lbase, 2 * kAttnStagePos)));
@@ -1317,12 +1328,15 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
   for (int l = 0; l < tree->depth; ++l) { key.push_back(tree->branch[l]); key.push_back(tree->beam[l]); }
   int nc[2] = {0, 0}, cs[2] = {0, 0};
   if (bf16) {
-    attn_mma_geom(h, L, false, nc[0], cs[0]);
-    attn_mma_geom(h, Lp, false, nc[1], cs[1]);
-    int wn[2], wc[2];  // the wide kernel's geometry (which levels take it follows from the tree and n_new)
-    attn_mma_geom(h, L, true, wn[0], wc[0]);
-    attn_mma_geom(h, Lp, true, wn[1], wc[1]);
-    key.insert(key.end(), {wn[0], wc[0], wn[1], wc[1], h->attn_wide_min});
+    attn_mma_geom(h, L, 0, nc[0], cs[0]);
+    attn_mma_geom(h, Lp, 0, nc[1], cs[1]);
+    for (int mode = 1; mode <= 2; ++mode) {  // the other kernels' geometry (which levels take them follows from the tree and n_new)
+      int wn[2], wc[2];
+      attn_mma_geom(h, L, mode, wn[0], wc[0]);
+      attn_mma_geom(h, Lp, mode, wn[1], wc[1]);
+      key.insert(key.end(), {wn[0], wc[0], wn[1], wc[1]});
+    }
+    key.insert(key.end(), {h->attn_wide_min, h->attn_qt2});
   } else {
     nc[0] = std::min(h->attn_chunks_cap, std::max(1, div_up(L, 2 * kAttnStagePos)));
     nc[1] = std::min(h->attn_chunks_cap, std::max(1, div_up(Lp, 2 * kAttnStagePos)));
@@ -1363,8 +1377,9 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
         ng.begin_params = kp;
         ng.begin_args.assign(kp.kernelParams, kp.kernelParams + 11);  // k_step_begin takes 11 arguments
         ng.begin_dv = *static_cast<const StepDyn*>(kp.kernelParams[0]);
-      } else if (kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64, 1>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128, 1>) ||
-                 kp.func == reinterpret_cast<void*>(k_tree_attention_mma<64, 4>) || kp.func == reinterpret_cast<void*>(k_tree_attention_mma<128, 4>)) {
+      } else if (kp.func == reinterpret_cast<void*>(attn_mma_kernel(64, 1)) || kp.func == reinterpret_cast<void*>(attn_mma_kernel(128, 1)) ||
+                 kp.func == reinterpret_cast<void*>(attn_mma_kernel(64, 2)) || kp.func == reinterpret_cast<void*>(attn_mma_kernel(128, 2)) ||
+                 kp.func == reinterpret_cast<void*>(attn_mma_kernel(64, 4)) || kp.func == reinterpret_cast<void*>(attn_mma_kernel(128, 4))) {
         ng.attn_nodes.push_back(nd);
         ng.attn_node_params.push_back(kp);
         ng.attn_params.push_back(*static_cast<const AttnParams*>(kp.kernelParams[0]));
@@ -1544,12 +1559,13 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   }
   if (es == 2 && !c.weight_quant) umma_init(h);
   if (es == 2) {  // how many clusters of each size the tensor-core attention kernel can have resident (attn_mma_geom)
-    for (int wide = 0; wide < 2; ++wide)
+    for (int mode = 0; mode < 3; ++mode)
       for (int cs = 1; cs <= 8; ++cs) {
+        const int qt = mode == 1 ? 4 : (mode == 2 ? 2 : 1);
         cudaLaunchConfig_t lc{};
         lc.gridDim = dim3(cs, c.n_kv_heads);
         lc.blockDim = dim3(kAmThreads);
-        lc.dynamicSmemBytes = am_smem_bytes(c.head_dim, wide ? 4 : 1);
+        lc.dynamicSmemBytes = am_smem_bytes(c.head_dim, qt);
         cudaLaunchAttribute at{};
         at.id = cudaLaunchAttributeClusterDimension;
         at.val.clusterDim.x = cs;
@@ -1557,10 +1573,9 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
         at.val.clusterDim.z = 1;
         lc.attrs = &at;
         lc.numAttrs = 1;
-        const void* fn = wide ? (c.head_dim == 128 ? reinterpret_cast<const void*>(k_tree_attention_mma<128, 4>) : reinterpret_cast<const void*>(k_tree_attention_mma<64, 4>))
-                              : (c.head_dim == 128 ? reinterpret_cast<const void*>(k_tree_attention_mma<128, 1>) : reinterpret_cast<const void*>(k_tree_attention_mma<64, 1>));
+        const void* fn = reinterpret_cast<const void*>(attn_mma_kernel(c.head_dim, qt));
         int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, fn, &lc) == cudaSuccess) h->attn_max_clusters[wide][cs] = n;
+        if (cudaOccupancyMaxActiveClusters(&n, fn, &lc) == cudaSuccess) h->attn_max_clusters[mode][cs] = n;
         else cudaGetLastError();
       }
   }
@@ -1858,6 +1873,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
     return DOVETAIL_OK;
   }
   if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
+  if (key == DOVETAIL_TUNE_ATTN_QT2 && (value == 0 || value == 1)) { h->attn_qt2 = value; return DOVETAIL_OK; }
   if (key == DOVETAIL_TUNE_ATTN_WIDE_MIN && value >= 0 && value <= 4096) { h->attn_wide_min = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);
 }
