@@ -17,10 +17,6 @@ __device__ __forceinline__ void tma_load_3d(void* dst, const CUtensorMap* map, i
       "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
-__device__ __forceinline__ void tma_prefetch_map(const CUtensorMap* map) {
-  asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
-}
-
 // One lane of a converged warp. Branching on this (not on lane == 0) tells ptxas that a single thread is active,
 // so the uniform-register operands of UTCHMMA / UTMALDG need no per-value waterfall loop.
 __device__ __forceinline__ bool elect_one() {
@@ -45,15 +41,10 @@ __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::
 // ---- tcgen05.mma, kind::f16 (bf16 x bf16 -> fp32), both operands in shared memory ----------------------------
 // Shared-memory matrix descriptor of a K-major tile in the 128-byte swizzled canonical layout: rows of 64
 // elements (128 bytes), 8-row groups of 1024 bytes `sbo` bytes apart. The tile base must be 1024-byte aligned;
-// a step of 16 elements along K inside the 64-element row is +32 bytes on the start address.
-__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t smem_addr, uint32_t sbo) {
-  uint64_t d = static_cast<uint64_t>((smem_addr & 0x3ffffu) >> 4);  // start address, bits [0, 14)
-  d |= static_cast<uint64_t>(1) << 16;                              // leading byte offset (unused when swizzled)
-  d |= static_cast<uint64_t>((sbo >> 4) & 0x3fffu) << 32;           // stride byte offset, bits [32, 46)
-  d |= static_cast<uint64_t>(1) << 46;                              // descriptor version of sm_100
-  d |= static_cast<uint64_t>(2) << 61;                              // layout type: 128-byte swizzle
-  return d;
-}
+// a step of 16 elements along K inside the 64-element row is +32 bytes on the start address. The 64-bit descriptor:
+// start address >> 4 in bits [0, 14), leading byte offset (unused when swizzled) = 1 at bit 16, stride byte offset >> 4
+// in bits [32, 46), descriptor version 1 at bit 46, layout type 2 (128-byte swizzle) at bits [61, 64); it is built as a
+// low and a high 32-bit word (umma_desc_lo / umma_desc_hi_sw128 below).
 // Instruction descriptor: D fp32, A and B bf16, both K-major, M x N tile (M = 64 or 128, N a multiple of 16).
 __host__ __device__ __forceinline__ uint32_t umma_idesc_bf16(int m, int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | (static_cast<uint32_t>(n >> 3) << 17) | (static_cast<uint32_t>(m >> 4) << 24);
