@@ -91,6 +91,16 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
  * pass over the cache instead of two); 0 = two passes of the 16-vector kernel. */
 #define DOVETAIL_TUNE_ATTN_QT2 4
 
+/* Host logic of the tcgen05 GEMV's row-exact work split (csrc/gemv_umma.cuh), callable without a GPU: for a group of
+ * n_mat matrices with rows[] rows dealt to `ctas` CTAs (paired: gate / up; pairperm: head_dim of rotary-paired QKV
+ * rows, else 0) returns per CTA the number of super-blocks n_sb[ctas], the 8-row boxes of each n_grp[ctas][8] and
+ * grp[ctas][8][16] ((matrix << 28) | first row), its row count cnt[ctas] and the tile position of every virtual row
+ * vpos[ctas][*vpos_ld] (super-block * 128 + tile row). Errors: EINVAL, ECAPACITY (more than 8 super-blocks per CTA or
+ * vpos_cap too small). */
+int dovetail_hooks_umma_tables(const int32_t rows[3], int32_t n_mat, int32_t paired, int32_t pairperm, int32_t ctas,
+                               int32_t* n_sb, int32_t* n_grp, int32_t* grp, uint16_t* vpos, int32_t vpos_cap, int32_t* vpos_ld,
+                               int32_t* cnt);
+
 /* Counters of the last dovetail_draft_step, for tests that must know which kernel ran.
  *   key 1: launches of the tcgen05 GEMV (k_gemv_umma). Unknown key or NULL handle: -1. */
 #define DOVETAIL_STAT_UMMA_LAUNCHES 1

@@ -21,7 +21,7 @@ EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_draft_prefill
            "dovetail_verify_plan", "dovetail_verify_accept", "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
-HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune", "dovetail_hooks_stat")
+HOOK_EXPORTS = ("dovetail_hooks_set", "dovetail_trace_enable", "dovetail_trace_read", "dovetail_probe_stream", "dovetail_hooks_tune", "dovetail_hooks_stat", "dovetail_hooks_umma_tables")
 
 
 class DovetailError(RuntimeError):
@@ -414,6 +414,29 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
 
 TUNE_UMMA_MIN_M, TUNE_GRAPHS, TUNE_ATTN_WIDE_MIN, TUNE_ATTN_QT2 = 1, 2, 3, 4
 STAT_UMMA_LAUNCHES, STAT_GRAPH = 1, 2
+
+
+def dovetail_hooks_umma_tables(rows, paired: int, pairperm: int, ctas: int) -> Dict:
+    """Row tables of the tcgen05 GEMV for one dealing (include/dovetail_hooks.h); host logic, no GPU needed."""
+    import numpy as np
+    lib = load()
+    n_mat = len(rows)
+    r = (C.c_int32 * 3)(*(list(rows) + [0] * (3 - n_mat)))
+    n_sb = np.zeros(ctas, np.int32)
+    cnt = np.zeros(ctas, np.int32)
+    n_grp = np.zeros((ctas, 8), np.int32)
+    grp = np.zeros((ctas, 8, 16), np.int32)
+    cap = ctas * (max(rows) * n_mat // ctas + 64)
+    vpos = np.zeros(cap, np.uint16)
+    ld = C.c_int32(0)
+    P = lambda a: a.ctypes.data_as(C.c_void_p)
+    f = lib.dovetail_hooks_umma_tables
+    f.restype = C.c_int
+    f.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_int32] + [C.c_void_p] * 4 + [C.c_int32, C.c_void_p, C.c_void_p]
+    rc = f(r, n_mat, paired, pairperm, ctas, P(n_sb), P(n_grp), P(grp), P(vpos), cap, C.byref(ld), P(cnt))
+    if rc != OK:
+        raise DovetailError(rc, "dovetail_hooks_umma_tables")
+    return dict(n_sb=n_sb, n_grp=n_grp, grp=grp, cnt=cnt, vpos=vpos[:ctas * ld.value].reshape(ctas, ld.value))
 
 
 def dovetail_hooks_stat(h: Draft, key: int) -> int:

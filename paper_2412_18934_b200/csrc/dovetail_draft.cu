@@ -466,24 +466,21 @@ void umma_init(dovetail_draft* h) {
 
 // Row tables of one dealing (gemv_umma.cuh UmmaCtaTab): the CTA's virtual rows sorted into contiguous memory
 // segments, each cut into 8-row boxes; boxes dealt to balanced super-blocks of <= 16 boxes.
-const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& G, int ctas) {
-  const std::array<int, 8> key = {G.rows[0], G.n_mat > 1 ? G.rows[1] : 0, G.n_mat > 2 ? G.rows[2] : 0, G.n_mat, G.paired,
-                                  G.pairperm, ctas, G.deal_base};
-  auto it = h->umma_tabs.find(key);
-  if (it != h->umma_tabs.end()) return it->second;
-  dovetail_draft::UmmaTable t;
+// Pure host logic (tested on the CPU through dovetail_hooks_umma_tables): fills tabs[ctas] and vpos[ctas * vpos_ld].
+// Returns false when a CTA would need more than kUmmaMaxSb super-blocks.
+bool build_umma_tables(const GemvGroup& G, int ctas, std::vector<UmmaCtaTab>& tabs, std::vector<uint16_t>& vpos, int& vpos_ld,
+                       int& g_max, int& g_min) {
   int max_cnt = 0;
   for (int c = 0; c < ctas; ++c) max_cnt = std::max(max_cnt, static_cast<int>(cta_rows(G, c, ctas).cnt));
-  t.vpos_ld = (max_cnt + 7) / 8 * 8;
-  std::vector<UmmaCtaTab> tabs(ctas);
-  std::vector<uint16_t> vpos(static_cast<size_t>(ctas) * std::max(1, t.vpos_ld), 0);
-  bool ok = max_cnt > 0;
-  t.g_max = 0;
-  t.g_min = kUmmaMaxGroups;
-  for (int c = 0; c < ctas && ok; ++c) {
+  vpos_ld = (max_cnt + 7) / 8 * 8;
+  tabs.assign(ctas, UmmaCtaTab{});
+  vpos.assign(static_cast<size_t>(ctas) * std::max(1, vpos_ld), 0);
+  g_max = 0;
+  g_min = kUmmaMaxGroups;
+  if (max_cnt <= 0) return false;
+  for (int c = 0; c < ctas; ++c) {
     const RowRange rr = cta_rows(G, c, ctas);
     UmmaCtaTab& T = tabs[c];
-    memset(&T, 0, sizeof T);
     if (rr.cnt == 0) continue;
     std::vector<std::array<int, 3>> rows(rr.cnt);
     for (int v = 0; v < rr.cnt; ++v) {
@@ -506,16 +503,28 @@ const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& 
     }
     const int Gt = static_cast<int>(gcode.size());
     const int n_sb = div_up(Gt, kUmmaMaxGroups), per = div_up(Gt, n_sb);
-    if (n_sb > kUmmaMaxSb) { ok = false; break; }
+    if (n_sb > kUmmaMaxSb) return false;
     T.n_sb = n_sb;
     for (int g = 0; g < Gt; ++g) {
       T.grp[g / per][g % per] = gcode[g];
       T.n_grp[g / per] = g % per + 1;
     }
-    for (int sb = 0; sb < n_sb; ++sb) { t.g_max = std::max(t.g_max, T.n_grp[sb]); t.g_min = std::min(t.g_min, T.n_grp[sb]); }
+    for (int sb = 0; sb < n_sb; ++sb) { g_max = std::max(g_max, T.n_grp[sb]); g_min = std::min(g_min, T.n_grp[sb]); }
     for (int v = 0; v < rr.cnt; ++v)
-      vpos[static_cast<size_t>(c) * t.vpos_ld + v] = static_cast<uint16_t>((pos[v].first / per) * 128 + (pos[v].first % per) * 8 + pos[v].second);
+      vpos[static_cast<size_t>(c) * vpos_ld + v] = static_cast<uint16_t>((pos[v].first / per) * 128 + (pos[v].first % per) * 8 + pos[v].second);
   }
+  return true;
+}
+
+const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& G, int ctas) {
+  const std::array<int, 8> key = {G.rows[0], G.n_mat > 1 ? G.rows[1] : 0, G.n_mat > 2 ? G.rows[2] : 0, G.n_mat, G.paired,
+                                  G.pairperm, ctas, G.deal_base};
+  auto it = h->umma_tabs.find(key);
+  if (it != h->umma_tabs.end()) return it->second;
+  dovetail_draft::UmmaTable t;
+  std::vector<UmmaCtaTab> tabs;
+  std::vector<uint16_t> vpos;
+  bool ok = build_umma_tables(G, ctas, tabs, vpos, t.vpos_ld, t.g_max, t.g_min);
   if (ok) {
     ok = cudaMalloc(reinterpret_cast<void**>(&t.tab), tabs.size() * sizeof(UmmaCtaTab)) == cudaSuccess &&
          cudaMalloc(reinterpret_cast<void**>(&t.vpos), vpos.size() * sizeof(uint16_t)) == cudaSuccess &&
@@ -1857,6 +1866,35 @@ int dovetail_hooks_set(dovetail_draft_t* h, const dovetail_hooks_t* hooks) {
 }
 
 int dovetail_last_launch_count(const dovetail_draft_t* h) { return h ? h->last_launches : 0; }
+
+int dovetail_hooks_umma_tables(const int32_t rows[3], int32_t n_mat, int32_t paired, int32_t pairperm, int32_t ctas,
+                               int32_t* n_sb, int32_t* n_grp, int32_t* grp, uint16_t* vpos, int32_t vpos_cap, int32_t* vpos_ld,
+                               int32_t* cnt) {
+  if (!rows || n_mat < 1 || n_mat > 3 || ctas < 1 || !n_sb || !n_grp || !grp || !vpos || !vpos_ld || !cnt) return DOVETAIL_EINVAL;
+  GemvGroup G{};
+  long tot = 0;
+  for (int j = 0; j < n_mat; ++j) { G.rows[j] = rows[j]; tot += rows[j]; }
+  G.n_mat = n_mat;
+  G.paired = paired;
+  G.pairperm = pairperm;
+  const long units = paired ? rows[0] : tot / (pairperm ? 2 : 1);  // the dealing of run_gemv
+  G.deal_base = static_cast<int32_t>(units / ctas);
+  G.deal_rem = static_cast<int32_t>(units % ctas);
+  std::vector<UmmaCtaTab> tabs;
+  std::vector<uint16_t> vp;
+  int ld = 0, g_max = 0, g_min = 0;
+  if (!build_umma_tables(G, ctas, tabs, vp, ld, g_max, g_min)) return DOVETAIL_ECAPACITY;
+  if (static_cast<long>(ctas) * ld > vpos_cap) return DOVETAIL_ECAPACITY;
+  *vpos_ld = ld;
+  for (int c = 0; c < ctas; ++c) {
+    n_sb[c] = tabs[c].n_sb;
+    cnt[c] = cta_rows(G, c, ctas).cnt;
+    memcpy(n_grp + static_cast<size_t>(c) * kUmmaMaxSb, tabs[c].n_grp, sizeof tabs[c].n_grp);
+    memcpy(grp + static_cast<size_t>(c) * kUmmaMaxSb * kUmmaMaxGroups, tabs[c].grp, sizeof tabs[c].grp);
+  }
+  memcpy(vpos, vp.data(), vp.size() * sizeof(uint16_t));
+  return DOVETAIL_OK;
+}
 
 int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
   if (!h) return -1;
