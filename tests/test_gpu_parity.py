@@ -249,7 +249,7 @@ def umma_cfg(**kw) -> DraftConfig:
 
 
 @pytest.mark.parametrize("variant", ["m1_forced", "m12", "m20", "m32_max_branch", "n_new33", "n_new64", "mha_dh128_gqa", "no_proj",
-                                     "final_norm", "big_vocab", "huge_vocab", "llama3_vocab_64_rows"])
+                                     "final_norm", "big_vocab", "huge_vocab", "llama3_vocab_64_rows", "tiny_dims"])
 def test_step_parity_umma(variant):
     kw, n_new, min_m = {}, 1, None
     if variant == "m1_forced":  # every level, 1 ... 5 rows, through the tcgen05 kernel (N = 16 columns)
@@ -276,6 +276,8 @@ def test_step_parity_umma(variant):
         kw.update(vocab=70000, tree=TreeSpec(2, (10, 2), (0, 10), 16))
     elif variant == "llama3_vocab_64_rows":  # 867 rows per CTA x 64 LM-head rows: the result buffer does not fit, the
         kw.update(vocab=128256, tree=TreeSpec(3, (8, 8, 1), (0, 8, 64), 40))  # level runs in two 32-row passes; 7 super-blocks
+    elif variant == "tiny_dims":  # fewer rows than CTAs (one row, one box per CTA), a single K-chunk of one slab
+        kw.update(hidden=64, n_q_heads=1, n_kv_heads=1, head_dim=64, ffn=64, vocab=120, tree=TreeSpec(2, (10, 2), (0, 10), 16))
     case = _boost(make_case(umma_cfg(**kw), n_new=n_new))
     s, gpu, ora = _run(case, umma_min_m=min_m)
     assert gpu["umma_launches"] > 0, "the tcgen05 GEMV did not run"
