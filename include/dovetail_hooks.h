@@ -90,6 +90,10 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value);
 /* key 4: 1 (default) = attention launches with 17 ... 32 query vectors use the 32-vectors-per-pass kernel (QT = 2: one
  * pass over the cache instead of two); 0 = two passes of the 16-vector kernel. */
 #define DOVETAIL_TUNE_ATTN_QT2 4
+/* key 5: the tcgen05 GEMVs whose CTAs hold one super-block (O, down, DGF) run with K split over CTA pairs
+ * (csrc/gemv_umma.cuh UmmaParams::ksplit) at levels of at least `value` rows, and at any tcgen05 level when the boxes of a
+ * pair fit a 64-row tile; default 48; 65 = never; 1 = always. */
+#define DOVETAIL_TUNE_UMMA_KSPLIT_MIN_M 5
 
 /* Host logic of the tcgen05 GEMV's row-exact work split (csrc/gemv_umma.cuh), callable without a GPU: for a group of
  * n_mat matrices with rows[] rows dealt to `ctas` CTAs (paired: gate / up; pairperm: head_dim of rotary-paired QKV
@@ -106,6 +110,9 @@ int dovetail_hooks_umma_tables(const int32_t rows[3], int32_t n_mat, int32_t pai
 #define DOVETAIL_STAT_UMMA_LAUNCHES 1
 /*   key 2: how the last step was launched: 0 direct launches, 1 graph replay, 2 graph captured and launched. */
 #define DOVETAIL_STAT_GRAPH 2
+/*   key 3: launches of the tcgen05 GEMV with K split over CTA pairs (direct launches only: a graph replay reports what its
+ *          capture counted). */
+#define DOVETAIL_STAT_KSPLIT_LAUNCHES 3
 int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key);
 
 /* Read-only HBM streaming ceilings, run by bench.py next to the step: reads `bytes`

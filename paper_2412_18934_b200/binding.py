@@ -412,8 +412,8 @@ def dovetail_trace_read(h: Draft, cap: int = 4096) -> Dict:
     return dict(step_us=(last - first) * 1e-3 if first is not None else 0.0, kinds=kinds, levels=levels)
 
 
-TUNE_UMMA_MIN_M, TUNE_GRAPHS, TUNE_ATTN_WIDE_MIN, TUNE_ATTN_QT2 = 1, 2, 3, 4
-STAT_UMMA_LAUNCHES, STAT_GRAPH = 1, 2
+TUNE_UMMA_MIN_M, TUNE_GRAPHS, TUNE_ATTN_WIDE_MIN, TUNE_ATTN_QT2, TUNE_UMMA_KSPLIT_MIN_M = 1, 2, 3, 4, 5
+STAT_UMMA_LAUNCHES, STAT_GRAPH, STAT_KSPLIT_LAUNCHES = 1, 2, 3
 
 
 def dovetail_hooks_umma_tables(rows, paired: int, pairperm: int, ctas: int) -> Dict:

@@ -95,6 +95,7 @@ struct dovetail_draft {
   int last_launches = 0;
   int launches = 0;
   int umma_launches = 0, last_umma_launches = 0;
+  int ksplit_launches = 0, last_ksplit_launches = 0;
   bool dry = false;  // shape-checking pass of dovetail_draft_step: nothing is launched
   // GEMVs queued by run_gemv, launched by flush_gemv
   struct QueuedGemv { GemvParams p; int n_groups, ctas, kind, max_cnt; int64_t bytes; };
@@ -103,13 +104,15 @@ struct dovetail_draft {
   // each: 1, 2, 4, 8 slabs of 64 k), row tables of every dealing seen so far
   int umma_min_m = 8;               // levels of at least this many rows take the tcgen05 kernel (65: never)
   int attn_max_clusters[3][9] = {};  // [mode][cluster size]: clusters of the attention kernel resident at once
+  int umma_ksplit_min_m = 48;       // levels of at least this many rows split K over CTA pairs whatever the tile (65: never)
   int attn_qt2 = 1;                 // 17 ... 32 query vectors take the 32-per-pass attention kernel
   int attn_wide_min = 32;           // levels with more query vectors (rows x q-heads per kv-head) take the wide attention kernel
   CUtensorMap* maps_dev = nullptr;  // [n_maps][4]
   std::map<const void*, int> wmap_of;  // weight matrix -> first map index
   struct PlaneBuf { const __nv_bfloat16* base; int64_t elems, ld; int cap, map; };
   std::vector<PlaneBuf> plane_bufs;
-  struct UmmaTable { UmmaCtaTab* tab = nullptr; uint16_t* vpos = nullptr; int vpos_ld = 0, g_max = 0, g_min = 0; bool ok = false; };
+  struct UmmaTable { UmmaCtaTab* tab = nullptr; uint16_t* vpos = nullptr; int vpos_ld = 0, g_max = 0, g_min = 0; bool ok = false;
+                     int pair_max = 0, pair_min = 0; };  // K split over CTA pairs: boxes of CTAs 2i and 2i + 1 together (0: not eligible)
   std::map<std::array<int, 8>, UmmaTable> umma_tabs;
   __nv_bfloat16* xs_par = nullptr;  // [3][max_rows][ld_d] parent hidden states of a wide level, gathered
   // One CUDA graph per (tree_spec, n_new, attention geometry): the step's launch sequence with its
@@ -525,6 +528,17 @@ const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& 
   std::vector<UmmaCtaTab> tabs;
   std::vector<uint16_t> vpos;
   bool ok = build_umma_tables(G, ctas, tabs, vpos, t.vpos_ld, t.g_max, t.g_min);
+  if (ok && ctas % 2 == 0) {  // pairs (2i, 2i + 1) of single-super-block CTAs whose boxes fit one tile together
+    t.pair_max = 0;
+    t.pair_min = 2 * kUmmaMaxGroups;
+    for (int c = 0; c < ctas; c += 2) {
+      if (tabs[c].n_sb != 1 || tabs[c + 1].n_sb != 1) { t.pair_max = 0; break; }
+      const int g2 = tabs[c].n_grp[0] + tabs[c + 1].n_grp[0];
+      t.pair_max = std::max(t.pair_max, g2);
+      t.pair_min = std::min(t.pair_min, g2);
+    }
+    if (t.pair_max > kUmmaMaxGroups) t.pair_max = 0;
+  }
   if (ok) {
     ok = cudaMalloc(reinterpret_cast<void**>(&t.tab), tabs.size() * sizeof(UmmaCtaTab)) == cudaSuccess &&
          cudaMalloc(reinterpret_cast<void**>(&t.vpos), vpos.size() * sizeof(uint16_t)) == cudaSuccess &&
@@ -538,12 +552,14 @@ const dovetail_draft::UmmaTable& umma_table(dovetail_draft* h, const GemvGroup& 
 
 struct UmmaGeom {
   bool ok;
-  int nslab, n_stages, stage_bytes, a_groups, b_groups, umma_m, tmem_cols, acc_cols, k_split, cnt_pad, ring_bytes, smem;
+  int nslab, n_stages, stage_bytes, a_groups, b_groups, umma_m, tmem_cols, acc_cols, k_split, cnt_pad, ring_bytes, smem, ksplit;
 };
 
 // Ring of one launch: the deepest K-chunk (64 * nslab elements) that leaves >= 3 stages or >= 120 KB in flight.
-UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
+// ks2 = true: K split over CTA pairs (gemv_umma.cuh UmmaParams::ksplit): g_max / g_min are the pair sums of boxes.
+UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt, bool ks2 = false, int g_min_pair = 0) {
   UmmaGeom u{};
+  u.ksplit = ks2 ? 2 : 1;
   const int M8 = (M + 7) / 8 * 8;
   u.acc_cols = (s_max * M8 + 15) / 16 * 16;
   u.b_groups = u.acc_cols / 8;
@@ -553,7 +569,7 @@ UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
   u.tmem_cols = 32;
   while (u.tmem_cols < 2 * u.k_split * u.acc_cols) u.tmem_cols *= 2;
   u.cnt_pad = (max_cnt + 3) / 4 * 4;
-  const int tail = 2544 + M * u.cnt_pad * 4;  // barriers, 1 / rms, row map, results (gemv_umma.cuh)
+  const int tail = 2544 + M * u.cnt_pad * 4 * (ks2 ? 2 : 1);  // barriers, 1 / rms, row map, results (+ outbox) (gemv_umma.cuh)
   UmmaGeom best{};
   for (int nslab = 8; nslab >= 1; nslab >>= 1) {
     if (K % (64 * nslab) != 0) continue;
@@ -563,7 +579,14 @@ UmmaGeom umma_geom(int K, int M, int s_max, int g_max, int max_cnt) {
     g.stage_bytes = (g.b_groups + g_max) * gb;
     // the tensor core reads whole 64- / 128-row tiles: past the weight groups into the activation part, and past
     // the last stage only by what that part does not cover
-    const int pad = std::max(0, g.umma_m / 8 - g_max - g.b_groups) * gb;
+    const int pad = std::max(0, g.umma_m / 8 - (ks2 ? g_min_pair : g_max) - g.b_groups) * gb;
+    if (ks2) {  // every CTA of a pair needs >= k_split chunks of its own
+      const int per_rank = K / (64 * nslab) / 2;
+      if (per_rank < 1) continue;
+      g.k_split = std::min(g.k_split, per_rank);
+      g.tmem_cols = 32;
+      while (g.tmem_cols < 2 * g.k_split * g.acc_cols) g.tmem_cols *= 2;
+    }
     g.n_stages = std::min(8, (kSmemMax - 1024 - tail - pad) / g.stage_bytes);
     if (g.n_stages < 2) continue;
     g.ring_bytes = g.n_stages * g.stage_bytes + pad;
@@ -582,7 +605,8 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
   GemvParams& p = q.p;
   if (p.K % 64 != 0 || !h->maps_dev) return DOVETAIL_OK;
   UmmaParams up{};
-  int s_max = 1, g_max = 0;
+  int s_max = 1, g_max = 0, pair_max = 0, pair_min = 2 * kUmmaMaxGroups;
+  bool pair_ok = true;
   for (int gi = 0; gi < q.n_groups; ++gi) {
     GemvGroup& G = p.g[gi];
     if (G.xkind != X_ROWS || G.xidx != nullptr || !G.xs) return DOVETAIL_OK;
@@ -607,13 +631,25 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
     if (gi > 0 && T.vpos_ld != up.vpos_ld) return DOVETAIL_OK;  // groups of one launch share the dealing shape
     up.vpos_ld = T.vpos_ld;
     g_max = std::max(g_max, T.g_max);
+    pair_max = std::max(pair_max, T.pair_max);
+    pair_min = std::min(pair_min, T.pair_min);
+    if (T.pair_max == 0) pair_ok = false;
   }
   const int Mtot = p.M;
   int Mc = Mtot;
-  UmmaGeom g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+  // CTAs with few rows at wide levels: K split over CTA pairs (half the activation operand and half the MMAs per CTA)
+  // Measured: at 64 rows per level it always pays (13B shape: down 59 -> 48 us, batch of 64 prompt rows 988 -> 925 us);
+  // below that only when the pair's boxes fit a 64-row tile (7B shape, 28 rows per CTA: down 24.8 -> 19.5 us at 10 rows;
+  // 13B shape, 35 rows per CTA and a 128-row tile: 679 -> 697 us per forward at 16 rows).
+  const bool ks2 = pair_ok && (Mtot >= h->umma_ksplit_min_m || (pair_max <= 8 && h->umma_ksplit_min_m <= kUmmaMaxM));
+  auto geom = [&](int m) {
+    UmmaGeom x = ks2 ? umma_geom(p.K, m, s_max, pair_max, q.max_cnt, true, pair_min) : UmmaGeom{};
+    return x.ok ? x : umma_geom(p.K, m, s_max, g_max, q.max_cnt);
+  };
+  UmmaGeom g = geom(Mc);
   while (!g.ok && Mc > 8) {
     Mc = (Mc / 2 + 7) / 8 * 8;
-    g = umma_geom(p.K, Mc, s_max, g_max, q.max_cnt);
+    g = geom(Mc);
   }
   if (!g.ok) return DOVETAIL_OK;
   int lg = 0;
@@ -623,7 +659,7 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
     for (int j = 0; j < p.g[gi].n_mat; ++j) up.wmap[gi][j] += lg;
   }
   up.nslab = g.nslab; up.n_stages = g.n_stages; up.stage_bytes = g.stage_bytes; up.a_groups = g.a_groups;
-  up.umma_m = g.umma_m; up.tmem_cols = g.tmem_cols; up.acc_cols = g.acc_cols; up.k_split = g.k_split; up.cnt_pad = g.cnt_pad;
+  up.umma_m = g.umma_m; up.tmem_cols = g.tmem_cols; up.acc_cols = g.acc_cols; up.k_split = g.k_split; up.ksplit = g.ksplit; up.cnt_pad = g.cnt_pad;
   up.ring_bytes = g.ring_bytes;
   p.n_groups = q.n_groups;
   p.ctas_per_group = q.ctas;
@@ -636,8 +672,8 @@ int run_umma(dovetail_draft* h, cudaStream_t st, dovetail_draft::QueuedGemv& q, 
     h->cur_bytes = m0 == 0 ? q.bytes : 0;  // the algorithmic bytes are counted once
     p.trace = trace_slot(h);
     up.p = p;
-    if (!h->dry) ++h->umma_launches;
-    cudaError_t e = launch(h, k_gemv_umma, dim3(q.n_groups * q.ctas), dim3(kUmmaThreads), g.smem, st, up);
+    if (!h->dry) { ++h->umma_launches; if (g.ksplit == 2) ++h->ksplit_launches; }
+    cudaError_t e = launch_c(h, g.ksplit, true, k_gemv_umma, dim3(q.n_groups * q.ctas), dim3(kUmmaThreads), g.smem, st, up);
     if (e != cudaSuccess) return fail(h, DOVETAIL_ECUDA, "GEMV (tcgen05) launch failed: %s", cudaGetErrorString(e));
   }
   p.M = Mtot;
@@ -942,6 +978,7 @@ int enqueue_step(dovetail_draft* h, cudaStream_t st, const float* hidden_feats, 
   int rc = DOVETAIL_OK;
   h->launches = 0;
   h->umma_launches = 0;
+  h->ksplit_launches = 0;
   const int d = c.hidden, F = c.ffn, V = c.vocab, dh = c.head_dim, half = dh / 2;
   const int dq = h->dq, dkv = h->dkv, ldq = h->ldq, nsm = h->num_sms;
   const int grp = c.n_q_heads / c.n_kv_heads;
@@ -1345,7 +1382,7 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
       attn_mma_geom(h, Lp, mode, wn[1], wc[1]);
       key.insert(key.end(), {wn[0], wc[0], wn[1], wc[1]});
     }
-    key.insert(key.end(), {h->attn_wide_min, h->attn_qt2});
+    key.insert(key.end(), {h->attn_wide_min, h->attn_qt2, h->umma_ksplit_min_m});
   } else {
     nc[0] = std::min(h->attn_chunks_cap, std::max(1, div_up(L, 2 * kAttnStagePos)));
     nc[1] = std::min(h->attn_chunks_cap, std::max(1, div_up(Lp, 2 * kAttnStagePos)));
@@ -1635,6 +1672,7 @@ int dovetail_draft_step(dovetail_draft_t* h, const float* hidden_feats, const in
   h->last_gamma = tree->gamma;
   h->last_launches = h->launches;
   h->last_umma_launches = h->umma_launches;
+  h->last_ksplit_launches = h->ksplit_launches;
   return DOVETAIL_OK;
 }
 
@@ -1900,6 +1938,7 @@ int dovetail_hooks_stat(const dovetail_draft_t* h, int32_t key) {
   if (!h) return -1;
   if (key == DOVETAIL_STAT_UMMA_LAUNCHES) return h->last_umma_launches;
   if (key == DOVETAIL_STAT_GRAPH) return h->last_graph;
+  if (key == DOVETAIL_STAT_KSPLIT_LAUNCHES) return h->last_ksplit_launches;
   return -1;
 }
 
@@ -1911,6 +1950,7 @@ int dovetail_hooks_tune(dovetail_draft_t* h, int32_t key, int32_t value) {
     return DOVETAIL_OK;
   }
   if (key == DOVETAIL_TUNE_GRAPHS && (value == 0 || value == 1)) { h->graphs_on = value != 0; return DOVETAIL_OK; }
+  if (key == DOVETAIL_TUNE_UMMA_KSPLIT_MIN_M && value >= 1 && value <= kUmmaMaxM + 1) { h->umma_ksplit_min_m = value; return DOVETAIL_OK; }
   if (key == DOVETAIL_TUNE_ATTN_QT2 && (value == 0 || value == 1)) { h->attn_qt2 = value; return DOVETAIL_OK; }
   if (key == DOVETAIL_TUNE_ATTN_WIDE_MIN && value >= 0 && value <= 4096) { h->attn_wide_min = value; return DOVETAIL_OK; }
   return fail(h, DOVETAIL_EINVAL, "unknown knob %d or value %d out of range", key, value);

@@ -27,6 +27,7 @@
 #pragma once
 #include <cuda_bf16.h>
 
+#include "attention_mma.cuh"  // thread-block cluster helpers (cluster rank, barrier, distributed shared memory loads)
 #include "gemv.cuh"
 #include "gemv_mma.cuh"
 #include "ptx.cuh"
@@ -67,6 +68,11 @@ struct UmmaParams {
                                   // core's fp32 accumulation rounds towards zero; chains of K / 16 steps into one
                                   // accumulator cost 3x the error of the mma.sync kernel's 8 shorter chains (measured),
                                   // so the chain is cut and the parts are added in fp32 by the epilogue
+  int32_t ksplit;                 // 2: the CTAs of a cluster pair split K. Each multiplies the rows of BOTH over its half of K
+                                  // (own rows = tile rows first, then the partner's), the partials of the partner's rows
+                                  // go to an outbox the partner adds through distributed shared memory. A CTA with few rows
+                                  // (O, down, DGF: 35 of a 64- / 128-row tile) then reads half of the activation operand
+                                  // and issues half of the MMAs -- at 32-64 columns those, not HBM, bound it. 1: off
   int32_t cnt_pad;                // row stride of the result buffer res[m][v]
   int32_t ring_bytes;             // ring + the pad the tensor core may read past the last stage
 };
@@ -89,6 +95,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
   float* rstd_s = reinterpret_cast<float*>(tslot + 4);                // [kUmmaMaxM]
   int16_t* rmap = reinterpret_cast<int16_t*>(rstd_s + kUmmaMaxM);     // [kUmmaMaxSb][128]: virtual row of a tile row, or -1
   float* res = reinterpret_cast<float*>(rmap + kUmmaMaxSb * 128);     // [M][cnt_pad]
+  float* outbox = res + static_cast<size_t>(p.M) * cp.cnt_pad;          // ksplit = 2: partials of the partner's rows, [M][cnt_pad]
 
   trace_begin(p.trace);
   if (tid < NS) {
@@ -118,6 +125,12 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
   const int N = (S * M8 + 15) & ~15;        // UMMA N
   const int n_chunks = p.K / (64 * nslab);
   const UmmaCtaTab* tab = c >= 0 ? cp.tab[gi] + c : nullptr;
+  // K split over a cluster pair: this CTA's chunks, the partner's boxes appended to its own
+  const bool ks2 = cp.ksplit == 2;
+  const int krank = ks2 ? static_cast<int>(cluster_ctarank()) : 0;
+  const int ch0 = ks2 && krank ? (n_chunks + 1) / 2 : 0, ch1 = ks2 && !krank ? (n_chunks + 1) / 2 : n_chunks;
+  const UmmaCtaTab* ptab = ks2 ? cp.tab[gi] + (c ^ 1) : nullptr;
+  const int png = ks2 ? ptab->n_grp[0] : 0;  // the partner's boxes (ksplit needs one super-block per CTA)
 
   if (warp == kConsumerWarps) {
     // ---------------- weight producer: one box per lane and stage; never waits for the previous kernel -------
@@ -126,11 +139,11 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
       const int n_sb = tab->n_sb;
       int slot = 0, round = 0;
       for (int sb = 0; sb < n_sb; ++sb) {
-        const int ng = tab->n_grp[sb];
-        const int gr = lane < ng ? tab->grp[sb][lane] : 0;
+        const int ng0 = tab->n_grp[sb], ng = ng0 + png;
+        const int gr = lane < ng ? (lane < ng0 ? tab->grp[sb][lane] : ptab->grp[0][lane - ng0]) : 0;
         const CUtensorMap* map = cp.wmap[gi][gr >> 28];
         const int row = gr & 0x0fffffff;
-        for (int ch = 0; ch < n_chunks; ++ch) {
+        for (int ch = ch0; ch < ch1; ++ch) {
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
           if (lane == 0) mbar_arrive_expect_tx(&full_a[slot], static_cast<uint32_t>(ng) * GB);
           __syncwarp();
@@ -153,7 +166,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
       const int row = s * cp.x_cap[gi] + cp.x_row0[gi] + p.m0 + g8 * 8;
       int slot = 0, round = 0;
       for (int sb = 0; sb < n_sb; ++sb) {
-        for (int ch = 0; ch < n_chunks; ++ch) {
+        for (int ch = ch0; ch < ch1; ++ch) {
           if (round > 0) mbar_wait(&empty[slot], (round & 1) ^ 1);
           if (lane == 0) mbar_arrive_expect_tx(&full_b[slot], static_cast<uint32_t>(nB) * GB);
           __syncwarp();
@@ -178,7 +191,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
         tc_fence_after();
         const uint32_t d_buf = tmem + static_cast<uint32_t>(buf * cp.k_split * cp.acc_cols);
         int ks = 0;
-        for (int ch = 0; ch < n_chunks; ++ch) {
+        for (int ch = ch0; ch < ch1; ++ch) {
           const uint32_t d_addr = d_buf + static_cast<uint32_t>(ks * cp.acc_cols);
           if (++ks == cp.k_split) ks = 0;
           mbar_wait(&full_a[slot], round & 1);
@@ -187,7 +200,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
           if (elect_one()) {
             const uint32_t a_base = ring_u + static_cast<uint32_t>(slot) * cp.stage_bytes;
             uint32_t a_lo = umma_desc_lo(a_base), b_lo = umma_desc_lo(a_base + static_cast<uint32_t>(cp.a_groups) * GB);
-            uint32_t accum = ch >= cp.k_split ? 1u : 0u;
+            uint32_t accum = ch - ch0 >= cp.k_split ? 1u : 0u;
             for (int sl = 0; sl < nslab; ++sl) {  // one slab = 64 k = four MMAs
               umma_bf16(d_addr, a_lo, b_lo, desc_hi, idesc, accum);
               umma_bf16(d_addr, a_lo + 2, b_lo + 2, desc_hi, idesc, 1u);
@@ -198,7 +211,7 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
               accum = 1u;
             }
             umma_commit(&empty[slot]);                       // the stage may be refilled once these MMAs have read it
-            if (ch == n_chunks - 1) umma_commit(&tm_full[buf]);  // the super-block's accumulators are complete
+            if (ch == ch1 - 1) umma_commit(&tm_full[buf]);  // the super-block's accumulators are complete
           }
           __syncwarp();
           if (++slot == NS) { slot = 0; ++round; }
@@ -211,6 +224,11 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
     if (c >= 0) {
       const uint16_t* vp = cp.vpos[gi] + static_cast<size_t>(c) * cp.vpos_ld;
       for (int v = tid; v < rr.cnt; v += kConsumerThreads) rmap[vp[v]] = static_cast<int16_t>(v);
+      if (ks2) {  // the partner's rows follow this CTA's boxes in the tile; marked by + 1024
+        const uint16_t* vq = cp.vpos[gi] + static_cast<size_t>(c ^ 1) * cp.vpos_ld;
+        const int pcnt = cta_rows(G, c ^ 1, p.ctas_per_group).cnt, shift = tab->n_grp[0] * 8;
+        for (int v = tid; v < pcnt; v += kConsumerThreads) rmap[vq[v] + shift] = static_cast<int16_t>(1024 + v);
+      }
     }
     pdl_wait();  // residual stream, [h1 || h2], sums of squares: written by the previous kernels
     if (c >= 0) {
@@ -274,7 +292,8 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
                 if (S >= 2) t += acc[1][i];
                 if (S == 3) t += acc[2][i];
                 if (p.ssq_in) t *= rstd_s[m];
-                res[m * cpad + v] = t;
+                if (v >= 1024) outbox[m * cpad + (v - 1024)] = t;
+                else res[m * cpad + v] = t;
               }
             }
           }
@@ -283,9 +302,22 @@ __global__ void __launch_bounds__(kUmmaThreads, 1) k_gemv_umma(const __grid_cons
         __syncwarp();
         if (lane == 0) mbar_arrive(&tm_empty[buf]);
       }
+      if (ks2) {
+        // both CTAs of the pair have drained: add the partner's partials of this CTA's rows (its outbox)
+        cluster_sync_all();
+        const uint32_t ob = smem_u32(outbox);
+        for (int idx = tid; idx < M * rr.cnt; idx += kConsumerThreads) {
+          const int m = idx / rr.cnt, v = idx - m * rr.cnt;
+          res[m * cpad + v] += ld_dsmem_f32(ob + static_cast<uint32_t>(m * cpad + v) * 4u, static_cast<uint32_t>(krank ^ 1));
+        }
+      }
       consumer_sync();  // res complete
       gemv_epilogue(p, G, rr, [&](int v, int m) -> float& { return res[m * cpad + v]; }, M, p.m0, c, p.ctas_per_group, true, &pre);
     }
+  }
+  if (ks2) {
+    if (warp >= kConsumerWarps) cluster_sync_all();  // the producer / MMA warps' share of the consumers' barrier above
+    cluster_sync_all();                               // no CTA of the pair exits while its outbox may still be read
   }
   tc_fence_before();
   __syncthreads();

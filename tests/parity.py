@@ -73,7 +73,7 @@ def _kv_torch(a: np.ndarray, like: torch.Tensor) -> torch.Tensor:
 
 
 def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: int = 128, max_branch: int = 32,
-            force: Optional[dict] = None, umma_min_m: Optional[int] = None):
+            force: Optional[dict] = None, umma_min_m: Optional[int] = None, umma_ksplit_min_m: Optional[int] = None):
     """One step through the C ABI. Returns (handle, kv, dict of host arrays).
 
     force = an oracle result: teacher forcing -- every level is computed from the oracle's hidden states,
@@ -85,6 +85,8 @@ def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: i
     kv = binding.KVCache(k, v, case.L)
     if umma_min_m is not None:  # which levels run on the tcgen05 GEMV (include/dovetail_hooks.h)
         binding.dovetail_hooks_tune(h, binding.TUNE_UMMA_MIN_M, umma_min_m)
+    if umma_ksplit_min_m is not None:  # from how many rows CTAs with few rows split K over cluster pairs
+        binding.dovetail_hooks_tune(h, binding.TUNE_UMMA_KSPLIT_MIN_M, umma_ksplit_min_m)
     hooks = {}
     n_new = case.tokens.shape[0]
     rows = n_new + tree.tree_rows()
@@ -111,7 +113,8 @@ def run_gpu(case: Case, taps: bool = True, max_rows: int = 64, max_tree_slots: i
                logits=g("tap_logits"), hhat=g("tap_hhat"), pool_token=g("tap_pool_token"), pool_cum=g("tap_pool_cum"),
                k=kv_np(hooks.get("tap_k", k)), v=kv_np(hooks.get("tap_v", v)), forced=force is not None,
                committed_len=kv.committed_len, launches=binding.dovetail_last_launch_count(h),
-               umma_launches=binding.dovetail_hooks_stat(h, binding.STAT_UMMA_LAUNCHES))
+               umma_launches=binding.dovetail_hooks_stat(h, binding.STAT_UMMA_LAUNCHES),
+               ksplit_launches=binding.dovetail_hooks_stat(h, binding.STAT_KSPLIT_LAUNCHES))
     return h, kv, res
 
 

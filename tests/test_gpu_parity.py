@@ -283,3 +283,29 @@ def test_step_parity_umma(variant):
     assert gpu["umma_launches"] > 0, "the tcgen05 GEMV did not run"
     assert s["same_tree"]
     assert s["free"]["same_tree"] or s["free"]["tie"] is not None
+
+
+@pytest.mark.parametrize("variant", ["m1_forced", "m12", "m32_max_branch", "n_new64", "mha_dh128_gqa", "no_proj", "tiny_dims"])
+def test_step_parity_umma_k_split(variant):
+    """The tcgen05 GEMV with K split over CTA pairs (csrc/gemv_umma.cuh UmmaParams::ksplit) forced on from one row:
+    O, down and the DGF matrices (one super-block per CTA) take it, the others do not."""
+    kw, n_new, min_m = {}, 1, None
+    if variant == "m1_forced":
+        min_m = 1
+    elif variant == "m12":
+        kw.update(tree=TreeSpec(3, (6, 3, 2), (0, 0, 12), 20))
+    elif variant == "m32_max_branch":
+        kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    elif variant == "n_new64":
+        n_new = 64
+    elif variant == "mha_dh128_gqa":
+        kw.update(hidden=256, n_q_heads=4, n_kv_heads=2, head_dim=128, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    elif variant == "no_proj":
+        kw.update(dgf_proj=0, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    elif variant == "tiny_dims":
+        kw.update(hidden=64, n_q_heads=1, n_kv_heads=1, head_dim=64, ffn=64, vocab=120, tree=TreeSpec(2, (10, 2), (0, 10), 16))
+    case = _boost(make_case(umma_cfg(**kw), n_new=n_new))
+    s, gpu, ora = _run(case, umma_min_m=min_m, umma_ksplit_min_m=1)
+    assert gpu["umma_launches"] > 0 and gpu["ksplit_launches"] > 0, "no GEMV ran with K split over a CTA pair"
+    assert s["same_tree"]
+    assert s["free"]["same_tree"] or s["free"]["tie"] is not None
