@@ -1486,7 +1486,7 @@ int dovetail_draft_init(const dovetail_weights_t* w, const dovetail_config_t* cf
   const dovetail_config_t& c = *cfg;
   if (c.hidden < 8 || c.n_q_heads < 1 || c.n_kv_heads < 1 || c.n_q_heads % c.n_kv_heads != 0 ||
       (c.head_dim != 64 && c.head_dim != 128) || c.n_layers < 1 || c.n_layers > DOVETAIL_MAX_LAYERS ||
-      c.ffn < 8 || c.vocab < 1 || !(c.rope_theta > 0.f) || !(c.rms_eps >= 0.f) ||
+      c.ffn < 8 || c.vocab < 1 || c.vocab > (1 << 24) - 2 || !(c.rope_theta > 0.f) || !(c.rms_eps >= 0.f) ||
       (c.dtype != DOVETAIL_F32 && c.dtype != DOVETAIL_BF16) ||
       (c.fusion != DOVETAIL_FUSION_DGF && c.fusion != DOVETAIL_FUSION_CONCAT_LINEAR) ||
       (c.fusion == DOVETAIL_FUSION_CONCAT_LINEAR && c.dgf_proj))

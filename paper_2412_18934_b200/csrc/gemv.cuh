@@ -80,7 +80,7 @@ struct GemvParams {
   int32_t d;
   int32_t b;             // LMHEAD: candidates kept per row
   int32_t vocab;
-  float* cand_val;       // LMHEAD: [kMaxRows][grid][kMaxBranch]
+  float* cand_val;       // LMHEAD: [kMaxRows][kMaxBranch][grid]
   int32_t* cand_id;
   float* stat;           // LMHEAD: [kMaxRows][grid][2] = (max, sum exp)
   float* tap;            // LMHEAD: optional logits tap rows [M, vocab]
@@ -339,7 +339,11 @@ __device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGro
           const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
           if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
         }
-        if (lane == 0) { p.cand_val[pc * kMaxBranch + jb] = bv; p.cand_id[pc * kMaxBranch + jb] = bi; }
+        if (lane == 0) {  // entry-major: the heads (jb = 0) of a row's lists are contiguous for k_tree_level
+          const int64_t o = (static_cast<int64_t>(mbase + m) * kMaxBranch + jb) * nct + c;
+          p.cand_val[o] = bv;
+          p.cand_id[o] = bi;
+        }
         lv = bv; li = bi;
       }
     }

@@ -36,6 +36,7 @@ struct RowTables {
   int32_t src[kMaxRows];    // step row whose output hidden state is this row's input feature
   int32_t slot[kMaxRows];   // new-region slot index j: cache row = Lbase + j
   int32_t pool[kMaxRows];   // pool index of the node forwarded at this row (-1 at level 0)
+  float cum[kMaxRows];      // that node's cumulative log-probability (0 at level 0)
   uint32_t mask[kMaxRows][kMaskWords];  // new-region slots the row attends (incl. itself)
 };
 

@@ -58,6 +58,7 @@ __global__ void k_step_begin(const StepDyn dynv, StepDyn* dyn, TreeState* ts, Ro
       rt0->src[m] = m;
       rt0->slot[m] = m;  // cache row L + m
       rt0->pool[m] = -1;
+      rt0->cum[m] = 0.f;
       for (int w = 0; w < kMaskWords; ++w) {  // causal among the level-0 rows: bits 0..m
         const int lo = w * 32;
         rt0->mask[m][w] = m >= lo + 31 ? 0xffffffffu : (m < lo ? 0u : (0xffffffffu >> (31 - (m - lo))));
@@ -199,67 +200,108 @@ __device__ __forceinline__ bool node_before(const float* cum, int a, int b) {
   return ca > cb || (ca == cb && a < b);
 }
 
+// A candidate (value, id) as an order-preserving pair of unsigned words: (key, lo) compares like cand_before
+// (larger value first, then smaller id). key 0 = no candidate (below every real value, -inf included);
+// -0 is canonicalised to +0 (cand_before treats them as equal). ids < 2^24 (dovetail_draft_init checks the vocabulary).
+__device__ __forceinline__ uint32_t cand_key(float v, int id) {
+  const uint32_t u = __float_as_uint(v + 0.f);
+  return id == 0x7fffffff ? 0u : ((u >> 31) ? ~u : (u | 0x80000000u));
+}
+__device__ __forceinline__ uint32_t cand_lo(int id, int cta) {
+  return id == 0x7fffffff ? 0u : ((static_cast<uint32_t>(0xffffff - id) << 8) | static_cast<uint32_t>(cta));
+}
+__device__ __forceinline__ float cand_key_value(uint32_t key) {
+  return key == 0u ? -INFINITY : __uint_as_float((key >> 31) ? (key & 0x7fffffffu) : ~key);
+}
+
+__device__ __forceinline__ uint64_t umax64(uint64_t a, uint64_t b) { return a > b ? a : b; }
+
 constexpr int kTreeThreads = 512;  // one warp per expanded row for levels of <= 16 rows (a row's merge is a serial chain)
 constexpr int kPoolSmem = 4352;  // >= kMaxBranch + kMaxTreeSlots * kMaxBranch + slack
+constexpr int kNoCand = 0x7fffffff;  // id of the "no candidate" entry (value -inf): after every real candidate
 
+// Pool::row of a child: >= 0 the step row it is forwarded at; -1 not forwarded; -2 not forwarded and outside its
+// own level's top-gamma, hence outside the step's top-gamma (S8 does not look at it).
 __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelParams p) {
-  // phases B / C: pool scores and keep flags
   __shared__ float s_raw[2 * kPoolSmem];
-  __shared__ int32_t s_cnt[kTreeThreads + 1];
   __shared__ int32_t s_tok[kMaxRows * kMaxBranch];  // this level's children: tokens (scores in s_cum), row-major [row][rank]
-  float* s_cum = s_raw;
-  int32_t* s_new = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);
+  __shared__ uint32_t s_bits[kPoolSmem / 32];       // S8: kept nodes, one bit per pool index
+  __shared__ int32_t s_nc;
+  float* s_cum = s_raw;                 // phases A / B: this level's children; S8: candidate scores
+  float* s_scr = s_raw + kPoolSmem;     // phase A: per-warp list tails; S8: candidate pool indices
   pdl_launch_dependents();
   trace_begin(p.trace);
-  pdl_wait();
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const Pool& P = p.pool;
+  // kernel parameters before the wait: their (cold) constant-bank misses overlap the LM head's tail
+  const int b = p.b, nct = p.nct;
+  const float* cv0 = p.cand_val;
+  const int32_t* ci0 = p.cand_id;
+  const float* st0 = p.stat;
+  asm volatile("" ::"r"(b), "r"(nct), "l"(cv0), "l"(ci0), "l"(st0));
+  pdl_wait();
 
   // ---- phase A: children of each expanded row --------------------------------
-  // One warp per row. The row's global top-b is a b-round merge of the per-CTA lists, each of which is sorted in the
-  // strict candidate order (gemv.cuh EPI_LMHEAD). Lane l owns the lists of CTAs l, l + 32, ... and keeps a window
-  // of two entries per list in registers: a round picks the best head of the warp, the owning lane shifts that
-  // list's window and requests the entry after it -- needed only if the same list wins twice more, so its L2
-  // round trip is off the critical path. (Staging whole lists through shared memory, two rows at a time, cost
-  // 53 us per level at 10 rows x 10 children; this takes the lists where they are.)
-  for (int m = warp; m < p.M; m += kTreeThreads / 32) {
-    const int parent = p.cur->pool[m];
-    const float pcum = parent < 0 ? 0.f : P.cum[parent];
-    const int base = p.pool_begin + m * p.b;
+  // One warp per row. The per-CTA lists of the LM head are sorted in the strict candidate order (gemv.cuh
+  // EPI_LMHEAD) and stored entry-major ([row][entry j][CTA c]): the heads of a row are contiguous.
+  //  (1) the warp reads every head (coalesced) and the (max, sum exp) pairs;
+  //  (2) b rounds of warp-argmax over the heads name the b lists with the best heads, in order (lane r keeps the
+  //      r-th). No other list can contribute: b heads come before each of its entries. Entry j of the r-th list has
+  //      r + j candidates before it, so only j < b - r matters;
+  //  (3) the second entry of every list comes with the heads; the other tail entries of the b lists (b > 2) are
+  //      fetched in one batch into shared memory;
+  //  (4) b rounds merge the <= b lists, lane r owning the r-th, without touching global memory.
+  // (A merge that fetched a list's next entry when its head won paid an L2 round trip per round -- the scoreboard
+  // waits for the load even where the value is not needed yet -- and its 128-byte-strided head loads cost 32 tag
+  // look-ups per instruction: 15 us at 10 rows x 10 children, 37 us at 32 rows x 2, 21 us at 1 row x 32.)
+  const int per_row = 2 * b * b;  // words of scratch per warp
+  const int n_act = max(1, min(kTreeThreads / 32, kPoolSmem / per_row));
+  for (int m = warp; m < p.M && warp < n_act; m += n_act) {
+    const int base = p.pool_begin + m * b;
     if (p.rp_tokens) {
-      if (lane < p.b) {
+      const int parent = p.cur->pool[m];
+      const float pcum = parent < 0 ? 0.f : p.cur->cum[m];
+      if (lane < b) {
         const size_t o = static_cast<size_t>(p.rp_row0 + m) * p.rp_maxb + lane;
         P.token[base + lane] = p.rp_tokens[o];
         P.parent[base + lane] = parent;
         P.depth[base + lane] = p.level + 1;
         P.cum[base + lane] = pcum + p.rp_logp[o];
         P.row[base + lane] = -1;
-        s_tok[m * p.b + lane] = p.rp_tokens[o];
-        s_cum[m * p.b + lane] = pcum + p.rp_logp[o];
+        s_tok[m * b + lane] = p.rp_tokens[o];
+        s_cum[m * b + lane] = pcum + p.rp_logp[o];
       }
       continue;
     }
-    const float* st = p.stat + static_cast<size_t>(m) * p.nct * 2;
-    const float* cv = p.cand_val + static_cast<size_t>(m) * p.nct * kMaxBranch;
-    const int32_t* ci = p.cand_id + static_cast<size_t>(m) * p.nct * kMaxBranch;
+    const size_t rowoff = static_cast<size_t>(m) * kMaxBranch * nct;
+    const float* cv = cv0 + rowoff;
+    const int32_t* ci = ci0 + rowoff;
+    const float2* st = reinterpret_cast<const float2*>(st0) + static_cast<size_t>(m) * nct;
     constexpr int kLists = 8;  // lists per lane: nct <= 256 (host)
-    float hv[kLists], nv[kLists], smx[kLists], sse[kLists];
-    int hi[kLists], ni[kLists], hp[kLists];
+    // A candidate as two words that compare like cand_before: hk = its value as an order-preserving unsigned key
+    // (0 = no candidate), lo = (0xffffff - id) << 8 | CTA. The warp's best is then two redux.sync.max.
+    uint64_t key[kLists];
+    float smx[kLists], sse[kLists], v1[kLists];  // v1 / i1: every list's second entry, fetched with the heads
+    int i1[kLists];
 #pragma unroll
     for (int k = 0; k < kLists; ++k) {  // every load of the row is issued before the first use
       const int c = lane + 32 * k;
-      hp[k] = 0;
-      hv[k] = nv[k] = smx[k] = -INFINITY;
-      hi[k] = ni[k] = 0x7fffffff;
+      key[k] = 0ull;
+      smx[k] = v1[k] = -INFINITY;
       sse[k] = 0.f;
-      if (c < p.nct) {
-        hv[k] = __ldcg(cv + c * kMaxBranch);
-        hi[k] = __ldcg(ci + c * kMaxBranch);
-        if (p.b > 1) { nv[k] = __ldcg(cv + c * kMaxBranch + 1); ni[k] = __ldcg(ci + c * kMaxBranch + 1); }
-        smx[k] = __ldcg(st + c * 2);
-        sse[k] = __ldcg(st + c * 2 + 1);
+      i1[k] = kNoCand;
+      if (c < nct) {
+        const float v = __ldcg(cv + c);
+        const int id = __ldcg(ci + c);
+        const float2 s2 = __ldcg(st + c);
+        if (b > 1) { v1[k] = __ldcg(cv + nct + c); i1[k] = __ldcg(ci + nct + c); }
+        key[k] = (static_cast<uint64_t>(cand_key(v, id)) << 32) | cand_lo(id, c);
+        smx[k] = s2.x;
+        sse[k] = s2.y;
       }
     }
+    const int parent = p.cur->pool[m];  // (after the loads above are in flight)
+    const float pcum = parent < 0 ? 0.f : p.cur->cum[m];
     // log-sum-exp over the vocabulary from the per-CTA (max, sum exp) pairs, fixed order (lane-major, then butterfly)
     float mg = -INFINITY;
 #pragma unroll
@@ -270,46 +312,90 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
     for (int k = 0; k < kLists; ++k) se += (smx[k] == -INFINITY) ? 0.f : sse[k] * expf(smx[k] - mg);
     se = warp_sum(se);
     const float logz = mg + logf(se);
-    for (int jb = 0; jb < p.b; ++jb) {
-      float bv = -INFINITY;
-      int bi = 0x7fffffff;
+    // (2) the b best heads: lane r keeps the r-th. The lane's best is a pairwise tree (a serial scan of the eight
+    // is a chain of ~50 dependent instructions per round); the winner is cleared by value, ids being unique.
+    uint32_t* sh = reinterpret_cast<uint32_t*>(s_scr) + warp * per_row;
+    uint32_t* sl = sh + b * b;
+    uint32_t th = 0u, tl = 0u;
+    for (int r = 0; r < b; ++r) {
+      const uint64_t m01 = umax64(key[0], key[1]), m23 = umax64(key[2], key[3]);
+      const uint64_t m45 = umax64(key[4], key[5]), m67 = umax64(key[6], key[7]);
+      const uint64_t best = umax64(umax64(m01, m23), umax64(m45, m67));
+      const uint32_t bh = static_cast<uint32_t>(best >> 32), bl = static_cast<uint32_t>(best);
+      const uint32_t gh = __reduce_max_sync(0xffffffffu, bh);
+      const uint32_t gl = __reduce_max_sync(0xffffffffu, bh == gh ? bl : 0u);
+      const uint64_t g = (static_cast<uint64_t>(gh) << 32) | gl;
 #pragma unroll
       for (int k = 0; k < kLists; ++k)
-        if (cand_before(hv[k], hi[k], bv, bi)) { bv = hv[k]; bi = hi[k]; }
-      const int mine = bi;
+        if (key[k] == g && gh != 0u) {  // the winner hands the list's second entry over: (r, 1)
+          key[k] = 0ull;
+          if (b > 1) { sh[r * b + 1] = cand_key(v1[k], i1[k]); sl[r * b + 1] = cand_lo(i1[k], 0); }
+        }
+      if (lane == r) { th = gh; tl = gl; }
+    }
+    const int tc = th != 0u ? static_cast<int>(tl & 255u) : -1;  // CTA of the r-th list
+    // (3) tails of those lists: entry (r, j), 2 <= j < b - r, at scratch [r * b + j] (a second round trip, b > 2 only)
+    constexpr int kU = 16;
+    const int binv = (65536 + b - 1) / b;  // e / b == (e * binv) >> 16 for e < 1024, b <= 32
+    for (int e0 = 0; e0 < b * b && b > 2; e0 += 32 * kU) {
+      float v[kU];
+      int id[kU];
+      bool ok2[kU];
 #pragma unroll
-      for (int o = 16; o > 0; o >>= 1) {
-        const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-        const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-        if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-      }
-      if (mine == bi && bi != 0x7fffffff) {  // token ids are unique across the lists: exactly one lane advances
-#pragma unroll
-        for (int k = 0; k < kLists; ++k) {
-          if (hi[k] == bi) {
-            const int c = lane + 32 * k;
-            ++hp[k];
-            hv[k] = nv[k];
-            hi[k] = ni[k];
-            if (hp[k] + 1 < p.b) { nv[k] = __ldcg(cv + c * kMaxBranch + hp[k] + 1); ni[k] = __ldcg(ci + c * kMaxBranch + hp[k] + 1); }
-            else { nv[k] = -INFINITY; ni[k] = 0x7fffffff; }
-          }
+      for (int u = 0; u < kU; ++u) {
+        const int e = e0 + 32 * u + lane;
+        const int r = (e * binv) >> 16, j = e - r * b;
+        const int cr = __shfl_sync(0xffffffffu, tc, r & 31);
+        const bool ok = e < b * b && j >= 2 && j < b - r && cr >= 0;
+        v[u] = -INFINITY;
+        id[u] = kNoCand;
+        ok2[u] = ok;
+        if (ok) {
+          v[u] = __ldcg(cv + j * nct + cr);
+          id[u] = __ldcg(ci + j * nct + cr);
         }
       }
-      if (lane == 0) {
-        P.token[base + jb] = bi;
-        P.parent[base + jb] = parent;
-        P.depth[base + jb] = p.level + 1;
-        P.cum[base + jb] = pcum + (bv - logz);  // cumulative log-probability
-        P.row[base + jb] = -1;
-        s_tok[m * p.b + jb] = bi;  // phase B works from shared memory: no round trip through the pool
-        s_cum[m * p.b + jb] = pcum + (bv - logz);
+#pragma unroll
+      for (int u = 0; u < kU; ++u) {
+        const int e = e0 + 32 * u + lane;
+        if (ok2[u]) { sh[e] = cand_key(v[u], id[u]); sl[e] = cand_lo(id[u], 0); }
       }
     }
+    __syncwarp();
+    // (4) merge: lane r owns the r-th list
+    uint32_t lh = th, ll = tl & ~255u;
+    int hp = 0;
+    const int lim = tc >= 0 ? b - lane : 0;
+    uint32_t oh = 0u, ol = 0u;
+    for (int jb = 0; jb < b; ++jb) {
+      const uint32_t gh = __reduce_max_sync(0xffffffffu, lh);
+      const uint32_t gl = __reduce_max_sync(0xffffffffu, lh == gh ? ll : 0u);
+      if (lh == gh && ll == gl && gh != 0u) {
+        ++hp;
+        if (hp < lim) { lh = sh[lane * b + hp]; ll = sl[lane * b + hp]; }
+        else { lh = ll = 0u; }
+      }
+      if (lane == jb) { oh = gh; ol = gl; }
+    }
+    if (lane < b) {
+      const float ov = cand_key_value(oh);
+      const int oi = oh != 0u ? static_cast<int>(0xffffffu - (ol >> 8)) : kNoCand;
+      const float cum = pcum + (ov - logz);  // cumulative log-probability
+      P.token[base + lane] = oi;
+      P.parent[base + lane] = parent;
+      P.depth[base + lane] = p.level + 1;
+      P.cum[base + lane] = cum;
+      P.row[base + lane] = -1;
+      s_tok[m * b + lane] = oi;  // phase B works from shared memory: no round trip through the pool
+      s_cum[m * b + lane] = cum;
+    }
+    __syncwarp();
   }
+  if (tid == 0) s_nc = 0;
+  for (int i = tid; i < kPoolSmem / 32; i += kTreeThreads) s_bits[i] = 0u;
   __syncthreads();
 
-  const int n = p.M * p.b;
+  const int n = p.M * b;
   if (p.tap_token != nullptr || p.force_token != nullptr) {  // hooks: never set in a plain step
     for (int i = tid; i < n; i += kTreeThreads) {
       const int node = p.pool_begin + i;
@@ -325,76 +411,73 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   }
 
   // ---- phase B: frontier of the next level = top-M_next children by score -----
-  if (p.M_next > 0) {
-    // Everything a selected child needs is its parent's row of THIS level (m = i / b): the node forwarded there
-    // (cur->pool[m]), that row's step row (cur_row0 + m) and its ancestor mask (cur->mask[m]) -- no dependent
-    // loads through the pool arrays.
-    for (int i = tid; i < n; i += kTreeThreads) {
-      int rank = 0;
-      for (int j = 0; j < n; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
-      if (rank < p.M_next) {
-        const int node = p.pool_begin + i, r = rank, m = i / p.b;
-        const bool root = p.level == 0;
-        const int t = p.next_t0 + r;  // tree-row index = new-region slot
-        p.next->token[r] = s_tok[i];
-        p.next->src[r] = root ? p.n_new - 1 : p.cur_row0 + m;
-        p.next->slot[r] = t;
-        p.next->pool[r] = node;
-        P.row[node] = p.next_row0 + r;
-        for (int w = 0; w < kMaskWords; ++w) {
-          uint32_t mk = root ? 0u : p.cur->mask[m][w];
-          if ((t >> 5) == w) mk |= 1u << (t & 31);
-          p.treemask[t * kMaskWords + w] = mk;
-          p.next->mask[r][w] = mk;
-        }
+  // Everything a selected child needs is its parent's row of THIS level (m = i / b): the node forwarded there
+  // (cur->pool[m]), that row's step row (cur_row0 + m) and its ancestor mask (cur->mask[m]) -- no dependent
+  // loads through the pool arrays. A child ranked gamma or later among its own level cannot be in the step's
+  // top-gamma: it is marked, and S8 ranks only the others (<= depth x gamma instead of the whole pool).
+  for (int i = tid; i < n; i += kTreeThreads) {
+    int rank = 0;
+    for (int j = 0; j < n; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
+    const int node = p.pool_begin + i;
+    if (rank < p.M_next) {
+      const int r = rank, m = i / b;
+      const bool root = p.level == 0;
+      const int t = p.next_t0 + r;  // tree-row index = new-region slot
+      p.next->token[r] = s_tok[i];
+      p.next->src[r] = root ? p.n_new - 1 : p.cur_row0 + m;
+      p.next->slot[r] = t;
+      p.next->pool[r] = node;
+      p.next->cum[r] = s_cum[i];
+      P.row[node] = p.next_row0 + r;
+      for (int w = 0; w < kMaskWords; ++w) {
+        uint32_t mk = root ? 0u : p.cur->mask[m][w];
+        if ((t >> 5) == w) mk |= 1u << (t & 31);
+        p.treemask[t * kMaskWords + w] = mk;
+        p.next->mask[r][w] = mk;
       }
+    } else if (rank >= p.gamma) {
+      P.row[node] = -2;
     }
-    __syncthreads();
+  }
+  __syncthreads();
+  if (p.M_next > 0) {
     trace_end(p.trace);
     return;
   }
 
-  // ---- phase C (last level): S8, top-gamma of the whole pool, pool order ------
+  // ---- S8 (last level): top-gamma of the whole pool, emitted in pool order ------
   const int Pn = p.pool_total;
-  for (int i = tid; i < Pn; i += kTreeThreads) s_cum[i] = P.cum[i];
-  __syncthreads();
   const int n_keep = min(p.gamma, Pn);
+  float* s_cc = s_raw;                                            // candidate scores
+  int32_t* s_ci = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);  // candidate pool indices
   for (int i = tid; i < Pn; i += kTreeThreads) {
+    if (P.row[i] != -2) {
+      const int k = atomicAdd(&s_nc, 1);
+      s_ci[k] = i;
+      s_cc[k] = P.cum[i];
+    }
+  }
+  __syncthreads();
+  const int C = s_nc;  // >= n_keep: every level contributes its min(gamma, size) best
+  for (int a = tid; a < C; a += kTreeThreads) {
+    const float ca = s_cc[a];
+    const int ia = s_ci[a];
     int rank = 0;
-    for (int j = 0; j < Pn; ++j) rank += (j != i && node_before(s_cum, j, i)) ? 1 : 0;
-    s_new[i] = rank < n_keep ? 1 : 0;
+    for (int j = 0; j < C; ++j) {
+      const float cj = s_cc[j];
+      rank += (cj > ca || (cj == ca && s_ci[j] < ia)) ? 1 : 0;
+    }
+    if (rank < n_keep) atomicOr(&s_bits[ia >> 5], 1u << (ia & 31));
   }
   __syncthreads();
-  // exclusive prefix count of the keep flags: contiguous chunk per thread
-  const int chunk = (Pn + kTreeThreads - 1) / kTreeThreads;
-  const int lo = min(Pn, tid * chunk), hi = min(Pn, lo + chunk);
-  int cnt = 0;
-  for (int i = lo; i < hi; ++i) cnt += s_new[i];
-  s_cnt[tid + 1] = cnt;
-  __syncthreads();
-  if (warp == 0) {  // inclusive prefix over the per-thread counts: kTreeThreads / 32 entries per lane, then a warp scan
-    constexpr int E = kTreeThreads / 32;
-    int loc = 0;
-    for (int j = 0; j < E; ++j) loc += s_cnt[1 + lane * E + j];
-    int inc = loc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int v = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += v;
+  // output index of a kept node = kept nodes before it in the pool
+  int32_t* s_map = reinterpret_cast<int32_t*>(s_raw);  // (scores are read again from the pool)
+  for (int i = tid; i < Pn; i += kTreeThreads) {
+    if ((s_bits[i >> 5] >> (i & 31)) & 1u) {
+      int o = __popc(s_bits[i >> 5] & ((1u << (i & 31)) - 1u));
+      for (int w = 0; w < (i >> 5); ++w) o += __popc(s_bits[w]);
+      s_map[i] = o;
     }
-    int run2 = inc - loc;
-    for (int j = 0; j < E; ++j) {
-      run2 += s_cnt[1 + lane * E + j];
-      s_cnt[1 + lane * E + j] = run2;
-    }
-    if (lane == 0) s_cnt[0] = 0;
-  }
-  __syncthreads();
-  int run = s_cnt[tid];
-  for (int i = lo; i < hi; ++i) {
-    const int k = s_new[i];
-    s_new[i] = k ? run : -1;  // output index of node i, or -1
-    run += k;
   }
   __syncthreads();
   const StepDyn* dyn = p.dyn;
@@ -404,12 +487,12 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   int32_t* o_depths = p.o_ids ? p.o_depths : dyn->out_depths;
   int32_t* o_n = p.o_ids ? p.o_n : dyn->out_n;
   for (int i = tid; i < Pn; i += kTreeThreads) {
-    const int o = s_new[i];
-    if (o < 0) continue;
+    if (!((s_bits[i >> 5] >> (i & 31)) & 1u)) continue;
+    const int o = s_map[i];
     const int parent = P.parent[i];
     o_ids[o] = P.token[i];
-    o_scores[o] = s_cum[i];
-    o_parents[o] = parent < 0 ? -1 : s_new[parent];  // kept set is ancestor-closed (A7)
+    o_scores[o] = P.cum[i];
+    o_parents[o] = parent < 0 ? -1 : s_map[parent];  // kept set is ancestor-closed (A7)
     if (o_depths) o_depths[o] = P.depth[i];
     p.out_pool_idx[o] = i;
   }

@@ -119,6 +119,31 @@ def test_paper_preset_tree_7b_shape_full_size():
     assert (np.diff(free["scores"][free["parents"] >= 0]) <= 1e30).all() and (free["scores"] <= 0).all()
 
 
+@pytest.mark.parametrize("variant", ["f32", "bf16", "bf16_wide_tcgen05", "bf16_b32"])
+def test_lm_head_merge_exact_ties(variant):
+    """Every LM-head row appears twice (token v and token v + V / 2 share their weights), in different CTAs of
+    the LM head: every logit is an exact two-way tie, so every top-b list, the merge of the per-CTA lists in
+    k_tree_level, every frontier and the final top-gamma are decided by the tie rule (smaller token id / smaller
+    pool index first, the oracle's stable order). The tree must be IDENTICAL to the oracle's: no tie excuse."""
+    kw = dict(dtype=F32 if variant == "f32" else BF16, tree=TreeSpec(3, (8, 4, 4), (0, 6, 10), 30))
+    if variant == "bf16_b32":  # 32 children per row: both tail batches of the merge, 12 rows per level
+        kw.update(tree=TreeSpec(3, (32, 32, 4), (0, 12, 12), 64))
+    case = _boost(make_case(small_cfg(**kw), n_new=2))
+    lm = case.top["lm_head"]
+    V = lm.shape[0]
+    lm[V // 2:] = lm[:V // 2]
+    ora = run_oracle(case)
+    h, kv, gpu = run_gpu(case)
+    binding.dovetail_draft_destroy(h)
+    if variant == "bf16_wide_tcgen05":
+        assert gpu["umma_launches"] > 0
+    for key in ("token_ids", "parents", "depths"):
+        assert np.array_equal(gpu[key], ora[key]), key
+    tok = ora["token_ids"]
+    assert ((tok[:, None] % (V // 2)) == (tok[None, :] % (V // 2))).sum() > len(tok)  # tied pairs were emitted
+    np.testing.assert_allclose(gpu["scores"], ora["scores"], rtol=2e-2, atol=1e-2)
+
+
 def test_determinism_run_to_run():
     cfg = small_cfg(dtype=BF16)
     case = _boost(make_case(cfg, n_new=2))
