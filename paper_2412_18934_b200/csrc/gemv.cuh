@@ -324,27 +324,27 @@ __device__ __forceinline__ void gemv_epilogue(const GemvParams& p, const GemvGro
       se = warp_sum(se);
       const int64_t pc = static_cast<int64_t>(mbase + m) * nct + c;
       if (lane == 0) { p.stat[pc * 2] = mx; p.stat[pc * 2 + 1] = se; }
-      // local top-b: b rounds of "best candidate strictly after the previous pick"
-      float lv = INFINITY; int li = -1;
+      // local top-b: b rounds of "best candidate strictly after the previous pick", on order-preserving keys
+      // (epilogue.cuh cand_key / cand_lo): a lane's best is a max over independent values and the warp's best two
+      // redux.sync.max (chains of cand_before and five shuffle rounds cost ~5 us per row at 10 children).
+      uint64_t bound = ~0ull;
       for (int jb = 0; jb < p.b; ++jb) {
-        float bv = -INFINITY; int bi = 0x7fffffff;
+        uint64_t best = 0ull;
+#pragma unroll 4
         for (int v = lane; v < cnt; v += 32) {
-          const float val = res(v, m);
           const int id = static_cast<int>(rr.g0) + v;
-          if (cand_before(lv, li, val, id) && cand_before(val, id, bv, bi)) { bv = val; bi = id; }
+          const uint64_t key = (static_cast<uint64_t>(cand_key(res(v, m), id)) << 32) | cand_lo(id, 0);
+          best = umax64(best, key < bound ? key : 0ull);
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          const float ov = __shfl_xor_sync(0xffffffffu, bv, o);
-          const int oi = __shfl_xor_sync(0xffffffffu, bi, o);
-          if (cand_before(ov, oi, bv, bi)) { bv = ov; bi = oi; }
-        }
+        const uint32_t bh = static_cast<uint32_t>(best >> 32), bl = static_cast<uint32_t>(best);
+        const uint32_t gh = __reduce_max_sync(0xffffffffu, bh);
+        const uint32_t gl = __reduce_max_sync(0xffffffffu, bh == gh ? bl : 0u);
+        bound = (static_cast<uint64_t>(gh) << 32) | gl;
         if (lane == 0) {  // entry-major: the heads (jb = 0) of a row's lists are contiguous for k_tree_level
           const int64_t o = (static_cast<int64_t>(mbase + m) * kMaxBranch + jb) * nct + c;
-          p.cand_val[o] = bv;
-          p.cand_id[o] = bi;
+          p.cand_val[o] = cand_key_value(gh);
+          p.cand_id[o] = gh != 0u ? static_cast<int>(0xffffffu - (gl >> 8)) : kNoCand;
         }
-        lv = bv; li = bi;
       }
     }
   }

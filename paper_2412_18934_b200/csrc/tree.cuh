@@ -200,25 +200,9 @@ __device__ __forceinline__ bool node_before(const float* cum, int a, int b) {
   return ca > cb || (ca == cb && a < b);
 }
 
-// A candidate (value, id) as an order-preserving pair of unsigned words: (key, lo) compares like cand_before
-// (larger value first, then smaller id). key 0 = no candidate (below every real value, -inf included);
-// -0 is canonicalised to +0 (cand_before treats them as equal). ids < 2^24 (dovetail_draft_init checks the vocabulary).
-__device__ __forceinline__ uint32_t cand_key(float v, int id) {
-  const uint32_t u = __float_as_uint(v + 0.f);
-  return id == 0x7fffffff ? 0u : ((u >> 31) ? ~u : (u | 0x80000000u));
-}
-__device__ __forceinline__ uint32_t cand_lo(int id, int cta) {
-  return id == 0x7fffffff ? 0u : ((static_cast<uint32_t>(0xffffff - id) << 8) | static_cast<uint32_t>(cta));
-}
-__device__ __forceinline__ float cand_key_value(uint32_t key) {
-  return key == 0u ? -INFINITY : __uint_as_float((key >> 31) ? (key & 0x7fffffffu) : ~key);
-}
-
-__device__ __forceinline__ uint64_t umax64(uint64_t a, uint64_t b) { return a > b ? a : b; }
 
 constexpr int kTreeThreads = 512;  // one warp per expanded row for levels of <= 16 rows (a row's merge is a serial chain)
 constexpr int kPoolSmem = 4352;  // >= kMaxBranch + kMaxTreeSlots * kMaxBranch + slack
-constexpr int kNoCand = 0x7fffffff;  // id of the "no candidate" entry (value -inf): after every real candidate
 
 // Pool::row of a child: >= 0 the step row it is forwarded at; -1 not forwarded; -2 not forwarded and outside its
 // own level's top-gamma, hence outside the step's top-gamma (S8 does not look at it).
