@@ -435,10 +435,12 @@ __global__ void __launch_bounds__(kTreeThreads) k_tree_level(const TreeLevelPara
   float* s_cc = s_raw;                                            // candidate scores
   int32_t* s_ci = reinterpret_cast<int32_t*>(s_raw + kPoolSmem);  // candidate pool indices
   for (int i = tid; i < Pn; i += kTreeThreads) {
-    if (P.row[i] != -2) {
+    const int row = P.row[i];
+    const float cum = P.cum[i];  // unconditional: one round trip, not two
+    if (row != -2) {
       const int k = atomicAdd(&s_nc, 1);
       s_ci[k] = i;
-      s_cc[k] = P.cum[i];
+      s_cc[k] = cum;
     }
   }
   __syncthreads();
