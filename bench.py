@@ -437,6 +437,59 @@ def bench_one(a, cfg, rank, world, local, dist):
                                    "bound at 64 rows per pass, not yet a tile-reuse GEMM)"}
         del k2, v2
 
+    # ---- what the verifier needs from the step and the acceptance rule (+ kv_commit) ----------
+    # Device time of each call on the last step's candidates; synthetic target answers (a seeded distribution per
+    # verifier row). Pre-built argument structs: the loop times the library's kernels, not tensor allocation.
+    if a.verify_leg and world == 1:
+        import ctypes as C
+        lib, g1, md = binding.load(), tree.gamma + 1, tree.depth
+        step_device()
+        torch.cuda.synchronize()
+        gen = torch.Generator(device="cuda").manual_seed(cfg.seed + 11)
+        par, tok = out["parents"][:tree.gamma].long(), out["token_ids"][:tree.gamma].long()
+        logits_t = torch.randn((g1, cfg.vocab), generator=gen, device="cuda") * 3.0
+        logits_t[par + 1, tok] += 12.0  # a target that mostly agrees with the draft: paths of several nodes get accepted
+        p_full = torch.softmax(logits_t, dim=-1).contiguous()
+        p_cand = p_full[par + 1, tok].contiguous()  # candidate i's token at its parent's row
+        tgt_argmax = p_full.argmax(dim=-1).to(torch.int32)
+        unif = torch.rand(g1, generator=gen, device="cuda")
+        plan = dict(mask=torch.zeros((g1, g1), dtype=torch.uint8, device="cuda"), pos=torch.zeros(g1, dtype=torch.int32, device="cuda"),
+                    paths=torch.zeros((tree.gamma, md), dtype=torch.int32, device="cuda"), n=torch.zeros(1, dtype=torch.int32, device="cuda"))
+        res = dict(path=torch.full((md,), -1, dtype=torch.int32, device="cuda"), n=torch.zeros(1, dtype=torch.int32, device="cuda"),
+                   bonus=torch.zeros(1, dtype=torch.int32, device="cuda"))
+        o_t = binding._out_t(out)
+        plan_t = binding.VerifyPlanT(*(binding._dp(plan[k]) for k in ("mask", "pos", "paths", "n")))
+        in_t = binding.VerifyInT(binding._dp(tgt_argmax), binding._dp(p_cand), binding._dp(unif), binding._dp(p_full))
+        res_t = binding.VerifyOutT(binding._dp(res["path"]), binding._dp(res["n"]), binding._dp(res["bonus"]))
+        sp = binding._stream(None)
+        calls = {"verify_plan_us": lambda: lib.dovetail_verify_plan(h.ptr, C.byref(o_t), tree.gamma, case.L, md, C.byref(plan_t), sp),
+                 "verify_accept_greedy_us": lambda: lib.dovetail_verify_accept(h.ptr, C.byref(o_t), tree.gamma, 0, md, C.byref(in_t), C.byref(res_t), sp),
+                 "verify_accept_sampling_us": lambda: lib.dovetail_verify_accept(h.ptr, C.byref(o_t), tree.gamma, 1, md, C.byref(in_t), C.byref(res_t), sp)}
+        vleg = {}
+        for name, fn in calls.items():
+            for _ in range(3):
+                assert fn() == 0, binding.dovetail_last_error(h)
+            vleg[name] = timed(fn, 50) / 50 * 1e3
+        torch.cuda.synchronize()
+        n_acc = int(res["n"].item())
+        path = [int(x) for x in res["path"][:n_acc].tolist()]
+
+        if n_acc > 0:  # a commit consumes its step: one step per commit, events around the commit alone
+            ts = []
+            for it in range(13):
+                step_device()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                binding.dovetail_kv_commit(h, kv, path, mode=1)  # plan + row moves + the host's read of the committed count
+                e1.record(stream)
+                torch.cuda.synchronize()
+                if it >= 3:
+                    ts.append(e0.elapsed_time(e1) * 1e3)
+            vleg["kv_commit_us"] = sorted(ts)[len(ts) // 2]
+        vleg.update(accepted_by_sampling=n_acc, note="synthetic target distributions, candidates of the last step; events around 50 back-to-back calls, so a figure of a few us is an upper bound set by the host's call rate, not the kernel's own time; kv_commit includes its read-back of the committed count")
+        line["verify"] = vleg
+        step_device()  # the commit moved cache rows of the tree region: leave the cache as a step leaves it
+
     # ---- reading A1 "report both": the same step with dgf_proj = 0 (W1 = W2 = I) ----------------------------
     if a.both_dgf and world == 1 and cfg.dgf_proj == 1 and cfg.fusion == 0:
         cfg0 = dataclasses.replace(cfg, dgf_proj=0)
@@ -483,6 +536,7 @@ def main():
     ap.add_argument("--prefill-rows", type=int, default=256, help="rows of the dovetail_draft_prefill leg (0: skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-trace", action="store_true")
+    ap.add_argument("--no-verify-leg", dest="verify_leg", action="store_false", help="skip the verify_plan / verify_accept / kv_commit timings")
     ap.add_argument("--no-both-dgf", dest="both_dgf", action="store_false")
     a = ap.parse_args()
     rank, world, local = dist_env()

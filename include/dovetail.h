@@ -80,7 +80,7 @@ typedef struct {
   int32_t head_dim;     /* dh, 64 or 128                                  */
   int32_t n_layers;     /* draft Transformer blocks (the paper's M), <= DOVETAIL_MAX_LAYERS */
   int32_t ffn;          /* F                                              */
-  int32_t vocab;        /* V                                              */
+  int32_t vocab;        /* V <= 2^24 - 2 (token ids travel in 24 bits of a candidate key) */
   float rope_theta;
   float rms_eps;
   int32_t dtype;        /* dovetail_dtype_t of weights, norm gains, bias and KV cache */

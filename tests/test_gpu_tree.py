@@ -193,6 +193,12 @@ def test_error_paths():
     with pytest.raises(binding.DovetailError) as ei:
         binding.dovetail_draft_init(c2.top, c2.layers, bad)
     assert ei.value.code == binding.EINVAL
+    # token ids are packed into 24 bits of a candidate key (k_tree_level): larger vocabularies are refused, checked
+    # before any weight is read
+    from dataclasses import replace
+    with pytest.raises(binding.DovetailError) as ei:
+        binding.dovetail_draft_init(case.top, case.layers, replace(cfg, vocab=(1 << 24) - 1))
+    assert ei.value.code == binding.EINVAL
 
 
 def test_two_steps_chained_through_commit_mode1():

@@ -83,6 +83,52 @@ def test_verify_accept_bit_exact(ti, mode):
     binding.dovetail_draft_destroy(h)
 
 
+def test_verify_accept_large_ragged_vocabulary():
+    """The bonus-token draw on a vocabulary that is neither small nor a multiple of 32 (50 003): several narrowing
+    rounds of the inverse-CDF search, rejected children removed from the row, thresholds at both ends of the row,
+    and a stopping row without any mass (a degenerate target answer: every child has probability 0 and is rejected,
+    nothing is left to draw from, bonus token -1 as include/dovetail.h states). Bit-exact against the oracle.
+    (A normalised row whose mass sits entirely on the node's children cannot end in -1: the remainder shrinks with
+    every rejection and the last sibling is accepted with probability 1 -- both sides agree on that too.)"""
+    tree = TreeSpec(3, (3, 2, 2), (0, 3, 4), 9)
+    cfg = small_cfg(dtype=BF16, tree=tree, vocab=50003)
+    case = _boost(make_case(cfg, n_new=1))
+    h = binding.dovetail_draft_init(case.top, case.layers, cfg)
+    kv = binding.KVCache(case.k.clone(), case.v.clone(), case.L)
+    out = binding.dovetail_draft_step(h, case.feats, case.tokens, kv, tree)
+    n, g, V = int(out["n_out"].item()), tree.gamma, cfg.vocab
+    tok, par = out["token_ids"][:n].cpu().numpy(), out["parents"][:n].cpu().numpy()
+    dev = lambda a: torch.from_numpy(a).cuda()
+    roots = [i for i in range(n) if par[i] == -1]
+    for seed in range(10):
+        rng = np.random.default_rng(77 + seed)
+        pf = rng.random((g + 1, V)).astype(np.float32) ** 6
+        for i in range(n):
+            pf[par[i] + 1, tok[i]] += np.float32(rng.random() * V / 30)
+        pf = (pf / pf.sum(1, keepdims=True)).astype(np.float32)
+        if seed >= 8:  # the root row carries no mass at all
+            pf[0] = 0
+        p_cand = np.zeros(g, np.float32)
+        p_cand[:n] = pf[par + 1, tok]
+        u = rng.random(g + 1).astype(np.float32)
+        if seed in (3, 4):  # reject every child of the root: the bonus token comes from the root row
+            u[roots] = np.float32(0.9999999)
+        if seed == 3:
+            u[n] = np.float32(0.0)
+        if seed == 4:
+            u[n] = np.float32(0.99999994)
+        ora = oracle.verify_accept(tok, par, 1, tgt_argmax=None, p_cand=p_cand[:n], uniforms=u[:n + 1], p_full=pf[:n + 1])
+        res = binding.dovetail_verify_accept(h, out, 1, tree.depth, p_cand=dev(p_cand), uniforms=dev(u), p_full=dev(pf))
+        torch.cuda.synchronize()
+        na = int(res["n_acc"].item())
+        assert na == ora["n_acc"], (seed, na, ora)
+        assert np.array_equal(res["accepted_path"][:na].cpu().numpy(), ora["accepted_path"])
+        assert int(res["bonus_token"].item()) == ora["bonus_token"], seed
+        if seed >= 8:
+            assert na == 0 and ora["bonus_token"] == -1
+    binding.dovetail_draft_destroy(h)
+
+
 def test_round_trip_step_verify_commit():
     """One whole round on device outputs: step, verifier inputs, greedy acceptance against a target that agrees with
     the draft's best chain, kv_commit (mode 1) of the accepted path."""
