@@ -43,7 +43,7 @@ def _run(case, **kw):
 
 @pytest.mark.parametrize("dtype", [F32, BF16])
 @pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "fusion_linear", "no_first_norm_final_norm", "n_new5",
-                                     "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch"])
+                                     "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch", "tiny_vocab"])
 def test_step_parity_small(dtype, variant):
     kw, n_new, prefix = dict(dtype=dtype), 1, None
     if variant == "mha_dh128":
@@ -70,6 +70,8 @@ def test_step_parity_small(dtype, variant):
         n_new = 33
     elif variant == "max_branch":  # 32 children of the root, all forwarded: b = max_branch, a 32-row level
         kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    elif variant == "tiny_vocab":  # fewer vocabulary rows than SMs: one row per LM-head CTA, per-CTA lists shorter than b
+        kw.update(vocab=120, tree=TreeSpec(3, (8, 4, 2), (0, 5, 6), 20))
     case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
     s, gpu, ora = _run(case)
     assert s["same_tree"]  # forced run: always; the free run's tree may differ only by a logged local tie
