@@ -315,6 +315,38 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree,
                          int32_t* pool_parent, int32_t* pool_depth, float* pool_cum,
                          int32_t* pool_size, void* cuda_stream);
 
+/* The same tree bookkeeping (PAPER.md:94 expansion and cumulative scores, :100
+ * reduction to the gamma candidates) for callers that cannot allocate: code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc. No handle, no dovetail_draft_init: the candidate pool, the row
+ * tables, the ancestor masks and the bookkeeping state live in ONE file-scope
+ * device array of DOVETAIL_STATIC_SCRATCH_BYTES inside the library (every GPU
+ * that loads the library holds it until the process exits). The call itself
+ * allocates nothing (no cudaMalloc / cudaFree / allocating library routine):
+ * it enqueues two cudaMemsetAsync and one k_tree_level launch per level.
+ *   cand_tokens, cand_logp, n_rows, max_b, out: as for dovetail_tree_replay
+ *        (device memory, caller-owned; out->depths may be NULL).
+ * Limits (beyond them: DOVETAIL_EINVAL and a message naming the limit, nothing
+ * is enqueued): depth <= DOVETAIL_MAX_DEPTH, branch[l] <= 32, rows forwarded
+ * per level <= 64, tree rows <= 128, candidate pool
+ * sum_l rows_l * branch[l] <= DOVETAIL_STATIC_MAX_POOL (half of what a handle
+ * can hold; the paper's own tree, width 10 / depth 7, needs 610).
+ * The array is shared by every call on the device and keeps the previous call's
+ * contents; the call clears what has to start clean (level-0 row table,
+ * bookkeeping state) on cuda_stream before the first launch. Two calls that
+ * overlap on the GPU (different streams, or graphs replayed concurrently) RACE
+ * on it: serialise them. The device current at the call must be the stream's;
+ * the array's address is resolved once per device, at the first call there
+ * (make that call outside stream capture).
+ * Asynchronous on cuda_stream. Errors: EINVAL (null pointers, limits, lists too
+ * short), ECUDA (no device, symbol lookup or launch failure);
+ * dovetail_last_error(NULL) holds the message. */
+#define DOVETAIL_STATIC_MAX_POOL 2048
+#define DOVETAIL_STATIC_SCRATCH_BYTES 65536
+int dovetail_tree_replay_static(const dovetail_tree_spec_t* tree, const int32_t* cand_tokens,
+                                const float* cand_logp, int32_t n_rows, int32_t max_b,
+                                const dovetail_draft_out_t* out, void* cuda_stream);
+
 /* Result of the device-side input checks of the steps enqueued so far on this
  * handle (the step consumes the accepted tokens; a token id outside
  * [0, vocab) has no embedding row). dovetail_draft_step itself never

@@ -18,6 +18,7 @@ OK, EINVAL, ECAPACITY, ECUDA, ENOMEM = 0, -1, -2, -3, -4
 
 # include/dovetail.h
 EXPORTS = ("dovetail_draft_init", "dovetail_draft_step", "dovetail_draft_prefill", "dovetail_kv_commit", "dovetail_tree_replay",
+           "dovetail_tree_replay_static",
            "dovetail_verify_plan", "dovetail_verify_accept", "dovetail_draft_status", "dovetail_last_launch_count", "dovetail_forward_bytes",
            "dovetail_draft_destroy", "dovetail_last_error")
 # include/dovetail_hooks.h (test and measurement hooks)
@@ -111,6 +112,9 @@ def load() -> C.CDLL:
         lib.dovetail_tree_replay.restype = C.c_int
         lib.dovetail_tree_replay.argtypes = [C.c_void_p, C.POINTER(TreeSpecT), C.c_void_p, C.c_void_p, C.c_int32,
                                              C.c_int32, C.POINTER(DraftOutT)] + [C.c_void_p] * 6
+        lib.dovetail_tree_replay_static.restype = C.c_int
+        lib.dovetail_tree_replay_static.argtypes = [C.POINTER(TreeSpecT), C.c_void_p, C.c_void_p, C.c_int32, C.c_int32,
+                                                    C.POINTER(DraftOutT), C.c_void_p]
         lib.dovetail_verify_plan.restype = C.c_int
         lib.dovetail_verify_plan.argtypes = [C.c_void_p, C.POINTER(DraftOutT), C.c_int32, C.c_int32, C.c_int32,
                                              C.POINTER(VerifyPlanT), C.c_void_p]
@@ -351,6 +355,21 @@ def dovetail_tree_replay(h: Draft, tree: TreeSpec, cand_tokens, cand_logp, out: 
                                      _dp(pool.get("depth")), _dp(pool.get("cum")), _dp(pool.get("size")),
                                      _stream(stream))
     _check(rc, h.ptr)
+    return out
+
+
+STATIC_MAX_POOL, STATIC_SCRATCH_BYTES = 2048, 65536  # include/dovetail.h
+
+
+def dovetail_tree_replay_static(tree: TreeSpec, cand_tokens, cand_logp, out: Dict, stream=None) -> Dict:
+    """The tree bookkeeping without a handle and without any allocation (include/dovetail.h): scratch in a
+    file-scope device array of the library. `out` must be pre-allocated (alloc_out) -- this wrapper allocates
+    nothing on the device either. Calls that overlap on the GPU race on the shared scratch."""
+    t = tree_spec_t(tree)
+    o = _out_t(out)
+    rc = load().dovetail_tree_replay_static(C.byref(t), _dp(cand_tokens), _dp(cand_logp), cand_tokens.shape[0],
+                                            cand_tokens.shape[1], C.byref(o), _stream(stream))
+    _check(rc, None)
     return out
 
 

@@ -15,6 +15,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -1476,6 +1477,50 @@ int step_by_graph(dovetail_draft* h, cudaStream_t st, const float* hidden_feats,
   return DOVETAIL_OK;
 }
 
+// ---- dovetail_tree_replay_static (include/dovetail.h): scratch that nobody allocates ---------------------------
+// What dovetail_draft_init gets from cudaMalloc for the tree bookkeeping, laid out over ONE file-scope device
+// array instead. Every GPU that loads the library holds these bytes until the process exits; every call on a
+// device shares them and finds the previous call's contents (the entry point clears what must start clean).
+struct ReplayScratch {
+  int32_t pool_token[DOVETAIL_STATIC_MAX_POOL];
+  int32_t pool_parent[DOVETAIL_STATIC_MAX_POOL];
+  int32_t pool_depth[DOVETAIL_STATIC_MAX_POOL];
+  float pool_cum[DOVETAIL_STATIC_MAX_POOL];
+  int32_t pool_row[DOVETAIL_STATIC_MAX_POOL];
+  int32_t out_pool_idx[DOVETAIL_STATIC_MAX_POOL];
+  uint32_t treemask[kMaxTreeSlots * kMaskWords];
+  RowTables rt[2];
+  TreeState ts;
+};
+static_assert(sizeof(ReplayScratch) <= DOVETAIL_STATIC_SCRATCH_BYTES, "the stated scratch size must hold the layout");
+static_assert(DOVETAIL_STATIC_MAX_POOL <= kPoolSmem, "k_tree_level stages the pool's scores in shared memory");
+static __device__ __align__(256) unsigned char g_replay_scratch[DOVETAIL_STATIC_SCRATCH_BYTES];
+
+// In host code `g_replay_scratch` is only a stand-in for the symbol, NOT a device address: a kernel handed it would
+// fault (or, where the GPU can reach host memory, quietly use the wrong bytes). The device address is looked up
+// once per device, with that device current, and kept.
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+ReplayScratch* g_static_ptr[kStaticMaxDevices] = {};
+
+int replay_scratch(ReplayScratch** out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return fail(nullptr, DOVETAIL_ECUDA, "no CUDA device: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, DOVETAIL_ECUDA, "device ordinal %d out of range", dev);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (g_static_ptr[dev] == nullptr) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_replay_scratch);
+    if (e != cudaSuccess || p == nullptr)
+      return fail(nullptr, DOVETAIL_ECUDA, "cudaGetSymbolAddress(static scratch) failed on device %d: %s", dev,
+                  cudaGetErrorString(e));
+    g_static_ptr[dev] = static_cast<ReplayScratch*>(p);
+  }
+  *out = g_static_ptr[dev];
+  return DOVETAIL_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -1887,6 +1932,95 @@ int dovetail_tree_replay(dovetail_draft_t* h, const dovetail_tree_spec_t* tree, 
   h->trace_on = trace_was;
   return DOVETAIL_OK;
 }
+
+// No allocation on this path: no cudaMalloc / cudaFree, no std::vector, no handle. (begin: no-alloc entry point)
+int dovetail_tree_replay_static(const dovetail_tree_spec_t* tree, const int32_t* cand_tokens, const float* cand_logp,
+                                int32_t n_rows, int32_t max_b, const dovetail_draft_out_t* out, void* cuda_stream) {
+  if (!tree || !cand_tokens || !cand_logp || !out || !out->token_ids || !out->scores || !out->parents || !out->n_out)
+    return fail(nullptr, DOVETAIL_EINVAL, "null argument");
+  // the level plan of validate_tree with n_new = 1, against the compile-time limits of the static scratch
+  if (tree->depth < 1 || tree->depth > DOVETAIL_MAX_DEPTH)
+    return fail(nullptr, DOVETAIL_EINVAL, "tree depth %d out of range [1, %d]", tree->depth, DOVETAIL_MAX_DEPTH);
+  if (tree->gamma < 1) return fail(nullptr, DOVETAIL_EINVAL, "gamma must be >= 1");
+  LevelPlan plan[DOVETAIL_MAX_DEPTH];
+  int m = 1, tree_rows = 0, need_rows = 1, maxb = 0;
+  long pool = 0;
+  for (int l = 0; l < tree->depth; ++l) {
+    if (tree->branch[l] < 1 || tree->branch[l] > kMaxBranch)
+      return fail(nullptr, DOVETAIL_EINVAL, "branch[%d] = %d out of range [1, %d]", l, tree->branch[l], kMaxBranch);
+    maxb = std::max(maxb, tree->branch[l]);
+    if (l >= 1) {
+      if (tree->beam[l] < 0) return fail(nullptr, DOVETAIL_EINVAL, "beam[%d] negative", l);
+      const long n = static_cast<long>(m) * tree->branch[l - 1];
+      const long mm = (tree->beam[l] > 0 && tree->beam[l] < n) ? tree->beam[l] : n;
+      if (mm > kMaxRows)
+        return fail(nullptr, DOVETAIL_EINVAL, "level %d forwards %ld rows > the static limit of %d rows per level", l, mm, kMaxRows);
+      m = static_cast<int>(mm);
+      plan[l] = LevelPlan{m, m, 1 + tree_rows, tree_rows, 0};
+      tree_rows += m;
+      need_rows += m;
+    } else {
+      plan[0] = LevelPlan{1, 1, 0, 0, 0};
+    }
+    plan[l].pool_begin = static_cast<int>(pool);
+    pool += static_cast<long>(plan[l].rows_lm) * tree->branch[l];
+    if (tree_rows > kMaxTreeSlots)
+      return fail(nullptr, DOVETAIL_EINVAL, "tree forwards %d rows > the static limit of %d tree rows", tree_rows, kMaxTreeSlots);
+    if (pool > DOVETAIL_STATIC_MAX_POOL)
+      return fail(nullptr, DOVETAIL_EINVAL, "candidate pool of %ld nodes exceeds DOVETAIL_STATIC_MAX_POOL = %d (the static scratch is %d bytes)",
+                  pool, DOVETAIL_STATIC_MAX_POOL, DOVETAIL_STATIC_SCRATCH_BYTES);
+  }
+  if (n_rows < need_rows || max_b < maxb)
+    return fail(nullptr, DOVETAIL_EINVAL, "replay needs %d rows of %d candidates", need_rows, maxb);
+  ReplayScratch* sc = nullptr;
+  const int rc = replay_scratch(&sc);
+  if (rc != DOVETAIL_OK) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  // the array keeps the previous call's contents: the level-0 row table (pool = -1: the root) and the bookkeeping
+  // state start clean; everything else (pool entries, masks, the other row table) is written before it is read
+  cudaError_t e = cudaMemsetAsync(&sc->rt[0], 0xff, sizeof(RowTables), st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(&sc->ts, 0, sizeof(TreeState), st);
+  if (e != cudaSuccess) return fail(nullptr, DOVETAIL_ECUDA, "memset failed: %s", cudaGetErrorString(e));
+  int row = 0;
+  for (int l = 0; l < tree->depth; ++l) {
+    const LevelPlan& lp = plan[l];
+    const bool last = l + 1 == tree->depth;
+    TreeLevelParams t{};
+    t.dyn = nullptr;  // never read: the explicit outputs below are set
+    t.ts = &sc->ts;
+    t.pool = Pool{sc->pool_token, sc->pool_parent, sc->pool_depth, sc->pool_cum, sc->pool_row};
+    t.treemask = sc->treemask;
+    t.rp_tokens = cand_tokens;
+    t.rp_logp = cand_logp;
+    t.rp_maxb = max_b;
+    t.rp_row0 = row;
+    t.M = lp.rows_lm;
+    t.b = tree->branch[l];
+    t.level = l;
+    t.pool_begin = lp.pool_begin;
+    t.M_next = last ? 0 : plan[l + 1].rows;
+    t.next_row0 = last ? 0 : plan[l + 1].row0;
+    t.cur_row0 = lp.row0;
+    t.next_t0 = last ? 0 : plan[l + 1].t0;
+    t.n_new = 1;
+    t.cur = &sc->rt[l & 1];
+    t.next = &sc->rt[(l + 1) & 1];
+    t.gamma = tree->gamma;
+    t.pool_total = static_cast<int>(pool);
+    t.out_pool_idx = sc->out_pool_idx;
+    t.o_ids = out->token_ids;
+    t.o_scores = out->scores;
+    t.o_parents = out->parents;
+    t.o_depths = out->depths;
+    t.o_n = out->n_out;
+    k_tree_level<<<1, kTreeThreads, 0, st>>>(t);  // plain stream order: each level sees the one before it complete
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(nullptr, DOVETAIL_ECUDA, "tree launch failed: %s", cudaGetErrorString(e));
+    row += lp.rows_lm;
+  }
+  return DOVETAIL_OK;
+}
+// (end: no-alloc entry point)
 
 int dovetail_hooks_set(dovetail_draft_t* h, const dovetail_hooks_t* hooks) {
   if (!h) return DOVETAIL_EINVAL;
