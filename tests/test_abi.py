@@ -84,3 +84,31 @@ def test_binding_refuses_missing_library(monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libdovetail_draft.so")
     with pytest.raises(FileNotFoundError):
         binding.load()
+
+
+def test_headers_compile_as_plain_c_and_a_c_program_links(tmp_path):
+    """The boundary is a C ABI: both headers are valid C99 and C++17 on their own (-Wall -Wextra -pedantic -Werror),
+    and a C program with no Python, torch or CUDA headers links against the library and gets error codes, not
+    aborts, from NULL arguments."""
+    import subprocess
+    inc = os.path.join(ROOT, "include")
+    libdir = os.path.join(ROOT, "paper_2412_18934_b200")
+    binding.load()  # builds the library if it is missing
+    for hdr in ("dovetail.h", "dovetail_hooks.h"):
+        for comp, std, lang in (("gcc", "-std=c99", "c"), ("g++", "-std=c++17", "c++")):
+            subprocess.run([comp, std, "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", "-x", lang, "-I", inc,
+                            os.path.join(inc, hdr)], check=True)
+    src = tmp_path / "main.c"
+    src.write_text('#include <stdio.h>\n#include <string.h>\n#include "dovetail.h"\n'
+                   "int main(void) {\n"
+                   "  if (dovetail_draft_init(NULL, NULL, NULL) != DOVETAIL_EINVAL) return 1;\n"
+                   "  if (dovetail_tree_replay_static(NULL, NULL, NULL, 0, 0, NULL, NULL) != DOVETAIL_EINVAL) return 2;\n"
+                   '  if (strstr(dovetail_last_error(NULL), "null") == NULL) return 3;\n'
+                   "  if (dovetail_forward_bytes(NULL, 0) != 0) return 4;\n"
+                   "  dovetail_draft_destroy(NULL);\n"
+                   '  puts("ok");\n  return 0;\n}\n')
+    exe = tmp_path / "main"
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", inc, str(src), "-o", str(exe), "-L", libdir,
+                    "-ldovetail_draft", f"-Wl,-rpath,{libdir}"], check=True)
+    out = subprocess.run([str(exe)], check=True, capture_output=True, text=True)
+    assert out.stdout.strip() == "ok"
