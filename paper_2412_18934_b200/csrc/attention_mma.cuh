@@ -651,42 +651,45 @@ __global__ void __launch_bounds__(kAmThreads, QT <= 2 ? 2 : 1) k_tree_attention_
       const int G = max(1, (kAmStages * BLK_BYTES / 4) / rec);  // query vectors per group
       for (int q0 = 0; q0 < qv_tot; q0 += G) {
         const int gq = min(G, qv_tot - q0);
-        const int n_el = gq * rec;
-        for (int base = 0; base < n_el; base += kAmConsumers * 8) {
-          float v[8];
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int e = base + i * kAmConsumers + tid;
-            v[i] = 0.f;
-            if (e < n_el) {
-              const int q = e / rec, rem = e - q * rec, cc = rem / WSTR, w = rem - cc * WSTR;
-              v[i] = __ldcg(p.ws + ((static_cast<size_t>(hk) * n_groups + cc) * p.qv_cap + q0 + q) * WSTR + w);
-            }
-          }
-#pragma unroll
-          for (int i = 0; i < 8; ++i) {
-            const int e = base + i * kAmConsumers + tid;
-            if (e < n_el) stg[e] = v[i];
-          }
+        // 16-byte asynchronous copies straight into shared memory, all in flight at once, from a loop of a few
+        // instructions: this code runs in one CTA per kv-head and launch, i.e. with a cold instruction cache --
+        // an unrolled register-staged copy (8 loads per thread and round, 4 rounds) took 4.6 us, and unrolling it
+        // further made it slower
+        const int rec4 = rec / 4, w4n = WSTR / 4;  // 16-byte pieces per query vector / per record
+        const uint32_t stg_u = smem_u32(stg);
+        const uint64_t pol_m = l2_policy_evict_last();
+        for (int e = tid; e < gq * rec4; e += kAmConsumers) {
+          const int q = e / rec4, rem = e - q * rec4, cc = rem / w4n, w4 = rem - cc * w4n;
+          cp_async16(stg_u + static_cast<uint32_t>(e) * 16u,
+                     p.ws + ((static_cast<size_t>(hk) * n_groups + cc) * p.qv_cap + q0 + q) * WSTR + w4 * 4, 16u, pol_m);
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");
         am_consumer_sync();
-        for (int idx = tid; idx < gq * DH; idx += kAmConsumers) {
-          const int q = idx / DH, dd = idx % DH, qv = q0 + q;
+        for (int idx = tid; idx < gq * (DH / 4); idx += kAmConsumers) {  // four d per thread: one set of weights per float4
+          const int q = idx / (DH / 4), dd = (idx % (DH / 4)) * 4, qv = q0 + q;
           const float* base = stg + q * rec;
           float mm = -INFINITY;
           for (int cc = 0; cc < n_groups; ++cc) mm = fmaxf(mm, base[cc * WSTR + DH]);
-          float ll = 0.f, oo = 0.f;
+          float ll = 0.f;
+          float4 oo = make_float4(0.f, 0.f, 0.f, 0.f);
           for (int cc = 0; cc < n_groups; ++cc) {
             const float* rr = base + cc * WSTR;
             const float cw = (rr[DH] == -INFINITY) ? 0.f : expf(rr[DH] - mm);
+            const float4 ov = *reinterpret_cast<const float4*>(rr + dd);
             ll += rr[DH + 1] * cw;
-            oo += rr[dd] * cw;
+            oo.x += ov.x * cw;
+            oo.y += ov.y * cw;
+            oo.z += ov.z * cw;
+            oo.w += ov.w * cw;
           }
           const int m = qv / grp, hq = hk * grp + qv % grp;
-          {
-            const float ov = oo / ll;
-            p.obuf[static_cast<size_t>(m) * dq + hq * DH + dd] = ov;
-            if (p.so.xs) store_split(p.so, m, hq * DH + dd, ov);
+          const float4 ov = make_float4(oo.x / ll, oo.y / ll, oo.z / ll, oo.w / ll);
+          *reinterpret_cast<float4*>(p.obuf + static_cast<size_t>(m) * dq + hq * DH + dd) = ov;
+          if (p.so.xs) {
+            store_split(p.so, m, hq * DH + dd, ov.x);
+            store_split(p.so, m, hq * DH + dd + 1, ov.y);
+            store_split(p.so, m, hq * DH + dd + 2, ov.z);
+            store_split(p.so, m, hq * DH + dd + 3, ov.w);
           }
         }
         am_consumer_sync();
