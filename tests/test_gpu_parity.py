@@ -43,7 +43,8 @@ def _run(case, **kw):
 
 @pytest.mark.parametrize("dtype", [F32, BF16])
 @pytest.mark.parametrize("variant", ["base", "mha_dh128", "mqa", "no_proj", "fusion_linear", "no_first_norm_final_norm", "n_new5",
-                                     "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch", "tiny_vocab"])
+                                     "no_prefix", "long_prefix", "wide", "very_wide", "n_new33", "max_branch", "tiny_vocab",
+                                     "prefix3100_three_clusters", "prefix3100_three_clusters_n_new40"])
 def test_step_parity_small(dtype, variant):
     kw, n_new, prefix = dict(dtype=dtype), 1, None
     if variant == "mha_dh128":
@@ -70,6 +71,10 @@ def test_step_parity_small(dtype, variant):
         n_new = 33
     elif variant == "max_branch":  # 32 children of the root, all forwarded: b = max_branch, a 32-row level
         kw.update(tree=TreeSpec(2, (32, 1), (0, 32), 40))
+    elif variant == "prefix3100_three_clusters":  # 49 blocks of 64 positions: 24 chunks per kv-head = 3 clusters of 8, merged across groups
+        prefix, n_new = 3100, 2
+    elif variant == "prefix3100_three_clusters_n_new40":  # 80 query vectors per kv-head: more than one staging round (62) of that merge
+        prefix, n_new = 3100, 40
     elif variant == "tiny_vocab":  # fewer vocabulary rows than SMs: one row per LM-head CTA, per-CTA lists shorter than b
         kw.update(vocab=120, tree=TreeSpec(3, (8, 4, 2), (0, 5, 6), 20))
     case = _boost(make_case(small_cfg(**kw), n_new=n_new, prefix=prefix))
